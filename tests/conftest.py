@@ -1,0 +1,21 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+
+
+@pytest.fixture(scope="session")
+def libset():
+    """The C-ABI library, built on demand (nvcc cross-compiles without a GPU)."""
+    from paper_2606_05495_b200 import build as _b
+    _b.build()
+    import paper_2606_05495_b200 as pkg
+    return pkg

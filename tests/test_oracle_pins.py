@@ -1,0 +1,393 @@
+"""Pins for the CPU oracle: every oracle function is checked against something other than itself --
+closed forms, invariants, textbook constants (tests/golden/), library routines on special cases, and
+pure-Python brute force on tiny inputs.  SURVEY.md §8(c) lists the pins per config.  CPU only."""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import inputgen
+import oracle
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(name):
+    rows = {}
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].split()
+        if line:
+            rows.setdefault(line[0], []).append([float(x) for x in line[1:]])
+    return rows
+
+
+# =============================================================== config 0: scan + hist64
+def test_c0_scan_last_is_sum_and_differences():
+    v = inputgen.config0_job(11)
+    s = oracle.scan_i32(v)
+    assert int(s[-1]) == int(v.astype(np.int64).sum())
+    assert s[0] == v[0]
+    assert np.array_equal(np.diff(s.astype(np.int64)), v[1:].astype(np.int64))
+
+
+def test_c0_all_ones_closed_form():
+    v = np.ones(4096, np.int32)
+    s = oracle.scan_i32(v)
+    assert np.array_equal(s, np.arange(1, 4097, dtype=np.int32))
+    h = oracle.hist_mod(s, 64)
+    assert np.array_equal(h, np.full(64, 64, np.uint32))
+
+
+def test_c0_bruteforce_tiny():
+    for n in (1, 2, 7, 33, 64):
+        v = inputgen.config0_job(100 + n, n)
+        s = oracle.scan_i32(v)
+        brute = [sum(int(v[k]) for k in range(i + 1)) for i in range(n)]  # O(n^2)
+        assert s.tolist() == brute
+        h = oracle.hist_mod(s, 64)
+        hb = [sum(1 for x in brute if x % 64 == b) for b in range(64)]
+        assert h.tolist() == hb
+
+
+def test_c0_hist_mass_and_input_variant_closed_form():
+    n = 4096
+    v = (np.arange(n) % 1000).astype(np.int32)
+    out = oracle.config0(v, hist_of_input=True)
+    h = out[n * 4:].view(np.uint32)
+    assert int(h.sum()) == n
+    # per full thousand: values 0..999 -> 16 per bin for b<40 (1000 = 15*64+40), 15 for b>=40;
+    # 4096 = 4 thousands + the values 0..95 (one more for every bin, one more again for b<32)
+    expect = np.array([4 * (16 if b < 40 else 15) + 1 + (1 if b < 32 else 0) for b in range(64)], np.uint32)
+    assert np.array_equal(h, expect)
+
+
+def test_c0_chain_layout_and_stage_order():
+    v = inputgen.config0_job(5)
+    out = oracle.config0(v)
+    assert out.size == 4096 * 4 + 256
+    scan = out[:4096 * 4].view(np.int32)
+    hist = out[4096 * 4:].view(np.uint32)
+    assert np.array_equal(scan, np.cumsum(v.astype(np.int64)).astype(np.int32))  # library routine
+    assert np.array_equal(hist, np.bincount(scan % 64, minlength=64).astype(np.uint32))
+    assert int(hist.sum()) == 4096
+    # reading C0-1: the histogram of the scan differs from the histogram of the input
+    assert not np.array_equal(hist, np.bincount(v % 64, minlength=64).astype(np.uint32))
+
+
+def test_c0_empty_and_single():
+    assert oracle.scan_i32(np.zeros(0, np.int32)).size == 0
+    assert oracle.hist_mod(np.zeros(0, np.int32)).sum() == 0
+    assert oracle.scan_i32(np.array([7], np.int32)).tolist() == [7]
+
+
+# =============================================================== config 1: fp32 chain + sum
+def test_c1_zero_input_golden():
+    g = _golden("config1_zero_input.txt")
+    z = np.zeros(16384, np.float32)
+    r, t4 = oracle.config1(z, z, want_t4=True)
+    assert np.all(t4 == np.float32(g["t4"][0][0]))
+    assert float(t4[0]) == g["t4"][0][0]
+    assert float(r) == g["sum"][0][0]
+    # the golden numbers themselves follow from exact rational arithmetic
+    tenth = Fraction(float(np.float32(0.1)))
+    sq = float(np.float32(float(tenth * tenth)))  # exact product -> one rounding to fp32 (double holds 48 bits)
+    assert sq == g["t4"][0][0]
+    assert float(np.float32(sq * 16384)) == g["sum"][0][0]
+
+
+def test_c1_relu_kills_negative_branch():
+    x = np.full(16384, -1.0, np.float32)
+    assert float(oracle.config1(x, np.zeros_like(x))) == 0.0
+    # bias is added BEFORE the ReLU: bias = +3 revives it: (2.5*-1+0.1+3)^2 = 0.6^2
+    r = oracle.config1(x, np.full_like(x, 3.0))
+    assert abs(float(r) / 16384 - 0.36) < 1e-6
+
+
+def test_c1_each_step_is_one_fp32_rounding():
+    j = inputgen.config1_job(3)
+    x, b = j[:16384], j[16384:]
+    _, t4 = oracle.config1(x, b, want_t4=True)
+    # independent route: evaluate every step exactly in double (operands are fp32, so product and sums are
+    # exact in double for these magnitudes) and round ONCE to fp32
+    xd, bd = x.astype(np.float64), b.astype(np.float64)
+    m = (2.5 * xd).astype(np.float32)
+    t1 = (m.astype(np.float64) + float(np.float32(0.1))).astype(np.float32)
+    t2 = (t1.astype(np.float64) + bd).astype(np.float32)
+    t3 = np.maximum(t2, np.float32(0))
+    t4r = (t3.astype(np.float64) ** 2).astype(np.float32)
+    assert np.array_equal(t4, t4r)
+    # and it is NOT the fused evaluation fl(2.5*x + 0.1) (reading C1-1): some elements must differ
+    fused = (2.5 * xd + float(np.float32(0.1))).astype(np.float32)
+    assert np.count_nonzero(fused != t1) > 100
+
+
+def test_c1_sum_in_double_vs_independent_double_chain():
+    for job in (0, 1, 2):
+        j = inputgen.config1_job(job)
+        x, b = j[:16384], j[16384:]
+        r, t4 = oracle.config1(x, b, want_t4=True)
+        assert float(r) >= 0.0
+        assert float(r) == float(np.float32(math.fsum(t4.astype(np.float64).tolist())))  # exact sum, one rounding
+        dbl = np.maximum(2.5 * x.astype(np.float64) + 0.1 + b.astype(np.float64), 0.0) ** 2
+        assert abs(float(r) - dbl.sum()) <= 1e-6 * dbl.sum()
+
+
+def test_c1_tiny_python_bruteforce():
+    x = np.array([0.5, -0.25, 0.75, -1.0, 0.0], np.float32)
+    b = np.array([0.0, 1.0, -3.0, 2.45, -0.1], np.float32)
+    f = np.float32
+    acc = 0.0
+    for xi, bi in zip(x, b):
+        t = f(f(f(2.5) * xi) + f(0.1))
+        t = f(t + bi)
+        t = t if t > 0 else f(0)
+        acc += float(f(t * t))
+    assert float(oracle.config1(x, b)) == float(f(acc))
+
+
+# =============================================================== config 2: Jacobi
+def test_c2_constant_field_interior_and_zero_halo_edges():
+    u = np.ones((16, 16), np.float32)
+    o = oracle.jacobi5_sweep(u)
+    assert np.all(o[1:-1, 1:-1] == np.float32(1.0))           # fl(0.2f*5) == 1
+    f = np.float32
+    assert o[0, 0] == f(0.2) * f(3) and o[0, 15] == f(0.2) * f(3) and o[15, 0] == f(0.2) * f(3)
+    assert np.all(o[0, 1:-1] == f(0.2) * f(4)) and np.all(o[1:-1, 0] == f(0.2) * f(4))
+    assert np.all(o[-1, 1:-1] == f(0.2) * f(4)) and np.all(o[1:-1, -1] == f(0.2) * f(4))
+    for t in (2, 3, 5):
+        o = oracle.config2(np.ones((32, 32), np.float32), t)
+        assert np.all(o[t:-t, t:-t] == np.float32(1.0))
+        assert o[t - 1, 16] != np.float32(1.0)
+
+
+def _walks(t, dx, dy):
+    """number of t-step walks over {stay, +-x, +-y} ending at (dx, dy) -- multinomial count"""
+    cnt = 0
+    for r in range(t + 1):              # right
+        l = r - dx
+        if l < 0: continue
+        for up in range(t + 1 - r - l):
+            d = up - dy
+            if d < 0: continue
+            s = t - r - l - up - d
+            if s < 0: continue
+            cnt += math.factorial(t) // (math.factorial(r) * math.factorial(l) * math.factorial(up)
+                                         * math.factorial(d) * math.factorial(s))
+    return cnt
+
+
+def test_c2_unit_impulse_walk_counts_and_mass():
+    n = 33
+    u = np.zeros((n, n), np.float32)
+    u[16, 16] = 1.0
+    o2 = oracle.config2(u, 2).astype(np.float64)
+    expect = {(0, 0): 5, (1, 0): 2, (0, 1): 2, (2, 0): 1, (0, 2): 1, (1, 1): 2, (2, 1): 0}
+    for (dy, dx), c in expect.items():
+        for sy in (1, -1):
+            for sx in (1, -1):
+                assert abs(o2[16 + sy * dy, 16 + sx * dx] - c / 25.0) <= 1e-6 * max(c / 25.0, 1e-30)
+    for t in (1, 3, 4, 7):
+        o = oracle.config2(u, t).astype(np.float64)
+        for dy in range(-t - 1, t + 2):
+            for dx in range(-t - 1, t + 2):
+                want = _walks(t, dx, dy) * 0.2 ** t
+                assert abs(o[16 + dy, 16 + dx] - want) <= 2e-6 * want + 1e-30
+        assert abs(o.sum() - 1.0) < 1e-5            # mass conserved while it has not reached the edge
+    # near the edge the zero halo loses mass
+    e = np.zeros((8, 8), np.float32); e[0, 0] = 1.0
+    assert abs(oracle.config2(e, 1).astype(np.float64).sum() - 0.6) < 1e-6
+
+
+def test_c2_scaling_by_two_is_exact():
+    u = inputgen.config2_job(7, 64, 48)
+    a = oracle.config2(u, 10)
+    b = oracle.config2(u * np.float32(2), 10)
+    assert np.array_equal(b, a * np.float32(2))
+
+
+def test_c2_association_order_pin():
+    # ((c + w) + e): c=1e8, w=-1e8, e=1 -> 1 ; the other order c+(w+e) would give 0 in fp32
+    u = np.zeros((3, 3), np.float32)
+    u[1, 1], u[1, 0], u[1, 2] = 1e8, -1e8, 1.0
+    o = oracle.jacobi5_sweep(u)
+    assert o[1, 1] == np.float32(0.2) * np.float32(1.0)
+    # n and s enter after w and e: c=1, w=1e8, e=-1e8 (cancel first), n=3, s=5 -> 0.2*9
+    u = np.zeros((3, 3), np.float32)
+    u[1, 1], u[1, 0], u[1, 2], u[0, 1], u[2, 1] = 1.0, 1e8, -1e8, 3.0, 5.0
+    # (1+1e8) = 1e8 in fp32, + -1e8 = 0, +3 +5 = 8
+    assert oracle.jacobi5_sweep(u)[1, 1] == np.float32(0.2) * np.float32(8.0)
+
+
+def test_c2_fp64_bruteforce_8x8_and_nonsquare():
+    for (h, w) in ((8, 8), (5, 9)):
+        u = inputgen.config2_job(3, h, w)
+        ref = [[float(u[i, j]) for j in range(w)] for i in range(h)]
+        for _ in range(10):
+            g = lambda i, j: ref[i][j] if 0 <= i < h and 0 <= j < w else 0.0
+            ref = [[0.2 * (g(i, j) + g(i, j - 1) + g(i, j + 1) + g(i - 1, j) + g(i + 1, j)) for j in range(w)]
+                   for i in range(h)]
+        o = oracle.config2(u, 10).astype(np.float64)
+        ref = np.array(ref)
+        assert np.abs(o - ref).max() <= 1e-6 * np.abs(ref).max()
+
+
+def test_c2_sweep_parity_and_input_untouched():
+    u = inputgen.config2_job(1, 12, 12)
+    keep = u.copy()
+    s = u
+    for t in range(0, 5):
+        assert np.array_equal(oracle.config2(u, t), s)
+        s = oracle.jacobi5_sweep(s)
+    assert np.array_equal(u, keep)
+
+
+# =============================================================== config 3: GEMM + bias + GELU
+def test_c3_gelu_textbook_values():
+    for line in open(os.path.join(GOLD, "gelu_values.txt")):
+        line = line.split("#")[0].split()
+        if line:
+            z, want = float(line[0]), float(line[1])
+            assert abs(oracle.gelu_erf(z) - want) < 5e-8
+    # identity GELU(z) - GELU(-z) = z
+    for z in (0.3, 1.7, 4.0):
+        assert abs(oracle.gelu_erf(z) - oracle.gelu_erf(-z) - z) < 1e-14
+
+
+def test_c3_bf16_rounding_rne():
+    assert oracle.f64_to_bf16_rne(1.0) == 0x3F80
+    assert oracle.f64_to_bf16_rne(1.0 + 2 ** -8) == 0x3F80          # tie -> even (down)
+    assert oracle.f64_to_bf16_rne(1.0 + 3 * 2 ** -8) == 0x3F82      # tie -> even (up)
+    assert oracle.f64_to_bf16_rne(1.0 + 2 ** -8 + 2 ** -30) == 0x3F81
+    assert oracle.f64_to_bf16_rne(-0.0) == 0x8000
+    assert oracle.f64_to_bf16_rne(float("inf")) == 0x7F80
+    assert oracle.f64_to_bf16_rne(1.9999999) == 0x4000               # carry into the exponent
+    import torch
+    x = (inputgen.gaussian(9, 0, 0, 20000) * np.exp(inputgen.gaussian(9, 0, 1, 20000) * 8)).astype(np.float32)
+    want = torch.from_numpy(x).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    got = np.array([oracle.f64_to_bf16_rne(float(v)) for v in x], np.uint16)
+    assert np.array_equal(got, want)
+    for b in (0x0001, 0x007F, 0x0080, 0x3F80, 0xC020, 0x7F7F):
+        assert oracle.f64_to_bf16_rne(oracle.bf16_to_f64(b)) == b
+
+
+def _c3_check(c_bits, z):
+    want = np.array([oracle.f64_to_bf16_rne(0.5 * v * (1.0 + math.erf(v / math.sqrt(2.0)))) for v in z.ravel()],
+                    np.uint16).reshape(z.shape)
+    assert np.array_equal(c_bits, want)
+
+
+def test_c3_identity_B_and_zero_A():
+    m = n = k = 32
+    a, _, bias = inputgen.config3_job(4, m, n, k)
+    eye = inputgen.f32_to_bf16_bits(np.eye(k, dtype=np.float32)).reshape(k, n)
+    c = oracle.config3(a, eye, bias)
+    _c3_check(c, inputgen.bf16_bits_to_f64(a) + bias.astype(np.float64)[None, :])      # bias indexed by column n
+    zero = np.zeros((m, k), np.uint16)
+    _, b, _ = inputgen.config3_job(5, m, n, k)
+    c = oracle.config3(zero, b, bias)
+    _c3_check(c, np.broadcast_to(bias.astype(np.float64)[None, :], (m, n)))
+
+
+def test_c3_nonsquare_vs_exact_fractions_and_library_matmul():
+    m, n, k = 5, 7, 16
+    a, b, bias = inputgen.config3_job(6, m, n, k)
+    a = a.reshape(-1)[:m * k].reshape(m, k); b = b.reshape(-1)[:k * n].reshape(k, n); bias = bias[:n]
+    ad, bd = inputgen.bf16_bits_to_f64(a), inputgen.bf16_bits_to_f64(b)
+    for i in range(m):
+        for j in range(n):
+            exact = sum(Fraction(float(ad[i, kk])) * Fraction(float(bd[kk, j])) for kk in range(k)) \
+                + Fraction(float(bias[j]))
+            assert abs(oracle.gemm_z_at(a, b, bias, i, j) - float(exact)) <= 1e-15 * max(1.0, abs(float(exact)))
+    m, n, k = 48, 80, 64     # all different: a transposed operand or swapped index cannot pass
+    a, b, bias = inputgen.config3_job(7, m, n, k)
+    # larger-magnitude operands so that A*B, not the bias, dominates z
+    a = inputgen.f32_to_bf16_bits((inputgen.gaussian(3, 70, 0, m * k)).astype(np.float32)).reshape(m, k)
+    b = inputgen.f32_to_bf16_bits((inputgen.gaussian(3, 70, 1, k * n) * 0.2).astype(np.float32)).reshape(k, n)
+    z = inputgen.bf16_bits_to_f64(a) @ inputgen.bf16_bits_to_f64(b) + bias.astype(np.float64)[None, :]
+    c = oracle.config3(a, b, bias)
+    got = inputgen.bf16_bits_to_f64(c)
+    want = 0.5 * z * (1.0 + np.vectorize(math.erf)(z / math.sqrt(2.0)))
+    # equal up to the final bf16 rounding (2^-9 relative) -- and bit-equal wherever the library z is not
+    # within 1e-12 of a rounding boundary
+    assert np.abs(got - want).max() <= 2 ** -8 * np.abs(want).max()
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < 3e-3
+    ms = np.array([0, 47, 13, 5], np.int64); ns = np.array([79, 0, 40, 5], np.int64)
+    assert np.array_equal(oracle.config3_sampled(a, b, bias, ms, ns), c[ms, ns])
+
+
+# =============================================================== config 4: gray -> blur -> hist256
+def test_c4_gray_weights_and_identity():
+    v = np.arange(256, dtype=np.uint8)
+    img = np.stack([v, v, v], axis=-1).reshape(16, 16, 3)
+    assert np.array_equal(oracle.gray_u8(img).ravel(), v)                  # 77+150+29 = 256
+    px = lambda r, g, b: int(oracle.gray_u8(np.array([[[r, g, b]]], np.uint8))[0, 0])
+    assert px(255, 0, 0) == (77 * 255) >> 8 == 76
+    assert px(0, 255, 0) == (150 * 255) >> 8 == 149
+    assert px(0, 0, 255) == (29 * 255) >> 8 == 28
+    assert px(1, 1, 0) == 0 and px(200, 100, 50) == (77 * 200 + 150 * 100 + 29 * 50) >> 8
+
+
+def test_c4_blur_golden_impulse_and_clamp():
+    g = _golden("blur_impulse.txt")
+    img = np.zeros((9, 11), np.uint8); img[4, 5] = 255
+    o = oracle.blur3x3_u8(img)
+    assert o[3:6, 4:7].ravel().tolist() == [int(x) for x in g["interior"][0]]
+    assert int(o.sum()) == sum(int(x) for x in g["interior"][0])
+    img = np.zeros((6, 7), np.uint8); img[0, 0] = 255
+    o = oracle.blur3x3_u8(img)
+    assert [int(o[0, 0]), int(o[0, 1]), int(o[1, 0]), int(o[1, 1])] == [int(x) for x in g["corner"][0]]
+    # constant image stays constant, borders included
+    for val in (0, 1, 17, 255):
+        c = np.full((7, 5), val, np.uint8)
+        assert np.all(oracle.blur3x3_u8(c) == val)
+
+
+def test_c4_blur_bruteforce_and_separable():
+    for (h, w) in ((4, 5), (1, 1), (1, 6), (7, 1), (2, 2)):
+        gimg = oracle.gray_u8(inputgen.config4_job(40 + h * w, (w, h)))
+        o = oracle.blur3x3_u8(gimg)
+        k = [[1, 2, 1], [2, 4, 2], [1, 2, 1]]
+        for y in range(h):
+            for x in range(w):
+                acc = 0
+                for dy in (-1, 0, 1):
+                    for dx in (-1, 0, 1):
+                        yy = min(max(y + dy, 0), h - 1); xx = min(max(x + dx, 0), w - 1)
+                        acc += k[dy + 1][dx + 1] * int(gimg[yy, xx])
+                assert int(o[y, x]) == acc >> 4
+    gimg = oracle.gray_u8(inputgen.config4_job(3, (64, 48)))
+    p = np.pad(gimg.astype(np.int32), 1, mode="edge")                      # library pad + separable passes
+    rows = p[:, :-2] + 2 * p[:, 1:-1] + p[:, 2:]
+    sep = (rows[:-2] + 2 * rows[1:-1] + rows[2:]) >> 4
+    assert np.array_equal(oracle.blur3x3_u8(gimg), sep.astype(np.uint8))
+
+
+def test_c4_chain_layout_and_hist_mass():
+    f = inputgen.config4_job(9, (64, 48))
+    out = oracle.config4(f)
+    assert out.size == 64 * 48 + 1024
+    blur = out[:64 * 48].reshape(48, 64)
+    hist = out[64 * 48:].copy().view(np.uint32)
+    assert int(hist.sum()) == 64 * 48
+    assert np.array_equal(blur, oracle.blur3x3_u8(oracle.gray_u8(f)))
+    assert np.array_equal(hist, np.bincount(blur.ravel(), minlength=256).astype(np.uint32))  # C4-4: of the blur
+    assert np.array_equal(oracle.hist256_u8(np.array([0, 255, 255, 7], np.uint8))[[0, 7, 255]], [1, 1, 2])
+
+
+# =============================================================== the generator is what DESIGN.md says it is
+def test_inputgen_distributions():
+    v = inputgen.config0_job(0)
+    assert v.dtype == np.int32 and v.min() >= 0 and v.max() < 1000 and v.size == 4096
+    assert not np.array_equal(v, inputgen.config0_job(1)) and np.array_equal(v, inputgen.config0_job(0))
+    j = inputgen.config1_job(0)
+    assert j.dtype == np.float32 and j.size == 32768 and j.min() >= -1 and j.max() <= 1 and abs(j.mean()) < 0.02
+    u = inputgen.config2_job(0, 256, 256)
+    assert abs(u.mean()) < 0.02 and abs(u.std() - 1) < 0.02
+    a, b, bias = inputgen.config3_job(0, 64, 64, 64)
+    assert abs(inputgen.bf16_bits_to_f64(a).std() - 0.02) < 2e-3 and abs(bias.std() - 1) < 0.3
+    sizes = [inputgen.config4_size(j) for j in range(300)]
+    assert set(sizes) == set(inputgen.FRAME_SIZES)
+    f = inputgen.config4_job(0, (32, 16))
+    assert f.shape == (16, 32, 3) and f.dtype == np.uint8 and abs(f.mean() - 127.5) < 8
