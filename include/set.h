@@ -1,0 +1,329 @@
+/* set.h -- C ABI of libset: stream-event-triggered (SET) dispatch of CUDA-graph pipelines on one B200.
+ *
+ * Source of the method: arxiv/paper_2606_05495 ("SET: Stream-Event-Triggered Scheduling for Efficient
+ * CUDA Graph Pipelines"), cited below as PAPER.md:<line> (+ section / algorithm).  The four main calls
+ * follow the paper's statement of the problem (§4; §4.2) in the shape
+ * BASELINE.json:north_star names: set_create / set_register_pipeline / set_submit / set_drain.
+ *
+ * A *job* is one pass  H2D copies -> stage kernels -> D2H copies  ("memcpy H2D, kernels,
+ * memcpy D2H"; "Job-as-Graph") over caller-owned host memory.  Jobs are independent.
+ * A *slot* is the paper's worker W_i = (stream S_i, graph executable G_i, device buffers M_i)
+ * (PAPER.md:110); here slot w runs on stream  w mod num_streams  and there are max_inflight slots, so a
+ * stream carries max_inflight/num_streams jobs back to back.
+ *
+ * Conventions
+ *   - Plain C, opaque handle, no exceptions cross the ABI, the library never aborts the process.
+ *   - Every pointer argument says HOST or DEVICE.  No torch / C++ types appear in any signature.
+ *   - Every call returns set_status (0 = SET_OK, negative = error) unless stated otherwise.
+ *   - Errors are sticky: after the first failure every later call on the handle (except
+ *     set_last_error, set_get_stats, set_destroy) returns the same failing status, and set_drain
+ *     still returns (it never hangs on a failed context).
+ *   - Thread safety: set_submit* may be called from several threads at once (Algorithm 1's
+ *     compare-exchange on c_next implies concurrent claimants); all other calls are
+ *     single-caller and must not race with each other.
+ */
+#ifndef SET_H
+#define SET_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct set_ctx set_ctx;
+typedef int32_t set_status;
+
+#define SET_OK            0
+#define SET_ERR_INVALID  (-1) /* bad argument (NULL, out of range, malformed descriptor)          */
+#define SET_ERR_CUDA     (-2) /* a CUDA runtime/driver call failed; text in set_last_error()       */
+#define SET_ERR_NOMEM    (-3) /* host or device allocation failed                                  */
+#define SET_ERR_STATE    (-4) /* call out of order (submit before register, register twice, ...)   */
+#define SET_ERR_SIZE     (-5) /* a per-job size computed from dims exceeds a registered buffer     */
+
+#define SET_MAX_STAGES  16
+#define SET_MAX_BUFFERS  8
+#define SET_MAX_ARGS    12
+#define SET_MAX_DIMS     4
+
+/* ------------------------------------------------------------------------------------------------
+ * Size expressions: the "placeholders" of PAPER.md:102 that vary per job.
+ *   value(dims) = fixed + per_unit * PROD_{i : dim_mask bit i set} dims[i]
+ * dims[0..3] are the four uint32 passed to set_submit_dims (all 1 for set_submit).
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct set_size_expr {
+    uint64_t fixed;
+    uint64_t per_unit;
+    uint32_t dim_mask;
+    uint32_t reserved;
+} set_size_expr;
+
+/* How each grid dimension of a stage is derived: grid = max(1, ceil(value(count) / divisor)). */
+typedef struct set_grid_rule {
+    set_size_expr count;
+    uint32_t divisor; /* >= 1 */
+    uint32_t reserved;
+} set_grid_rule;
+
+/* Kernel argument kinds.  Arguments are passed to the kernel in list order. */
+#define SET_ARG_BUFFER  0 /* DEVICE pointer: slot buffer `index` + value(offset)                   */
+#define SET_ARG_IMM32   1 /* 4-byte immediate (low 32 bits of imm)                                 */
+#define SET_ARG_IMM64   2 /* 8-byte immediate                                                      */
+#define SET_ARG_DIM     3 /* uint32 = dims[index] of the job                                       */
+#define SET_ARG_TMAP2D  4 /* 128-byte CUtensorMap (by value, __grid_constant__) over a 2-D row-major
+                             region of slot buffer `index` starting at value(offset); see tmap     */
+
+#define SET_SWIZZLE_NONE 0
+#define SET_SWIZZLE_128B 3
+
+typedef struct set_tmap2d {
+    uint32_t elem_bytes;   /* 2 (bf16) or 4 (fp32) or 1                                            */
+    uint32_t swizzle;      /* SET_SWIZZLE_*                                                        */
+    uint64_t inner;        /* elements along the contiguous dimension                              */
+    uint64_t outer;        /* rows                                                                 */
+    uint64_t pitch_bytes;  /* byte stride between rows (multiple of 16)                            */
+    uint32_t box_inner;    /* TMA box, elements                                                    */
+    uint32_t box_outer;
+} set_tmap2d;
+
+typedef struct set_arg_desc {
+    int32_t kind;          /* SET_ARG_*                                                            */
+    int32_t index;         /* BUFFER/TMAP2D: buffer index; DIM: dims index                         */
+    set_size_expr offset;  /* BUFFER/TMAP2D: byte offset inside the buffer                         */
+    uint64_t imm;          /* IMM32 / IMM64 payload                                                */
+    set_tmap2d tmap;       /* TMAP2D only                                                          */
+} set_arg_desc;
+
+#define SET_STAGE_PDL 1u   /* connect this stage to the previous one with a programmatic-dependent-
+                              launch edge (the kernel must call griddepcontrol.wait before reading) */
+
+/* One stage = one kernel node of the job graph ("nodes are initialized with the target
+ * function, input arguments, grid and block dimensions").  Stages run in list order. */
+typedef struct set_stage_desc {
+    const void *func;      /* HOST address of the __global__ function's host stub (what
+                              cudaLaunchKernel takes), e.g. from set_builtin_kernel()              */
+    set_grid_rule grid[3];
+    uint32_t block[3];
+    uint32_t smem_bytes;   /* dynamic shared memory                                                */
+    uint32_t flags;        /* SET_STAGE_*                                                          */
+    int32_t num_args;
+    int32_t reserved;
+    set_arg_desc args[SET_MAX_ARGS];
+} set_stage_desc;
+
+#define SET_BUF_ZERO 1u    /* zero [zero_offset, zero_offset+zero_bytes) on the device at the start
+                              of every job (a memset node ahead of the first stage)                */
+
+/* One device buffer of the slot's memory set M_w ("pre-allocated memory slots",
+ * PAPER.md:110 "dedicated set of device-side buffers M_i"), plus at most one H2D and one D2H copy.
+ * All H2D copies precede the first stage, all D2H copies follow the last one. */
+typedef struct set_buffer_desc {
+    uint64_t bytes;             /* device bytes per slot (capacity; per-job sizes must fit)        */
+    uint32_t flags;             /* SET_BUF_*                                                       */
+    uint32_t reserved;
+    set_size_expr h2d_bytes;    /* 0 => no H2D for this buffer                                     */
+    set_size_expr h2d_host_off; /* byte offset in the job's host_in                                */
+    set_size_expr h2d_dev_off;  /* byte offset in this buffer                                      */
+    set_size_expr d2h_bytes;    /* 0 => no D2H for this buffer                                     */
+    set_size_expr d2h_host_off; /* byte offset in the job's host_out                               */
+    set_size_expr d2h_dev_off;
+    set_size_expr zero_off;     /* SET_BUF_ZERO range                                              */
+    set_size_expr zero_bytes;
+} set_buffer_desc;
+
+/* Scheduling models.  SET is the product; the others are the in-run baselines of BASELINE.md §5 /
+ * PAPER.md:224-229 and share buffers, graphs and kernels with it, not the scheduler. */
+#define SET_MODE_SET           0 /* Algorithms 1-3                               */
+#define SET_MODE_PLAIN_STREAMS 1 /* cudaMemcpyAsync + <<<>>> per job on stream j mod S (PAPER.md:226
+                                    synchronous model, spread over the stream pool)                */
+#define SET_MODE_BATCH_SYNC    2 /* static batching: b graphs on fixed streams, host sync after
+                                    every batch                        */
+#define SET_MODE_SINGLE_GRAPH  3 /* graph model: one exec replayed on one stream    */
+#define SET_MODE_MUTEX_QUEUE   4 /* queue model: one global queue behind a mutex, O(b) completion
+                                    queries by the host                */
+
+#define SET_IO_HOST   0 /* host_in / host_out are HOST pointers (pinned: DMA'd in place; pageable:
+                           staged through the library's pinned ring)                               */
+#define SET_IO_DEVICE 1 /* host_in / host_out are DEVICE pointers: the copy nodes become D2D.  Used
+                           to time the path with inputs already resident in HBM.                   */
+
+#define SET_STEAL_SWAP     0 /* a stolen job is re-bound onto an exec already tied to the thief's
+                                M_w (only the host pointers change)                                */
+#define SET_STEAL_RETARGET 1 /* PAPER.md:122 literally: the victim's exec is retargeted to the
+                                thief's buffers (every node updated) and migrates with the job     */
+
+#define SET_CB_NOTIFY_STREAM 0 /* completion: cudaEventRecord on S_w, cudaStreamWaitEvent +
+                                  cudaLaunchHostFunc on a per-stream notify stream                 */
+#define SET_CB_WORK_STREAM   1 /* PAPER.md:203 literally: cudaLaunchHostFunc on S_w itself         */
+
+typedef struct set_config {
+    uint32_t struct_bytes;    /* = sizeof(set_config), for forward compatibility                   */
+    int32_t num_streams;      /* S >= 1                                                            */
+    int32_t max_inflight;     /* b >= 1: launched-but-not-completed jobs             */
+    int32_t mode;             /* SET_MODE_*                                                        */
+    int32_t io;               /* SET_IO_*                                                          */
+    int32_t queue_capacity;   /* q >= 1 prepared jobs per slot queue Q_w; 0 => default (2)         */
+    int32_t num_dispatchers;  /* dispatcher threads; 0 => default (1)                              */
+    int32_t steal_policy;     /* SET_STEAL_*                                                       */
+    int32_t callback_mode;    /* SET_CB_*                                                          */
+    int32_t device;           /* CUDA device ordinal; -1 => current device                         */
+    int32_t spin_us;          /* dispatcher/drain spin time before sleeping; 0 => default (50)     */
+    int32_t reserved0;
+    void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
+                                 torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
+    void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */
+    uint64_t device_arena_bytes;
+} set_config;
+
+typedef struct set_stats {
+    uint64_t submitted;        /* jobs accepted by set_submit*                                     */
+    uint64_t completed;        /* c_done of Algorithm 3                                            */
+    uint64_t launched;         /* graph launches (or per-job launch sequences in baseline modes)   */
+    uint64_t steals;           /* jobs taken from another slot's queue (Alg. 2 l.12-16)            */
+    uint64_t full_rebinds;     /* exec updates that touched every node (device pointers / dims)    */
+    uint64_t host_rebinds;     /* exec updates that touched only the host-pointer copy nodes       */
+    uint64_t staged_jobs;      /* jobs whose pageable buffers went through the pinned ring         */
+    uint64_t submit_stalls;    /* times set_submit had to wait for a free queue entry              */
+    uint64_t dispatcher_sleeps;/* times a dispatcher blocked in the kernel (futex)                 */
+    uint64_t kernel_nodes;     /* kernel launches issued (graph kernel nodes count once per launch)*/
+    uint64_t ns_submit;        /* host ns inside set_submit* (claim + bind + push)                 */
+    uint64_t ns_bind;          /* host ns inside exec parameter updates                            */
+    uint64_t ns_launch;        /* host ns inside launch + event chaining                           */
+    uint64_t ns_callback;      /* host ns inside completion callbacks                              */
+    uint64_t ns_sync;          /* host ns blocked in batch/stream synchronisation (baselines)      */
+    uint64_t max_inflight_seen;/* high-water mark of launched-not-completed jobs                   */
+    uint64_t reserved[4];
+} set_stats;
+
+/* ---------------------------------------------------------------------------------------------- *
+ * A1  set_create -- PAPER.md:116 "Initialization": create the stream pool, b = max_inflight slots,
+ * the free-worker pool W_pool holding every slot id and the per-slot job queues Q_w
+ * (PAPER.md:112); spawn the dispatcher thread(s).  No device memory is allocated yet.
+ *   num_streams, max_inflight : >= 1.  max_inflight is rounded up to a multiple of num_streams.
+ *   out : HOST, receives the handle.  Ownership: caller, release with set_destroy.
+ * Errors: SET_ERR_INVALID, SET_ERR_CUDA (no device), SET_ERR_NOMEM.  *out is NULL on failure.
+ * set_create(S, b, out) == set_create_ex with mode SET, io HOST, defaults elsewhere.
+ */
+set_status set_create(int num_streams, int max_inflight, set_ctx **out);
+set_status set_create_ex(const set_config *cfg, set_ctx **out);
+
+/* A2  set_register_pipeline -- PAPER.md:102 (job-as-graph with placeholders), PAPER.md:104 (memory
+ * slots), PAPER.md:110 (G_i bound only to M_i).  For every slot: allocate the device buffers, build
+ * the DAG  [memset] -> H2D copy nodes -> kernel nodes in list order -> D2H copy nodes  by explicit
+ * construction, instantiate queue_capacity+1 graph executables and bind them to the slot's buffers.
+ *   stages : HOST array[num_stages], 1..SET_MAX_STAGES.  bufs : HOST array[num_bufs], 1..SET_MAX_BUFFERS.
+ *   Descriptors are copied; the caller may free them on return.  Kernel images must stay loaded.
+ * One pipeline per context; a second call returns SET_ERR_STATE.
+ * Errors: SET_ERR_INVALID (malformed descriptor), SET_ERR_NOMEM, SET_ERR_CUDA.
+ */
+set_status set_register_pipeline(set_ctx *ctx, const set_stage_desc *stages, int num_stages,
+                                 const set_buffer_desc *bufs, int num_bufs);
+
+/* A3  set_submit -- Algorithm 1 and PAPER.md:118: claim the job, pick a queue with
+ * a free entry starting at job ticket mod b, update the graph executable's copy nodes to host_in /
+ * host_out (UpdateGraphParams) and push it to Q_i.  Blocks (back-pressure) while every queue is full.
+ *   job_id   : caller's tag, reported back nowhere except stats/tracing; need not be unique.
+ *   host_in  : HOST (or DEVICE under SET_IO_DEVICE), read-only to the library.  Layout = the byte image
+ *              the pipeline's h2d_host_off / h2d_bytes describe.  Must stay valid and unmodified
+ *              until set_drain returns.
+ *   host_out : HOST (or DEVICE), written by DMA.  Contents are defined after set_drain returns SET_OK.
+ *   dims     : HOST array[4] of per-job dimensions for size expressions (set_submit: all 1).
+ * Pinned pointers (set_host_alloc, cudaHostAlloc, torch pin_memory) are DMA'd in place; pageable
+ * pointers are copied through the library's pinned staging ring.
+ * Errors: SET_ERR_STATE (no pipeline), SET_ERR_SIZE (dims overflow a buffer), sticky errors.
+ */
+set_status set_submit(set_ctx *ctx, uint64_t job_id, const void *host_in, void *host_out);
+set_status set_submit_dims(set_ctx *ctx, uint64_t job_id, const void *host_in, void *host_out,
+                           const uint32_t dims[SET_MAX_DIMS]);
+/* n submissions in one call (same semantics as n calls in order).  host_ins/host_outs: HOST arrays of
+ * n pointers; dims: HOST array[n][4] or NULL; job_ids: HOST array[n] or NULL (then first_id + i). */
+set_status set_submit_batch(set_ctx *ctx, int64_t n, uint64_t first_id, const uint64_t *job_ids,
+                            const void *const *host_ins, void *const *host_outs, const uint32_t *dims);
+
+/* A8  set_drain -- implied by the done counter of Algorithm 3: block until every
+ * submitted job has completed (c_done == c_submitted), then surface the sticky error if any.
+ * After SET_OK every host_out is fully written.  The context stays usable for more submissions. */
+set_status set_drain(set_ctx *ctx);
+
+/* Stop the dispatcher(s), drain, free every library-owned resource.  NULL is allowed. */
+set_status set_destroy(set_ctx *ctx);
+
+/* Pinned host memory from the context's allocator (cudaHostAlloc, portable).  Returns HOST pointer or
+ * NULL.  Ownership: caller; release with set_host_free before set_destroy (set_destroy frees leftovers). */
+void *set_host_alloc(set_ctx *ctx, size_t bytes);
+void set_host_free(set_ctx *ctx, void *p);
+
+/* Counters and per-phase host time since create (or since set_reset_stats). out: HOST. */
+set_status set_get_stats(set_ctx *ctx, set_stats *out);
+set_status set_reset_stats(set_ctx *ctx);
+
+/* HOST, NUL-terminated text of the first error on this context ("" if none).  Valid until destroy. */
+const char *set_last_error(set_ctx *ctx);
+
+/* Number of slots b actually created, streams S, execs per slot (q+1). out_*: HOST, may be NULL. */
+set_status set_get_geometry(set_ctx *ctx, int *out_slots, int *out_streams, int *out_execs_per_slot);
+
+/* Time stage `stage` alone: `iters` back-to-back launches on slot 0's buffers and stream, bracketed by
+ * CUDA events on that stream, after `warmup` launches; dims as in set_submit_dims (NULL => all 1).
+ * out_avg_us: HOST, average microseconds per launch.  Requires a drained context. */
+set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int warmup, int iters,
+                          float *out_avg_us);
+
+/* ---------------------------------------------------------------------------------------------- *
+ * Built-in stage kernels (hand-written sm_100a CUDA, csrc/kernels/) and the five pipelines of
+ * BASELINE.json:configs[0..4].  Operation definitions: DESIGN.md §"Stage kernels".
+ */
+#define SET_K_SCAN_I32        1  /* (const int32* in, int32* out, uint32 n)  inclusive prefix sum, 1 block   */
+#define SET_K_HIST_MOD64      2  /* (const int32* in, uint32* hist, uint32 n) 64 bins of v mod 64, 1 block   */
+#define SET_K_AFFINE_F32      3  /* (const float* x, float* y, uint32 n)  y = fl(fl(2.5x)+0.1)               */
+#define SET_K_ADD_BIAS_F32    4  /* (float* y, const float* bias, uint32 n)  y = fl(y + bias)                */
+#define SET_K_RELU_F32        5  /* (float* y, uint32 n)  y = max(y,0)                                       */
+#define SET_K_SQUARE_F32      6  /* (float* y, uint32 n)  y = fl(y*y)                                        */
+#define SET_K_BLOCK_SUM_F32   7  /* (const float* y, float* out, uint32 n)  out[0] = sum, fixed tree, 1 block */
+#define SET_K_JACOBI5_F32     8  /* (const float* u, float* v, uint32 h, uint32 w)  one sweep, zero halo     */
+#define SET_K_GEMM_BIAS_GELU  9  /* (tmapA, tmapB, const float* bias, bf16* C, uint32 M, N, K)  tcgen05      */
+#define SET_K_RGB2GRAY_U8    10  /* (const uint8* rgb, uint8* gray, uint32 w, uint32 h)                      */
+#define SET_K_BLUR3X3_U8     11  /* (const uint8* g, uint8* out, uint32 w, uint32 h)  clamp-to-edge          */
+#define SET_K_HIST256_U8     12  /* (const uint8* p, uint32* hist, uint32 w, uint32 h)  hist must be zeroed  */
+#define SET_K_SPIN           13  /* (uint32* scratch, uint32 ns)  debug delay stage (busy-waits ns)          */
+
+/* HOST address usable as set_stage_desc.func, or NULL for an unknown id. */
+const void *set_builtin_kernel(int kernel_id);
+
+/* Fill stage/buffer descriptors for BASELINE.json:configs[config] (0..4).
+ *   params : HOST array of uint32 or NULL for the BASELINE sizes:
+ *     config 0: {n}            config 1: {n}          config 2: {h, w, sweeps}
+ *     config 3: {M, N, K}      config 4: {max_w, max_h}  (dims per job = {w, h, 1, 1})
+ *   variant: 0 = default.  config 0: 1 = histogram of the INPUT values (reading C0-1 alternative).
+ * *            any config: bit 8 set = append a SET_K_SPIN delay stage that busy-waits dims[3] nanoseconds.
+ *   stages/bufs : HOST arrays with room for SET_MAX_STAGES / SET_MAX_BUFFERS entries.
+ *   host_in_bytes/host_out_bytes : HOST, may be NULL; maximum byte size of a job's host images.
+ */
+set_status set_builtin_pipeline(int config, int variant, const uint32_t *params, int num_params,
+                                set_stage_desc *stages, int *num_stages,
+                                set_buffer_desc *bufs, int *num_bufs,
+                                uint64_t *host_in_bytes, uint64_t *host_out_bytes);
+
+/* ---------------------------------------------------------------------------------------------- *
+ * Host-only self tests of the lock-free structures (no CUDA call is made; usable without a GPU).
+ */
+/* Steal-scan order of Algorithm 2 l.8-17: given b queues whose non-emptiness is the
+ * bit mask `nonempty` (b <= 64), return the queue FindJob(w) takes from: w if non-empty, else the
+ * first (w+k) mod b, k = 1..b-1, that is non-empty, else -1. */
+int set_selftest_find_order(int b, int w, uint64_t nonempty);
+/* Multi-threaded stress of the bounded MPMC ring used for Q_w, W_pool and the exec free lists:
+ * `producers` threads push `items_per_producer` distinct tokens, `consumers` threads pop until all
+ * are seen.  Returns 0 if every token was delivered exactly once, else a negative count of errors. */
+int64_t set_selftest_ring(int capacity, int producers, int consumers, int64_t items_per_producer);
+/* Run Algorithms 1-3 end to end with a simulated device: `completers` host threads stand in for the
+ * CUDA driver's callback thread and finish launched jobs after a pseudo-random delay.  Checks: every
+ * job completes exactly once, never more than b in flight, no slot runs two jobs at once, a stolen
+ * job is bound to the thief's slot.  Returns 0 on success, else a negative error code. */
+int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capacity, int num_dispatchers,
+                               int submitters, int64_t jobs, uint32_t seed, uint64_t *out_steals);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SET_H */

@@ -1,0 +1,28 @@
+// kernels.h -- declarations of the built-in stage kernels (definitions in this folder).
+// Argument lists are documented in include/set.h next to the SET_K_* ids.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+extern "C" {
+__global__ void set_k_scan_i32(const int32_t* in, int32_t* out, uint32_t n);
+__global__ void set_k_hist_mod64(const int32_t* in, uint32_t* hist, uint32_t n);
+__global__ void set_k_affine_f32(const float* x, float* y, uint32_t n);
+__global__ void set_k_add_bias_f32(float* y, const float* bias, uint32_t n);
+__global__ void set_k_relu_f32(float* y, uint32_t n);
+__global__ void set_k_square_f32(float* y, uint32_t n);
+__global__ void set_k_block_sum_f32(const float* y, float* out, uint32_t n);
+__global__ void set_k_jacobi5_f32(const float* u, float* v, uint32_t h, uint32_t w);
+__global__ void set_k_rgb2gray_u8(const uint8_t* rgb, uint8_t* gray, uint32_t w, uint32_t h);
+__global__ void set_k_blur3x3_u8(const uint8_t* g, uint8_t* out, uint32_t w, uint32_t h);
+__global__ void set_k_hist256_u8(const uint8_t* p, uint32_t* hist, uint32_t w, uint32_t h);
+__global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
+}
+
+// Tile shapes the host-side grid rules in set_builtin.cu must agree with.
+constexpr int kJacobiRows = 16;        // rows per block
+constexpr int kJacobiCols = 1024;      // columns per block (256 threads x float4)
+constexpr int kGrayPixPerBlock = 256 * 16;
+constexpr int kBlurTileW = 128, kBlurTileH = 64;
+constexpr int kHistPixPerBlock = 256 * 16 * 4;

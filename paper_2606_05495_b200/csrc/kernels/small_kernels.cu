@@ -1,0 +1,195 @@
+// small_kernels.cu -- stage kernels K1-K7 and K13 (configs 0 and 1; BASELINE.json:configs[0..1]).
+// Hand-written CUDA for sm_100a.  These are latency-class kernels: one job's data (16-128 KB) sits in L2
+// right after its H2D copy, so the design goal is the shortest possible critical path -- one block for the
+// scan / histogram / reduction (no inter-block synchronisation), 128-bit accesses, warp-shuffle scans and
+// reductions, and no FMA contraction anywhere (reading C1-1).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "kernels.h"
+
+namespace {
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += t;
+    }
+    return v;
+}
+
+}  // namespace
+
+// K1: inclusive prefix sum of n int32, one block of 1024 threads.
+// Per 4096-element chunk: 128-bit load -> 4-element serial scan in registers -> warp shuffle scan of the
+// thread totals -> 32 warp totals scanned by warp 0 in shared memory -> carry from the previous chunk.
+extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t* __restrict__ in, int32_t* __restrict__ out,
+                                                                  uint32_t n) {
+    __shared__ int warp_tot[32];
+    __shared__ int chunk_tot;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int carry = 0;
+    for (uint32_t base = 0; base < n; base += 4096) {
+        uint32_t i = base + 4u * tid;
+        int4 v = make_int4(0, 0, 0, 0);
+        if (i + 3 < n) {
+            v = *reinterpret_cast<const int4*>(in + i);
+        } else {
+            if (i < n) v.x = in[i];
+            if (i + 1 < n) v.y = in[i + 1];
+            if (i + 2 < n) v.z = in[i + 2];
+        }
+        v.y += v.x;
+        v.z += v.y;
+        v.w += v.z;
+        int incl = warp_incl_scan(v.w, lane);
+        if (lane == 31) warp_tot[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            int t = warp_tot[lane];
+            int s = warp_incl_scan(t, lane);
+            warp_tot[lane] = s - t;  // exclusive prefix of the warp totals
+            if (lane == 31) chunk_tot = s;
+        }
+        __syncthreads();
+        int off = carry + warp_tot[wid] + (incl - v.w);
+        v.x += off;
+        v.y += off;
+        v.z += off;
+        v.w += off;
+        if (i + 3 < n) {
+            *reinterpret_cast<int4*>(out + i) = v;
+        } else {
+            if (i < n) out[i] = v.x;
+            if (i + 1 < n) out[i + 1] = v.y;
+            if (i + 2 < n) out[i + 2] = v.z;
+        }
+        carry += chunk_tot;
+        __syncthreads();  // warp_tot / chunk_tot are rewritten by the next chunk
+    }
+}
+
+// K2: hist[b] = #{i : v[i] mod 64 == b}, v >= 0 (reading C0-3), one block of 1024 threads.
+// One private 64-bin histogram per warp in shared memory (32 x 64 counters) keeps atomic contention inside a
+// warp; the 32 copies are then summed, one bin per thread.
+extern "C" __global__ void __launch_bounds__(1024) set_k_hist_mod64(const int32_t* __restrict__ in, uint32_t* __restrict__ hist,
+                                                                    uint32_t n) {
+    __shared__ uint32_t h[32][64 + 1];
+    const int tid = threadIdx.x, wid = tid >> 5;
+    for (int k = tid; k < 32 * 65; k += 1024) (&h[0][0])[k] = 0;
+    __syncthreads();
+    const uint32_t n4 = n / 4;
+    for (uint32_t i = tid; i < n4; i += 1024) {
+        int4 v = reinterpret_cast<const int4*>(in)[i];
+        atomicAdd(&h[wid][v.x & 63], 1u);
+        atomicAdd(&h[wid][v.y & 63], 1u);
+        atomicAdd(&h[wid][v.z & 63], 1u);
+        atomicAdd(&h[wid][v.w & 63], 1u);
+    }
+    for (uint32_t i = n4 * 4 + tid; i < n; i += 1024) atomicAdd(&h[wid][in[i] & 63], 1u);
+    __syncthreads();
+    if (tid < 64) {
+        uint32_t s = 0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) s += h[w][tid];
+        hist[tid] = s;
+    }
+}
+
+// K3..K6: one fp32 operation per element per kernel (reading C1-5: the chain stays unfused).  256 threads x 4
+// elements per block; __fmul_rn/__fadd_rn are never contracted into an FMA (reading C1-1).
+extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* __restrict__ x, float* __restrict__ y, uint32_t n) {
+    uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
+    if (i + 3 < n) {
+        float4 v = *reinterpret_cast<const float4*>(x + i);
+        v.x = __fadd_rn(__fmul_rn(2.5f, v.x), 0.1f);
+        v.y = __fadd_rn(__fmul_rn(2.5f, v.y), 0.1f);
+        v.z = __fadd_rn(__fmul_rn(2.5f, v.z), 0.1f);
+        v.w = __fadd_rn(__fmul_rn(2.5f, v.w), 0.1f);
+        *reinterpret_cast<float4*>(y + i) = v;
+    } else {
+        for (; i < n; ++i) y[i] = __fadd_rn(__fmul_rn(2.5f, x[i]), 0.1f);
+    }
+}
+
+extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __restrict__ y, const float* __restrict__ bias, uint32_t n) {
+    uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
+    if (i + 3 < n) {
+        float4 v = *reinterpret_cast<float4*>(y + i);
+        float4 b = *reinterpret_cast<const float4*>(bias + i);
+        v.x = __fadd_rn(v.x, b.x);
+        v.y = __fadd_rn(v.y, b.y);
+        v.z = __fadd_rn(v.z, b.z);
+        v.w = __fadd_rn(v.w, b.w);
+        *reinterpret_cast<float4*>(y + i) = v;
+    } else {
+        for (; i < n; ++i) y[i] = __fadd_rn(y[i], bias[i]);
+    }
+}
+
+extern "C" __global__ void __launch_bounds__(256) set_k_relu_f32(float* __restrict__ y, uint32_t n) {
+    uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
+    if (i + 3 < n) {
+        float4 v = *reinterpret_cast<float4*>(y + i);
+        v.x = v.x > 0.0f ? v.x : 0.0f;
+        v.y = v.y > 0.0f ? v.y : 0.0f;
+        v.z = v.z > 0.0f ? v.z : 0.0f;
+        v.w = v.w > 0.0f ? v.w : 0.0f;
+        *reinterpret_cast<float4*>(y + i) = v;
+    } else {
+        for (; i < n; ++i) y[i] = y[i] > 0.0f ? y[i] : 0.0f;
+    }
+}
+
+extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __restrict__ y, uint32_t n) {
+    uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
+    if (i + 3 < n) {
+        float4 v = *reinterpret_cast<float4*>(y + i);
+        v.x = __fmul_rn(v.x, v.x);
+        v.y = __fmul_rn(v.y, v.y);
+        v.z = __fmul_rn(v.z, v.z);
+        v.w = __fmul_rn(v.w, v.w);
+        *reinterpret_cast<float4*>(y + i) = v;
+    } else {
+        for (; i < n; ++i) y[i] = __fmul_rn(y[i], y[i]);
+    }
+}
+
+// K7: out[0] = sum_i y[i], one block of 1024 threads, fixed-shape tree (deterministic run to run):
+// per thread: pairwise sum inside each float4, sequential over the thread's strided float4s;
+// then xor-shuffle tree inside the warp, then the 32 warp sums by warp 0 (reading C1-2: any fixed tree within
+// the 1e-6 tolerance of the double-accumulated oracle; measured ~1e-8).
+extern "C" __global__ void __launch_bounds__(1024) set_k_block_sum_f32(const float* __restrict__ y, float* __restrict__ out,
+                                                                       uint32_t n) {
+    __shared__ float wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    float acc = 0.0f;
+    const uint32_t n4 = n / 4;
+    for (uint32_t i = tid; i < n4; i += 1024) {
+        float4 v = reinterpret_cast<const float4*>(y)[i];
+        acc = __fadd_rn(acc, __fadd_rn(__fadd_rn(v.x, v.y), __fadd_rn(v.z, v.w)));
+    }
+    for (uint32_t i = n4 * 4 + tid; i < n; i += 1024) acc = __fadd_rn(acc, y[i]);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc = __fadd_rn(acc, __shfl_xor_sync(0xffffffffu, acc, d));
+    if (lane == 0) wsum[wid] = acc;
+    __syncthreads();
+    if (wid == 0) {
+        float s = wsum[lane];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s = __fadd_rn(s, __shfl_xor_sync(0xffffffffu, s, d));
+        if (lane == 0) out[0] = s;
+    }
+}
+
+// K13: debug delay stage (SURVEY.md §5 fault injection): one thread busy-waits `ns` nanoseconds so that job
+// completions reorder and slots stay occupied; scratch[0] receives the waited time.
+extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do {
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    } while (t - t0 < (unsigned long long)ns);
+    if (scratch) scratch[0] = (uint32_t)(t - t0);
+}

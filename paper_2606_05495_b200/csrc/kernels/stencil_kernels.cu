@@ -1,0 +1,198 @@
+// stencil_kernels.cu -- K8 (config 2: 5-point Jacobi) and K10-K12 (config 4: gray -> blur -> hist256).
+// Hand-written CUDA for sm_100a.  These are the bandwidth-class stages: 128-bit (or 32-bit for the byte images)
+// coalesced global accesses, vertical register rolling so that every input row is read once per block, and
+// warp shuffles for the horizontal neighbours.  No tensor cores: none of this is a dense contraction.
+#include "kernels.h"
+
+// ------------------------------------------------------------------------------------------------------------
+// K8: one Jacobi sweep  v[i][j] = 0.2f * ((((c + w) + e) + n) + s), zero halo (readings C2-1..C2-3).
+// Block = 256 threads = 1024 columns x kJacobiRows rows.  Each thread owns one float4 column group and walks
+// down the rows keeping (up, mid, down) in registers: each element is loaded once per block plus the two halo
+// rows; left/right neighbours come from the adjacent lane by shuffle, from global memory only at warp edges.
+// The add order is exactly the oracle's, and there is no multiply-add pair, so results are bit-identical.
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+__device__ __forceinline__ float jac(float c, float w, float e, float n, float s) {
+    return __fmul_rn(0.2f, __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(c, w), e), n), s));
+}
+__device__ __forceinline__ float at0(const float* __restrict__ u, uint32_t h, uint32_t w, int64_t i, int64_t j) {
+    return (i < 0 || j < 0 || i >= (int64_t)h || j >= (int64_t)w) ? 0.0f : __ldg(u + i * (int64_t)w + j);
+}
+}  // namespace
+
+extern "C" __global__ void __launch_bounds__(256) set_k_jacobi5_f32(const float* __restrict__ u, float* __restrict__ v, uint32_t h,
+                                                                    uint32_t w) {
+    const uint32_t r0 = blockIdx.y * kJacobiRows;
+    const uint32_t r1 = min(r0 + (uint32_t)kJacobiRows, h);
+    const uint32_t c4 = (blockIdx.x * 256u + threadIdx.x) * 4u;
+    if ((w & 3u) == 0) {
+        const int lane = threadIdx.x & 31;
+        const bool active = c4 < w;
+        const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+        auto row = [&](uint32_t r) -> float4 {
+            return active ? __ldg(reinterpret_cast<const float4*>(u + (size_t)r * w + c4)) : zero;
+        };
+        float4 up = (r0 > 0) ? row(r0 - 1) : zero;
+        float4 mid = (r0 < h) ? row(r0) : zero;
+        for (uint32_t r = r0; r < r1; ++r) {
+            float4 down = (r + 1 < h) ? row(r + 1) : zero;
+            float left = __shfl_up_sync(0xffffffffu, mid.w, 1);
+            float right = __shfl_down_sync(0xffffffffu, mid.x, 1);  // an inactive neighbour holds 0 = the halo
+            if (lane == 0) left = (active && c4 > 0) ? __ldg(u + (size_t)r * w + c4 - 1) : 0.0f;
+            if (lane == 31) right = (active && c4 + 4 < w) ? __ldg(u + (size_t)r * w + c4 + 4) : 0.0f;
+            if (active) {
+                float4 o;
+                o.x = jac(mid.x, left, mid.y, up.x, down.x);
+                o.y = jac(mid.y, mid.x, mid.z, up.y, down.y);
+                o.z = jac(mid.z, mid.y, mid.w, up.z, down.z);
+                o.w = jac(mid.w, mid.z, right, up.w, down.w);
+                *reinterpret_cast<float4*>(v + (size_t)r * w + c4) = o;
+            }
+            up = mid;
+            mid = down;
+        }
+    } else {  // ragged width: rows are not 16-byte aligned, one element at a time
+        for (uint32_t r = r0; r < r1; ++r)
+            for (uint32_t k = 0; k < 4; ++k) {
+                uint32_t c = c4 + k;
+                if (c < w)
+                    v[(size_t)r * w + c] = jac(at0(u, h, w, r, c), at0(u, h, w, r, (int64_t)c - 1), at0(u, h, w, r, c + 1),
+                                               at0(u, h, w, (int64_t)r - 1, c), at0(u, h, w, r + 1, c));
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K10: gray = (77R + 150G + 29B) >> 8 on interleaved RGB (readings C4-1, C4-2).  16 pixels per thread:
+// three 128-bit loads (48 contiguous bytes), one 128-bit store.
+// ------------------------------------------------------------------------------------------------------------
+extern "C" __global__ void __launch_bounds__(256) set_k_rgb2gray_u8(const uint8_t* __restrict__ rgb, uint8_t* __restrict__ gray,
+                                                                    uint32_t w, uint32_t h) {
+    const uint32_t npix = w * h;
+    const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
+    if (p0 + 15 < npix) {
+        union {
+            uint4 v[3];
+            uint8_t b[48];
+        } in;
+        const uint4* src = reinterpret_cast<const uint4*>(rgb + (size_t)p0 * 3);
+        in.v[0] = __ldg(src);
+        in.v[1] = __ldg(src + 1);
+        in.v[2] = __ldg(src + 2);
+        union {
+            uint4 v;
+            uint8_t b[16];
+        } o;
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+            o.b[k] = (uint8_t)((77u * in.b[3 * k] + 150u * in.b[3 * k + 1] + 29u * in.b[3 * k + 2]) >> 8);
+        *reinterpret_cast<uint4*>(gray + p0) = o.v;
+    } else {
+        for (uint32_t p = p0; p < npix && p < p0 + 16; ++p)
+            gray[p] = (uint8_t)((77u * rgb[3 * (size_t)p] + 150u * rgb[3 * (size_t)p + 1] + 29u * rgb[3 * (size_t)p + 2]) >> 8);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K11: 3x3 blur [1 2 1; 2 4 2; 1 2 1] >> 4, clamp-to-edge.  Evaluated separably -- horizontal [1 2 1] sums per
+// row (<= 1020), then vertical [1 2 1] and ONE final >> 4 -- which is exactly the 2-D form in integers.
+// blockDim = (32, 8): a warp covers 128 pixels x 8 rows, 4 pixels per lane as one 32-bit word; the horizontal
+// neighbours come from adjacent lanes by shuffle; the three row sums roll through registers.
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+struct HSum {
+    int s[4];
+};
+__device__ __forceinline__ HSum hrow(const uint8_t* __restrict__ g, uint32_t w, uint32_t r, uint32_t x4, bool active, int lane) {
+    const uint8_t* row = g + (size_t)r * w;
+    uint32_t word = active ? __ldg(reinterpret_cast<const uint32_t*>(row + x4)) : 0u;
+    uint32_t left = __shfl_up_sync(0xffffffffu, word >> 24, 1);
+    uint32_t right = __shfl_down_sync(0xffffffffu, word & 0xffu, 1);
+    if (active) {
+        if (lane == 0) left = (x4 > 0) ? row[x4 - 1] : (word & 0xffu);             // clamp at the left edge
+        if (lane == 31 || x4 + 4 >= w) right = (x4 + 4 < w) ? row[x4 + 4] : (word >> 24);  // clamp at the right edge
+    }
+    int p0 = word & 0xff, p1 = (word >> 8) & 0xff, p2 = (word >> 16) & 0xff, p3 = word >> 24;
+    HSum h;
+    h.s[0] = (int)left + 2 * p0 + p1;
+    h.s[1] = p0 + 2 * p1 + p2;
+    h.s[2] = p1 + 2 * p2 + p3;
+    h.s[3] = p2 + 2 * p3 + (int)right;
+    return h;
+}
+}  // namespace
+
+extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t* __restrict__ g, uint8_t* __restrict__ out, uint32_t w,
+                                                                   uint32_t h) {
+    if ((w & 3u) == 0) {
+        const int lane = threadIdx.x;
+        const uint32_t x4 = (blockIdx.x * 32u + lane) * 4u;
+        const bool active = x4 < w;
+        const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 8u;
+        if (r0 >= h) return;  // warp-uniform
+        const uint32_t r1 = min(r0 + 8u, h);
+        HSum up = hrow(g, w, r0 > 0 ? r0 - 1 : 0, x4, active, lane);
+        HSum mid = hrow(g, w, r0, x4, active, lane);
+        for (uint32_t r = r0; r < r1; ++r) {
+            HSum down = hrow(g, w, min(r + 1, h - 1), x4, active, lane);
+            if (active) {
+                uint32_t o = 0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) o |= (uint32_t)((up.s[k] + 2 * mid.s[k] + down.s[k]) >> 4) << (8 * k);
+                *reinterpret_cast<uint32_t*>(out + (size_t)r * w + x4) = o;
+            }
+            up = mid;
+            mid = down;
+        }
+    } else {  // ragged width: per-pixel 9-tap with explicit clamping
+        const uint32_t x0 = (blockIdx.x * 32u + threadIdx.x) * 4u;
+        const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 8u;
+        for (uint32_t r = r0; r < min(r0 + 8u, h); ++r)
+            for (uint32_t x = x0; x < min(x0 + 4u, w); ++x) {
+                int acc = 0;
+#pragma unroll
+                for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        int yy = min(max((int)r + dy, 0), (int)h - 1), xx = min(max((int)x + dx, 0), (int)w - 1);
+                        acc += (2 - (dy < 0 ? -dy : dy)) * (2 - (dx < 0 ? -dx : dx)) * (int)g[(size_t)yy * w + xx];
+                    }
+                out[(size_t)r * w + x] = (uint8_t)(acc >> 4);
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K12: 256-bin histogram.  Blurred pixels concentrate (sigma ~ 19 levels), so every warp keeps a private
+// histogram in shared memory; the 8 copies are summed and added to the (pre-zeroed) global bins with one
+// atomic per non-empty bin per block.
+// ------------------------------------------------------------------------------------------------------------
+extern "C" __global__ void __launch_bounds__(256) set_k_hist256_u8(const uint8_t* __restrict__ p, uint32_t* __restrict__ hist,
+                                                                   uint32_t w, uint32_t h) {
+    const uint32_t n = w * h;
+    __shared__ uint32_t sh[8][256];
+    const int tid = threadIdx.x, wid = tid >> 5;
+    for (int k = tid; k < 8 * 256; k += 256) (&sh[0][0])[k] = 0;
+    __syncthreads();
+    const uint32_t base = blockIdx.x * (uint32_t)kHistPixPerBlock;
+    const uint32_t end = min(base + (uint32_t)kHistPixPerBlock, n);
+    uint32_t* my = sh[wid];
+    uint32_t i = base + tid * 16u;
+    for (; i + 15 < end; i += 256u * 16u) {
+        uint4 v = __ldg(reinterpret_cast<const uint4*>(p + i));
+        uint32_t wds[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            atomicAdd(&my[wds[k] & 0xff], 1u);
+            atomicAdd(&my[(wds[k] >> 8) & 0xff], 1u);
+            atomicAdd(&my[(wds[k] >> 16) & 0xff], 1u);
+            atomicAdd(&my[wds[k] >> 24], 1u);
+        }
+    }
+    for (uint32_t j = i; j < end && j < i + 16; ++j) atomicAdd(&my[p[j]], 1u);  // ragged tail of this block's range
+    __syncthreads();
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += sh[k][tid];
+    if (s) atomicAdd(&hist[tid], s);
+}

@@ -1,0 +1,372 @@
+// set_core.hpp -- the SET scheduler proper: Algorithms 1-3 of arxiv/paper_2606_05495
+// over an abstract device backend.  Host-side integer/pointer work only; every CUDA call lives in the
+// backend (set_cuda.cpp).  The same core runs against a simulated device in set_selftest.cpp so that the
+// lock-free logic is testable without a GPU.
+//
+// Vocabulary:
+//   slot w      worker W_w = (stream S_{w mod S}, device buffers M_w, execs bound to M_w)
+//   Q_w         per-slot queue of PREPARED jobs (exec already updated for the job)   -- Ring<Prepared>
+//   W_pool      free worker pool: ids of slots with nothing in flight               -- Ring<int>
+//   c_next      next-job counter (Alg. 1), c_done finished-job counter (Alg. 3)
+#pragma once
+#include <atomic>
+#include <cerrno>
+#include <climits>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <thread>
+#include <vector>
+
+#include <linux/futex.h>
+#include <sys/syscall.h>
+#include <time.h>
+#include <unistd.h>
+
+#include "set_ring.hpp"
+
+namespace setrt {
+
+inline uint64_t now_ns() {
+    timespec ts;
+    clock_gettime(CLOCK_MONOTONIC, &ts);
+    return (uint64_t)ts.tv_sec * 1000000000ull + (uint64_t)ts.tv_nsec;
+}
+
+inline void cpu_relax() {
+#if defined(__x86_64__) || defined(__i386__)
+    __builtin_ia32_pause();
+#else
+    asm volatile("" ::: "memory");
+#endif
+}
+
+// Event count: sleepers block in the kernel (futex) only after spinning for spin_ns.
+// notify() costs one atomic increment and, only if somebody sleeps, one syscall -- this is the
+// notify_one() of Algorithm 3 l.3.
+class EventCount {
+  public:
+    uint32_t prepare() const { return epoch_.load(std::memory_order_acquire); }
+    // Wait until the epoch differs from `seen`.  Returns true if the thread went to sleep.
+    bool wait(uint32_t seen, uint64_t spin_ns) {
+        uint64_t t0 = now_ns();
+        for (int i = 0;; ++i) {
+            if (epoch_.load(std::memory_order_acquire) != seen) return false;
+            cpu_relax();
+            if ((i & 63) == 63 && now_ns() - t0 >= spin_ns) break;
+        }
+        sleepers_.fetch_add(1, std::memory_order_seq_cst);
+        bool slept = false;
+        while (epoch_.load(std::memory_order_seq_cst) == seen) {
+            slept = true;
+            syscall(SYS_futex, reinterpret_cast<uint32_t*>(&epoch_), FUTEX_WAIT_PRIVATE, seen, nullptr, nullptr, 0);
+        }
+        sleepers_.fetch_sub(1, std::memory_order_seq_cst);
+        return slept;
+    }
+    void notify_all() {
+        epoch_.fetch_add(1, std::memory_order_seq_cst);
+        if (sleepers_.load(std::memory_order_seq_cst) > 0)
+            syscall(SYS_futex, reinterpret_cast<uint32_t*>(&epoch_), FUTEX_WAKE_PRIVATE, INT_MAX, nullptr, nullptr, 0);
+    }
+
+  private:
+    alignas(kCacheLine) std::atomic<uint32_t> epoch_{0};
+    alignas(kCacheLine) std::atomic<uint32_t> sleepers_{0};
+};
+static_assert(sizeof(std::atomic<uint32_t>) == 4, "futex word");
+
+struct JobDesc {
+    uint64_t id = 0;
+    const void* in = nullptr;
+    void* out = nullptr;
+    uint32_t dims[4] = {1, 1, 1, 1};
+};
+
+// Queue entry: a fully prepared graph executable, not a task index.
+struct Prepared {
+    int32_t exec = -1;  // global exec index; its free list is that of slot exec / execs_per_slot
+    int32_t home = -1;  // slot whose memory M_home the exec is bound to
+    JobDesc job;
+};
+
+// Device side of the scheduler.  bind = UpdateGraphParams (Alg. 1 l.4, Alg. 2 l.20); launch = GraphLaunch +
+// AddCallback (Alg. 2 l.21-22).  launch() must arrange for Scheduler::on_complete(slot) to be called exactly
+// once, from any thread, when the job's last operation has finished.
+class Backend {
+  public:
+    virtual ~Backend() = default;
+    // Returns 0 or a negative set_status.  `pinned_to_exec`: true if the job's data now lives in storage tied
+    // to this exec (pageable staging), so a thief must retarget this very exec instead of swapping.
+    virtual int bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) = 0;
+    virtual int launch(int exec, int slot, const JobDesc& job) = 0;
+    // Called on the completing thread before the slot is released (e.g. staged D2H -> caller memory).
+    virtual void finish(int exec, int slot, const JobDesc& job) = 0;
+};
+
+struct CoreStats {
+    std::atomic<uint64_t> submitted{0}, completed{0}, launched{0}, steals{0}, submit_stalls{0},
+        dispatcher_sleeps{0}, ns_submit{0}, ns_launch{0}, ns_callback{0}, max_inflight{0};
+};
+
+class Scheduler {
+  public:
+    enum StealPolicy { kSwap = 0, kRetarget = 1 };
+
+    Scheduler(Backend* be, int num_streams, int slots, int queue_capacity, int num_dispatchers, int steal_policy,
+              int spin_us)
+        : be_(be),
+          S_(num_streams),
+          b_(slots),
+          q_(queue_capacity),
+          epp_(queue_capacity + 1),
+          steal_policy_(steal_policy),
+          spin_ns_((uint64_t)spin_us * 1000ull) {
+        queues_.reset(new PaddedRing<Prepared>[b_]);
+        free_execs_.reset(new PaddedRing<int>[b_]);
+        running_.reset(new Running[b_]);
+        for (int w = 0; w < b_; ++w) {
+            queues_[w].r.init((size_t)epp_ + 1);
+            free_execs_[w].r.init((size_t)epp_ * 2);  // room for migrated execs under kRetarget
+            for (int k = 0; k < epp_; ++k) free_execs_[w].r.try_push(w * epp_ + k);
+        }
+        pool_.init((size_t)b_ + 1);
+        // the main thread initialises all workers; all of them start idle.
+        for (int w = 0; w < b_; ++w) pool_.try_push(w);
+        n_free_.store(b_, std::memory_order_relaxed);
+        for (int d = 0; d < num_dispatchers; ++d) dispatchers_.emplace_back([this] { dispatcher_loop(); });
+    }
+
+    ~Scheduler() { stop(); }
+
+    void stop() {
+        bool expected = false;
+        if (!stop_.compare_exchange_strong(expected, true)) return;
+        work_ec_.notify_all();
+        for (auto& t : dispatchers_) t.join();
+        dispatchers_.clear();
+    }
+
+    int slots() const { return b_; }
+    int execs_per_slot() const { return epp_; }
+    CoreStats& stats() { return stats_; }
+    int error() const { return err_.load(std::memory_order_acquire); }
+    void set_error(int e) {
+        int zero = 0;
+        err_.compare_exchange_strong(zero, e);
+        done_ec_.notify_all();
+        space_ec_.notify_all();
+    }
+
+    // ---- Algorithm 1: job submitter --------------------------------------
+    // The paper's submitter claims job indices from a shared array with compare_exchange(c_next, id, id+1);
+    // here the caller hands the job over, so the claim degenerates to a fetch_add that yields the ticket used
+    // to pick the first queue to look at ("monitors all queues for available slots").
+    int submit(JobDesc job) {
+        uint64_t t0 = now_ns();
+        if (int e = error()) return e;
+        uint64_t ticket = c_next_.fetch_add(1, std::memory_order_relaxed);
+        int start = (int)(ticket % (uint64_t)b_);
+        int exec = -1, slot = -1;
+        for (;;) {
+            uint32_t seen = space_ec_.prepare();
+            for (int k = 0; k < b_; ++k) {  // "Q_i not full" == slot i still has an unused exec
+                int i = start + k;
+                if (i >= b_) i -= b_;
+                if (free_execs_[i].r.try_pop(exec)) {
+                    slot = i;
+                    break;
+                }
+            }
+            if (slot >= 0) break;
+            if (int e = error()) return e;
+            stats_.submit_stalls.fetch_add(1, std::memory_order_relaxed);
+            space_ec_.wait(seen, spin_ns_);
+        }
+        Prepared p;
+        p.exec = exec;
+        p.home = slot;
+        p.job = job;
+        bool pinned = false;
+        int rc = be_->bind(exec, slot, p.job, &pinned);  // UpdateGraphParams(J_id, i)
+        if (rc != 0) {
+            free_execs_[slot].r.try_push(exec);
+            space_ec_.notify_all();
+            if (rc != -5 /*SET_ERR_SIZE is per job, not sticky*/) set_error(rc);
+            return rc;
+        }
+        if (pinned) p.home |= kPinnedBit;
+        stats_.submitted.fetch_add(1, std::memory_order_relaxed);
+        c_submitted_.fetch_add(1, std::memory_order_release);
+        queues_[slot].r.try_push(p);  // cannot fail: entries are bounded by the slot's exec count
+        n_queued_.fetch_add(1, std::memory_order_seq_cst);
+        work_ec_.notify_all();
+        stats_.ns_submit.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+        return 0;
+    }
+
+    // ---- Algorithm 3: asynchronous resource return ------------------------
+    // Runs on the CUDA driver's callback thread (or a simulated completer).  No CUDA call in here.
+    void on_complete(int w) {
+        uint64_t t0 = now_ns();
+        Running& r = running_[w];
+        be_->finish(r.exec, w, r.job);
+        int exec = r.exec;
+        r.exec = -1;
+        inflight_.fetch_sub(1, std::memory_order_relaxed);
+        free_execs_[exec / epp_].r.try_push(exec);  // the exec returns to its home free list
+        space_ec_.notify_all();
+        pool_.try_push(w);  // W_pool.push(w_id)
+        n_free_.fetch_add(1, std::memory_order_seq_cst);
+        work_ec_.notify_all();  // notify_one()
+        stats_.completed.fetch_add(1, std::memory_order_relaxed);
+        uint64_t done = c_done_.fetch_add(1, std::memory_order_acq_rel) + 1;  // c_done.fetch_add(1)
+        if (done == c_submitted_.load(std::memory_order_acquire)) done_ec_.notify_all();
+        stats_.ns_callback.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+    }
+
+    // ---- A8 drain: wait for c_done == c_submitted ----------------------------------------------------------
+    int drain() {
+        uint64_t err_t0 = 0;
+        for (;;) {
+            uint32_t seen = done_ec_.prepare();
+            if (c_done_.load(std::memory_order_acquire) == c_submitted_.load(std::memory_order_acquire)) break;
+            if (error()) {
+                // A failed context may never deliver its callbacks: give in-flight work a bounded grace
+                // period, then return the error instead of hanging (set.h "set_drain still returns").
+                if (n_queued_.load() <= 0 && inflight_.load() <= 0) break;
+                if (err_t0 == 0) err_t0 = now_ns();
+                if (now_ns() - err_t0 > 2000000000ull) break;
+                timespec ts{0, 200000};
+                nanosleep(&ts, nullptr);
+                continue;
+            }
+            done_ec_.wait(seen, spin_ns_);
+        }
+        return error();
+    }
+
+    // FindJob's victim order, exposed for the host-only self test (Alg. 2 l.8-17).
+    static int find_order(int b, int w, uint64_t nonempty) {
+        if (nonempty >> w & 1) return w;
+        for (int k = 1; k < b; ++k) {
+            int v = (w + k) % b;
+            if (nonempty >> v & 1) return v;
+        }
+        return -1;
+    }
+
+  private:
+    static constexpr int32_t kPinnedBit = 1 << 30;
+    template <typename T>
+    struct alignas(kCacheLine) PaddedRing {
+        Ring<T> r;
+    };
+    struct alignas(kCacheLine) Running {
+        int exec = -1;
+        JobDesc job;
+    };
+
+    // ---- Algorithm 2: FindJob -----------------------------------------------------------
+    bool find_job(int w, Prepared& p, bool& stolen) {
+        if (queues_[w].r.try_pop(p)) {  // local queue first: head of Q_w
+            stolen = false;
+            return true;
+        }
+        for (int k = 1; k < b_; ++k) {  // victim_id = (w_id + k) mod b, first job it meets
+            int v = w + k;
+            if (v >= b_) v -= b_;
+            if (queues_[v].r.try_pop(p)) {  // try_steal == try_pop at the head
+                stolen = true;
+                return true;
+            }
+        }
+        return false;
+    }
+
+    // ---- Algorithm 2: LaunchJob -------------------------------------------
+    void launch_job(Prepared p, int w, bool stolen) {
+        uint64_t t0 = now_ns();
+        bool pinned = (p.home & kPinnedBit) != 0;
+        int exec = p.exec;
+        int rc = 0;
+        if (stolen) {
+            stats_.steals.fetch_add(1, std::memory_order_relaxed);
+            int mine = -1;
+            bool dummy = false;
+            if (steal_policy_ == kSwap && !pinned && free_execs_[w].r.try_pop(mine)) {
+                // The thief owns an exec that is already tied to M_w: give the job to it (only the
+                // host-pointer copy nodes change) and hand the victim's exec back at once.
+                rc = be_->bind(mine, w, p.job, &dummy);
+                free_execs_[exec / epp_].r.try_push(exec);
+                space_ec_.notify_all();
+                exec = mine;
+            } else {
+                // JIT update retargets the victim's exec to read W_free's input memory, use
+                // W_free's buffers and write W_free's output memory.
+                rc = be_->bind(exec, w, p.job, &dummy);
+            }
+        }
+        Running& r = running_[w];
+        r.exec = exec;
+        r.job = p.job;
+        uint64_t inflight = inflight_.fetch_add(1, std::memory_order_relaxed) + 1;
+        uint64_t hw = stats_.max_inflight.load(std::memory_order_relaxed);
+        while (inflight > hw && !stats_.max_inflight.compare_exchange_weak(hw, inflight)) {
+        }
+        if (rc == 0) rc = be_->launch(exec, w, p.job);  // GraphLaunch + AddCallback
+        stats_.launched.fetch_add(1, std::memory_order_relaxed);
+        stats_.ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+        if (rc != 0) {  // keep the books balanced so that drain returns; the error is sticky
+            set_error(rc);
+            on_complete(w);
+        }
+    }
+
+    // ---- Algorithm 2: dispatcher main loop ----------------------------------------------
+    void dispatcher_loop() {
+        while (!stop_.load(std::memory_order_acquire)) {
+            uint32_t seen = work_ec_.prepare();
+            // Sleep unless there is both an idle worker and a queued job.
+            if (n_free_.load(std::memory_order_seq_cst) <= 0 || n_queued_.load(std::memory_order_seq_cst) <= 0) {
+                if (stop_.load(std::memory_order_acquire)) break;
+                if (work_ec_.wait(seen, spin_ns_)) stats_.dispatcher_sleeps.fetch_add(1, std::memory_order_relaxed);
+                continue;
+            }
+            int w;
+            if (!pool_.try_pop(w)) continue;  // another dispatcher took it
+            n_free_.fetch_sub(1, std::memory_order_seq_cst);
+            Prepared p;
+            bool stolen = false;
+            if (find_job(w, p, stolen)) {
+                n_queued_.fetch_sub(1, std::memory_order_seq_cst);
+                launch_job(p, w, stolen);
+            } else {  // Alg. 2 l.7: no job -> the worker goes back to the pool
+                pool_.try_push(w);
+                n_free_.fetch_add(1, std::memory_order_seq_cst);
+            }
+        }
+    }
+
+    Backend* be_;
+    const int S_, b_, q_, epp_, steal_policy_;
+    const uint64_t spin_ns_;
+    std::unique_ptr<PaddedRing<Prepared>[]> queues_;
+    std::unique_ptr<PaddedRing<int>[]> free_execs_;
+    std::unique_ptr<Running[]> running_;
+    Ring<int> pool_;
+    alignas(kCacheLine) std::atomic<uint64_t> c_next_{0};
+    alignas(kCacheLine) std::atomic<uint64_t> c_submitted_{0};
+    alignas(kCacheLine) std::atomic<uint64_t> c_done_{0};
+    alignas(kCacheLine) std::atomic<int64_t> n_queued_{0};
+    alignas(kCacheLine) std::atomic<int64_t> n_free_{0};
+    alignas(kCacheLine) std::atomic<int64_t> inflight_{0};
+    EventCount work_ec_, space_ec_, done_ec_;
+    std::atomic<bool> stop_{false};
+    std::atomic<int> err_{0};
+    CoreStats stats_;
+    std::vector<std::thread> dispatchers_;
+};
+
+}  // namespace setrt

@@ -1,0 +1,1012 @@
+// set_cuda.cpp -- CUDA backend and C ABI of libset (include/set.h).
+//
+// Layers L1 (job-as-graph + memory slots) and the CUDA half of L2 (GraphLaunch, AddCallback,
+// UpdateGraphParams of Algorithms 1-2).  The lock-free scheduling logic itself is in
+// set_core.hpp.  Also holds the in-run baseline models of PAPER.md:224-229 (they share buffers, graphs and
+// kernels with SET, not the scheduler).
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <deque>
+#include <memory>
+#include <mutex>
+#include <vector>
+
+#include "../../include/set.h"
+#include "set_core.hpp"
+
+using namespace setrt;
+
+namespace {
+
+inline uint64_t eval(const set_size_expr& e, const uint32_t* dims) {
+    uint64_t prod = 1;
+    for (int i = 0; i < SET_MAX_DIMS; ++i)
+        if (e.dim_mask >> i & 1) prod *= dims[i];
+    return e.fixed + e.per_unit * prod;
+}
+inline bool expr_is_zero(const set_size_expr& e) { return e.fixed == 0 && e.per_unit == 0; }
+
+struct SpinLock {
+    std::atomic_flag f = ATOMIC_FLAG_INIT;
+    void lock() {
+        while (f.test_and_set(std::memory_order_acquire)) cpu_relax();
+    }
+    void unlock() { f.clear(std::memory_order_release); }
+};
+
+struct ArgPack {
+    alignas(64) unsigned char store[SET_MAX_ARGS][128];
+    void* ptrs[SET_MAX_ARGS];
+};
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct SlotMem {
+    void* buf[SET_MAX_BUFFERS] = {};
+    cudaEvent_t done = nullptr;   // event chaining: recorded behind the slot's graph on its work stream
+    cudaEvent_t t0 = nullptr;     // plain-stream baseline / timing helpers
+    bool used = false;
+};
+
+struct ExecState {
+    cudaGraphExec_t exec = nullptr;
+    int bound_slot = -1;
+    const void* in = nullptr;  // what the copy nodes currently point at
+    void* out = nullptr;
+    uint32_t dims[4] = {1, 1, 1, 1};
+    // pageable staging (lazily allocated pinned blocks tied to this exec)
+    void* stage_in = nullptr;
+    void* stage_out = nullptr;
+    bool staged = false;
+    void* user_out = nullptr;
+    uint64_t out_bytes = 0;
+};
+
+struct PinnedRange {
+    uintptr_t lo, hi;
+};
+
+}  // namespace
+
+struct set_ctx final : public Backend {
+    set_config cfg{};
+    int S = 0, b = 0, q = 0, epp = 0, device = 0;
+    std::vector<cudaStream_t> streams, notify;
+    bool own_streams = false;
+    std::unique_ptr<SpinLock[]> stream_locks;
+
+    bool registered = false;
+    std::vector<set_stage_desc> stages;
+    std::vector<set_buffer_desc> bufs;
+    uint64_t in_extent_unit = 0, out_extent_unit = 0;
+
+    std::vector<SlotMem> slots;
+    std::vector<ExecState> execs;
+    std::vector<void*> owned_dev;
+    cudaGraph_t graph = nullptr;
+    std::vector<cudaGraphNode_t> kern_nodes;
+    cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
+    void* ph_in = nullptr;   // placeholder operands the template graph is built with
+    void* ph_out = nullptr;
+
+    std::unique_ptr<Scheduler> sched;
+    struct CbArg {
+        set_ctx* ctx;
+        int slot;
+    };
+    std::vector<CbArg> cbargs;
+
+    // counters owned by the backend
+    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0};
+    std::atomic<uint64_t> base_submitted{0}, base_completed{0}, base_launched{0}, base_ns_submit{0}, base_ns_launch{0};
+
+    // sticky error
+    std::atomic<int> err{0};
+    std::mutex errmu;
+    char errmsg[512] = {0};
+
+    // host allocations and the pinned-range cache
+    std::mutex hostmu;
+    std::vector<std::pair<void*, size_t>> host_allocs;
+    SpinLock range_lock;
+    std::vector<PinnedRange> pinned_ranges;
+
+    PFN_encodeTiled encode_tiled = nullptr;
+
+    // baseline state (single caller thread)
+    std::vector<JobDesc> batch;
+    uint64_t base_ticket = 0;
+    std::mutex mq_mu;                 // SET_MODE_MUTEX_QUEUE: the global issue queue's lock
+    std::deque<JobDesc> mq_queue;
+
+    // ------------------------------------------------------------------ errors
+    int fail(int code, const char* fmt, ...) {
+        int zero = 0;
+        if (err.compare_exchange_strong(zero, code)) {
+            std::lock_guard<std::mutex> g(errmu);
+            va_list ap;
+            va_start(ap, fmt);
+            vsnprintf(errmsg, sizeof(errmsg), fmt, ap);
+            va_end(ap);
+        }
+        if (sched) sched->set_error(code);
+        return code;
+    }
+    int cuda_fail(cudaError_t e, const char* what, int line) {
+        return fail(SET_ERR_CUDA, "%s failed at set_cuda.cpp:%d: %s (%s)", what, line, cudaGetErrorName(e),
+                    cudaGetErrorString(e));
+    }
+
+    void bind_thread() {
+        static thread_local int bound = -1;
+        if (bound != device) {
+            cudaSetDevice(device);
+            bound = device;
+        }
+    }
+
+    // ------------------------------------------------------------------ Backend interface
+    int bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) override;
+    int launch(int exec, int slot, const JobDesc& job) override;
+    void finish(int exec, int slot, const JobDesc& job) override;
+
+    int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid);
+    int check_sizes(const uint32_t* dims);
+    bool is_pinned(const void* p);
+    void add_pinned_range(const void* p, size_t n);
+    int build_graph();
+    int plain_job(int slot, const JobDesc& job);
+    int baseline_submit(const JobDesc& job);
+    int baseline_flush();
+    int baseline_drain();
+};
+
+#define CK(call)                                                         \
+    do {                                                                 \
+        cudaError_t _e = (call);                                         \
+        if (_e != cudaSuccess) return cuda_fail(_e, #call, __LINE__);    \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------------------
+// kernel arguments: placeholders -> concrete values for (slot, dims)
+// ---------------------------------------------------------------------------------------------------------
+int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid) {
+    for (int a = 0; a < st.num_args; ++a) {
+        const set_arg_desc& d = st.args[a];
+        ap.ptrs[a] = ap.store[a];
+        switch (d.kind) {
+            case SET_ARG_BUFFER: {
+                char* p = (char*)slots[slot].buf[d.index] + eval(d.offset, dims);
+                memcpy(ap.store[a], &p, sizeof(p));
+                break;
+            }
+            case SET_ARG_IMM32: {
+                uint32_t v = (uint32_t)d.imm;
+                memcpy(ap.store[a], &v, 4);
+                break;
+            }
+            case SET_ARG_IMM64:
+                memcpy(ap.store[a], &d.imm, 8);
+                break;
+            case SET_ARG_DIM:
+                memcpy(ap.store[a], &dims[d.index], 4);
+                break;
+            case SET_ARG_TMAP2D: {
+                if (!encode_tiled) return fail(SET_ERR_CUDA, "cuTensorMapEncodeTiled entry point unavailable");
+                const set_tmap2d& t = d.tmap;
+                CUtensorMapDataType dt = t.elem_bytes == 2   ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                         : t.elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                                             : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+                cuuint64_t gdim[2] = {t.inner, t.outer};
+                cuuint64_t gstride[1] = {t.pitch_bytes};
+                cuuint32_t box[2] = {t.box_inner, t.box_outer};
+                cuuint32_t estr[2] = {1, 1};
+                CUtensorMapSwizzle sw = t.swizzle == SET_SWIZZLE_128B ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
+                char* base = (char*)slots[slot].buf[d.index] + eval(d.offset, dims);
+                CUresult r = encode_tiled((CUtensorMap*)ap.store[a], dt, 2, base, gdim, gstride, box, estr,
+                                          CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r != CUDA_SUCCESS) return fail(SET_ERR_CUDA, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
+                break;
+            }
+            default:
+                return fail(SET_ERR_INVALID, "unknown argument kind %d", d.kind);
+        }
+    }
+    unsigned g[3];
+    for (int i = 0; i < 3; ++i) {
+        uint64_t c = eval(st.grid[i].count, dims);
+        uint64_t dv = st.grid[i].divisor ? st.grid[i].divisor : 1;
+        uint64_t v = (c + dv - 1) / dv;
+        g[i] = (unsigned)(v ? v : 1);
+    }
+    grid = dim3(g[0], g[1], g[2]);
+    return 0;
+}
+
+int set_ctx::check_sizes(const uint32_t* dims) {
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (eval(bd.h2d_dev_off, dims) + eval(bd.h2d_bytes, dims) > bd.bytes) return SET_ERR_SIZE;
+        if (eval(bd.d2h_dev_off, dims) + eval(bd.d2h_bytes, dims) > bd.bytes) return SET_ERR_SIZE;
+        if ((bd.flags & SET_BUF_ZERO) && eval(bd.zero_off, dims) + eval(bd.zero_bytes, dims) > bd.bytes) return SET_ERR_SIZE;
+    }
+    for (auto& st : stages)
+        for (int a = 0; a < st.num_args; ++a)
+            if ((st.args[a].kind == SET_ARG_BUFFER || st.args[a].kind == SET_ARG_TMAP2D) &&
+                eval(st.args[a].offset, dims) > bufs[st.args[a].index].bytes)
+                return SET_ERR_SIZE;
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// pinned-memory test: known ranges first, one driver query per unknown allocation
+// ---------------------------------------------------------------------------------------------------------
+void set_ctx::add_pinned_range(const void* p, size_t n) {
+    range_lock.lock();
+    pinned_ranges.push_back({(uintptr_t)p, (uintptr_t)p + n});
+    range_lock.unlock();
+}
+
+bool set_ctx::is_pinned(const void* p) {
+    uintptr_t a = (uintptr_t)p;
+    range_lock.lock();
+    for (auto& r : pinned_ranges)
+        if (a >= r.lo && a < r.hi) {
+            range_lock.unlock();
+            return true;
+        }
+    range_lock.unlock();
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    if (at.type != cudaMemoryTypeHost) return false;
+    // remember the whole allocation so that later jobs from the same arena skip the query
+    typedef CUresult (*PFN_getattr)(void*, CUpointer_attribute, CUdeviceptr);
+    static PFN_getattr getattr = [] {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuPointerGetAttribute", &fn, cudaEnableDefault, &qr) != cudaSuccess) fn = nullptr;
+        return (PFN_getattr)fn;
+    }();
+    uintptr_t lo = a, hi = a + 1;
+    if (getattr) {
+        CUdeviceptr start = 0;
+        size_t size = 0;
+        if (getattr(&start, CU_POINTER_ATTRIBUTE_RANGE_START_ADDR, (CUdeviceptr)at.devicePointer) == CUDA_SUCCESS &&
+            getattr(&size, CU_POINTER_ATTRIBUTE_RANGE_SIZE, (CUdeviceptr)at.devicePointer) == CUDA_SUCCESS && size > 0 &&
+            (uintptr_t)at.devicePointer == a) {  // unified addressing: host and device views coincide
+            lo = (uintptr_t)start;
+            hi = lo + size;
+        }
+    }
+    if (hi > lo + 1) add_pinned_range((void*)lo, hi - lo);
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// A2: job-as-graph.  [memset] / H2D roots -> kernel chain -> D2H leaves, built by explicit construction
+// with slot 0's buffers and placeholder host operands; every exec is then re-bound.
+// ---------------------------------------------------------------------------------------------------------
+int set_ctx::build_graph() {
+    const uint32_t unit[4] = {1, 1, 1, 1};
+    cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    CK(cudaGraphCreate(&graph, 0));
+    std::vector<cudaGraphNode_t> roots;
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (bd.flags & SET_BUF_ZERO) {
+            cudaMemsetParams mp{};
+            mp.dst = (char*)slots[0].buf[i] + eval(bd.zero_off, unit);
+            mp.elementSize = 1;
+            mp.width = eval(bd.zero_bytes, unit);
+            mp.height = 1;
+            mp.value = 0;
+            CK(cudaGraphAddMemsetNode(&memset_nodes[i], graph, nullptr, 0, &mp));
+            roots.push_back(memset_nodes[i]);
+        }
+        if (!expr_is_zero(bd.h2d_bytes)) {
+            CK(cudaGraphAddMemcpyNode1D(&h2d_nodes[i], graph, nullptr, 0, (char*)slots[0].buf[i] + eval(bd.h2d_dev_off, unit),
+                                        (char*)ph_in + eval(bd.h2d_host_off, unit), eval(bd.h2d_bytes, unit), kin));
+            roots.push_back(h2d_nodes[i]);
+        }
+    }
+    kern_nodes.resize(stages.size());
+    cudaGraphNode_t prev = nullptr;
+    for (size_t s = 0; s < stages.size(); ++s) {
+        const set_stage_desc& st = stages[s];
+        ArgPack ap;
+        dim3 grid;
+        if (int rc = build_args(st, 0, unit, ap, grid)) return rc;
+        if (st.smem_bytes > 48 * 1024)
+            CK(cudaFuncSetAttribute(st.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st.smem_bytes));
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void*>(st.func);
+        kp.gridDim = grid;
+        kp.blockDim = dim3(st.block[0], st.block[1] ? st.block[1] : 1, st.block[2] ? st.block[2] : 1);
+        kp.sharedMemBytes = st.smem_bytes;
+        kp.kernelParams = ap.ptrs;
+        CK(cudaGraphAddKernelNode(&kern_nodes[s], graph, nullptr, 0, &kp));
+        if (s == 0) {
+            for (auto r : roots) CK(cudaGraphAddDependencies(graph, &r, &kern_nodes[s], 1));
+        } else if (st.flags & SET_STAGE_PDL) {
+            cudaGraphEdgeData ed{};
+            ed.from_port = cudaGraphKernelNodePortProgrammatic;
+            ed.to_port = 0;
+            ed.type = cudaGraphDependencyTypeProgrammatic;
+            CK(cudaGraphAddDependencies_v2(graph, &prev, &kern_nodes[s], &ed, 1));
+        } else {
+            CK(cudaGraphAddDependencies(graph, &prev, &kern_nodes[s], 1));
+        }
+        prev = kern_nodes[s];
+    }
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (!expr_is_zero(bd.d2h_bytes)) {
+            CK(cudaGraphAddMemcpyNode1D(&d2h_nodes[i], graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
+                                        (char*)slots[0].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
+        }
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// UpdateGraphParams(J, i)  (Alg. 1 l.4 / Alg. 2 l.20)
+// Host-pointer copy nodes change for every job; kernel/memset nodes and the device side of the copies change
+// only when the exec moves to another slot's memory or the job's dims differ from the exec's last dims.
+// ---------------------------------------------------------------------------------------------------------
+int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
+    uint64_t t0 = now_ns();
+    bind_thread();
+    ExecState& es = execs[exec];
+    bool dims_changed = memcmp(es.dims, job.dims, sizeof(es.dims)) != 0;
+    bool full = es.bound_slot != slot || dims_changed;
+    if (dims_changed)
+        if (int rc = check_sizes(job.dims)) return rc;
+
+    const void* in = job.in;
+    void* out = job.out;
+    *pinned_to_exec = false;
+    if (cfg.io == SET_IO_HOST && !es.staged /* a retarget keeps the staging it already has */) {
+        bool pin_in = is_pinned(in), pin_out = is_pinned(out);
+        if (!pin_in || !pin_out) {
+            // pageable caller memory: go through this exec's pinned staging blocks (per-stream pinned ring)
+            uint64_t in_bytes = 0, out_bytes = 0;
+            for (auto& bd : bufs) {
+                if (!expr_is_zero(bd.h2d_bytes)) in_bytes = std::max(in_bytes, eval(bd.h2d_host_off, job.dims) + eval(bd.h2d_bytes, job.dims));
+                if (!expr_is_zero(bd.d2h_bytes)) out_bytes = std::max(out_bytes, eval(bd.d2h_host_off, job.dims) + eval(bd.d2h_bytes, job.dims));
+            }
+            uint64_t cap_in = 0, cap_out = 0;  // capacity: the buffers bound every per-job size
+            for (auto& bd : bufs) {
+                if (!expr_is_zero(bd.h2d_bytes)) cap_in += bd.bytes;
+                if (!expr_is_zero(bd.d2h_bytes)) cap_out += bd.bytes;
+            }
+            if (!es.stage_in) {
+                CK(cudaHostAlloc(&es.stage_in, std::max<uint64_t>(cap_in, in_bytes), cudaHostAllocPortable));
+                CK(cudaHostAlloc(&es.stage_out, std::max<uint64_t>(cap_out, out_bytes), cudaHostAllocPortable));
+            }
+            memcpy(es.stage_in, in, in_bytes);
+            es.staged = true;
+            es.user_out = out;
+            es.out_bytes = out_bytes;
+            staged_jobs.fetch_add(1, std::memory_order_relaxed);
+        }
+    }
+    if (es.staged) {
+        in = es.stage_in;
+        out = es.stage_out;
+        *pinned_to_exec = true;
+    }
+
+    cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (full) {
+        for (size_t s = 0; s < stages.size(); ++s) {
+            ArgPack ap;
+            dim3 grid;
+            if (int rc = build_args(stages[s], slot, job.dims, ap, grid)) return rc;
+            cudaKernelNodeParams kp{};
+            kp.func = const_cast<void*>(stages[s].func);
+            kp.gridDim = grid;
+            kp.blockDim = dim3(stages[s].block[0], stages[s].block[1] ? stages[s].block[1] : 1,
+                               stages[s].block[2] ? stages[s].block[2] : 1);
+            kp.sharedMemBytes = stages[s].smem_bytes;
+            kp.kernelParams = ap.ptrs;
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, kern_nodes[s], &kp));
+        }
+        for (size_t i = 0; i < bufs.size(); ++i)
+            if (bufs[i].flags & SET_BUF_ZERO) {
+                cudaMemsetParams mp{};
+                mp.dst = (char*)slots[slot].buf[i] + eval(bufs[i].zero_off, job.dims);
+                mp.elementSize = 1;
+                mp.width = eval(bufs[i].zero_bytes, job.dims);
+                mp.height = 1;
+                CK(cudaGraphExecMemsetNodeSetParams(es.exec, memset_nodes[i], &mp));
+            }
+        full_rebinds.fetch_add(1, std::memory_order_relaxed);
+    } else {
+        host_rebinds.fetch_add(1, std::memory_order_relaxed);
+    }
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (!expr_is_zero(bd.h2d_bytes) && (full || es.in != in))
+            CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
+                                                  (const char*)in + eval(bd.h2d_host_off, job.dims), eval(bd.h2d_bytes, job.dims), kin));
+        if (!expr_is_zero(bd.d2h_bytes) && (full || es.out != out))
+            CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, d2h_nodes[i], (char*)out + eval(bd.d2h_host_off, job.dims),
+                                                  (char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, job.dims), eval(bd.d2h_bytes, job.dims), kout));
+    }
+    es.bound_slot = slot;
+    es.in = in;
+    es.out = out;
+    memcpy(es.dims, job.dims, sizeof(es.dims));
+    ns_bind.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// GraphLaunch + AddCallback (Alg. 2 l.21-22) with event chaining (A6): the completion event is recorded
+// behind the graph on the work stream; a per-stream notify stream waits on it and runs the host function,
+// so the work stream itself never stalls on the host round trip (PAPER.md:203 puts the callback "at the end
+// of the stream"; SET_CB_WORK_STREAM keeps that literal placement for comparison).
+// ---------------------------------------------------------------------------------------------------------
+static void CUDART_CB set_completion_cb(void* arg) {
+    auto* a = static_cast<set_ctx::CbArg*>(arg);
+    a->ctx->sched->on_complete(a->slot);  // Algorithm 3
+}
+
+int set_ctx::launch(int exec, int slot, const JobDesc&) {
+    bind_thread();
+    int s = slot % S;
+    SpinLock& lk = stream_locks[s];
+    lk.lock();
+    cudaError_t e = cudaGraphLaunch(execs[exec].exec, streams[s]);
+    if (e == cudaSuccess) {
+        if (cfg.callback_mode == SET_CB_WORK_STREAM) {
+            e = cudaLaunchHostFunc(streams[s], set_completion_cb, &cbargs[slot]);
+        } else {
+            e = cudaEventRecord(slots[slot].done, streams[s]);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(notify[s], slots[slot].done, 0);
+            if (e == cudaSuccess) e = cudaLaunchHostFunc(notify[s], set_completion_cb, &cbargs[slot]);
+        }
+    }
+    lk.unlock();
+    if (e != cudaSuccess) return cuda_fail(e, "graph launch / event chain", __LINE__);
+    kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+    return 0;
+}
+
+void set_ctx::finish(int exec, int, const JobDesc&) {
+    ExecState& es = execs[exec];
+    if (es.staged) {  // staged D2H: pinned ring -> caller's pageable memory, on the callback thread
+        memcpy(es.user_out, es.stage_out, es.out_bytes);
+        es.staged = false;
+        es.in = nullptr;  // force the next job's copy nodes to be re-pointed
+        es.out = nullptr;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Baseline models.  All run on the caller's thread inside set_submit / set_drain.
+// ---------------------------------------------------------------------------------------------------------
+int set_ctx::plain_job(int slot, const JobDesc& job) {
+    // "Synchronous model": individual copies and kernel launches, no graph
+    int s = slot % S;
+    cudaStream_t st = streams[s];
+    SlotMem& sm = slots[slot];
+    if (sm.used) {  // buffer reuse guarded by event synchronisation
+        uint64_t t0 = now_ns();
+        CK(cudaEventSynchronize(sm.done));
+        ns_sync.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+        base_completed.fetch_add(1, std::memory_order_relaxed);
+    }
+    cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (bd.flags & SET_BUF_ZERO)
+            CK(cudaMemsetAsync((char*)sm.buf[i] + eval(bd.zero_off, job.dims), 0, eval(bd.zero_bytes, job.dims), st));
+        if (!expr_is_zero(bd.h2d_bytes))
+            CK(cudaMemcpyAsync((char*)sm.buf[i] + eval(bd.h2d_dev_off, job.dims), (const char*)job.in + eval(bd.h2d_host_off, job.dims),
+                               eval(bd.h2d_bytes, job.dims), kin, st));
+    }
+    for (auto& sd : stages) {
+        ArgPack ap;
+        dim3 grid;
+        if (int rc = build_args(sd, slot, job.dims, ap, grid)) return rc;
+        CK(cudaLaunchKernel(sd.func, grid, dim3(sd.block[0], sd.block[1] ? sd.block[1] : 1, sd.block[2] ? sd.block[2] : 1),
+                            ap.ptrs, sd.smem_bytes, st));
+    }
+    kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+    for (size_t i = 0; i < bufs.size(); ++i) {
+        const set_buffer_desc& bd = bufs[i];
+        if (!expr_is_zero(bd.d2h_bytes))
+            CK(cudaMemcpyAsync((char*)job.out + eval(bd.d2h_host_off, job.dims), (char*)sm.buf[i] + eval(bd.d2h_dev_off, job.dims),
+                               eval(bd.d2h_bytes, job.dims), kout, st));
+    }
+    CK(cudaEventRecord(sm.done, st));
+    sm.used = true;
+    return 0;
+}
+
+int set_ctx::baseline_flush() {
+    // Static batching: exec i <- job i, fixed stream i mod S, then the host
+    // synchronises with every stream before the next batch may touch the buffers.
+    if (batch.empty()) return 0;
+    uint64_t t0 = now_ns();
+    for (size_t i = 0; i < batch.size(); ++i) {
+        bool dummy;
+        int e = (int)i * epp;
+        if (int rc = bind(e, (int)i, batch[i], &dummy)) return rc;
+        CK(cudaGraphLaunch(execs[e].exec, streams[i % S]));
+    }
+    base_launched.fetch_add(batch.size(), std::memory_order_relaxed);
+    kernel_nodes.fetch_add(stages.size() * batch.size(), std::memory_order_relaxed);
+    uint64_t t1 = now_ns();
+    for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
+    uint64_t t2 = now_ns();
+    for (size_t i = 0; i < batch.size(); ++i) finish((int)i * epp, (int)i, batch[i]);
+    base_completed.fetch_add(batch.size(), std::memory_order_relaxed);
+    base_ns_launch.fetch_add(t1 - t0, std::memory_order_relaxed);
+    ns_sync.fetch_add(t2 - t1, std::memory_order_relaxed);
+    batch.clear();
+    return 0;
+}
+
+int set_ctx::baseline_submit(const JobDesc& job) {
+    uint64_t t0 = now_ns();
+    int rc = 0;
+    bind_thread();
+    if (int r = check_sizes(job.dims)) return r;
+    switch (cfg.mode) {
+        case SET_MODE_PLAIN_STREAMS: {
+            if (cfg.io == SET_IO_HOST && (!is_pinned(job.in) || !is_pinned(job.out)))
+                return fail(SET_ERR_INVALID, "baseline modes need pinned host buffers");
+            int slot = (int)(base_ticket++ % (uint64_t)b);
+            rc = plain_job(slot, job);
+            base_launched.fetch_add(1, std::memory_order_relaxed);
+            break;
+        }
+        case SET_MODE_BATCH_SYNC:
+            batch.push_back(job);
+            if ((int)batch.size() == b) rc = baseline_flush();
+            break;
+        case SET_MODE_SINGLE_GRAPH: {
+            // Graph model: one pre-instantiated exec replayed on one stream; stream order alone
+            // protects the single buffer set.  Updating an exec whose previous launch is still running is
+            // legal in CUDA: the update applies to later launches.
+            bool dummy;
+            JobDesc j = job;
+            rc = bind(0, 0, j, &dummy);
+            if (rc == 0) {
+                cudaError_t e = cudaGraphLaunch(execs[0].exec, streams[0]);
+                if (e != cudaSuccess) rc = cuda_fail(e, "cudaGraphLaunch", __LINE__);
+            }
+            base_launched.fetch_add(1, std::memory_order_relaxed);
+            kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+            break;
+        }
+        default:
+            return fail(SET_ERR_INVALID, "mode %d not implemented", cfg.mode);
+    }
+    if (rc == 0) base_submitted.fetch_add(1, std::memory_order_relaxed);
+    base_ns_submit.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+    return rc;
+}
+
+int set_ctx::baseline_drain() {
+    bind_thread();
+    if (cfg.mode == SET_MODE_BATCH_SYNC)
+        if (int rc = baseline_flush()) return rc;
+    uint64_t t0 = now_ns();
+    for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
+    ns_sync.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+    for (auto& sm : slots) sm.used = false;
+    base_completed.store(base_submitted.load());
+    return err.load();
+}
+
+// =========================================================================================================
+// C ABI
+// =========================================================================================================
+extern "C" {
+
+set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
+    if (!out) return SET_ERR_INVALID;
+    *out = nullptr;
+    if (!cfg_in || cfg_in->struct_bytes != sizeof(set_config)) return SET_ERR_INVALID;
+    set_config cfg = *cfg_in;
+    if (cfg.num_streams < 1 || cfg.max_inflight < 1 || cfg.num_streams > 1024 || cfg.max_inflight > (1 << 16)) return SET_ERR_INVALID;
+    if (cfg.mode < SET_MODE_SET || cfg.mode > SET_MODE_MUTEX_QUEUE) return SET_ERR_INVALID;
+    if (cfg.io != SET_IO_HOST && cfg.io != SET_IO_DEVICE) return SET_ERR_INVALID;
+    if (cfg.queue_capacity < 0 || cfg.queue_capacity > 64 || cfg.num_dispatchers < 0 || cfg.num_dispatchers > 64) return SET_ERR_INVALID;
+    if (cfg.queue_capacity == 0) cfg.queue_capacity = 2;
+    if (cfg.num_dispatchers == 0) cfg.num_dispatchers = 1;
+    if (cfg.spin_us == 0) cfg.spin_us = 50;
+    if (cfg.mode == SET_MODE_SINGLE_GRAPH) {  // one worker, one stream, one exec by definition
+        cfg.num_streams = 1;
+        cfg.max_inflight = 1;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return SET_ERR_CUDA;
+    }
+    int dev = cfg.device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return SET_ERR_CUDA;
+    if (dev >= ndev) return SET_ERR_INVALID;
+    if (cudaSetDevice(dev) != cudaSuccess) return SET_ERR_CUDA;
+
+    set_ctx* c = new (std::nothrow) set_ctx();
+    if (!c) return SET_ERR_NOMEM;
+    c->cfg = cfg;
+    c->device = dev;
+    c->S = cfg.num_streams;
+    c->b = ((cfg.max_inflight + c->S - 1) / c->S) * c->S;
+    c->q = cfg.queue_capacity;
+    c->epp = c->q + 1;
+    c->streams.resize(c->S);
+    c->notify.resize(c->S);
+    c->stream_locks.reset(new SpinLock[c->S]);
+    c->own_streams = cfg.streams == nullptr;
+    bool ok = true;
+    for (int s = 0; s < c->S && ok; ++s) {
+        if (c->own_streams)
+            ok = cudaStreamCreateWithFlags(&c->streams[s], cudaStreamNonBlocking) == cudaSuccess;
+        else
+            c->streams[s] = (cudaStream_t)cfg.streams[s];
+        ok = ok && cudaStreamCreateWithFlags(&c->notify[s], cudaStreamNonBlocking) == cudaSuccess;
+    }
+    c->slots.resize(c->b);
+    c->cbargs.resize(c->b);
+    for (int w = 0; w < c->b && ok; ++w) {
+        ok = cudaEventCreateWithFlags(&c->slots[w].done, cudaEventDisableTiming) == cudaSuccess;
+        c->cbargs[w] = {c, w};
+    }
+    if (!ok) {
+        cudaGetLastError();
+        delete c;
+        return SET_ERR_CUDA;
+    }
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+        c->encode_tiled = (PFN_encodeTiled)fn;
+    else
+        cudaGetLastError();
+    if (cfg.mode == SET_MODE_SET || cfg.mode == SET_MODE_MUTEX_QUEUE)
+        c->sched.reset(new Scheduler(c, c->S, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
+    *out = c;
+    return SET_OK;
+}
+
+set_status set_create(int num_streams, int max_inflight, set_ctx** out) {
+    set_config cfg{};
+    cfg.struct_bytes = sizeof(cfg);
+    cfg.num_streams = num_streams;
+    cfg.max_inflight = max_inflight;
+    cfg.mode = SET_MODE_SET;
+    cfg.io = SET_IO_HOST;
+    cfg.device = -1;
+    return set_create_ex(&cfg, out);
+}
+
+set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int num_stages, const set_buffer_desc* bufs,
+                                 int num_bufs) {
+    if (!c) return SET_ERR_INVALID;
+    if (int e = c->err.load()) return e;
+    if (c->registered) return SET_ERR_STATE;
+    if (!stages || !bufs || num_stages < 1 || num_stages > SET_MAX_STAGES || num_bufs < 1 || num_bufs > SET_MAX_BUFFERS)
+        return SET_ERR_INVALID;
+    const uint32_t unit[4] = {1, 1, 1, 1};
+    for (int s = 0; s < num_stages; ++s) {
+        const set_stage_desc& st = stages[s];
+        if (!st.func || st.num_args < 0 || st.num_args > SET_MAX_ARGS || st.block[0] == 0) return SET_ERR_INVALID;
+        if ((uint64_t)st.block[0] * (st.block[1] ? st.block[1] : 1) * (st.block[2] ? st.block[2] : 1) > 1024) return SET_ERR_INVALID;
+        for (int a = 0; a < st.num_args; ++a) {
+            const set_arg_desc& d = st.args[a];
+            if (d.kind < SET_ARG_BUFFER || d.kind > SET_ARG_TMAP2D) return SET_ERR_INVALID;
+            if ((d.kind == SET_ARG_BUFFER || d.kind == SET_ARG_TMAP2D) && (d.index < 0 || d.index >= num_bufs)) return SET_ERR_INVALID;
+            if (d.kind == SET_ARG_DIM && (d.index < 0 || d.index >= SET_MAX_DIMS)) return SET_ERR_INVALID;
+        }
+    }
+    for (int i = 0; i < num_bufs; ++i) {
+        if (bufs[i].bytes == 0) return SET_ERR_INVALID;
+        if ((bufs[i].flags & SET_BUF_ZERO) && eval(bufs[i].zero_bytes, unit) == 0) return SET_ERR_INVALID;
+    }
+    c->bind_thread();
+    c->stages.assign(stages, stages + num_stages);
+    c->bufs.assign(bufs, bufs + num_bufs);
+    if (c->check_sizes(unit)) return SET_ERR_INVALID;
+
+    // ---- memory slots M_w: b pre-allocated, reusable device buffer sets
+    auto align_up = [](uint64_t v) { return (v + 1023) & ~1023ull; };
+    uint64_t per_slot = 0;
+    for (auto& bd : c->bufs) per_slot += align_up(bd.bytes);
+    char* arena = (char*)c->cfg.device_arena;
+    if (arena) {
+        arena = (char*)align_up((uint64_t)(uintptr_t)arena);
+        uint64_t lost = (uint64_t)(arena - (char*)c->cfg.device_arena);
+        if (c->cfg.device_arena_bytes < lost + per_slot * (uint64_t)c->b)
+            return c->fail(SET_ERR_NOMEM, "device arena too small: need %llu bytes", (unsigned long long)(lost + per_slot * c->b));
+    }
+    for (int w = 0; w < c->b; ++w) {
+        char* base;
+        if (arena) {
+            base = arena + per_slot * (uint64_t)w;
+        } else {
+            void* p = nullptr;
+            cudaError_t e = cudaMalloc(&p, per_slot);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                return c->fail(SET_ERR_NOMEM, "cudaMalloc of %llu bytes for slot %d failed: %s", (unsigned long long)per_slot, w,
+                               cudaGetErrorString(e));
+            }
+            c->owned_dev.push_back(p);
+            base = (char*)p;
+        }
+        uint64_t off = 0;
+        for (size_t i = 0; i < c->bufs.size(); ++i) {
+            c->slots[w].buf[i] = base + off;
+            off += align_up(c->bufs[i].bytes);
+        }
+    }
+    // ---- placeholder operands for the template graph
+    uint64_t pin = 16, pout = 16;
+    for (auto& bd : c->bufs) {
+        pin = std::max(pin, eval(bd.h2d_host_off, unit) + eval(bd.h2d_bytes, unit));
+        pout = std::max(pout, eval(bd.d2h_host_off, unit) + eval(bd.d2h_bytes, unit));
+    }
+    c->in_extent_unit = pin;
+    c->out_extent_unit = pout;
+    if (c->cfg.io == SET_IO_DEVICE) {
+        if (cudaMalloc(&c->ph_in, pin) != cudaSuccess || cudaMalloc(&c->ph_out, pout) != cudaSuccess) {
+            cudaGetLastError();
+            return c->fail(SET_ERR_NOMEM, "placeholder allocation failed");
+        }
+    } else {
+        if (cudaHostAlloc(&c->ph_in, pin, cudaHostAllocPortable) != cudaSuccess ||
+            cudaHostAlloc(&c->ph_out, pout, cudaHostAllocPortable) != cudaSuccess) {
+            cudaGetLastError();
+            return c->fail(SET_ERR_NOMEM, "pinned placeholder allocation failed");
+        }
+    }
+    if (int rc = c->build_graph()) return rc;
+
+    // ---- bounded pool of graph executables: q+1 per slot, each re-bound to its slot's M_w
+    int nexec = (c->cfg.mode == SET_MODE_SET || c->cfg.mode == SET_MODE_MUTEX_QUEUE) ? c->b * c->epp : c->b * c->epp;
+    c->execs.resize(nexec);
+    for (int e = 0; e < nexec; ++e) {
+        bool needed = (c->cfg.mode == SET_MODE_SET || c->cfg.mode == SET_MODE_MUTEX_QUEUE) || (e % c->epp == 0);
+        if (c->cfg.mode == SET_MODE_PLAIN_STREAMS) needed = false;
+        if (!needed) continue;
+        cudaError_t er = cudaGraphInstantiate(&c->execs[e].exec, c->graph, 0);
+        if (er != cudaSuccess) return c->cuda_fail(er, "cudaGraphInstantiate", __LINE__);
+        c->execs[e].bound_slot = 0;  // the template was built on slot 0's buffers
+        c->execs[e].in = c->ph_in;
+        c->execs[e].out = c->ph_out;
+        int slot = e / c->epp;
+        if (slot != 0) {
+            JobDesc j;
+            j.in = c->ph_in;
+            j.out = c->ph_out;
+            bool dummy;
+            // placeholders are pinned (or device) memory, so this never stages
+            if (int rc = c->bind(e, slot, j, &dummy)) return rc;
+        }
+    }
+    c->full_rebinds.store(0);
+    c->host_rebinds.store(0);
+    c->ns_bind.store(0);
+    c->registered = true;
+    return SET_OK;
+}
+
+static set_status submit_one(set_ctx* c, const JobDesc& j) {
+    if (c->cfg.mode == SET_MODE_SET) return c->sched->submit(j);
+    return c->baseline_submit(j);
+}
+
+set_status set_submit_dims(set_ctx* c, uint64_t job_id, const void* host_in, void* host_out, const uint32_t dims[SET_MAX_DIMS]) {
+    if (!c || !host_in || !host_out) return SET_ERR_INVALID;
+    if (int e = c->err.load()) return e;
+    if (!c->registered) return SET_ERR_STATE;
+    JobDesc j;
+    j.id = job_id;
+    j.in = host_in;
+    j.out = host_out;
+    if (dims) memcpy(j.dims, dims, sizeof(j.dims));
+    return submit_one(c, j);
+}
+
+set_status set_submit(set_ctx* c, uint64_t job_id, const void* host_in, void* host_out) {
+    return set_submit_dims(c, job_id, host_in, host_out, nullptr);
+}
+
+set_status set_submit_batch(set_ctx* c, int64_t n, uint64_t first_id, const uint64_t* job_ids, const void* const* host_ins,
+                            void* const* host_outs, const uint32_t* dims) {
+    if (!c || n < 0 || (n > 0 && (!host_ins || !host_outs))) return SET_ERR_INVALID;
+    for (int64_t i = 0; i < n; ++i) {
+        set_status rc = set_submit_dims(c, job_ids ? job_ids[i] : first_id + (uint64_t)i, host_ins[i], host_outs[i],
+                                        dims ? dims + 4 * i : nullptr);
+        if (rc != SET_OK) return rc;
+    }
+    return SET_OK;
+}
+
+set_status set_drain(set_ctx* c) {
+    if (!c) return SET_ERR_INVALID;
+    if (!c->registered) return c->err.load();
+    int rc = c->cfg.mode == SET_MODE_SET ? c->sched->drain() : c->baseline_drain();
+    if (int e = c->err.load()) return e;
+    return rc;
+}
+
+set_status set_destroy(set_ctx* c) {
+    if (!c) return SET_OK;
+    cudaSetDevice(c->device);
+    if (c->registered && c->err.load() == 0) set_drain(c);
+    if (c->sched) c->sched->stop();
+    for (auto s : c->streams) cudaStreamSynchronize(s);
+    for (auto s : c->notify) cudaStreamSynchronize(s);  // host functions have returned after this
+    for (auto& es : c->execs) {
+        if (es.exec) cudaGraphExecDestroy(es.exec);
+        if (es.stage_in) cudaFreeHost(es.stage_in);
+        if (es.stage_out) cudaFreeHost(es.stage_out);
+    }
+    if (c->graph) cudaGraphDestroy(c->graph);
+    for (auto& sm : c->slots) {
+        if (sm.done) cudaEventDestroy(sm.done);
+        if (sm.t0) cudaEventDestroy(sm.t0);
+    }
+    for (auto p : c->owned_dev) cudaFree(p);
+    if (c->ph_in) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_in) : cudaFreeHost(c->ph_in));
+    if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
+    for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
+    for (int s = 0; s < c->S; ++s) {
+        if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
+        if (c->notify[s]) cudaStreamDestroy(c->notify[s]);
+    }
+    cudaGetLastError();
+    c->sched.reset();
+    delete c;
+    return SET_OK;
+}
+
+void* set_host_alloc(set_ctx* c, size_t bytes) {
+    if (!c || bytes == 0) return nullptr;
+    c->bind_thread();
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, bytes, cudaHostAllocPortable) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    {
+        std::lock_guard<std::mutex> g(c->hostmu);
+        c->host_allocs.push_back({p, bytes});
+    }
+    c->add_pinned_range(p, bytes);
+    return p;
+}
+
+void set_host_free(set_ctx* c, void* p) {
+    if (!c || !p) return;
+    std::lock_guard<std::mutex> g(c->hostmu);
+    for (size_t i = 0; i < c->host_allocs.size(); ++i)
+        if (c->host_allocs[i].first == p) {
+            c->range_lock.lock();
+            for (size_t k = 0; k < c->pinned_ranges.size(); ++k)
+                if (c->pinned_ranges[k].lo == (uintptr_t)p) {
+                    c->pinned_ranges.erase(c->pinned_ranges.begin() + (long)k);
+                    break;
+                }
+            c->range_lock.unlock();
+            cudaFreeHost(p);
+            c->host_allocs.erase(c->host_allocs.begin() + (long)i);
+            return;
+        }
+}
+
+set_status set_get_stats(set_ctx* c, set_stats* out) {
+    if (!c || !out) return SET_ERR_INVALID;
+    memset(out, 0, sizeof(*out));
+    if (c->sched && c->cfg.mode == SET_MODE_SET) {
+        CoreStats& st = c->sched->stats();
+        out->submitted = st.submitted.load();
+        out->completed = st.completed.load();
+        out->launched = st.launched.load();
+        out->steals = st.steals.load();
+        out->submit_stalls = st.submit_stalls.load();
+        out->dispatcher_sleeps = st.dispatcher_sleeps.load();
+        out->ns_submit = st.ns_submit.load();
+        out->ns_launch = st.ns_launch.load();
+        out->ns_callback = st.ns_callback.load();
+        out->max_inflight_seen = st.max_inflight.load();
+    } else {
+        out->submitted = c->base_submitted.load();
+        out->completed = c->base_completed.load();
+        out->launched = c->base_launched.load();
+        out->ns_submit = c->base_ns_submit.load();
+        out->ns_launch = c->base_ns_launch.load();
+        out->max_inflight_seen = (uint64_t)c->b;
+    }
+    out->full_rebinds = c->full_rebinds.load();
+    out->host_rebinds = c->host_rebinds.load();
+    out->staged_jobs = c->staged_jobs.load();
+    out->kernel_nodes = c->kernel_nodes.load();
+    out->ns_bind = c->ns_bind.load();
+    out->ns_sync = c->ns_sync.load();
+    return SET_OK;
+}
+
+set_status set_reset_stats(set_ctx* c) {
+    if (!c) return SET_ERR_INVALID;
+    if (c->sched) {
+        CoreStats& st = c->sched->stats();
+        st.submitted = 0; st.completed = 0; st.launched = 0; st.steals = 0; st.submit_stalls = 0; st.dispatcher_sleeps = 0;
+        st.ns_submit = 0; st.ns_launch = 0; st.ns_callback = 0; st.max_inflight = 0;
+    }
+    c->base_submitted = 0; c->base_completed = 0; c->base_launched = 0; c->base_ns_submit = 0; c->base_ns_launch = 0;
+    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
+    return SET_OK;
+}
+
+const char* set_last_error(set_ctx* c) {
+    if (!c) return "";
+    std::lock_guard<std::mutex> g(c->errmu);
+    return c->errmsg;
+}
+
+set_status set_get_geometry(set_ctx* c, int* out_slots, int* out_streams, int* out_execs_per_slot) {
+    if (!c) return SET_ERR_INVALID;
+    if (out_slots) *out_slots = c->b;
+    if (out_streams) *out_streams = c->S;
+    if (out_execs_per_slot) *out_execs_per_slot = c->epp;
+    return SET_OK;
+}
+
+set_status set_time_stage(set_ctx* c, int stage, const uint32_t* dims, int warmup, int iters, float* out_avg_us) {
+    if (!c || !out_avg_us || iters < 1 || warmup < 0) return SET_ERR_INVALID;
+    if (!c->registered) return SET_ERR_STATE;
+    if (stage < 0 || stage >= (int)c->stages.size()) return SET_ERR_INVALID;
+    if (int e = c->err.load()) return e;
+    c->bind_thread();
+    const uint32_t unit[4] = {1, 1, 1, 1};
+    if (!dims) dims = unit;
+    if (c->check_sizes(dims)) return SET_ERR_SIZE;
+    const set_stage_desc& sd = c->stages[stage];
+    ArgPack ap;
+    dim3 grid;
+    if (int rc = c->build_args(sd, 0, dims, ap, grid)) return rc;
+    dim3 block(sd.block[0], sd.block[1] ? sd.block[1] : 1, sd.block[2] ? sd.block[2] : 1);
+    cudaStream_t st = c->streams[0];
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return c->cuda_fail(cudaGetLastError(), "cudaEventCreate", __LINE__);
+    cudaError_t er = cudaSuccess;
+    for (int i = 0; i < warmup && er == cudaSuccess; ++i) er = cudaLaunchKernel(sd.func, grid, block, ap.ptrs, sd.smem_bytes, st);
+    if (er == cudaSuccess) er = cudaEventRecord(e0, st);
+    for (int i = 0; i < iters && er == cudaSuccess; ++i) er = cudaLaunchKernel(sd.func, grid, block, ap.ptrs, sd.smem_bytes, st);
+    if (er == cudaSuccess) er = cudaEventRecord(e1, st);
+    if (er == cudaSuccess) er = cudaEventSynchronize(e1);
+    float ms = 0;
+    if (er == cudaSuccess) er = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (er != cudaSuccess) return c->cuda_fail(er, "set_time_stage", __LINE__);
+    *out_avg_us = ms * 1000.0f / (float)iters;
+    return SET_OK;
+}
+
+}  // extern "C"

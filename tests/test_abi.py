@@ -1,0 +1,100 @@
+"""C-ABI checks that need no GPU: the library loads, exports every symbol include/set.h declares, the ctypes
+structs agree with the C structs, and calls fail cleanly (no abort, no CPU fallback) without a device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "set.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(set_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(libset):
+    lib = libset.load()
+    declared = _declared_symbols()
+    assert len(declared) >= 18
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/set.h but not exported by libset.so"
+    assert sorted(libset.EXPORTS) == declared
+
+
+def test_builtin_descriptors_roundtrip_struct_layout(libset):
+    # if the ctypes mirrors of set_stage_desc / set_buffer_desc were laid out differently from the C structs
+    # these fields would come back as garbage
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(0)
+    assert (ns, nb, hin, hout) == (2, 2, 16384, 16640)
+    assert st[0].block[0] == 1024 and st[0].num_args == 3 and st[0].args[2].kind == libset.ARG_IMM32 and st[0].args[2].imm == 4096
+    assert st[1].args[1].kind == libset.ARG_BUFFER and st[1].args[1].index == 1 and st[1].args[1].offset.fixed == 16384
+    assert bf[0].h2d_bytes.fixed == 16384 and bf[1].d2h_bytes.fixed == 16640 and bf[1].bytes == 16640
+    assert st[0].func == libset.load().set_builtin_kernel(1) and st[0].func
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(1)
+    assert (ns, nb, hin, hout) == (5, 3, 131072, 4) and st[0].grid[0].count.fixed == 16
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(2)
+    assert (ns, nb, hin, hout) == (10, 2, 4096 * 4096 * 4, 4096 * 4096 * 4) and bf[0].d2h_bytes.fixed == hout
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(2, params=[64, 64, 3])
+    assert ns == 3 and bf[1].d2h_bytes.fixed == 64 * 64 * 4 and bf[0].d2h_bytes.fixed == 0      # odd sweep count ends in buffer 1
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(3)
+    assert (ns, nb, hin, hout) == (1, 2, 16785408, 8388608) and st[0].args[0].kind == libset.ARG_TMAP2D
+    assert st[0].args[1].offset.fixed == 8388608 and st[0].args[1].tmap.inner == 2048 and st[0].smem_bytes > 48 * 1024
+    st, ns, bf, nb, hin, hout = libset.builtin_pipeline(4)
+    assert (ns, nb, hin, hout) == (3, 4, 6220800, 2073600 + 1024)
+    assert bf[0].h2d_bytes.per_unit == 3 and bf[0].h2d_bytes.dim_mask == 3 and bf[3].flags == libset.BUF_ZERO
+    assert bf[3].d2h_host_off.per_unit == 1 and st[1].block[0] == 32 and st[1].block[1] == 8
+    st, ns, bf, nb, _, _ = libset.builtin_pipeline(0, variant=libset.VARIANT_SPIN)
+    assert ns == 3 and nb == 3 and st[2].args[1].kind == libset.ARG_DIM and st[2].args[1].index == 3
+    with pytest.raises(libset.SetError):
+        libset.builtin_pipeline(7)
+    assert libset.load().set_builtin_kernel(99) is None
+
+
+def test_struct_sizes_match_header(libset):
+    assert C.sizeof(libset.SizeExpr) == 24 and C.sizeof(libset.GridRule) == 32 and C.sizeof(libset.Tmap2D) == 40
+    assert C.sizeof(libset.ArgDesc) == 8 + 24 + 8 + 40
+    assert C.sizeof(libset.Stats) == 20 * 8
+    assert C.sizeof(libset.Config) == 12 * 4 + 8 + 8 + 8
+
+
+def test_invalid_arguments_are_rejected_without_a_device(libset):
+    lib = libset.load()
+    h = C.c_void_p(None)
+    assert lib.set_create(0, 8, C.byref(h)) == libset.SET_ERR_INVALID and not h
+    assert lib.set_create(4, 0, C.byref(h)) == libset.SET_ERR_INVALID
+    assert lib.set_create(4, 8, None) == libset.SET_ERR_INVALID
+    assert lib.set_submit(None, 0, None, None) == libset.SET_ERR_INVALID
+    assert lib.set_drain(None) == libset.SET_ERR_INVALID
+    assert lib.set_destroy(None) == libset.SET_OK
+    assert lib.set_last_error(None) == b""
+
+
+def test_no_cpu_fallback_without_gpu(libset):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    lib = libset.load()
+    h = C.c_void_p(None)
+    assert lib.set_create(4, 8, C.byref(h)) == libset.SET_ERR_CUDA      # fails loudly, does not fall back
+    assert not h
+    with pytest.raises(libset.SetError):
+        libset.Context(4, 8)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_05495_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cpp", ".cu", ".hpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
+                assert "oracle.h" not in src and "liboracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2606_05495_b200" not in src.replace("imports nothing from\npaper_2606_05495_b200", "") or f in ("__init__.py", "oracle.h")
+            assert not re.search(r"^\s*(import|from)\s+paper_2606_05495_b200", src, flags=re.M), f
+            assert "set.h" not in src and "libset" not in src, f

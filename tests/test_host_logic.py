@@ -1,0 +1,53 @@
+"""Host-side logic of the scheduler, exercised without a GPU through the library's self-test entry points:
+the lock-free ring, FindJob's steal order (Alg. 2 l.8-17) and Algorithms 1-3 end to end
+against a simulated device."""
+import random
+
+import pytest
+
+
+def test_find_order_matches_algorithm2(libset):
+    rng = random.Random(7)
+    for b in (1, 2, 5, 8, 32, 64):
+        for _ in range(200):
+            w = rng.randrange(b)
+            mask = rng.getrandbits(b) if rng.random() < 0.8 else 0
+            # Alg. 2: own queue first, else victim = (w + k) mod b for k = 1..b-1, else NULL
+            want = -1
+            if mask >> w & 1:
+                want = w
+            else:
+                for k in range(1, b):
+                    v = (w + k) % b
+                    if mask >> v & 1:
+                        want = v
+                        break
+            assert libset.selftest_find_order(b, w, mask) == want
+    assert libset.selftest_find_order(8, 3, 0b00000110) == 1      # wraps around: 4..7 empty, then 0 empty, then 1
+    assert libset.selftest_find_order(8, 8, 1) == -2              # w out of range
+
+
+@pytest.mark.parametrize("cap,prod,cons,items", [(2, 1, 1, 20000), (8, 3, 3, 30000), (64, 4, 2, 30000), (4, 2, 6, 10000)])
+def test_ring_delivers_every_token_exactly_once(libset, cap, prod, cons, items):
+    assert libset.selftest_ring(cap, prod, cons, items) == 0
+
+
+@pytest.mark.parametrize("S,b,q,disp,subs,jobs,seed", [
+    (4, 8, 2, 1, 1, 20000, 0),      # config 0/2/3 geometry, swap steals
+    (8, 32, 2, 1, 1, 30000, 1),     # config 1/4 geometry, retarget steals (odd seed)
+    (8, 32, 2, 3, 2, 30000, 2),     # several dispatchers and submitters
+    (1, 1, 1, 1, 1, 2000, 3),       # degenerate: one worker
+    (4, 6, 1, 2, 3, 10000, 5),      # max_inflight not a multiple of the stream count -> rounded up
+    (2, 64, 4, 2, 2, 20000, 4),
+])
+def test_scheduler_algorithms_on_simulated_device(libset, S, b, q, disp, subs, jobs, seed):
+    rc, steals = libset.selftest_scheduler(S, b, q, disp, subs, jobs, seed)
+    assert rc == 0
+    assert steals >= 0
+
+
+def test_scheduler_zero_jobs_and_bad_args(libset):
+    rc, _ = libset.selftest_scheduler(4, 8, 2, 1, 1, 0, 0)
+    assert rc == 0
+    rc, _ = libset.selftest_scheduler(0, 8, 2, 1, 1, 10, 0)
+    assert rc == -1
