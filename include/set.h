@@ -264,8 +264,9 @@ const char *set_last_error(set_ctx *ctx);
 /* Number of slots b actually created, streams S, execs per slot (q+1). out_*: HOST, may be NULL. */
 set_status set_get_geometry(set_ctx *ctx, int *out_slots, int *out_streams, int *out_execs_per_slot);
 
-/* Time stage `stage` alone: `iters` back-to-back launches on slot 0's buffers and stream, bracketed by
- * CUDA events on that stream, after `warmup` launches; dims as in set_submit_dims (NULL => all 1).
+/* Time stage `stage` alone on slot 0's buffers and stream: a graph holding a chain of `iters` launches of the
+ * stage's kernel (no host launch cost between them), run once or more for warm-up (`warmup` > 0) and then once
+ * bracketed by CUDA events on that stream; dims as in set_submit_dims (NULL => all 1).
  * out_avg_us: HOST, average microseconds per launch.  Requires a drained context. */
 set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int warmup, int iters,
                           float *out_avg_us);

@@ -19,6 +19,12 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     return v;
 }
 
+// 128-bit accesses need 16-byte aligned operands; the device image mirrors the host image, so an operand that
+// starts at byte 4n of a buffer (the bias vector of config 1) is only aligned when n is a multiple of 4.
+__device__ __forceinline__ bool aligned16(const void* a, const void* b = nullptr) {
+    return (((uintptr_t)a | (uintptr_t)b) & 15u) == 0;
+}
+
 }  // namespace
 
 // K1: inclusive prefix sum of n int32, one block of 1024 threads.
@@ -101,7 +107,7 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_hist_mod64(const int32_
 // elements per block; __fmul_rn/__fadd_rn are never contracted into an FMA (reading C1-1).
 extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* __restrict__ x, float* __restrict__ y, uint32_t n) {
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
-    if (i + 3 < n) {
+    if (i + 3 < n && aligned16(x, y)) {
         float4 v = *reinterpret_cast<const float4*>(x + i);
         v.x = __fadd_rn(__fmul_rn(2.5f, v.x), 0.1f);
         v.y = __fadd_rn(__fmul_rn(2.5f, v.y), 0.1f);
@@ -109,13 +115,13 @@ extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* 
         v.w = __fadd_rn(__fmul_rn(2.5f, v.w), 0.1f);
         *reinterpret_cast<float4*>(y + i) = v;
     } else {
-        for (; i < n; ++i) y[i] = __fadd_rn(__fmul_rn(2.5f, x[i]), 0.1f);
+        for (uint32_t e = i + 4; i < n && i < e; ++i) y[i] = __fadd_rn(__fmul_rn(2.5f, x[i]), 0.1f);
     }
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __restrict__ y, const float* __restrict__ bias, uint32_t n) {
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
-    if (i + 3 < n) {
+    if (i + 3 < n && aligned16(y, bias)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
         float4 b = *reinterpret_cast<const float4*>(bias + i);
         v.x = __fadd_rn(v.x, b.x);
@@ -124,13 +130,13 @@ extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __re
         v.w = __fadd_rn(v.w, b.w);
         *reinterpret_cast<float4*>(y + i) = v;
     } else {
-        for (; i < n; ++i) y[i] = __fadd_rn(y[i], bias[i]);
+        for (uint32_t e = i + 4; i < n && i < e; ++i) y[i] = __fadd_rn(y[i], bias[i]);
     }
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_relu_f32(float* __restrict__ y, uint32_t n) {
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
-    if (i + 3 < n) {
+    if (i + 3 < n && aligned16(y)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
         v.x = v.x > 0.0f ? v.x : 0.0f;
         v.y = v.y > 0.0f ? v.y : 0.0f;
@@ -138,13 +144,13 @@ extern "C" __global__ void __launch_bounds__(256) set_k_relu_f32(float* __restri
         v.w = v.w > 0.0f ? v.w : 0.0f;
         *reinterpret_cast<float4*>(y + i) = v;
     } else {
-        for (; i < n; ++i) y[i] = y[i] > 0.0f ? y[i] : 0.0f;
+        for (uint32_t e = i + 4; i < n && i < e; ++i) y[i] = y[i] > 0.0f ? y[i] : 0.0f;
     }
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __restrict__ y, uint32_t n) {
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
-    if (i + 3 < n) {
+    if (i + 3 < n && aligned16(y)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
         v.x = __fmul_rn(v.x, v.x);
         v.y = __fmul_rn(v.y, v.y);
@@ -152,7 +158,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __rest
         v.w = __fmul_rn(v.w, v.w);
         *reinterpret_cast<float4*>(y + i) = v;
     } else {
-        for (; i < n; ++i) y[i] = __fmul_rn(y[i], y[i]);
+        for (uint32_t e = i + 4; i < n && i < e; ++i) y[i] = __fmul_rn(y[i], y[i]);
     }
 }
 

@@ -48,8 +48,9 @@ inline void cpu_relax() {
 class EventCount {
   public:
     uint32_t prepare() const { return epoch_.load(std::memory_order_acquire); }
-    // Wait until the epoch differs from `seen`.  Returns true if the thread went to sleep.
-    bool wait(uint32_t seen, uint64_t spin_ns) {
+    // Wait until the epoch differs from `seen` (or, with timeout_ns != 0, until about that much time has passed
+    // in the kernel).  Returns true if the thread went to sleep.  Callers re-check their condition in a loop.
+    bool wait(uint32_t seen, uint64_t spin_ns, uint64_t timeout_ns = 0) {
         uint64_t t0 = now_ns();
         for (int i = 0;; ++i) {
             if (epoch_.load(std::memory_order_acquire) != seen) return false;
@@ -58,9 +59,12 @@ class EventCount {
         }
         sleepers_.fetch_add(1, std::memory_order_seq_cst);
         bool slept = false;
+        timespec ts{(time_t)(timeout_ns / 1000000000ull), (long)(timeout_ns % 1000000000ull)};
         while (epoch_.load(std::memory_order_seq_cst) == seen) {
             slept = true;
-            syscall(SYS_futex, reinterpret_cast<uint32_t*>(&epoch_), FUTEX_WAIT_PRIVATE, seen, nullptr, nullptr, 0);
+            long rc = syscall(SYS_futex, reinterpret_cast<uint32_t*>(&epoch_), FUTEX_WAIT_PRIVATE, seen,
+                              timeout_ns ? &ts : nullptr, nullptr, 0);
+            if (timeout_ns && rc == -1 && errno == ETIMEDOUT) break;
         }
         sleepers_.fetch_sub(1, std::memory_order_seq_cst);
         return slept;
@@ -103,6 +107,10 @@ class Backend {
     virtual int launch(int exec, int slot, const JobDesc& job) = 0;
     // Called on the completing thread before the slot is released (e.g. staged D2H -> caller memory).
     virtual void finish(int exec, int slot, const JobDesc& job) = 0;
+    // Called from a blocked submit/drain every kPollNs: report an asynchronous device failure (a faulting stage
+    // kernel) as a negative set_status.  The driver never runs a host function behind failed work, so without
+    // this check a fault would leave c_done short of c_submitted forever.
+    virtual int poll() { return 0; }
 };
 
 struct CoreStats {
@@ -182,7 +190,8 @@ class Scheduler {
             if (slot >= 0) break;
             if (int e = error()) return e;
             stats_.submit_stalls.fetch_add(1, std::memory_order_relaxed);
-            space_ec_.wait(seen, spin_ns_);
+            if (space_ec_.wait(seen, spin_ns_, kPollNs))
+                if (int e = be_->poll()) set_error(e);
         }
         Prepared p;
         p.exec = exec;
@@ -242,7 +251,8 @@ class Scheduler {
                 nanosleep(&ts, nullptr);
                 continue;
             }
-            done_ec_.wait(seen, spin_ns_);
+            if (done_ec_.wait(seen, spin_ns_, kPollNs))
+                if (int e = be_->poll()) set_error(e);
         }
         return error();
     }
@@ -259,6 +269,7 @@ class Scheduler {
 
   private:
     static constexpr int32_t kPinnedBit = 1 << 30;
+    static constexpr uint64_t kPollNs = 20000000ull;  // 20 ms
     template <typename T>
     struct alignas(kCacheLine) PaddedRing {
         Ring<T> r;

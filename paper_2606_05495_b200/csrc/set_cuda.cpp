@@ -158,6 +158,7 @@ struct set_ctx final : public Backend {
     int bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) override;
     int launch(int exec, int slot, const JobDesc& job) override;
     void finish(int exec, int slot, const JobDesc& job) override;
+    int poll() override;
 
     int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid);
     int check_sizes(const uint32_t* dims);
@@ -485,6 +486,15 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     lk.unlock();
     if (e != cudaSuccess) return cuda_fail(e, "graph launch / event chain", __LINE__);
     kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+    return 0;
+}
+
+int set_ctx::poll() {
+    bind_thread();
+    for (int s = 0; s < S; ++s) {
+        cudaError_t e = cudaStreamQuery(streams[s]);
+        if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(e, "asynchronous failure on a work stream", __LINE__);
+    }
     return 0;
 }
 
@@ -992,18 +1002,39 @@ set_status set_time_stage(set_ctx* c, int stage, const uint32_t* dims, int warmu
     if (int rc = c->build_args(sd, 0, dims, ap, grid)) return rc;
     dim3 block(sd.block[0], sd.block[1] ? sd.block[1] : 1, sd.block[2] ? sd.block[2] : 1);
     cudaStream_t st = c->streams[0];
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return c->cuda_fail(cudaGetLastError(), "cudaEventCreate", __LINE__);
-    cudaError_t er = cudaSuccess;
-    for (int i = 0; i < warmup && er == cudaSuccess; ++i) er = cudaLaunchKernel(sd.func, grid, block, ap.ptrs, sd.smem_bytes, st);
+    if (sd.smem_bytes > 48 * 1024) cudaFuncSetAttribute(sd.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sd.smem_bytes);
+    // A chain of `iters` kernel nodes in one graph: no host launch cost between the kernels, so the average is the
+    // kernel's device time plus the graph's node-to-node hand-off -- what the kernel costs inside a job graph.
+    cudaGraph_t g = nullptr;
+    cudaGraphExec_t ge = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t er = cudaGraphCreate(&g, 0);
+    cudaGraphNode_t prev = nullptr;
+    for (int i = 0; i < iters && er == cudaSuccess; ++i) {
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void*>(sd.func);
+        kp.gridDim = grid;
+        kp.blockDim = block;
+        kp.sharedMemBytes = sd.smem_bytes;
+        kp.kernelParams = ap.ptrs;
+        cudaGraphNode_t node;
+        er = cudaGraphAddKernelNode(&node, g, prev ? &prev : nullptr, prev ? 1 : 0, &kp);
+        prev = node;
+    }
+    if (er == cudaSuccess) er = cudaGraphInstantiate(&ge, g, 0);
+    if (er == cudaSuccess) er = cudaEventCreate(&e0);
+    if (er == cudaSuccess) er = cudaEventCreate(&e1);
+    for (int i = 0; i < (warmup > 0 ? 1 + warmup / iters : 0) && er == cudaSuccess; ++i) er = cudaGraphLaunch(ge, st);
     if (er == cudaSuccess) er = cudaEventRecord(e0, st);
-    for (int i = 0; i < iters && er == cudaSuccess; ++i) er = cudaLaunchKernel(sd.func, grid, block, ap.ptrs, sd.smem_bytes, st);
+    if (er == cudaSuccess) er = cudaGraphLaunch(ge, st);
     if (er == cudaSuccess) er = cudaEventRecord(e1, st);
     if (er == cudaSuccess) er = cudaEventSynchronize(e1);
     float ms = 0;
     if (er == cudaSuccess) er = cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (ge) cudaGraphExecDestroy(ge);
+    if (g) cudaGraphDestroy(g);
     if (er != cudaSuccess) return c->cuda_fail(er, "set_time_stage", __LINE__);
     *out_avg_us = ms * 1000.0f / (float)iters;
     return SET_OK;

@@ -169,8 +169,10 @@ def test_work_stealing_with_jittered_jobs_max_depth(libset, policy):
     """config 4 geometry (8 streams, 32 in flight) with a random-length delay stage: completions reorder, queues
     drain unevenly, idle slots steal.  Every output must still equal F(in) of its own job."""
     from paper_2606_05495_b200.workloads import Workload
+    # jobs 0, 32, 64, ... start in slot 0's queue and hold it for 2 ms each while the other 31 slots run short
+    # jobs and go idle: whatever is still queued behind a long job must be stolen (Alg. 2 l.12-16).
     wl = Workload(4, (1920, 1080), variant=libset.VARIANT_SPIN, jobs=160, num_streams=8, max_inflight=32,
-                  extra={"spin_ns": lambda j: int(inputgen.uniform24(99, j, 0, 1)[0] % 400) * 1000})
+                  extra={"spin_ns": lambda j: 2_000_000 if j % 32 == 0 else int(inputgen.uniform24(99, j, 0, 1)[0] % 400) * 1000})
     st = check(libset, wl, list(range(wl.jobs)), steal_policy=policy, num_dispatchers=2)
     assert st["steals"] > 0
     assert st["max_inflight_seen"] <= 32
