@@ -533,6 +533,14 @@ def main():
         kr = kernel_rooflines(setlib, wl, pk, d if wl.config == 4 else None)
         extra["kernels"] = kr
         if not args.no_baselines:
+            cm = {}
+            for name, cb in (("hostfunc_notify_stream", 1), ("hostfunc_work_stream", 2)):
+                p_, r_ = LAYOUT[wl.config]
+                r = run_arm(setlib, wl, ids, "set", False, steps, warmup, p_, r_, verify=2, ctx_kw={"callback_mode": cb}, flush=flush)
+                log(f"[bench]   {wl.config} set/{name:24s} host   {r['jobs_per_s']:12.1f} jobs/s  host us/job {r['host_us_per_job']}")
+                cm[name + "_e2e"] = {"jobs_per_s": round(r["jobs_per_s"], 1), "ms_per_step": round(r["ms_per_step"], 3),
+                                     "host_us_per_job": r["host_us_per_job"], "mismatches": r["mismatches"]}
+            extra["completion_modes"] = dict(cm, flag_poll_e2e={"jobs_per_s": round(e2e_value, 1)})
             base = {}
             for mode in ("batch_sync_graphs", "plain_streams", "single_graph"):
                 for io_device in (False, True):
@@ -592,7 +600,7 @@ def main():
                 "clocks": clocks,
                 "e2e": {"value": round(e2e_value, 1), "unit": "jobs/s", "h2d_bytes_per_step": int(e2e_arm["h2d_bytes"] * world),
                         "d2h_bytes_per_step": int(e2e_arm["d2h_bytes"] * world), "ms_per_step": round(ms_e2e, 4)},
-                "gpu_launches": int(dev_arm["kernel_launches"] * world),
+                "gpu_launches": int((dev_arm["kernel_launches"] + dev_arm["stats"]["signal_nodes"]) * world),
                 "mismatches": dev_arm["mismatches"] + e2e_arm["mismatches"],
                 "host_us_per_job": {"device": dev_arm["host_us_per_job"], "e2e": e2e_arm["host_us_per_job"]},
                 "sched_stats": {k: e2e_arm["stats"][k] for k in ("steals", "submit_stalls", "dispatcher_sleeps", "max_inflight_seen",

@@ -23,7 +23,7 @@ SET_MAX_STAGES, SET_MAX_BUFFERS, SET_MAX_ARGS, SET_MAX_DIMS = 16, 8, 12, 4
 MODE_SET, MODE_PLAIN_STREAMS, MODE_BATCH_SYNC, MODE_SINGLE_GRAPH, MODE_MUTEX_QUEUE = 0, 1, 2, 3, 4
 IO_HOST, IO_DEVICE = 0, 1
 STEAL_SWAP, STEAL_RETARGET = 0, 1
-CB_NOTIFY_STREAM, CB_WORK_STREAM = 0, 1
+CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL = 0, 1, 2, 3
 ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D = 0, 1, 2, 3, 4
 STAGE_PDL = 1
 BUF_ZERO = 1
@@ -78,7 +78,7 @@ class Stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in
                 ("submitted", "completed", "launched", "steals", "full_rebinds", "host_rebinds", "staged_jobs", "submit_stalls",
                  "dispatcher_sleeps", "kernel_nodes", "ns_submit", "ns_bind", "ns_launch", "ns_callback", "ns_sync",
-                 "max_inflight_seen")] + [("reserved", C.c_uint64 * 4)]
+                 "max_inflight_seen", "signal_nodes")] + [("reserved", C.c_uint64 * 3)]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if n != "reserved"}
@@ -157,7 +157,7 @@ class Context:
     """Owner of one set_ctx handle.  All pointers are plain integer addresses."""
 
     def __init__(self, num_streams: int, max_inflight: int, mode: int = MODE_SET, io: int = IO_HOST, queue_capacity: int = 0,
-                 num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_NOTIFY_STREAM,
+                 num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_DEFAULT,
                  device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0):
         self._lib = load()
         self._h = C.c_void_p(None)

@@ -199,3 +199,11 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
     } while (t - t0 < (unsigned long long)ns);
     if (scratch) scratch[0] = (uint32_t)(t - t0);
 }
+
+// K14: completion signal of SET_CB_FLAG_POLL.  Last node of the job graph (it depends on every D2H copy node, so
+// the job's output is already in host memory): one thread stores 1 to the slot's word in mapped pinned host
+// memory, which the dispatcher thread is watching.  The fence orders the store after everything this GPU wrote.
+extern "C" __global__ void set_k_signal(uint32_t* flag) {
+    __threadfence_system();
+    *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+}

@@ -90,6 +90,7 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_BLUR3X3_U8: return (const void*)set_k_blur3x3_u8;
         case SET_K_HIST256_U8: return (const void*)set_k_hist256_u8;
         case SET_K_SPIN: return (const void*)set_k_spin;
+        case SET_K_SIGNAL: return (const void*)set_k_signal;
         default: return nullptr;
     }
 }

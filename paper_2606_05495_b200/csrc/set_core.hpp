@@ -111,7 +111,13 @@ class Backend {
     // kernel) as a negative set_status.  The driver never runs a host function behind failed work, so without
     // this check a fault would leave c_done short of c_submitted forever.
     virtual int poll() { return 0; }
+    // Flag-polled completion (SET_CB_FLAG_POLL): non-null => the last node of every job graph stores a non-zero
+    // word to done_flags()[slot * kFlagStride] (pinned host memory the GPU writes directly); no host function is
+    // enqueued, the dispatcher itself watches the words and runs Algorithm 3.  The core clears the word before launch().
+    virtual volatile uint32_t* done_flags() { return nullptr; }
 };
+
+constexpr int kFlagStride = 16;  // one 64-byte line per slot: the GPU's write invalidates only that slot's line
 
 struct CoreStats {
     std::atomic<uint64_t> submitted{0}, completed{0}, launched{0}, steals{0}, submit_stalls{0},
@@ -134,6 +140,7 @@ class Scheduler {
         queues_.reset(new PaddedRing<Prepared>[b_]);
         free_execs_.reset(new PaddedRing<int>[b_]);
         running_.reset(new Running[b_]);
+        flags_ = be_->done_flags();
         for (int w = 0; w < b_; ++w) {
             queues_[w].r.init((size_t)epp_ + 1);
             free_execs_[w].r.init((size_t)epp_ * 2);  // room for migrated execs under kRetarget
@@ -223,7 +230,8 @@ class Scheduler {
         be_->finish(r.exec, w, r.job);
         int exec = r.exec;
         r.exec = -1;
-        inflight_.fetch_sub(1, std::memory_order_relaxed);
+        r.state.store(0, std::memory_order_release);
+        inflight_.fetch_sub(1, std::memory_order_seq_cst);
         free_execs_[exec / epp_].r.try_push(exec);  // the exec returns to its home free list
         space_ec_.notify_all();
         pool_.try_push(w);  // W_pool.push(w_id)
@@ -276,8 +284,24 @@ class Scheduler {
     };
     struct alignas(kCacheLine) Running {
         int exec = -1;
+        std::atomic<int> state{0};  // 0 idle, 1 in flight, 2 completion claimed by a polling dispatcher
         JobDesc job;
     };
+
+    // Flag-polled completion: scan the in-flight slots' words; whoever wins the 1 -> 2 claim runs Algorithm 3.
+    bool poll_flags() {
+        bool any = false;
+        for (int w = 0; w < b_; ++w) {
+            Running& r = running_[w];
+            if (r.state.load(std::memory_order_relaxed) != 1) continue;
+            if (__atomic_load_n(&flags_[w * kFlagStride], __ATOMIC_ACQUIRE) == 0) continue;
+            int one = 1;
+            if (!r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) continue;
+            on_complete(w);
+            any = true;
+        }
+        return any;
+    }
 
     // ---- Algorithm 2: FindJob -----------------------------------------------------------
     bool find_job(int w, Prepared& p, bool& stolen) {
@@ -322,16 +346,21 @@ class Scheduler {
         Running& r = running_[w];
         r.exec = exec;
         r.job = p.job;
-        uint64_t inflight = inflight_.fetch_add(1, std::memory_order_relaxed) + 1;
+        uint64_t inflight = inflight_.fetch_add(1, std::memory_order_seq_cst) + 1;
         uint64_t hw = stats_.max_inflight.load(std::memory_order_relaxed);
         while (inflight > hw && !stats_.max_inflight.compare_exchange_weak(hw, inflight)) {
+        }
+        if (flags_) {  // clear the slot's completion word BEFORE it becomes visible as in flight
+            __atomic_store_n(&flags_[w * kFlagStride], 0u, __ATOMIC_RELAXED);
+            r.state.store(1, std::memory_order_release);
         }
         if (rc == 0) rc = be_->launch(exec, w, p.job);  // GraphLaunch + AddCallback
         stats_.launched.fetch_add(1, std::memory_order_relaxed);
         stats_.ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
         if (rc != 0) {  // keep the books balanced so that drain returns; the error is sticky
             set_error(rc);
-            on_complete(w);
+            int one = 1;
+            if (!flags_ || r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) on_complete(w);
         }
     }
 
@@ -339,28 +368,36 @@ class Scheduler {
     void dispatcher_loop() {
         while (!stop_.load(std::memory_order_acquire)) {
             uint32_t seen = work_ec_.prepare();
-            // Sleep unless there is both an idle worker and a queued job.
-            if (n_free_.load(std::memory_order_seq_cst) <= 0 || n_queued_.load(std::memory_order_seq_cst) <= 0) {
-                if (stop_.load(std::memory_order_acquire)) break;
-                if (work_ec_.wait(seen, spin_ns_)) stats_.dispatcher_sleeps.fetch_add(1, std::memory_order_relaxed);
+            bool progressed = flags_ ? poll_flags() : false;
+            if (n_free_.load(std::memory_order_seq_cst) > 0 && n_queued_.load(std::memory_order_seq_cst) > 0) {
+                int w;
+                if (!pool_.try_pop(w)) continue;  // another dispatcher took it
+                n_free_.fetch_sub(1, std::memory_order_seq_cst);
+                Prepared p;
+                bool stolen = false;
+                if (find_job(w, p, stolen)) {
+                    n_queued_.fetch_sub(1, std::memory_order_seq_cst);
+                    launch_job(p, w, stolen);
+                } else {  // Alg. 2 l.7: no job -> the worker goes back to the pool
+                    pool_.try_push(w);
+                    n_free_.fetch_add(1, std::memory_order_seq_cst);
+                }
                 continue;
             }
-            int w;
-            if (!pool_.try_pop(w)) continue;  // another dispatcher took it
-            n_free_.fetch_sub(1, std::memory_order_seq_cst);
-            Prepared p;
-            bool stolen = false;
-            if (find_job(w, p, stolen)) {
-                n_queued_.fetch_sub(1, std::memory_order_seq_cst);
-                launch_job(p, w, stolen);
-            } else {  // Alg. 2 l.7: no job -> the worker goes back to the pool
-                pool_.try_push(w);
-                n_free_.fetch_add(1, std::memory_order_seq_cst);
+            if (progressed) continue;
+            if (stop_.load(std::memory_order_acquire)) break;
+            if (flags_ && inflight_.load(std::memory_order_seq_cst) > 0) {
+                // Nobody will wake this thread when the GPU stores a flag: keep watching while work is in flight.
+                cpu_relax();
+                continue;
             }
+            // Sleep until there is both an idle worker and a queued job (or, polled mode, until a submit arrives).
+            if (work_ec_.wait(seen, spin_ns_)) stats_.dispatcher_sleeps.fetch_add(1, std::memory_order_relaxed);
         }
     }
 
     Backend* be_;
+    volatile uint32_t* flags_ = nullptr;
     const int S_, b_, q_, epp_, steal_policy_;
     const uint64_t spin_ns_;
     std::unique_ptr<PaddedRing<Prepared>[]> queues_;

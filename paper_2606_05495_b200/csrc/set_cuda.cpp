@@ -95,6 +95,10 @@ struct set_ctx final : public Backend {
     cudaGraph_t graph = nullptr;
     std::vector<cudaGraphNode_t> kern_nodes;
     cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
+    cudaGraphNode_t signal_node = nullptr;     // SET_CB_FLAG_POLL: last node, stores the slot's completion word
+    uint32_t* flags_host = nullptr;            // b words, kFlagStride apart, mapped pinned host memory
+    uint32_t* flags_dev = nullptr;             // the device's address of the same memory
+    bool flag_poll = false;
     void* ph_in = nullptr;   // placeholder operands the template graph is built with
     void* ph_out = nullptr;
 
@@ -106,7 +110,7 @@ struct set_ctx final : public Backend {
     std::vector<CbArg> cbargs;
 
     // counters owned by the backend
-    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0};
+    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0}, signal_nodes{0};
     std::atomic<uint64_t> base_submitted{0}, base_completed{0}, base_launched{0}, base_ns_submit{0}, base_ns_launch{0};
 
     // sticky error
@@ -159,6 +163,7 @@ struct set_ctx final : public Backend {
     int launch(int exec, int slot, const JobDesc& job) override;
     void finish(int exec, int slot, const JobDesc& job) override;
     int poll() override;
+    volatile uint32_t* done_flags() override { return flag_poll ? flags_host : nullptr; }
 
     int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid);
     int check_sizes(const uint32_t* dims);
@@ -353,12 +358,25 @@ int set_ctx::build_graph() {
         }
         prev = kern_nodes[s];
     }
+    std::vector<cudaGraphNode_t> leaves;
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
         if (!expr_is_zero(bd.d2h_bytes)) {
             CK(cudaGraphAddMemcpyNode1D(&d2h_nodes[i], graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
                                         (char*)slots[0].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
+            leaves.push_back(d2h_nodes[i]);
         }
+    }
+    if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished
+        if (leaves.empty()) leaves.push_back(prev);
+        uint32_t* flag = flags_dev;
+        void* args[1] = {&flag};
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
+        kp.gridDim = dim3(1);
+        kp.blockDim = dim3(1);
+        kp.kernelParams = args;
+        CK(cudaGraphAddKernelNode(&signal_node, graph, leaves.data(), leaves.size(), &kp));
     }
     return 0;
 }
@@ -436,6 +454,16 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
                 mp.height = 1;
                 CK(cudaGraphExecMemsetNodeSetParams(es.exec, memset_nodes[i], &mp));
             }
+        if (signal_node && es.bound_slot != slot) {
+            uint32_t* flag = flags_dev + (size_t)slot * kFlagStride;
+            void* args[1] = {&flag};
+            cudaKernelNodeParams kp{};
+            kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
+            kp.gridDim = dim3(1);
+            kp.blockDim = dim3(1);
+            kp.kernelParams = args;
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, signal_node, &kp));
+        }
         full_rebinds.fetch_add(1, std::memory_order_relaxed);
     } else {
         host_rebinds.fetch_add(1, std::memory_order_relaxed);
@@ -474,7 +502,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     SpinLock& lk = stream_locks[s];
     lk.lock();
     cudaError_t e = cudaGraphLaunch(execs[exec].exec, streams[s]);
-    if (e == cudaSuccess) {
+    if (e == cudaSuccess && !flag_poll) {
         if (cfg.callback_mode == SET_CB_WORK_STREAM) {
             e = cudaLaunchHostFunc(streams[s], set_completion_cb, &cbargs[slot]);
         } else {
@@ -486,6 +514,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     lk.unlock();
     if (e != cudaSuccess) return cuda_fail(e, "graph launch / event chain", __LINE__);
     kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+    if (flag_poll) signal_nodes.fetch_add(1, std::memory_order_relaxed);
     return 0;
 }
 
@@ -645,6 +674,8 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.queue_capacity == 0) cfg.queue_capacity = 2;
     if (cfg.num_dispatchers == 0) cfg.num_dispatchers = 1;
     if (cfg.spin_us == 0) cfg.spin_us = 50;
+    if (cfg.callback_mode < SET_CB_DEFAULT || cfg.callback_mode > SET_CB_FLAG_POLL) return SET_ERR_INVALID;
+    if (cfg.callback_mode == SET_CB_DEFAULT) cfg.callback_mode = SET_CB_FLAG_POLL;
     if (cfg.mode == SET_MODE_SINGLE_GRAPH) {  // one worker, one stream, one exec by definition
         cfg.num_streams = 1;
         cfg.max_inflight = 1;
@@ -696,6 +727,18 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
         c->encode_tiled = (PFN_encodeTiled)fn;
     else
         cudaGetLastError();
+    if (cfg.mode == SET_MODE_SET && cfg.callback_mode == SET_CB_FLAG_POLL) {
+        // one 64-byte line per slot in mapped pinned memory; the GPU stores, the dispatcher loads
+        size_t bytes = (size_t)c->b * kFlagStride * sizeof(uint32_t);
+        if (cudaHostAlloc((void**)&c->flags_host, bytes, cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess ||
+            cudaHostGetDevicePointer((void**)&c->flags_dev, c->flags_host, 0) != cudaSuccess) {
+            cudaGetLastError();
+            delete c;
+            return SET_ERR_CUDA;
+        }
+        memset(c->flags_host, 0, bytes);
+        c->flag_poll = true;
+    }
     if (cfg.mode == SET_MODE_SET || cfg.mode == SET_MODE_MUTEX_QUEUE)
         c->sched.reset(new Scheduler(c, c->S, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
     *out = c;
@@ -885,6 +928,7 @@ set_status set_destroy(set_ctx* c) {
     if (c->ph_in) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_in) : cudaFreeHost(c->ph_in));
     if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
+    if (c->flags_host) cudaFreeHost(c->flags_host);
     for (int s = 0; s < c->S; ++s) {
         if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
         if (c->notify[s]) cudaStreamDestroy(c->notify[s]);
@@ -956,6 +1000,7 @@ set_status set_get_stats(set_ctx* c, set_stats* out) {
     out->host_rebinds = c->host_rebinds.load();
     out->staged_jobs = c->staged_jobs.load();
     out->kernel_nodes = c->kernel_nodes.load();
+    out->signal_nodes = c->signal_nodes.load();
     out->ns_bind = c->ns_bind.load();
     out->ns_sync = c->ns_sync.load();
     return SET_OK;
@@ -969,7 +1014,7 @@ set_status set_reset_stats(set_ctx* c) {
         st.ns_submit = 0; st.ns_launch = 0; st.ns_callback = 0; st.max_inflight = 0;
     }
     c->base_submitted = 0; c->base_completed = 0; c->base_launched = 0; c->base_ns_submit = 0; c->base_ns_launch = 0;
-    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
+    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
     return SET_OK;
 }
 

@@ -66,8 +66,9 @@ namespace {
 // Simulated device: launch() hands (slot, due time) to completer threads, which call on_complete(slot).
 class SimBackend : public Backend {
   public:
-    SimBackend(int slots, int epp, int completers, int64_t jobs, uint32_t seed)
-        : b_(slots), epp_(epp), jobs_(jobs), seed_(seed), inbox_((size_t)slots + 1) {
+    SimBackend(int slots, int epp, int completers, int64_t jobs, uint32_t seed, bool polled)
+        : b_(slots), epp_(epp), jobs_(jobs), seed_(seed), inbox_((size_t)slots + 1), polled_(polled) {
+        flags_.assign((size_t)slots * kFlagStride, 0u);
         bound_slot_.assign((size_t)slots * epp, -1);
         for (int e = 0; e < slots * epp; ++e) bound_slot_[(size_t)e] = e / epp;  // execs start tied to M_home
         exec_busy_ = std::vector<std::atomic<int>>((size_t)slots * epp);
@@ -116,6 +117,8 @@ class SimBackend : public Backend {
         slot_busy_[(size_t)slot].store(0);
         inflight_.fetch_sub(1);
     }
+    // polled completion: the completer threads play the GPU and store the slot's word
+    volatile uint32_t* done_flags() override { return polled_ ? flags_.data() : nullptr; }
     int64_t check_all_done_once() {
         int64_t bad = 0;
         for (auto& d : done_count_)
@@ -141,7 +144,10 @@ class SimBackend : public Backend {
                     int slot = held[i].slot;
                     held[i] = held.back();
                     held.pop_back();
-                    sched_->on_complete(slot);
+                    if (polled_)
+                        __atomic_store_n(&flags_[(size_t)slot * kFlagStride], 1u, __ATOMIC_RELEASE);
+                    else
+                        sched_->on_complete(slot);
                     any = true;
                 } else {
                     ++i;
@@ -155,6 +161,8 @@ class SimBackend : public Backend {
     uint32_t seed_;
     int ncompleters_ = 1;
     Ring<Item> inbox_;
+    bool polled_ = false;
+    std::vector<uint32_t> flags_;
     std::vector<int> bound_slot_;
     int bound_job_[1] = {0};
     std::vector<std::atomic<int>> exec_busy_, slot_busy_, done_count_;
@@ -172,7 +180,7 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
         return -1;
     int b = ((max_inflight + num_streams - 1) / num_streams) * num_streams;
     int policy = (seed & 1) ? Scheduler::kRetarget : Scheduler::kSwap;
-    SimBackend be(b, queue_capacity + 1, 2, jobs, seed);
+    SimBackend be(b, queue_capacity + 1, 2, jobs, seed, /*polled=*/(seed & 2) != 0);
     int64_t rc = 0;
     {
         Scheduler sched(&be, num_streams, b, queue_capacity, num_dispatchers, policy, 20);

@@ -184,9 +184,22 @@ def test_same_inputs_twice_give_identical_bits(libset):
         wl = small_workload(config)
         ids = list(range(6))
         a, _, _, _ = run_jobs(libset, wl, ids)
-        b, _, _, _ = run_jobs(libset, wl, ids, num_dispatchers=2, callback_mode=1)
+        b, _, _, _ = run_jobs(libset, wl, ids, num_dispatchers=2, callback_mode=libset.CB_WORK_STREAM)
         for x, y in zip(a, b):
             assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("cb", [1, 2, 3])
+@pytest.mark.parametrize("disp", [1, 2])
+def test_every_completion_mode_delivers_every_job(libset, cb, disp):
+    """A6/A7: event chain + cudaLaunchHostFunc on a notify stream (1), host function on the work stream (2, PAPER.md:203
+    literally) and the GPU-written flag watched by the dispatcher (3) all release each slot exactly once."""
+    from paper_2606_05495_b200.workloads import small_workload
+    for config in (0, 4):
+        wl = small_workload(config)
+        st = check(libset, wl, list(range(wl.jobs)), callback_mode=cb, num_dispatchers=disp)
+        assert st["signal_nodes"] == (wl.jobs if cb == 3 else 0)
+        assert st["max_inflight_seen"] <= wl.max_inflight
 
 
 def test_submit_before_register_and_double_register(libset):
