@@ -1,5 +1,228 @@
-// gemm_sm100.cu -- K9 placeholder (filled in by the tcgen05 kernel).
+// gemm_sm100.cu -- K9: C = bf16( GELU( A.B + bias ) ), bf16 operands, fp32 accumulation on the 5th-generation tensor
+// cores (BASELINE.json:configs[3]; readings C3-1..C3-4).  Hand-written for sm_100a: TMA
+// (cp.async.bulk.tensor) stages 128-byte-swizzled operand tiles in shared memory, one elected thread issues
+// tcgen05.mma with the accumulator in tensor memory (TMEM), four epilogue warps read it back with tcgen05.ld and
+// apply bias + erf-GELU + round-to-nearest-even bf16 on the way to global memory.
+//
+//   A : bf16 [M][K] row-major  -> K-major operand,  TMA box 64 (K) x 128 (M) = 16 KiB per stage
+//   B : bf16 [K][N] row-major  -> MN-major operand (no host transpose), 4 TMA boxes 64 (N) x 64 (K) = 32 KiB per stage
+//   D : fp32 128 x 256 accumulator = 256 TMEM columns x 128 lanes; one tile per CTA, grid = (N/256, M/128)
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..5 = epilogue
+// (warp w may only touch TMEM lanes 32*(w%4) .. 32*(w%4)+31, so the four warps cover lanes 64..127, 0..63).
+// Ragged shapes: TMA zero-fills out-of-bounds rows/columns of a box, so partial tiles in M, N and K contribute
+// zeros; the epilogue stores only rows < M and columns < N (N and K must be multiples of 8: 16-byte TMA pitches).
+#include <cuda_bf16.h>
+
 #include "kernels.h"
-extern "C" __global__ void set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                                                     const float* bias, uint16_t* C, uint32_t M, uint32_t N, uint32_t K) {}
-extern "C" uint32_t set_gemm_smem_bytes(void) { return 0; }
+
+namespace {
+
+constexpr uint32_t kBlockM = 128, kBlockN = 256, kBlockK = 64, kUmmaK = 16;
+constexpr uint32_t kStages = 4;
+constexpr uint32_t kABytes = kBlockM * kBlockK * 2;          // 16 KiB
+constexpr uint32_t kBBoxN = 64;                              // one 128-byte swizzle atom of N per box
+constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
+constexpr uint32_t kBBytes = kBBoxBytes * (kBlockN / kBBoxN);  // 32 KiB
+constexpr uint32_t kStageBytes = kABytes + kBBytes;          // 48 KiB
+constexpr uint32_t kTmemCols = 256;
+constexpr uint32_t kBarrierBytes = 256;
+constexpr uint32_t kSmemBytes = kStages * kStageBytes + kBarrierBytes + 1024;  // + slack for 1024-byte alignment
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int32_t c_inner, int32_t c_outer) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+                 "l"(tm), "r"(bar), "r"(c_inner), "r"(c_outer)
+                 : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
+// Shared-memory matrix descriptor (tcgen05): start address, leading / stride byte offsets (all >> 4), descriptor
+// version 1, 128-byte swizzle.  K-major A tile [128 rows][64 k]: 8-row groups are 1024 B apart (SBO), LBO unused.
+// MN-major B tile: 64 (N) x 8 (K) swizzle atoms; the next 8 K rows are 1024 B on (SBO), the next 64 columns of N
+// are one TMA box = 8 KiB on (LBO).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((addr >> 4) & 0x3fffu);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3fffu) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3fffu) << 32;
+    d |= 1ull << 46;  // descriptor version (Blackwell)
+    d |= 2ull << 61;  // SWIZZLE_128B
+    return d;
+}
+
+// Instruction descriptor, kind::f16: D fp32, A and B bf16, A K-major, B MN-major, N >> 3, M >> 4.
+constexpr uint32_t kInstrDesc = (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((kBlockN >> 3) << 17) | ((kBlockM >> 4) << 24);
+
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate)
+        : "memory");
+}
+// Arrives on the mbarrier once every tcgen05.mma issued so far by this thread has completed.
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+
+// GELU, exact erf form (reading C3-3): 0.5 z (1 + erf(z / sqrt 2)), evaluated in fp32.
+__device__ __forceinline__ float gelu_erf(float z) { return 0.5f * z * (1.0f + erff(z * 0.70710678118654752440f)); }
+
+}  // namespace
+
+extern "C" uint32_t set_gemm_smem_bytes(void) { return kSmemBytes; }
+
+extern "C" __global__ void __launch_bounds__(192, 1)
+set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const float* __restrict__ bias,
+                          uint16_t* __restrict__ C, uint32_t M, uint32_t N, uint32_t K) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // 128-byte swizzle atoms repeat every 1024 B
+    const uint32_t bars = base + kStages * kStageBytes;
+    // barrier block: full[kStages], empty[kStages], accum_full, then the TMEM base address written by tcgen05.alloc
+    auto full_bar = [&](uint32_t s) { return bars + 8u * s; };
+    auto empty_bar = [&](uint32_t s) { return bars + 8u * (kStages + s); };
+    const uint32_t accum_bar = bars + 8u * (2 * kStages);
+    const uint32_t tmem_slot = bars + 8u * (2 * kStages + 1);
+    auto a_tile = [&](uint32_t s) { return base + s * kStageBytes; };
+    auto b_tile = [&](uint32_t s) { return base + s * kStageBytes + kABytes; };
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t m0 = blockIdx.y * kBlockM, n0 = blockIdx.x * kBlockN;
+    const uint32_t num_kb = (K + kBlockK - 1) / kBlockK;
+    // B boxes of this tile that start inside the matrix (a box that starts at or beyond N is never requested; the
+    // accumulator columns it would feed are never stored)
+    const uint32_t n_boxes = min((N - n0 + kBBoxN - 1) / kBBoxN, kBlockN / kBBoxN);
+    const uint32_t stage_tx = kABytes + n_boxes * kBBoxBytes;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        for (uint32_t s = 0; s < kStages; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), 1);
+        }
+        mbar_init(accum_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {  // TMEM: 256 columns for the 128 x 256 fp32 accumulator
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (elect_one()) {
+            for (uint32_t kb = 0; kb < num_kb; ++kb) {
+                const uint32_t s = kb % kStages, round = kb / kStages;
+                mbar_wait(empty_bar(s), (round & 1u) ^ 1u);  // first pass over the ring falls through
+                mbar_expect_tx(full_bar(s), stage_tx);
+                tma_load_2d(a_tile(s), &tmA, full_bar(s), (int32_t)(kb * kBlockK), (int32_t)m0);
+                for (uint32_t j = 0; j < n_boxes; ++j)
+                    tma_load_2d(b_tile(s) + j * kBBoxBytes, &tmB, full_bar(s), (int32_t)(n0 + j * kBBoxN), (int32_t)(kb * kBlockK));
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: one thread drives the tensor core for the whole CTA =====
+        if (elect_one()) {
+            for (uint32_t kb = 0; kb < num_kb; ++kb) {
+                const uint32_t s = kb % kStages, round = kb / kStages;
+                mbar_wait(full_bar(s), round & 1u);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (uint32_t k = 0; k < kBlockK / kUmmaK; ++k) {
+                    // A: 16 K-elements = 32 bytes further along the swizzled 128-byte row
+                    const uint64_t adesc = smem_desc(a_tile(s) + k * kUmmaK * 2u, 16u, 1024u);
+                    // B: 16 K-rows = two 8-row groups = 2048 bytes further
+                    const uint64_t bdesc = smem_desc(b_tile(s) + k * kUmmaK * 128u, kBBoxBytes, 1024u);
+                    umma_bf16(tmem_base, adesc, bdesc, (kb | k) != 0u);
+                }
+                umma_commit(empty_bar(s));  // the stage may be refilled once these MMAs have read it
+            }
+            umma_commit(accum_bar);  // accumulator complete
+        }
+    } else {
+        // ===== epilogue: TMEM -> registers -> bias + GELU -> bf16 -> global =====
+        mbar_wait(accum_bar, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t quarter = warp & 3u;  // the TMEM lane quarter this warp may read
+        const uint32_t row = m0 + quarter * 32u + lane;
+        uint16_t* crow = C + (size_t)row * N;
+#pragma unroll 1
+        for (uint32_t c = 0; c < kBlockN; c += 32) {
+            if (n0 + c >= N) break;  // warp-uniform
+            uint32_t v[32];
+            tmem_ld32(tmem_base + ((quarter * 32u) << 16) + c, v);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (uint32_t g = 0; g < 4; ++g) {  // 8 columns -> one 16-byte store
+                const uint32_t n = n0 + c + 8u * g;
+                if (row < M && n < N) {
+                    const float4 b0 = __ldg(reinterpret_cast<const float4*>(bias + n));
+                    const float4 b1 = __ldg(reinterpret_cast<const float4*>(bias + n + 4));
+                    const float z[8] = {__uint_as_float(v[8 * g + 0]) + b0.x, __uint_as_float(v[8 * g + 1]) + b0.y,
+                                        __uint_as_float(v[8 * g + 2]) + b0.z, __uint_as_float(v[8 * g + 3]) + b0.w,
+                                        __uint_as_float(v[8 * g + 4]) + b1.x, __uint_as_float(v[8 * g + 5]) + b1.y,
+                                        __uint_as_float(v[8 * g + 6]) + b1.z, __uint_as_float(v[8 * g + 7]) + b1.w};
+                    uint4 o;
+                    uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        __nv_bfloat162 h = __floats2bfloat162_rn(gelu_erf(z[2 * q]), gelu_erf(z[2 * q + 1]));
+                        ow[q] = *reinterpret_cast<uint32_t*>(&h);
+                    }
+                    *reinterpret_cast<uint4*>(crow + n) = o;
+                }
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    }
+}

@@ -133,6 +133,14 @@ def test_config2_ragged_grids(libset, h, w, sweeps):
     check(libset, Workload(2, (h, w, sweeps), jobs=3, num_streams=2, max_inflight=4), list(range(3)))
 
 
+@pytest.mark.parametrize("m,n,k", [(128, 256, 64), (128, 256, 576), (200, 264, 72), (130, 8, 8), (1, 2048, 40), (300, 768, 320)])
+def test_config3_ragged_shapes(libset, m, n, k):
+    """One tile exactly; more k-blocks than pipeline stages (the smem ring wraps twice); partial tiles in M, N and K;
+    degenerate thin shapes."""
+    from paper_2606_05495_b200.workloads import Workload
+    check(libset, Workload(3, (m, n, k), jobs=3, num_streams=2, max_inflight=4), list(range(3)))
+
+
 @pytest.mark.parametrize("size", [(1, 1), (5, 4), (7, 3), (128, 64), (132, 65), (644, 9)])
 def test_config4_ragged_frames(libset, size):
     from paper_2606_05495_b200.workloads import Workload
