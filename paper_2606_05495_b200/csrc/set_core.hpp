@@ -144,11 +144,11 @@ class Scheduler {
         for (int w = 0; w < b_; ++w) {
             queues_[w].r.init((size_t)epp_ + 1);
             free_execs_[w].r.init((size_t)epp_ * 2);  // room for migrated execs under kRetarget
-            for (int k = 0; k < epp_; ++k) free_execs_[w].r.try_push(w * epp_ + k);
+            for (int k = 0; k < epp_; ++k) free_execs_[w].r.push(w * epp_ + k);
         }
         pool_.init((size_t)b_ + 1);
         // the main thread initialises all workers; all of them start idle.
-        for (int w = 0; w < b_; ++w) pool_.try_push(w);
+        for (int w = 0; w < b_; ++w) pool_.push(w);
         n_free_.store(b_, std::memory_order_relaxed);
         for (int d = 0; d < num_dispatchers; ++d) dispatchers_.emplace_back([this] { dispatcher_loop(); });
     }
@@ -207,7 +207,7 @@ class Scheduler {
         bool pinned = false;
         int rc = be_->bind(exec, slot, p.job, &pinned);  // UpdateGraphParams(J_id, i)
         if (rc != 0) {
-            free_execs_[slot].r.try_push(exec);
+            free_execs_[slot].r.push(exec);
             space_ec_.notify_all();
             if (rc != -5 /*SET_ERR_SIZE is per job, not sticky*/) set_error(rc);
             return rc;
@@ -215,7 +215,7 @@ class Scheduler {
         if (pinned) p.home |= kPinnedBit;
         stats_.submitted.fetch_add(1, std::memory_order_relaxed);
         c_submitted_.fetch_add(1, std::memory_order_release);
-        queues_[slot].r.try_push(p);  // cannot fail: entries are bounded by the slot's exec count
+        queues_[slot].r.push(p);  // room is guaranteed: entries are bounded by the slot's exec count
         n_queued_.fetch_add(1, std::memory_order_seq_cst);
         work_ec_.notify_all();
         stats_.ns_submit.fetch_add(now_ns() - t0, std::memory_order_relaxed);
@@ -232,9 +232,9 @@ class Scheduler {
         r.exec = -1;
         r.state.store(0, std::memory_order_release);
         inflight_.fetch_sub(1, std::memory_order_seq_cst);
-        free_execs_[exec / epp_].r.try_push(exec);  // the exec returns to its home free list
+        free_execs_[exec / epp_].r.push(exec);  // the exec returns to its home free list
         space_ec_.notify_all();
-        pool_.try_push(w);  // W_pool.push(w_id)
+        pool_.push(w);  // W_pool.push(w_id)
         n_free_.fetch_add(1, std::memory_order_seq_cst);
         work_ec_.notify_all();  // notify_one()
         stats_.completed.fetch_add(1, std::memory_order_relaxed);
@@ -293,7 +293,7 @@ class Scheduler {
         bool any = false;
         for (int w = 0; w < b_; ++w) {
             Running& r = running_[w];
-            if (r.state.load(std::memory_order_relaxed) != 1) continue;
+            if (r.state.load(std::memory_order_acquire) != 1) continue;
             if (__atomic_load_n(&flags_[w * kFlagStride], __ATOMIC_ACQUIRE) == 0) continue;
             int one = 1;
             if (!r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) continue;
@@ -334,7 +334,7 @@ class Scheduler {
                 // The thief owns an exec that is already tied to M_w: give the job to it (only the
                 // host-pointer copy nodes change) and hand the victim's exec back at once.
                 rc = be_->bind(mine, w, p.job, &dummy);
-                free_execs_[exec / epp_].r.try_push(exec);
+                free_execs_[exec / epp_].r.push(exec);
                 space_ec_.notify_all();
                 exec = mine;
             } else {
@@ -366,12 +366,17 @@ class Scheduler {
 
     // ---- Algorithm 2: dispatcher main loop ----------------------------------------------
     void dispatcher_loop() {
+        Backoff idle(4096);
         while (!stop_.load(std::memory_order_acquire)) {
             uint32_t seen = work_ec_.prepare();
             bool progressed = flags_ ? poll_flags() : false;
             if (n_free_.load(std::memory_order_seq_cst) > 0 && n_queued_.load(std::memory_order_seq_cst) > 0) {
                 int w;
-                if (!pool_.try_pop(w)) continue;  // another dispatcher took it
+                if (!pool_.try_pop(w)) {  // another dispatcher took it
+                    idle.pause();
+                    continue;
+                }
+                idle = Backoff(4096);
                 n_free_.fetch_sub(1, std::memory_order_seq_cst);
                 Prepared p;
                 bool stolen = false;
@@ -379,20 +384,25 @@ class Scheduler {
                     n_queued_.fetch_sub(1, std::memory_order_seq_cst);
                     launch_job(p, w, stolen);
                 } else {  // Alg. 2 l.7: no job -> the worker goes back to the pool
-                    pool_.try_push(w);
+                    pool_.push(w);
                     n_free_.fetch_add(1, std::memory_order_seq_cst);
                 }
                 continue;
             }
-            if (progressed) continue;
+            if (progressed) {
+                idle = Backoff(4096);
+                continue;
+            }
             if (stop_.load(std::memory_order_acquire)) break;
             if (flags_ && inflight_.load(std::memory_order_seq_cst) > 0) {
-                // Nobody will wake this thread when the GPU stores a flag: keep watching while work is in flight.
-                cpu_relax();
+                // Nobody will wake this thread when the GPU stores a flag: keep watching while work is in flight
+                // (PAUSE for the first few thousand rounds, then yield between looks).
+                idle.pause();
                 continue;
             }
             // Sleep until there is both an idle worker and a queued job (or, polled mode, until a submit arrives).
             if (work_ec_.wait(seen, spin_ns_)) stats_.dispatcher_sleeps.fetch_add(1, std::memory_order_relaxed);
+            idle = Backoff(4096);
         }
     }
 

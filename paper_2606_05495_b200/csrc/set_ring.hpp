@@ -19,9 +19,30 @@
 #include <memory>
 #include <new>
 
+#include <sched.h>
+
 namespace setrt {
 
 constexpr size_t kCacheLine = 64;
+
+// Spin politely: PAUSE for the first `spins` rounds, then give the core away each round, so that a waiter never
+// starves the thread it is waiting for when there are fewer cores than threads.
+struct Backoff {
+    explicit Backoff(int spins = 128) : left(spins) {}
+    void pause() {
+        if (left > 0) {
+            --left;
+#if defined(__x86_64__) || defined(__i386__)
+            __builtin_ia32_pause();
+#else
+            asm volatile("" ::: "memory");
+#endif
+        } else {
+            sched_yield();
+        }
+    }
+    int left;
+};
 
 template <typename T>
 class Ring {
@@ -67,6 +88,15 @@ class Ring {
                 pos = tail_.load(std::memory_order_relaxed);
             }
         }
+    }
+
+    // For pushes that are logically guaranteed room (the entry count is bounded below the capacity by the
+    // caller's own accounting).  try_push can still report "full" for a moment: a consumer that claimed the
+    // cell one lap earlier may have been preempted between its head_ CAS and its seq store.  That state is
+    // transient, so wait it out instead of dropping the entry.
+    void push(const T& v) {
+        Backoff bo;
+        while (!try_push(v)) bo.pause();
     }
 
     bool try_pop(T& out) {

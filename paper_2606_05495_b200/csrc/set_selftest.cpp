@@ -29,19 +29,22 @@ extern "C" int64_t set_selftest_ring(int capacity, int producers, int consumers,
         th.emplace_back([&, p] {
             for (int64_t i = 0; i < items_per_producer; ++i) {
                 uint64_t tok = (uint64_t)p * (uint64_t)items_per_producer + (uint64_t)i;
-                while (!ring.try_push(tok)) cpu_relax();
+                Backoff bo;
+                while (!ring.try_push(tok)) bo.pause();
             }
         });
     for (int c = 0; c < consumers; ++c)
         th.emplace_back([&] {
             uint64_t last_from[64];
             for (auto& l : last_from) l = 0;
+            Backoff bo;
             while (popped.load(std::memory_order_relaxed) < total) {
                 uint64_t tok;
                 if (!ring.try_pop(tok)) {
-                    cpu_relax();
+                    bo.pause();
                     continue;
                 }
+                bo = Backoff();
                 if (tok >= (uint64_t)total) { errors.fetch_add(1); continue; }
                 if (seen[(size_t)tok].fetch_add(1) != 0) errors.fetch_add(1);  // delivered twice
                 // FIFO per producer as observed by ONE consumer: tokens of a producer arrive in order
@@ -108,7 +111,7 @@ class SimBackend : public Backend {
         h ^= h >> 15;
         uint64_t due = now_ns() + (uint64_t)(h % 40u) * 1000ull;
         Item it{slot, exec, job.id, due};
-        while (!inbox_.try_push(it)) cpu_relax();
+        inbox_.push(it);
         return 0;
     }
     void finish(int exec, int slot, const JobDesc& job) override {
@@ -134,6 +137,7 @@ class SimBackend : public Backend {
     };
     void completer() {
         std::vector<Item> held;
+        Backoff bo;
         while (!stop_.load(std::memory_order_acquire) || !held.empty() || !inbox_.empty_approx()) {
             Item it;
             while (inbox_.try_pop(it)) held.push_back(it);
@@ -153,7 +157,10 @@ class SimBackend : public Backend {
                     ++i;
                 }
             }
-            if (!any) cpu_relax();
+            if (any)
+                bo = Backoff();
+            else
+                bo.pause();
         }
     }
     int b_, epp_;
