@@ -194,7 +194,7 @@ MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3
 
 
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
-            verify: int = 0, ctx_kw=None, flush=None, clock_windows=None):
+            verify: int = 0, ctx_kw=None, flush=None, clock_windows=None, trace=None):
     """W untimed + K timed steps of (submit every job, drain).  Returns a dict with per-step ms (CUDA events on
     torch's current stream, recorded around the host-synchronous submit..drain region), wall ms and library stats."""
     import torch
@@ -213,6 +213,14 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
             step()
         torch.cuda.synchronize()
         ctx.reset_stats()
+        if trace is not None:
+            # gap pass: one step under CUPTI activity tracing; never used for a throughput number
+            trace.start()
+            step()
+            torch.cuda.synchronize()
+            g = trace.stop()
+            js.keep.clear()
+            return {"mode": mode, "io": "device" if io_device else "host", "jobs": n, "gaps": g}
         ev_ms, wall_ms = [], []
         for _ in range(steps):
             if flush is not None:
@@ -411,6 +419,43 @@ def cpu_baseline(wl, job_ids, budget_s=15.0, passes=10):
 # ------------------------------------------------------------------------------------------------ main
 # distinct-input pool / output ring per config (0 = one per job).  Rings are >= b*(q+1) outstanding jobs.
 LAYOUT = {0: (0, 0), 1: (0, 0), 2: (16, 32), 3: (8, 64), 4: (96, 128)}
+GAP_JOBS = {0: 256, 1: 2000, 2: 64, 3: 200, 4: 512}  # jobs traced per arm in the gap pass (records stay in host memory)
+
+
+def gap_pass(setlib, wl, ids, all_configs: bool, warmup: int):
+    """Inter-kernel gaps and device idle fraction from CUPTI activity records (include/set_trace.h), for SET and for the
+    batch-synchronous-graph baseline on the same jobs.  Runs after every timed arm: tracing slows the launch path, so no
+    throughput figure comes from here."""
+    out = {"how": "one step per arm under CUPTI activity tracing (kernel, memcpy, memset records), after all timed arms; "
+                  "gap = start(next) - end(previous) of operations consecutive on one stream; idle_frac = 1 - |union of "
+                  "activity| / wall (DESIGN.md reading S12)"}
+    try:
+        from paper_2606_05495_b200 import trace
+        trace.load()
+    except Exception as e:
+        return {"unavailable": str(e)[:200]}
+    from paper_2606_05495_b200.workloads import baseline_workload
+    todo = [(wl, ids)]
+    if all_configs:
+        todo += [(baseline_workload(c), None) for c in range(5) if c != wl.config]
+    for w, job_ids in todo:
+        job_ids = list(range(w.jobs)) if job_ids is None else job_ids
+        job_ids = job_ids[:GAP_JOBS[w.config]]
+        p, r = LAYOUT[w.config]
+        res = {"jobs": len(job_ids)}
+        for mode in ("set", "batch_sync_graphs"):
+            for io_device in (True, False):
+                key = f"{mode}_{'device' if io_device else 'e2e'}"
+                try:
+                    g = run_arm(setlib, w, job_ids, mode, io_device, 1, max(1, min(warmup, 2)), p, r, trace=trace)["gaps"]
+                    res[key] = g
+                    log(f"[bench]   gaps config{w.config} {key:28s} kernel->kernel mean {g['kernel_kernel']['mean_us']:.2f} us "
+                        f"p99 {g['kernel_kernel']['p99_us']:.2f}  inter-job mean {g['inter_job']['mean_us']:.2f} us  idle {g['idle_frac']:.3f}")
+                except Exception as e:
+                    res[key] = {"error": str(e)[:200]}
+                    log(f"[bench]   gaps config{w.config} {key} failed: {e}")
+        out[f"config{w.config}"] = res
+    return out
 
 
 def workload_for(config, jobs_override=None):
@@ -469,6 +514,7 @@ def main():
     ap.add_argument("--impl", default="set", choices=["set", "reference"])
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
     ap.add_argument("--out", default=None, help="also write the JSON line to this file")
     args = ap.parse_args()
 
@@ -581,6 +627,8 @@ def main():
             extra["workloads"] = others
     sampler.stop()
     clocks = sampler.summary(windows)
+    if world == 1 and not args.no_gaps:
+        extra["gaps"] = gap_pass(setlib, wl, ids, args.suite == "all", warmup)
 
     if rank == 0:
         dom = max(extra.get("kernels", [{"total_us": 0}]), key=lambda r: r.get("total_us", 0)) if extra.get("kernels") else None

@@ -14,6 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libset.so")
+TRACE_LIB = os.path.join(HERE, "libsettrace.so")  # CUPTI gap tracer (include/set_trace.h): measurement only
 BUILD_DIR = os.path.join(HERE, "build")
 
 CUDA_SOURCES = ["kernels/small_kernels.cu", "kernels/stencil_kernels.cu", "kernels/gemm_sm100.cu", "set_builtin.cu"]
@@ -60,7 +61,22 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
             raise RuntimeError("link failed")
+    build_trace(force)
     return LIB
+
+
+def build_trace(force: bool = False) -> str:
+    """libsettrace.so: host-only C++ against the CUPTI headers; libcupti itself is dlopen'ed at run time."""
+    src = os.path.join(CSRC, "set_trace.cpp")
+    if force or _stale(TRACE_LIB, [src, os.path.join(INCLUDE, "set_trace.h"), os.path.abspath(__file__)]):
+        cuda = os.path.dirname(os.path.dirname(os.path.realpath(NVCC)))
+        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-Wall", "-Wextra", "-I", INCLUDE, "-I", os.path.join(cuda, "include"),
+               "-o", TRACE_LIB, src, "-ldl", "-lpthread"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+            raise RuntimeError("building libsettrace.so failed")
+    return TRACE_LIB
 
 
 if __name__ == "__main__":
