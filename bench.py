@@ -193,15 +193,20 @@ def build_jobs(setlib, ctx, wl, job_ids, io_device: bool, pool: int, out_ring: i
 MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3, "mutex_queue": 4}
 
 
+# graph-shape options of every arm (SET and the in-run baselines share the job graph): --sm-copy / --pdl
+OPTS = {"sm_copy_max_bytes": 0, "pdl": True}
+
+
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
-            verify: int = 0, ctx_kw=None, flush=None, clock_windows=None, trace=None):
+            verify: int = 0, ctx_kw=None, flush=None, clock_windows=None, trace=None, opts=None):
     """W untimed + K timed steps of (submit every job, drain).  Returns a dict with per-step ms (CUDA events on
     torch's current stream, recorded around the host-synchronous submit..drain region), wall ms and library stats."""
     import torch
+    o = dict(OPTS, **(opts or {}))
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=MODES[mode], io=setlib.IO_DEVICE if io_device else setlib.IO_HOST,
-                         **(ctx_kw or {}))
+                         sm_copy_max_bytes=o["sm_copy_max_bytes"], **(ctx_kw or {}))
     try:
-        ctx.register_builtin(wl.config, wl.variant, list(wl.params))
+        ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=o["pdl"])
         js = build_jobs(setlib, ctx, wl, job_ids, io_device, pool, out_ring)
         n = js.n
 
@@ -257,7 +262,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
                "wall_ms_per_step": float(np.sum(wall_ms)) / steps, "jobs_per_s": n / (ms * 1e-3),
                "step_ms": [round(x, 4) for x in ev_ms], "h2d_bytes": 0 if io_device else js.in_bytes,
                "d2h_bytes": 0 if io_device else js.out_bytes, "in_bytes": js.in_bytes, "out_bytes": js.out_bytes,
-               "kernel_launches": st["kernel_nodes"], "verified": len(picks) if verify else 0, "mismatches": bad,
+               "kernel_launches": st["kernel_nodes"] + st["copy_nodes"] + st["signal_nodes"], "verified": len(picks) if verify else 0, "mismatches": bad,
                "stats": st}
         jobs_total = max(1, st["submitted"])
         out["host_us_per_job"] = {k: st["ns_" + k] / jobs_total / 1e3 for k in ("submit", "bind", "launch", "callback", "sync")}
@@ -515,8 +520,11 @@ def main():
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
+    ap.add_argument("--sm-copy", type=int, default=0, help="set_config.sm_copy_max_bytes: 0 = library default, -1 = copy engines only")
+    ap.add_argument("--pdl", type=int, default=1, help="1: programmatic-dependent-launch edges between kernel nodes (default), 0: plain edges")
     ap.add_argument("--out", default=None, help="also write the JSON line to this file")
     args = ap.parse_args()
+    OPTS["sm_copy_max_bytes"], OPTS["pdl"] = args.sm_copy, bool(args.pdl)
 
     from paper_2606_05495_b200 import multi
     if args.impl == "reference":
@@ -587,6 +595,16 @@ def main():
                 cm[name + "_e2e"] = {"jobs_per_s": round(r["jobs_per_s"], 1), "ms_per_step": round(r["ms_per_step"], 3),
                                      "host_us_per_job": r["host_us_per_job"], "mismatches": r["mismatches"]}
             extra["completion_modes"] = dict(cm, flag_poll_e2e={"jobs_per_s": round(e2e_value, 1)})
+            gv = {}
+            for name, o in (("ce_copies_plain_edges", {"sm_copy_max_bytes": -1, "pdl": False}), ("ce_copies_pdl", {"sm_copy_max_bytes": -1, "pdl": True}),
+                            ("sm_copies_plain_edges", {"sm_copy_max_bytes": 0, "pdl": False}), ("sm_copies_pdl", {"sm_copy_max_bytes": 0, "pdl": True})):
+                p_, r_ = LAYOUT[wl.config]
+                for io_device in (False, True):
+                    r = run_arm(setlib, wl, ids, "set", io_device, steps, warmup, p_, r_, verify=2, flush=flush, opts=o)
+                    gv[f"{name}_{'device' if io_device else 'e2e'}"] = {"jobs_per_s": round(r["jobs_per_s"], 1), "mismatches": r["mismatches"],
+                                                                        "host_us_per_job": r["host_us_per_job"]}
+                    log(f"[bench]   {wl.config} set/{name:24s} {'device' if io_device else 'host  '} {r['jobs_per_s']:12.1f} jobs/s")
+            extra["graph_variants"] = gv
             base = {}
             for mode in ("batch_sync_graphs", "plain_streams", "single_graph"):
                 for io_device in (False, True):
@@ -642,13 +660,14 @@ def main():
                 "ms_per_step": round(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": wl.dtype, "data": "synthetic",
                 "config": {"workload": wl.name, "jobs_per_step_per_gpu": len(ids), "num_streams": wl.num_streams,
+                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or "library default: 262144 for host buffers, copy engines for device-resident I/O", "pdl_edges": OPTS["pdl"],
                            "max_inflight": wl.max_inflight, "io": "value: inputs/outputs resident in HBM (D2D copy nodes); e2e: pinned host buffers",
                            "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer rewritten between timed steps; distinct job inputs "
                                  f"{dev_arm['in_bytes'] / 1e6:.0f} MB per step"},
                 "clocks": clocks,
                 "e2e": {"value": round(e2e_value, 1), "unit": "jobs/s", "h2d_bytes_per_step": int(e2e_arm["h2d_bytes"] * world),
                         "d2h_bytes_per_step": int(e2e_arm["d2h_bytes"] * world), "ms_per_step": round(ms_e2e, 4)},
-                "gpu_launches": int((dev_arm["kernel_launches"] + dev_arm["stats"]["signal_nodes"]) * world),
+                "gpu_launches": int(dev_arm["kernel_launches"] * world),
                 "mismatches": dev_arm["mismatches"] + e2e_arm["mismatches"],
                 "host_us_per_job": {"device": dev_arm["host_us_per_job"], "e2e": e2e_arm["host_us_per_job"]},
                 "sched_stats": {k: e2e_arm["stats"][k] for k in ("steals", "submit_stalls", "dispatcher_sleeps", "max_inflight_seen",

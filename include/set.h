@@ -95,8 +95,10 @@ typedef struct set_arg_desc {
     set_tmap2d tmap;       /* TMAP2D only                                                          */
 } set_arg_desc;
 
-#define SET_STAGE_PDL 1u   /* connect this stage to the previous one with a programmatic-dependent-
-                              launch edge (the kernel must call griddepcontrol.wait before reading) */
+#define SET_STAGE_PDL 1u   /* connect this stage to the node before it (the previous stage; for the first stage,
+                              an SM copy node) with a programmatic-dependent-launch edge: the kernel must
+                              execute griddepcontrol.wait before it reads or writes job data (every built-in
+                              kernel does).  Ignored where the predecessor is a copy-engine node.           */
 
 /* One stage = one kernel node of the job graph ("nodes are initialized with the target
  * function, input arguments, grid and block dimensions").  Stages run in list order. */
@@ -175,7 +177,12 @@ typedef struct set_config {
     int32_t callback_mode;    /* SET_CB_*                                                          */
     int32_t device;           /* CUDA device ordinal; -1 => current device                         */
     int32_t spin_us;          /* dispatcher/drain spin time before sleeping; 0 => default (50)     */
-    int32_t reserved0;
+    int32_t sm_copy_max_bytes;/* H2D/D2H copies of a fixed size up to this many bytes become kernel nodes
+                                 (SET_K_COPY: the SMs read/write pinned host memory over the link) instead of
+                                 copy-engine memcpy nodes; 0 => default (262144 under SET_IO_HOST, never under
+                                 SET_IO_DEVICE), -1 => never.  One D2H copy
+                                 done this way also carries the SET_CB_FLAG_POLL completion signal.
+                                 DESIGN.md "SM copies"                                                  */
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */
@@ -200,7 +207,8 @@ typedef struct set_stats {
     uint64_t ns_sync;          /* host ns blocked in batch/stream synchronisation (baselines)      */
     uint64_t max_inflight_seen;/* high-water mark of launched-not-completed jobs                   */
     uint64_t signal_nodes;     /* completion-signal kernel launches (SET_CB_FLAG_POLL: one per job)*/
-    uint64_t reserved[3];
+    uint64_t copy_nodes;       /* SET_K_COPY kernel launches (copies done by the SMs)                 */
+    uint64_t reserved[2];
 } set_stats;
 
 /* ---------------------------------------------------------------------------------------------- *
@@ -289,20 +297,24 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_RELU_F32        5  /* (float* y, uint32 n)  y = max(y,0)                                       */
 #define SET_K_SQUARE_F32      6  /* (float* y, uint32 n)  y = fl(y*y)                                        */
 #define SET_K_BLOCK_SUM_F32   7  /* (const float* y, float* out, uint32 n)  out[0] = sum, fixed tree, 1 block */
-#define SET_K_JACOBI5_F32     8  /* (const float* u, float* v, uint32 h, uint32 w)  one sweep, zero halo     */
-#define SET_K_GEMM_BIAS_GELU  9  /* (tmapA, tmapB, const float* bias, bf16* C, uint32 M, N, K)  tcgen05      */
+#define SET_K_JACOBI5_F32     8  /* (const float* u, float* v, uint32 h, uint32 w, uint32 flip)  one sweep, zero
+                                    halo; flip = 1 walks the row blocks bottom-up (L2 reuse between sweeps)  */
+#define SET_K_GEMM_BIAS_GELU  9  /* (tmapA, tmapB, tmapC, const float* bias, uint32 M, N, K)  tcgen05 + TMA   */
 #define SET_K_RGB2GRAY_U8    10  /* (const uint8* rgb, uint8* gray, uint32 w, uint32 h)                      */
 #define SET_K_BLUR3X3_U8     11  /* (const uint8* g, uint8* out, uint32 w, uint32 h)  clamp-to-edge          */
 #define SET_K_HIST256_U8     12  /* (const uint8* p, uint32* hist, uint32 w, uint32 h)  hist must be zeroed  */
 #define SET_K_SPIN           13  /* (uint32* scratch, uint32 ns)  debug delay stage (busy-waits ns)          */
 #define SET_K_SIGNAL         14  /* (uint32* flag)  *flag = 1 in mapped pinned HOST memory (SET_CB_FLAG_POLL) */
+#define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes, uint32* ctr, uint32* flag)
+                                    copy by the SMs; src/dst may be pinned HOST or DEVICE memory; flag != NULL:
+                                    the last block stores *flag = 1 after every block's data is visible       */
 
 /* HOST address usable as set_stage_desc.func, or NULL for an unknown id. */
 const void *set_builtin_kernel(int kernel_id);
 
 /* Fill stage/buffer descriptors for BASELINE.json:configs[config] (0..4).
  *   params : HOST array of uint32 or NULL for the BASELINE sizes:
- *     config 0: {n}            config 1: {n}          config 2: {h, w, sweeps}
+ *     config 0: {n}            config 1: {n}          config 2: {h, w, sweeps[, alternate = 1]}
  *     config 3: {M, N, K}      config 4: {max_w, max_h}  (dims per job = {w, h, 1, 1})
  *   variant: 0 = default.  config 0: 1 = histogram of the INPUT values (reading C0-1 alternative).
  * *            any config: bit 8 set = append a SET_K_SPIN delay stage that busy-waits dims[3] nanoseconds.

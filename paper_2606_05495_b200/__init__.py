@@ -26,6 +26,7 @@ STEAL_SWAP, STEAL_RETARGET = 0, 1
 CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL = 0, 1, 2, 3
 ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D = 0, 1, 2, 3, 4
 STAGE_PDL = 1
+K_COPY = 15
 BUF_ZERO = 1
 VARIANT_SPIN = 0x100
 
@@ -70,7 +71,7 @@ class BufferDesc(C.Structure):
 class Config(C.Structure):
     _fields_ = [("struct_bytes", C.c_uint32), ("num_streams", C.c_int32), ("max_inflight", C.c_int32), ("mode", C.c_int32),
                 ("io", C.c_int32), ("queue_capacity", C.c_int32), ("num_dispatchers", C.c_int32), ("steal_policy", C.c_int32),
-                ("callback_mode", C.c_int32), ("device", C.c_int32), ("spin_us", C.c_int32), ("reserved0", C.c_int32),
+                ("callback_mode", C.c_int32), ("device", C.c_int32), ("spin_us", C.c_int32), ("sm_copy_max_bytes", C.c_int32),
                 ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64)]
 
 
@@ -78,7 +79,7 @@ class Stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in
                 ("submitted", "completed", "launched", "steals", "full_rebinds", "host_rebinds", "staged_jobs", "submit_stalls",
                  "dispatcher_sleeps", "kernel_nodes", "ns_submit", "ns_bind", "ns_launch", "ns_callback", "ns_sync",
-                 "max_inflight_seen", "signal_nodes")] + [("reserved", C.c_uint64 * 3)]
+                 "max_inflight_seen", "signal_nodes", "copy_nodes")] + [("reserved", C.c_uint64 * 2)]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if n != "reserved"}
@@ -158,7 +159,8 @@ class Context:
 
     def __init__(self, num_streams: int, max_inflight: int, mode: int = MODE_SET, io: int = IO_HOST, queue_capacity: int = 0,
                  num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_DEFAULT,
-                 device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0):
+                 device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0,
+                 sm_copy_max_bytes: int = 0):
         self._lib = load()
         self._h = C.c_void_p(None)
         cfg = Config()
@@ -166,6 +168,7 @@ class Context:
         cfg.num_streams, cfg.max_inflight, cfg.mode, cfg.io = num_streams, max_inflight, mode, io
         cfg.queue_capacity, cfg.num_dispatchers, cfg.steal_policy = queue_capacity, num_dispatchers, steal_policy
         cfg.callback_mode, cfg.device, cfg.spin_us = callback_mode, device, spin_us
+        cfg.sm_copy_max_bytes = sm_copy_max_bytes
         self._streams_arr = None
         if streams is not None:
             self._streams_arr = (C.c_void_p * len(streams))(*[int(s) for s in streams])
@@ -205,8 +208,11 @@ class Context:
         self._check(self._lib.set_register_pipeline(self._h, stages, num_stages, bufs, num_bufs), "set_register_pipeline")
         self.num_stages = num_stages
 
-    def register_builtin(self, config: int, variant: int = 0, params=None):
+    def register_builtin(self, config: int, variant: int = 0, params=None, pdl: bool = False):
         st, ns, bf, nb, hin, hout = builtin_pipeline(config, variant, params)
+        if pdl:  # programmatic-dependent-launch edges between consecutive kernel nodes (set.h SET_STAGE_PDL)
+            for i in range(ns):
+                st[i].flags |= STAGE_PDL
         self.register_pipeline(st, ns, bf, nb)
         self.host_in_bytes, self.host_out_bytes = hin, hout
         return hin, hout

@@ -1,17 +1,19 @@
 // gemm_sm100.cu -- K9: C = bf16( GELU( A.B + bias ) ), bf16 operands, fp32 accumulation on the 5th-generation tensor
 // cores (BASELINE.json:configs[3]; readings C3-1..C3-4).  Hand-written for sm_100a: TMA
 // (cp.async.bulk.tensor) stages 128-byte-swizzled operand tiles in shared memory, one elected thread issues
-// tcgen05.mma with the accumulator in tensor memory (TMEM), four epilogue warps read it back with tcgen05.ld and
-// apply bias + erf-GELU + round-to-nearest-even bf16 on the way to global memory.
+// tcgen05.mma with the accumulator in tensor memory (TMEM), eight epilogue warps read it back with tcgen05.ld and
+// apply bias + erf-GELU + round-to-nearest-even bf16 and store the tile through TMA.
 //
 //   A : bf16 [M][K] row-major  -> K-major operand,  TMA box 64 (K) x 128 (M) = 16 KiB per stage
 //   B : bf16 [K][N] row-major  -> MN-major operand (no host transpose), 4 TMA boxes 64 (N) x 64 (K) = 32 KiB per stage
 //   D : fp32 128 x 256 accumulator = 256 TMEM columns x 128 lanes; one tile per CTA, grid = (N/256, M/128)
 //
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..5 = epilogue
-// (warp w may only touch TMEM lanes 32*(w%4) .. 32*(w%4)+31, so the four warps cover lanes 64..127, 0..63).
-// Ragged shapes: TMA zero-fills out-of-bounds rows/columns of a box, so partial tiles in M, N and K contribute
-// zeros; the epilogue stores only rows < M and columns < N (N and K must be multiples of 8: 16-byte TMA pitches).
+// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..9 = epilogue
+// (warp w may only touch TMEM lanes 32*(w%4) .. 32*(w%4)+31; two warps share each lane quarter and split the 256
+// columns).  The epilogue writes bf16 rows into 128-byte-swizzled shared memory and hands each 32 x 64 piece to the
+// TMA unit (cp.async.bulk.tensor store): C leaves the SM as full 128-byte lines instead of 16 bytes per row.
+// Ragged shapes: TMA zero-fills out-of-bounds rows/columns of a load box, so partial tiles in M, N and K contribute
+// zeros, and clips a store box to the matrix (N and K must be multiples of 8: 16-byte TMA pitches).
 #include <cuda_bf16.h>
 
 #include "kernels.h"
@@ -25,6 +27,8 @@ constexpr uint32_t kBBoxN = 64;                              // one 128-byte swi
 constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
 constexpr uint32_t kBBytes = kBBoxBytes * (kBlockN / kBBoxN);  // 32 KiB
 constexpr uint32_t kStageBytes = kABytes + kBBytes;          // 48 KiB
+constexpr uint32_t kCBoxBytes = 64 * 32 * 2;                 // epilogue staging: one TMA store box, 64 columns x 32 rows of bf16
+static_assert(16 * kCBoxBytes <= kStages * kStageBytes, "the epilogue stages its 16 boxes in the idle operand ring");
 constexpr uint32_t kTmemCols = 256;
 constexpr uint32_t kBarrierBytes = 256;
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + kBarrierBytes + 1024;  // + slack for 1024-byte alignment
@@ -111,9 +115,9 @@ __device__ __forceinline__ float gelu_erf(float z) { return 0.5f * z * (1.0f + e
 
 extern "C" uint32_t set_gemm_smem_bytes(void) { return kSmemBytes; }
 
-extern "C" __global__ void __launch_bounds__(192, 1)
-set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const float* __restrict__ bias,
-                          uint16_t* __restrict__ C, uint32_t M, uint32_t N, uint32_t K) {
+extern "C" __global__ void __launch_bounds__(320, 1)
+set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                          const __grid_constant__ CUtensorMap tmC, const float* __restrict__ bias, uint32_t M, uint32_t N, uint32_t K) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // 128-byte swizzle atoms repeat every 1024 B
     const uint32_t bars = base + kStages * kStageBytes;
@@ -136,6 +140,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         for (uint32_t s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);
             mbar_init(empty_bar(s), 1);
@@ -185,39 +190,56 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
             umma_commit(accum_bar);  // accumulator complete
         }
     } else {
-        // ===== epilogue: TMEM -> registers -> bias + GELU -> bf16 -> global =====
+        // ===== epilogue: TMEM -> registers -> bias + GELU -> bf16 -> swizzled smem -> TMA store =====
+        // Eight warps: warp w reads TMEM lane quarter q = w % 4 (the only lanes it may touch) and column half
+        // h = (w - 2) / 4, i.e. a 32-row x 128-column piece of the tile = two 64-column TMA boxes of 4 KiB.  The
+        // operand ring is idle once accum_bar has fired (every MMA has read it), so the boxes are staged there.
         mbar_wait(accum_bar, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t quarter = warp & 3u;  // the TMEM lane quarter this warp may read
-        const uint32_t row = m0 + quarter * 32u + lane;
-        uint16_t* crow = C + (size_t)row * N;
+        const uint32_t q = warp & 3u, h = (warp - 2u) >> 2;
+        const uint32_t stage0 = base + ((h * 4u + q) * 2u) * kCBoxBytes;
 #pragma unroll 1
-        for (uint32_t c = 0; c < kBlockN; c += 32) {
-            if (n0 + c >= N) break;  // warp-uniform
-            uint32_t v[32];
-            tmem_ld32(tmem_base + ((quarter * 32u) << 16) + c, v);
+        for (uint32_t j = 0; j < 2; ++j) {  // one 64-column box per round
+            const uint32_t c0 = h * 128u + j * 64u;
+            if (n0 + c0 >= N) break;  // warp-uniform: nothing of this box lies inside the matrix
+            uint32_t v[64];
+            tmem_ld32(tmem_base + ((q * 32u) << 16) + c0, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+            tmem_ld32(tmem_base + ((q * 32u) << 16) + c0 + 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            const uint32_t srow = stage0 + j * kCBoxBytes + lane * 128u;  // this lane's 128-byte row of the box
 #pragma unroll
-            for (uint32_t g = 0; g < 4; ++g) {  // 8 columns -> one 16-byte store
-                const uint32_t n = n0 + c + 8u * g;
-                if (row < M && n < N) {
-                    const float4 b0 = __ldg(reinterpret_cast<const float4*>(bias + n));
-                    const float4 b1 = __ldg(reinterpret_cast<const float4*>(bias + n + 4));
-                    const float z[8] = {__uint_as_float(v[8 * g + 0]) + b0.x, __uint_as_float(v[8 * g + 1]) + b0.y,
-                                        __uint_as_float(v[8 * g + 2]) + b0.z, __uint_as_float(v[8 * g + 3]) + b0.w,
-                                        __uint_as_float(v[8 * g + 4]) + b1.x, __uint_as_float(v[8 * g + 5]) + b1.y,
-                                        __uint_as_float(v[8 * g + 6]) + b1.z, __uint_as_float(v[8 * g + 7]) + b1.w};
-                    uint4 o;
-                    uint32_t* ow = reinterpret_cast<uint32_t*>(&o);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        __nv_bfloat162 h = __floats2bfloat162_rn(gelu_erf(z[2 * q]), gelu_erf(z[2 * q + 1]));
-                        ow[q] = *reinterpret_cast<uint32_t*>(&h);
-                    }
-                    *reinterpret_cast<uint4*>(crow + n) = o;
+            for (uint32_t g = 0; g < 8; ++g) {  // 8 columns -> one 16-byte chunk
+                const uint32_t n = n0 + c0 + 8u * g;
+                float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+                if (n < N) {  // N is a multiple of 8: a chunk is inside or outside as a whole
+                    b0 = __ldg(reinterpret_cast<const float4*>(bias + n));
+                    b1 = __ldg(reinterpret_cast<const float4*>(bias + n + 4));
                 }
+                const float z[8] = {__uint_as_float(v[8 * g + 0]) + b0.x, __uint_as_float(v[8 * g + 1]) + b0.y,
+                                    __uint_as_float(v[8 * g + 2]) + b0.z, __uint_as_float(v[8 * g + 3]) + b0.w,
+                                    __uint_as_float(v[8 * g + 4]) + b1.x, __uint_as_float(v[8 * g + 5]) + b1.y,
+                                    __uint_as_float(v[8 * g + 6]) + b1.z, __uint_as_float(v[8 * g + 7]) + b1.w};
+                uint32_t o[4];
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    __nv_bfloat162 hh = __floats2bfloat162_rn(gelu_erf(z[2 * t]), gelu_erf(z[2 * t + 1]));
+                    o[t] = *reinterpret_cast<uint32_t*>(&hh);
+                }
+                // 128-byte swizzle: chunk g of row r lives at chunk position g ^ (r mod 8)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(srow + ((g ^ (lane & 7u)) << 4)), "r"(o[0]), "r"(o[1]),
+                             "r"(o[2]), "r"(o[3])
+                             : "memory");
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
+            __syncwarp();
+            if (lane == 0 && m0 + q * 32u < M) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
+                asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(&tmC),
+                             "r"(stage0 + j * kCBoxBytes), "r"((int32_t)(n0 + c0)), "r"((int32_t)(m0 + q * 32u))
+                             : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
         }
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // stores done before smem goes away
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();

@@ -13,17 +13,30 @@ __global__ void set_k_add_bias_f32(float* y, const float* bias, uint32_t n);
 __global__ void set_k_relu_f32(float* y, uint32_t n);
 __global__ void set_k_square_f32(float* y, uint32_t n);
 __global__ void set_k_block_sum_f32(const float* y, float* out, uint32_t n);
-__global__ void set_k_jacobi5_f32(const float* u, float* v, uint32_t h, uint32_t w);
+__global__ void set_k_jacobi5_f32(const float* u, float* v, uint32_t h, uint32_t w, uint32_t flip);
 __global__ void set_k_rgb2gray_u8(const uint8_t* rgb, uint8_t* gray, uint32_t w, uint32_t h);
 __global__ void set_k_blur3x3_u8(const uint8_t* g, uint8_t* out, uint32_t w, uint32_t h);
 __global__ void set_k_hist256_u8(const uint8_t* p, uint32_t* hist, uint32_t w, uint32_t h);
 __global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
 __global__ void set_k_signal(uint32_t* flag);
+__global__ void set_k_copy(const void* src, void* dst, uint32_t bytes, uint32_t* done_ctr, uint32_t* flag);
 }
+
+// Programmatic dependent launch (SET_STAGE_PDL edges of the job graph): let the next kernel node be scheduled now,
+// then wait until every kernel this one depends on has finished and its writes are visible.  Both instructions do
+// nothing in a kernel that was launched over an ordinary edge, so every built-in kernel starts with this.
+#ifdef __CUDACC__
+__device__ __forceinline__ void set_pdl_sync() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
 
 // Tile shapes the host-side grid rules in set_builtin.cu must agree with.
 constexpr int kJacobiRows = 16;        // rows per block
 constexpr int kJacobiCols = 1024;      // columns per block (256 threads x float4)
+constexpr unsigned kJacobiUnroll = 4;  // rows whose loads are in flight together
 constexpr int kGrayPixPerBlock = 256 * 16;
 constexpr int kBlurTileW = 128, kBlurTileH = 64;
 constexpr int kHistPixPerBlock = 256 * 16 * 4;
+constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words

@@ -32,6 +32,7 @@ __device__ __forceinline__ bool aligned16(const void* a, const void* b = nullptr
 // thread totals -> 32 warp totals scanned by warp 0 in shared memory -> carry from the previous chunk.
 extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t* __restrict__ in, int32_t* __restrict__ out,
                                                                   uint32_t n) {
+    set_pdl_sync();
     __shared__ int warp_tot[32];
     __shared__ int chunk_tot;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -81,6 +82,7 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t*
 // warp; the 32 copies are then summed, one bin per thread.
 extern "C" __global__ void __launch_bounds__(1024) set_k_hist_mod64(const int32_t* __restrict__ in, uint32_t* __restrict__ hist,
                                                                     uint32_t n) {
+    set_pdl_sync();
     __shared__ uint32_t h[32][64 + 1];
     const int tid = threadIdx.x, wid = tid >> 5;
     for (int k = tid; k < 32 * 65; k += 1024) (&h[0][0])[k] = 0;
@@ -106,6 +108,7 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_hist_mod64(const int32_
 // K3..K6: one fp32 operation per element per kernel (reading C1-5: the chain stays unfused).  256 threads x 4
 // elements per block; __fmul_rn/__fadd_rn are never contracted into an FMA (reading C1-1).
 extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* __restrict__ x, float* __restrict__ y, uint32_t n) {
+    set_pdl_sync();
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(x, y)) {
         float4 v = *reinterpret_cast<const float4*>(x + i);
@@ -120,6 +123,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* 
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __restrict__ y, const float* __restrict__ bias, uint32_t n) {
+    set_pdl_sync();
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(y, bias)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
@@ -135,6 +139,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __re
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_relu_f32(float* __restrict__ y, uint32_t n) {
+    set_pdl_sync();
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(y)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
@@ -149,6 +154,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_relu_f32(float* __restri
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __restrict__ y, uint32_t n) {
+    set_pdl_sync();
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(y)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
@@ -168,6 +174,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __rest
 // the 1e-6 tolerance of the double-accumulated oracle; measured ~1e-8).
 extern "C" __global__ void __launch_bounds__(1024) set_k_block_sum_f32(const float* __restrict__ y, float* __restrict__ out,
                                                                        uint32_t n) {
+    set_pdl_sync();
     __shared__ float wsum[32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     float acc = 0.0f;
@@ -204,6 +211,47 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
 // the job's output is already in host memory): one thread stores 1 to the slot's word in mapped pinned host
 // memory, which the dispatcher thread is watching.  The fence orders the store after everything this GPU wrote.
 extern "C" __global__ void set_k_signal(uint32_t* flag) {
+    set_pdl_sync();
     __threadfence_system();
     *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+}
+
+// K15: copy node executed by the SMs.  A job of configs 0-1 moves 16-128 KB per direction;
+// a copy-engine memcpy node costs ~10 us of engine hand-off on each side of it, far more than the wire time, so
+// copies up to set_config.sm_copy_max_bytes are kernel nodes instead: the SMs read pinned host memory directly
+// over the link (H2D) or store into it (D2H).  Each thread moves two 128-bit words, both loads issued before the
+// first store so that 8 KB per block are in flight; unaligned operands or sizes fall back to a byte loop.
+// With flag != NULL this is also the completion signal of SET_CB_FLAG_POLL: every block fences its stores
+// system-wide and bumps the slot's counter; the last block resets the counter and stores the slot's word.
+extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes,
+                                                             uint32_t* done_ctr, uint32_t* flag) {
+    set_pdl_sync();
+    const uint32_t tid = threadIdx.x;
+    const uint32_t base = blockIdx.x * (uint32_t)kCopyBytesPerBlock;
+    if (aligned16(src, dst)) {
+        const uint32_t o0 = base + tid * 16u, o1 = o0 + 256u * 16u;
+        uint4 a = make_uint4(0, 0, 0, 0), b = a;
+        const bool f0 = o0 + 16u <= bytes, f1 = o1 + 16u <= bytes;
+        if (f0) a = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o0);
+        if (f1) b = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o1);
+        if (f0) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o0) = a;
+        if (f1) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o1) = b;
+        // ragged tail (< 16 bytes), by the thread whose word would have covered it
+        if (!f0 && o0 < bytes)
+            for (uint32_t k = o0; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
+        if (!f1 && o1 < bytes)
+            for (uint32_t k = o1; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
+    } else {
+        const uint32_t end = min(base + (uint32_t)kCopyBytesPerBlock, bytes);
+        for (uint32_t k = base + tid; k < end; k += 256u) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
+    }
+    if (flag) {
+        __threadfence_system();  // this thread's stores are visible system-wide before anything it does next
+        __syncthreads();
+        if (tid == 0 && atomicAdd(done_ctr, 1u) == gridDim.x - 1) {
+            *done_ctr = 0;  // ready for the slot's next job (which starts only after the host has seen the flag)
+            __threadfence_system();
+            *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+        }
+    }
 }

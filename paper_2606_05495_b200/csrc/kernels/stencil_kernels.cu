@@ -21,8 +21,12 @@ __device__ __forceinline__ float at0(const float* __restrict__ u, uint32_t h, ui
 }  // namespace
 
 extern "C" __global__ void __launch_bounds__(256) set_k_jacobi5_f32(const float* __restrict__ u, float* __restrict__ v, uint32_t h,
-                                                                    uint32_t w) {
-    const uint32_t r0 = blockIdx.y * kJacobiRows;
+                                                                    uint32_t w, uint32_t flip) {
+    set_pdl_sync();
+    // flip = 1: walk the row blocks bottom-up.  Consecutive sweeps alternate direction, so a sweep starts on the rows
+    // the previous sweep wrote last -- the part of the ping-pong pair (2 x 64 MiB) that is still in the 126 MB L2.
+    const uint32_t by = flip ? gridDim.y - 1u - blockIdx.y : blockIdx.y;
+    const uint32_t r0 = by * kJacobiRows;
     const uint32_t r1 = min(r0 + (uint32_t)kJacobiRows, h);
     const uint32_t c4 = (blockIdx.x * 256u + threadIdx.x) * 4u;
     if ((w & 3u) == 0) {
@@ -32,24 +36,47 @@ extern "C" __global__ void __launch_bounds__(256) set_k_jacobi5_f32(const float*
         auto row = [&](uint32_t r) -> float4 {
             return active ? __ldg(reinterpret_cast<const float4*>(u + (size_t)r * w + c4)) : zero;
         };
+        // the warp's edge lanes need one scalar from the neighbouring column group (0 outside the grid = the halo)
+        auto edge = [&](uint32_t r) -> float {
+            if (lane == 0) return (active && c4 > 0) ? __ldg(u + (size_t)r * w + c4 - 1) : 0.0f;
+            if (lane == 31) return (active && c4 + 4 < w) ? __ldg(u + (size_t)r * w + c4 + 4) : 0.0f;
+            return 0.0f;
+        };
         float4 up = (r0 > 0) ? row(r0 - 1) : zero;
-        float4 mid = (r0 < h) ? row(r0) : zero;
-        for (uint32_t r = r0; r < r1; ++r) {
-            float4 down = (r + 1 < h) ? row(r + 1) : zero;
-            float left = __shfl_up_sync(0xffffffffu, mid.w, 1);
-            float right = __shfl_down_sync(0xffffffffu, mid.x, 1);  // an inactive neighbour holds 0 = the halo
-            if (lane == 0) left = (active && c4 > 0) ? __ldg(u + (size_t)r * w + c4 - 1) : 0.0f;
-            if (lane == 31) right = (active && c4 + 4 < w) ? __ldg(u + (size_t)r * w + c4 + 4) : 0.0f;
-            if (active) {
-                float4 o;
-                o.x = jac(mid.x, left, mid.y, up.x, down.x);
-                o.y = jac(mid.y, mid.x, mid.z, up.y, down.y);
-                o.z = jac(mid.z, mid.y, mid.w, up.z, down.z);
-                o.w = jac(mid.w, mid.z, right, up.w, down.w);
-                *reinterpret_cast<float4*>(v + (size_t)r * w + c4) = o;
+        float4 mid = row(r0);
+        float e_mid = edge(r0);
+        // kJacobiUnroll rows per round: all of the round's loads are issued before the first add, so every thread keeps
+        // kJacobiUnroll 128-bit loads in flight (one load per thread does not cover the HBM latency at 7 blocks per SM)
+        for (uint32_t r = r0; r < r1; r += kJacobiUnroll) {
+            float4 dn[kJacobiUnroll];
+            float e_dn[kJacobiUnroll];
+#pragma unroll
+            for (uint32_t k = 0; k < kJacobiUnroll; ++k) {
+                const uint32_t rr = r + 1 + k;  // row below output row r + k; row r1 is the block's lower halo
+                const bool need = rr < h && rr <= r1;
+                dn[k] = need ? row(rr) : zero;
+                e_dn[k] = (need && rr < r1) ? edge(rr) : 0.0f;
             }
-            up = mid;
-            mid = down;
+#pragma unroll
+            for (uint32_t k = 0; k < kJacobiUnroll; ++k) {
+                if (r + k < r1) {
+                    float left = __shfl_up_sync(0xffffffffu, mid.w, 1);
+                    float right = __shfl_down_sync(0xffffffffu, mid.x, 1);  // an inactive neighbour holds 0 = the halo
+                    if (lane == 0) left = e_mid;
+                    if (lane == 31) right = e_mid;
+                    if (active) {
+                        float4 o;
+                        o.x = jac(mid.x, left, mid.y, up.x, dn[k].x);
+                        o.y = jac(mid.y, mid.x, mid.z, up.y, dn[k].y);
+                        o.z = jac(mid.z, mid.y, mid.w, up.z, dn[k].z);
+                        o.w = jac(mid.w, mid.z, right, up.w, dn[k].w);
+                        *reinterpret_cast<float4*>(v + (size_t)(r + k) * w + c4) = o;
+                    }
+                    up = mid;
+                    mid = dn[k];
+                    e_mid = e_dn[k];
+                }
+            }
         }
     } else {  // ragged width: rows are not 16-byte aligned, one element at a time
         for (uint32_t r = r0; r < r1; ++r)

@@ -7,7 +7,8 @@
 #include "kernels/kernels.h"
 
 extern "C" __global__ void set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                                                     const float* bias, uint16_t* C, uint32_t M, uint32_t N, uint32_t K);
+                                                     const __grid_constant__ CUtensorMap tmC, const float* bias, uint32_t M, uint32_t N,
+                                                     uint32_t K);
 extern "C" uint32_t set_gemm_smem_bytes(void);
 
 namespace {
@@ -91,6 +92,7 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_HIST256_U8: return (const void*)set_k_hist256_u8;
         case SET_K_SPIN: return (const void*)set_k_spin;
         case SET_K_SIGNAL: return (const void*)set_k_signal;
+        case SET_K_COPY: return (const void*)set_k_copy;
         default: return nullptr;
     }
 }
@@ -140,7 +142,7 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             break;
         }
         case 2: {  // `sweeps` Jacobi sweeps, ping-pong between buffers 0 and 1   (configs[2]; readings C2-1..C2-3)
-            uint32_t h = P(0, 4096), w = P(1, 4096), sweeps = P(2, 10);
+            uint32_t h = P(0, 4096), w = P(1, 4096), sweeps = P(2, 10), alternate = P(3, 1);
             if (h == 0 || w == 0 || sweeps == 0) return SET_ERR_INVALID;
             in_bytes = out_bytes = 4ull * h * w;
             bf[0] = buffer(in_bytes);
@@ -154,7 +156,7 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
                 {
                     st[ns++] = stage(SET_K_JACOBI5_F32, grid_fixed((w + kJacobiCols - 1) / kJacobiCols),
                                      grid_fixed((h + kJacobiRows - 1) / kJacobiRows), 256, 1, 0,
-                                     {arg_buf(cur), arg_buf(cur ^ 1), arg_u32(h), arg_u32(w)});
+                                     {arg_buf(cur), arg_buf(cur ^ 1), arg_u32(h), arg_u32(w), arg_u32(alternate ? (sweeps - left) & 1u : 0u)});
                     left -= 1;
                 }
                 cur ^= 1;
@@ -174,9 +176,10 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[1].d2h_bytes = fixed(out_bytes);
             nb = 2;
             // A: row-major MxK, box = 64 K-elements (128 B) x 128 rows.  B: row-major KxN, box = 64 N-elements x 64 K-rows.
-            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed((N + 255) / 256), grid_fixed((M + 127) / 128), 192, 1, set_gemm_smem_bytes(),
-                             {arg_tmap(0, 0, 2, K, M, 64, 128), arg_tmap(0, a_bytes, 2, N, K, 64, 64), arg_buf(0, fixed(a_bytes + b_bytes)),
-                              arg_buf(1), arg_u32(M), arg_u32(N), arg_u32(K)});
+            // C: row-major MxN, store box = 64 N-elements x 32 rows (one epilogue warp's piece).
+            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed((N + 255) / 256), grid_fixed((M + 127) / 128), 320, 1, set_gemm_smem_bytes(),
+                             {arg_tmap(0, 0, 2, K, M, 64, 128), arg_tmap(0, a_bytes, 2, N, K, 64, 64), arg_tmap(1, 0, 2, N, M, 64, 32),
+                              arg_buf(0, fixed(a_bytes + b_bytes)), arg_u32(M), arg_u32(N), arg_u32(K)});
             break;
         }
         case 4: {  // gray -> blur -> hist256; dims = {w, h}   (configs[4]; readings C4-1..C4-4)

@@ -23,6 +23,8 @@
 
 using namespace setrt;
 
+#define SET_COPY_BYTES_PER_BLOCK 8192u  // kernels/kernels.h kCopyBytesPerBlock (SET_K_COPY: 256 threads x 2 x 16 B)
+
 namespace {
 
 inline uint64_t eval(const set_size_expr& e, const uint32_t* dims) {
@@ -96,6 +98,12 @@ struct set_ctx final : public Backend {
     std::vector<cudaGraphNode_t> kern_nodes;
     cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
     cudaGraphNode_t signal_node = nullptr;     // SET_CB_FLAG_POLL: last node, stores the slot's completion word
+    // SM copies (set_config.sm_copy_max_bytes): h2d_nodes[i] / d2h_nodes[i] are SET_K_COPY kernel nodes where set
+    bool h2d_sm[SET_MAX_BUFFERS] = {}, d2h_sm[SET_MAX_BUFFERS] = {};
+    int n_sm_copies = 0;
+    int fused_signal_buf = -1;                 // the one D2H SM copy that also stores the completion word, or -1
+    bool pdl = false;                          // some stage asked for SET_STAGE_PDL: kernel-to-kernel edges are programmatic
+    uint32_t* ctrs_dev = nullptr;              // per-slot block counters of the fused copy+signal node (DEVICE)
     uint32_t* flags_host = nullptr;            // b words, kFlagStride apart, mapped pinned host memory
     uint32_t* flags_dev = nullptr;             // the device's address of the same memory
     bool flag_poll = false;
@@ -110,7 +118,7 @@ struct set_ctx final : public Backend {
     std::vector<CbArg> cbargs;
 
     // counters owned by the backend
-    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0}, signal_nodes{0};
+    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0}, signal_nodes{0}, copy_nodes{0};
     std::atomic<uint64_t> base_submitted{0}, base_completed{0}, base_launched{0}, base_ns_submit{0}, base_ns_launch{0};
 
     // sticky error
@@ -125,6 +133,12 @@ struct set_ctx final : public Backend {
     std::vector<PinnedRange> pinned_ranges;
 
     PFN_encodeTiled encode_tiled = nullptr;
+
+    // SET_DRIVER_LOCK=1 (environment, read at create): every graph update and graph launch takes this one lock.
+    // Only for runs under Nsight Compute 2025.2, whose injection library double-frees when one thread updates a
+    // graph executable while another thread is inside cudaGraphLaunch (profiles/r1_ncu.md); never set for timing.
+    bool driver_lock = false;
+    std::mutex driver_mu;
 
     // baseline state (single caller thread)
     std::vector<JobDesc> batch;
@@ -166,6 +180,17 @@ struct set_ctx final : public Backend {
     volatile uint32_t* done_flags() override { return flag_poll ? flags_host : nullptr; }
 
     int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid);
+    // SET_K_COPY node parameters for buffer i of `slot`: H2D (host_or_dev = job input) or D2H (job output)
+    struct CopyArgs {
+        const void* src;
+        void* dst;
+        uint32_t bytes;
+        uint32_t* ctr;
+        uint32_t* flag;
+        void* ptrs[5];
+        cudaKernelNodeParams kp;
+    };
+    void copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims);
     int check_sizes(const uint32_t* dims);
     bool is_pinned(const void* p);
     void add_pinned_range(const void* p, size_t n);
@@ -239,6 +264,34 @@ int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims
     return 0;
 }
 
+void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims) {
+    const set_buffer_desc& bd = bufs[i];
+    if (to_device) {
+        ca.src = (const char*)host + eval(bd.h2d_host_off, dims);
+        ca.dst = (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, dims);
+        ca.bytes = (uint32_t)eval(bd.h2d_bytes, dims);
+        ca.ctr = nullptr;
+        ca.flag = nullptr;
+    } else {
+        ca.src = (const char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, dims);
+        ca.dst = (char*)host + eval(bd.d2h_host_off, dims);
+        ca.bytes = (uint32_t)eval(bd.d2h_bytes, dims);
+        bool sig = fused_signal_buf == i;
+        ca.ctr = sig ? ctrs_dev + (size_t)slot * kFlagStride : nullptr;
+        ca.flag = sig ? flags_dev + (size_t)slot * kFlagStride : nullptr;
+    }
+    ca.ptrs[0] = &ca.src;
+    ca.ptrs[1] = &ca.dst;
+    ca.ptrs[2] = &ca.bytes;
+    ca.ptrs[3] = &ca.ctr;
+    ca.ptrs[4] = &ca.flag;
+    ca.kp = cudaKernelNodeParams{};
+    ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
+    ca.kp.gridDim = dim3((ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK);
+    ca.kp.blockDim = dim3(256);
+    ca.kp.kernelParams = ca.ptrs;
+}
+
 int set_ctx::check_sizes(const uint32_t* dims) {
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
@@ -278,6 +331,9 @@ bool set_ctx::is_pinned(const void* p) {
         return false;
     }
     if (at.type != cudaMemoryTypeHost) return false;
+    // SM copies dereference the caller's pointer on the device: registered memory whose device alias differs (or
+    // that is not mapped at all) goes through the library's own pinned staging blocks like pageable memory
+    if (n_sm_copies && at.devicePointer != p) return false;
     // remember the whole allocation so that later jobs from the same arena skip the query
     typedef CUresult (*PFN_getattr)(void*, CUpointer_attribute, CUdeviceptr);
     static PFN_getattr getattr = [] {
@@ -309,8 +365,18 @@ int set_ctx::build_graph() {
     const uint32_t unit[4] = {1, 1, 1, 1};
     cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    // dependency helper: a programmatic (PDL) edge where both ends are kernel nodes and the pipeline asked for it
+    auto depend = [&](cudaGraphNode_t from, cudaGraphNode_t to, bool programmatic) -> cudaError_t {
+        if (!programmatic) return cudaGraphAddDependencies(graph, &from, &to, 1);
+        cudaGraphEdgeData ed{};
+        ed.from_port = cudaGraphKernelNodePortProgrammatic;
+        ed.to_port = 0;
+        ed.type = cudaGraphDependencyTypeProgrammatic;
+        return cudaGraphAddDependencies_v2(graph, &from, &to, &ed, 1);
+    };
     CK(cudaGraphCreate(&graph, 0));
     std::vector<cudaGraphNode_t> roots;
+    std::vector<bool> root_is_kernel;
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
         if (bd.flags & SET_BUF_ZERO) {
@@ -322,11 +388,19 @@ int set_ctx::build_graph() {
             mp.value = 0;
             CK(cudaGraphAddMemsetNode(&memset_nodes[i], graph, nullptr, 0, &mp));
             roots.push_back(memset_nodes[i]);
+            root_is_kernel.push_back(false);
         }
         if (!expr_is_zero(bd.h2d_bytes)) {
-            CK(cudaGraphAddMemcpyNode1D(&h2d_nodes[i], graph, nullptr, 0, (char*)slots[0].buf[i] + eval(bd.h2d_dev_off, unit),
-                                        (char*)ph_in + eval(bd.h2d_host_off, unit), eval(bd.h2d_bytes, unit), kin));
+            if (h2d_sm[i]) {
+                CopyArgs ca;
+                copy_params(ca, 0, (int)i, true, ph_in, unit);
+                CK(cudaGraphAddKernelNode(&h2d_nodes[i], graph, nullptr, 0, &ca.kp));
+            } else {
+                CK(cudaGraphAddMemcpyNode1D(&h2d_nodes[i], graph, nullptr, 0, (char*)slots[0].buf[i] + eval(bd.h2d_dev_off, unit),
+                                            (char*)ph_in + eval(bd.h2d_host_off, unit), eval(bd.h2d_bytes, unit), kin));
+            }
             roots.push_back(h2d_nodes[i]);
+            root_is_kernel.push_back(h2d_sm[i]);
         }
     }
     kern_nodes.resize(stages.size());
@@ -345,16 +419,13 @@ int set_ctx::build_graph() {
         kp.sharedMemBytes = st.smem_bytes;
         kp.kernelParams = ap.ptrs;
         CK(cudaGraphAddKernelNode(&kern_nodes[s], graph, nullptr, 0, &kp));
+        const bool want_pdl = (st.flags & SET_STAGE_PDL) != 0;
         if (s == 0) {
-            for (auto r : roots) CK(cudaGraphAddDependencies(graph, &r, &kern_nodes[s], 1));
-        } else if (st.flags & SET_STAGE_PDL) {
-            cudaGraphEdgeData ed{};
-            ed.from_port = cudaGraphKernelNodePortProgrammatic;
-            ed.to_port = 0;
-            ed.type = cudaGraphDependencyTypeProgrammatic;
-            CK(cudaGraphAddDependencies_v2(graph, &prev, &kern_nodes[s], &ed, 1));
+            // a kernel may have at most one programmatic predecessor worth having: use it only for a lone SM-copy root
+            for (size_t r = 0; r < roots.size(); ++r)
+                CK(depend(roots[r], kern_nodes[s], want_pdl && roots.size() == 1 && root_is_kernel[r]));
         } else {
-            CK(cudaGraphAddDependencies(graph, &prev, &kern_nodes[s], 1));
+            CK(depend(prev, kern_nodes[s], want_pdl));
         }
         prev = kern_nodes[s];
     }
@@ -362,12 +433,19 @@ int set_ctx::build_graph() {
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
         if (!expr_is_zero(bd.d2h_bytes)) {
-            CK(cudaGraphAddMemcpyNode1D(&d2h_nodes[i], graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
-                                        (char*)slots[0].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
+            if (d2h_sm[i]) {
+                CopyArgs ca;
+                copy_params(ca, 0, (int)i, false, ph_out, unit);
+                CK(cudaGraphAddKernelNode(&d2h_nodes[i], graph, nullptr, 0, &ca.kp));
+                CK(depend(prev, d2h_nodes[i], pdl));
+            } else {
+                CK(cudaGraphAddMemcpyNode1D(&d2h_nodes[i], graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
+                                            (char*)slots[0].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
+            }
             leaves.push_back(d2h_nodes[i]);
         }
     }
-    if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished
+    if (flag_poll && fused_signal_buf < 0) {  // completion signal: runs after every D2H copy of the job has finished
         if (leaves.empty()) leaves.push_back(prev);
         uint32_t* flag = flags_dev;
         void* args[1] = {&flag};
@@ -389,6 +467,8 @@ int set_ctx::build_graph() {
 int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
     uint64_t t0 = now_ns();
     bind_thread();
+    std::unique_lock<std::mutex> dl(driver_mu, std::defer_lock);
+    if (driver_lock) dl.lock();
     ExecState& es = execs[exec];
     bool dims_changed = memcmp(es.dims, job.dims, sizeof(es.dims)) != 0;
     bool full = es.bound_slot != slot || dims_changed;
@@ -470,12 +550,26 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
     }
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
-        if (!expr_is_zero(bd.h2d_bytes) && (full || es.in != in))
-            CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
-                                                  (const char*)in + eval(bd.h2d_host_off, job.dims), eval(bd.h2d_bytes, job.dims), kin));
-        if (!expr_is_zero(bd.d2h_bytes) && (full || es.out != out))
-            CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, d2h_nodes[i], (char*)out + eval(bd.d2h_host_off, job.dims),
-                                                  (char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, job.dims), eval(bd.d2h_bytes, job.dims), kout));
+        if (!expr_is_zero(bd.h2d_bytes) && (full || es.in != in)) {
+            if (h2d_sm[i]) {
+                CopyArgs ca;
+                copy_params(ca, slot, (int)i, true, in, job.dims);
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, h2d_nodes[i], &ca.kp));
+            } else {
+                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
+                                                      (const char*)in + eval(bd.h2d_host_off, job.dims), eval(bd.h2d_bytes, job.dims), kin));
+            }
+        }
+        if (!expr_is_zero(bd.d2h_bytes) && (full || es.out != out)) {
+            if (d2h_sm[i]) {
+                CopyArgs ca;
+                copy_params(ca, slot, (int)i, false, out, job.dims);
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, d2h_nodes[i], &ca.kp));
+            } else {
+                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, d2h_nodes[i], (char*)out + eval(bd.d2h_host_off, job.dims),
+                                                      (char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, job.dims), eval(bd.d2h_bytes, job.dims), kout));
+            }
+        }
     }
     es.bound_slot = slot;
     es.in = in;
@@ -499,6 +593,8 @@ static void CUDART_CB set_completion_cb(void* arg) {
 int set_ctx::launch(int exec, int slot, const JobDesc&) {
     bind_thread();
     int s = slot % S;
+    std::unique_lock<std::mutex> dl(driver_mu, std::defer_lock);
+    if (driver_lock) dl.lock();
     SpinLock& lk = stream_locks[s];
     lk.lock();
     cudaError_t e = cudaGraphLaunch(execs[exec].exec, streams[s]);
@@ -514,7 +610,8 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     lk.unlock();
     if (e != cudaSuccess) return cuda_fail(e, "graph launch / event chain", __LINE__);
     kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
-    if (flag_poll) signal_nodes.fetch_add(1, std::memory_order_relaxed);
+    if (n_sm_copies) copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
+    if (signal_node) signal_nodes.fetch_add(1, std::memory_order_relaxed);
     return 0;
 }
 
@@ -557,9 +654,16 @@ int set_ctx::plain_job(int slot, const JobDesc& job) {
         const set_buffer_desc& bd = bufs[i];
         if (bd.flags & SET_BUF_ZERO)
             CK(cudaMemsetAsync((char*)sm.buf[i] + eval(bd.zero_off, job.dims), 0, eval(bd.zero_bytes, job.dims), st));
-        if (!expr_is_zero(bd.h2d_bytes))
-            CK(cudaMemcpyAsync((char*)sm.buf[i] + eval(bd.h2d_dev_off, job.dims), (const char*)job.in + eval(bd.h2d_host_off, job.dims),
-                               eval(bd.h2d_bytes, job.dims), kin, st));
+        if (!expr_is_zero(bd.h2d_bytes)) {
+            if (h2d_sm[i]) {  // the same node list as the job graph, launched one by one
+                CopyArgs ca;
+                copy_params(ca, slot, (int)i, true, job.in, job.dims);
+                CK(cudaLaunchKernel(ca.kp.func, ca.kp.gridDim, ca.kp.blockDim, ca.ptrs, 0, st));
+            } else {
+                CK(cudaMemcpyAsync((char*)sm.buf[i] + eval(bd.h2d_dev_off, job.dims), (const char*)job.in + eval(bd.h2d_host_off, job.dims),
+                                   eval(bd.h2d_bytes, job.dims), kin, st));
+            }
+        }
     }
     for (auto& sd : stages) {
         ArgPack ap;
@@ -571,10 +675,20 @@ int set_ctx::plain_job(int slot, const JobDesc& job) {
     kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
-        if (!expr_is_zero(bd.d2h_bytes))
-            CK(cudaMemcpyAsync((char*)job.out + eval(bd.d2h_host_off, job.dims), (char*)sm.buf[i] + eval(bd.d2h_dev_off, job.dims),
-                               eval(bd.d2h_bytes, job.dims), kout, st));
+        if (!expr_is_zero(bd.d2h_bytes)) {
+            if (d2h_sm[i]) {
+                CopyArgs ca;
+                copy_params(ca, slot, (int)i, false, job.out, job.dims);
+                ca.ctr = nullptr;  // no completion word outside SET mode
+                ca.flag = nullptr;
+                CK(cudaLaunchKernel(ca.kp.func, ca.kp.gridDim, ca.kp.blockDim, ca.ptrs, 0, st));
+            } else {
+                CK(cudaMemcpyAsync((char*)job.out + eval(bd.d2h_host_off, job.dims), (char*)sm.buf[i] + eval(bd.d2h_dev_off, job.dims),
+                                   eval(bd.d2h_bytes, job.dims), kout, st));
+            }
+        }
     }
+    if (n_sm_copies) copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
     CK(cudaEventRecord(sm.done, st));
     sm.used = true;
     return 0;
@@ -593,6 +707,7 @@ int set_ctx::baseline_flush() {
     }
     base_launched.fetch_add(batch.size(), std::memory_order_relaxed);
     kernel_nodes.fetch_add(stages.size() * batch.size(), std::memory_order_relaxed);
+    copy_nodes.fetch_add((uint64_t)n_sm_copies * batch.size(), std::memory_order_relaxed);
     uint64_t t1 = now_ns();
     for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
     uint64_t t2 = now_ns();
@@ -635,6 +750,7 @@ int set_ctx::baseline_submit(const JobDesc& job) {
             }
             base_launched.fetch_add(1, std::memory_order_relaxed);
             kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+            copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
             break;
         }
         default:
@@ -694,6 +810,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (!c) return SET_ERR_NOMEM;
     c->cfg = cfg;
     c->device = dev;
+    if (const char* dlk = getenv("SET_DRIVER_LOCK")) c->driver_lock = dlk[0] == '1';
     c->S = cfg.num_streams;
     c->b = ((cfg.max_inflight + c->S - 1) / c->S) * c->S;
     c->q = cfg.queue_capacity;
@@ -836,6 +953,31 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
             return c->fail(SET_ERR_NOMEM, "pinned placeholder allocation failed");
         }
     }
+    // ---- which copies become SET_K_COPY kernel nodes: fixed size (the grid never changes), at most sm_copy_max_bytes
+    {
+        // default: 256 KiB across the host link; off for SET_IO_DEVICE, where a D2D memcpy node runs on a copy engine
+        // beside the kernels while an SM copy would lengthen the stream's kernel chain (measured, profiles/r1_bench.md)
+        int64_t lim = c->cfg.sm_copy_max_bytes != 0 ? c->cfg.sm_copy_max_bytes : (c->cfg.io == SET_IO_DEVICE ? -1 : 262144);
+        int n_d2h = 0, last_sm = -1;
+        for (size_t i = 0; i < c->bufs.size(); ++i) {
+            const set_buffer_desc& bd = c->bufs[i];
+            auto small = [&](const set_size_expr& e) { return e.per_unit == 0 && e.fixed > 0 && (int64_t)e.fixed <= lim; };
+            c->h2d_sm[i] = small(bd.h2d_bytes);
+            c->d2h_sm[i] = small(bd.d2h_bytes);
+            c->n_sm_copies += (int)c->h2d_sm[i] + (int)c->d2h_sm[i];
+            if (!expr_is_zero(bd.d2h_bytes)) ++n_d2h;
+            if (c->d2h_sm[i]) last_sm = (int)i;
+        }
+        if (c->flag_poll && n_d2h == 1 && last_sm >= 0) c->fused_signal_buf = last_sm;
+        for (auto& st : c->stages) c->pdl = c->pdl || (st.flags & SET_STAGE_PDL);
+        if (c->fused_signal_buf >= 0) {
+            size_t bytes = (size_t)c->b * kFlagStride * sizeof(uint32_t);
+            if (cudaMalloc((void**)&c->ctrs_dev, bytes) != cudaSuccess || cudaMemset(c->ctrs_dev, 0, bytes) != cudaSuccess) {
+                cudaGetLastError();
+                return c->fail(SET_ERR_NOMEM, "counter allocation failed");
+            }
+        }
+    }
     if (int rc = c->build_graph()) return rc;
 
     // ---- bounded pool of graph executables: q+1 per slot, each re-bound to its slot's M_w
@@ -929,6 +1071,7 @@ set_status set_destroy(set_ctx* c) {
     if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
     if (c->flags_host) cudaFreeHost(c->flags_host);
+    if (c->ctrs_dev) cudaFree(c->ctrs_dev);
     for (int s = 0; s < c->S; ++s) {
         if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
         if (c->notify[s]) cudaStreamDestroy(c->notify[s]);
@@ -1001,6 +1144,7 @@ set_status set_get_stats(set_ctx* c, set_stats* out) {
     out->staged_jobs = c->staged_jobs.load();
     out->kernel_nodes = c->kernel_nodes.load();
     out->signal_nodes = c->signal_nodes.load();
+    out->copy_nodes = c->copy_nodes.load();
     out->ns_bind = c->ns_bind.load();
     out->ns_sync = c->ns_sync.load();
     return SET_OK;
@@ -1014,7 +1158,7 @@ set_status set_reset_stats(set_ctx* c) {
         st.ns_submit = 0; st.ns_launch = 0; st.ns_callback = 0; st.max_inflight = 0;
     }
     c->base_submitted = 0; c->base_completed = 0; c->base_launched = 0; c->base_ns_submit = 0; c->base_ns_launch = 0;
-    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
+    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->copy_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
     return SET_OK;
 }
 

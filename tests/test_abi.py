@@ -53,6 +53,15 @@ def test_builtin_descriptors_roundtrip_struct_layout(libset):
     assert libset.load().set_builtin_kernel(99) is None
 
 
+def test_every_builtin_kernel_id_in_the_header_resolves(libset):
+    text = open(os.path.join(ROOT, "include", "set.h")).read()
+    ids = {name: int(v) for name, v in re.findall(r"#define\s+(SET_K_[A-Z0-9_]+)\s+(\d+)", text)}
+    assert len(ids) >= 15 and sorted(ids.values()) == list(range(1, len(ids) + 1))
+    lib = libset.load()
+    for name, v in ids.items():
+        assert lib.set_builtin_kernel(v), f"{name} = {v} has no entry in set_builtin_kernel()"
+
+
 def test_struct_sizes_match_header(libset):
     assert C.sizeof(libset.SizeExpr) == 24 and C.sizeof(libset.GridRule) == 32 and C.sizeof(libset.Tmap2D) == 40
     assert C.sizeof(libset.ArgDesc) == 8 + 24 + 8 + 40

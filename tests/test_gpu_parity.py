@@ -12,12 +12,12 @@ pytestmark = pytest.mark.gpu
 SENTINEL = 0xA5
 
 
-def run_jobs(setlib, wl, job_ids, mode=0, pageable=False, io_check=True, **ctx_kw):
+def run_jobs(setlib, wl, job_ids, mode=0, pageable=False, io_check=True, pdl=False, misalign=0, **ctx_kw):
     """Submit the jobs through the C ABI; returns (list of output uint8 arrays, list of input images, dims, stats)."""
     from paper_2606_05495_b200.workloads import PinnedArena
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=mode, **ctx_kw)
     try:
-        ctx.register_builtin(wl.config, wl.variant, list(wl.params))
+        ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=pdl)
         ins = [wl.make_input(j) for j in job_ids]
         dims = [wl.dims(j) for j in job_ids]
         if "spin_ns" in wl.extra:
@@ -33,13 +33,14 @@ def run_jobs(setlib, wl, job_ids, mode=0, pageable=False, io_check=True, **ctx_k
             arena = PinnedArena(ctx, sum(in_sz) + sum(out_sz) + (2 * len(ins) + 2) * (pad + 256) + 4096)
             arena.view[:] = SENTINEL
             in_bufs, out_bufs = [], []
+            m = misalign  # byte offset that breaks the 16-byte alignment the vector paths want
             for x, n in zip(ins, in_sz):
                 a, v = arena.take(n + pad)
-                v[:n] = x
-                in_bufs.append(v[:n])
+                v[m:m + n] = x
+                in_bufs.append(v[m:m + n])
             for n in out_sz:
                 a, v = arena.take(n + pad)
-                out_bufs.append(v[:n])
+                out_bufs.append(v[m:m + n])
         for k, j in enumerate(job_ids):
             ctx.submit(j, in_bufs[k].ctypes.data, out_bufs[k].ctypes.data, dims[k] if wl.config == 4 or "spin_ns" in wl.extra else None)
         ctx.drain()
@@ -206,8 +207,38 @@ def test_every_completion_mode_delivers_every_job(libset, cb, disp):
     for config in (0, 4):
         wl = small_workload(config)
         st = check(libset, wl, list(range(wl.jobs)), callback_mode=cb, num_dispatchers=disp)
-        assert st["signal_nodes"] == (wl.jobs if cb == 3 else 0)
+        # config 0: its one D2H copy is an SM copy node that carries the completion word itself; config 4 has two D2H copies
+        assert st["signal_nodes"] == (wl.jobs if cb == 3 and config == 4 else 0)
+        assert st["copy_nodes"] == wl.jobs * (2 if config == 0 else 1)
         assert st["max_inflight_seen"] <= wl.max_inflight
+
+
+@pytest.mark.parametrize("config", [0, 1, 4])
+@pytest.mark.parametrize("sm_copy", [-1, 0, 4096])
+@pytest.mark.parametrize("pdl", [False, True])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_graph_shapes_compute_the_same(libset, config, sm_copy, pdl, mode):
+    """Copy-engine memcpy nodes or SM copy nodes (set_config.sm_copy_max_bytes), ordinary or programmatic (PDL) edges:
+    the job graph's result is the same in SET and in the baseline models that share the graph."""
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(config)
+    st = check(libset, wl, list(range(min(wl.jobs, 48))), mode=mode, sm_copy_max_bytes=sm_copy, pdl=pdl)
+    if sm_copy == -1:
+        assert st["copy_nodes"] == 0
+
+
+@pytest.mark.parametrize("misalign", [4, 1])
+def test_sm_copies_with_unaligned_pinned_pointers(libset, misalign):
+    from paper_2606_05495_b200.workloads import Workload
+    check(libset, Workload(0, (1001,), jobs=12, num_streams=2, max_inflight=4), list(range(12)), misalign=misalign, pdl=True)
+
+
+def test_sm_copy_completion_signal_survives_many_jobs_per_slot(libset):
+    """The fused copy+signal node counts its blocks in a per-slot device word that the last block resets: 600 jobs over
+    4 slots, outputs of three blocks each (config 0 with n = 5000 -> 20,256 bytes)."""
+    from paper_2606_05495_b200.workloads import Workload
+    st = check(libset, Workload(0, (5000,), jobs=600, num_streams=2, max_inflight=4), list(range(600)), pdl=True)
+    assert st["signal_nodes"] == 0 and st["copy_nodes"] == 1200
 
 
 def test_submit_before_register_and_double_register(libset):
