@@ -606,7 +606,7 @@ def main():
                     log(f"[bench]   {wl.config} set/{name:24s} {'device' if io_device else 'host  '} {r['jobs_per_s']:12.1f} jobs/s")
             extra["graph_variants"] = gv
             base = {}
-            for mode in ("batch_sync_graphs", "plain_streams", "single_graph"):
+            for mode in ("batch_sync_graphs", "plain_streams", "single_graph", "mutex_queue"):
                 for io_device in (False, True):
                     r = arm(wl, ids, mode, io_device, verify=2)
                     base[f"{mode}_{'device' if io_device else 'e2e'}"] = {"jobs_per_s": round(r["jobs_per_s"], 1),

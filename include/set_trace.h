@@ -39,7 +39,7 @@ typedef struct set_trace_stats {
     double idle_frac;          /* t_schedule / T = 1 - busy/wall                                       */
     double kernel_mean_us;     /* mean duration of the stage kernels (signal kernels excluded)         */
     double sum_op_us;          /* sum of all op durations (> busy_us when streams overlap)             */
-    set_gap_summary kernel_kernel; /* stage kernel -> next stage kernel, nothing else between them:
+    set_gap_summary kernel_kernel; /* stage kernel -> next stage kernel of the SAME job, nothing else between them:
                                       the "inter-kernel gap" of BASELINE.json:metric                   */
     set_gap_summary intra_job; /* consecutive ops of ONE job (same launch correlation id)              */
     set_gap_summary inter_job; /* last op of a job -> first op of the next job on that stream          */

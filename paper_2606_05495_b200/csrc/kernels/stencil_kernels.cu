@@ -95,6 +95,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_jacobi5_f32(const float*
 // ------------------------------------------------------------------------------------------------------------
 extern "C" __global__ void __launch_bounds__(256) set_k_rgb2gray_u8(const uint8_t* __restrict__ rgb, uint8_t* __restrict__ gray,
                                                                     uint32_t w, uint32_t h) {
+    set_pdl_sync();
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     if (p0 + 15 < npix) {
@@ -122,60 +123,80 @@ extern "C" __global__ void __launch_bounds__(256) set_k_rgb2gray_u8(const uint8_
 
 // ------------------------------------------------------------------------------------------------------------
 // K11: 3x3 blur [1 2 1; 2 4 2; 1 2 1] >> 4, clamp-to-edge.  Evaluated separably -- horizontal [1 2 1] sums per
-// row (<= 1020), then vertical [1 2 1] and ONE final >> 4 -- which is exactly the 2-D form in integers.
-// blockDim = (32, 8): a warp covers 128 pixels x 8 rows, 4 pixels per lane as one 32-bit word; the horizontal
-// neighbours come from adjacent lanes by shuffle; the three row sums roll through registers.
+// row (<= 1020), then vertical [1 2 1] (<= 4080) and ONE final >> 4 -- which is exactly the 2-D form in integers.
+// blockDim = (32, 8), tile = 512 pixels x 32 rows: a lane owns 16 pixels (one 128-bit word) of 4 consecutive rows.
+// All six input rows of a lane (4 + the row above and below) are loaded before the first add, so 96 bytes per
+// thread are in flight; horizontal neighbours come from the adjacent lanes by shuffle.  Sums are kept as two 16-bit
+// halves per register (even pixels / odd pixels of a 32-bit word): every partial sum fits 16 bits, so packed adds
+// never carry between the halves.
 // ------------------------------------------------------------------------------------------------------------
 namespace {
-struct HSum {
-    int s[4];
+struct HRow {
+    uint32_t ev[4], od[4];  // horizontal sums of the even (b0, b2) and odd (b1, b3) pixels of each 32-bit word
 };
-__device__ __forceinline__ HSum hrow(const uint8_t* __restrict__ g, uint32_t w, uint32_t r, uint32_t x4, bool active, int lane) {
-    const uint8_t* row = g + (size_t)r * w;
-    uint32_t word = active ? __ldg(reinterpret_cast<const uint32_t*>(row + x4)) : 0u;
-    uint32_t left = __shfl_up_sync(0xffffffffu, word >> 24, 1);
-    uint32_t right = __shfl_down_sync(0xffffffffu, word & 0xffu, 1);
-    if (active) {
-        if (lane == 0) left = (x4 > 0) ? row[x4 - 1] : (word & 0xffu);             // clamp at the left edge
-        if (lane == 31 || x4 + 4 >= w) right = (x4 + 4 < w) ? row[x4 + 4] : (word >> 24);  // clamp at the right edge
+// wd: the lane's 16 pixels; lb / rb: the pixel left of b0 and right of b15 (already clamped at the image edge)
+__device__ __forceinline__ HRow hsum16(const uint4& wd, uint32_t lb, uint32_t rb) {
+    const uint32_t x[4] = {wd.x, wd.y, wd.z, wd.w};
+    HRow h;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t ev = x[k] & 0x00ff00ffu, od = (x[k] >> 8) & 0x00ff00ffu;
+        const uint32_t prev_b3 = k == 0 ? lb : x[k - 1] >> 24;
+        const uint32_t next_b0 = k == 3 ? rb : x[k + 1] & 0xffu;
+        h.ev[k] = ((od << 16) | prev_b3) + 2u * ev + od;            // (b-1 + 2 b0 + b1, b1 + 2 b2 + b3)
+        h.od[k] = ev + 2u * od + ((ev >> 16) | (next_b0 << 16));    // (b0 + 2 b1 + b2, b2 + 2 b3 + b4)
     }
-    int p0 = word & 0xff, p1 = (word >> 8) & 0xff, p2 = (word >> 16) & 0xff, p3 = word >> 24;
-    HSum h;
-    h.s[0] = (int)left + 2 * p0 + p1;
-    h.s[1] = p0 + 2 * p1 + p2;
-    h.s[2] = p1 + 2 * p2 + p3;
-    h.s[3] = p2 + 2 * p3 + (int)right;
     return h;
 }
 }  // namespace
 
 extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t* __restrict__ g, uint8_t* __restrict__ out, uint32_t w,
                                                                    uint32_t h) {
-    if ((w & 3u) == 0) {
-        const int lane = threadIdx.x;
-        const uint32_t x4 = (blockIdx.x * 32u + lane) * 4u;
-        const bool active = x4 < w;
-        const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 8u;
+    set_pdl_sync();
+    const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
+    if ((w & 15u) == 0) {
+        const uint32_t lane = threadIdx.x;
+        const uint32_t x16 = (blockIdx.x * 32u + lane) * 16u;
+        const bool active = x16 < w;
         if (r0 >= h) return;  // warp-uniform
-        const uint32_t r1 = min(r0 + 8u, h);
-        HSum up = hrow(g, w, r0 > 0 ? r0 - 1 : 0, x4, active, lane);
-        HSum mid = hrow(g, w, r0, x4, active, lane);
-        for (uint32_t r = r0; r < r1; ++r) {
-            HSum down = hrow(g, w, min(r + 1, h - 1), x4, active, lane);
-            if (active) {
-                uint32_t o = 0;
+        uint4 wd[6];
+        uint32_t le[6], re[6];  // edge pixels fetched from memory by the warp's first / last lane
 #pragma unroll
-                for (int k = 0; k < 4; ++k) o |= (uint32_t)((up.s[k] + 2 * mid.s[k] + down.s[k]) >> 4) << (8 * k);
-                *reinterpret_cast<uint32_t*>(out + (size_t)r * w + x4) = o;
-            }
-            up = mid;
-            mid = down;
+        for (int k = 0; k < 6; ++k) {
+            const uint32_t rr = min(max((int)r0 - 1 + k, 0), (int)h - 1);  // clamp-to-edge rows
+            const uint8_t* row = g + (size_t)rr * w;
+            wd[k] = active ? __ldg(reinterpret_cast<const uint4*>(row + x16)) : make_uint4(0, 0, 0, 0);
+            le[k] = (active && lane == 0 && x16 > 0) ? __ldg(row + x16 - 1) : 0u;
+            re[k] = (active && lane == 31 && x16 + 16 < w) ? __ldg(row + x16 + 16) : 0u;
         }
-    } else {  // ragged width: per-pixel 9-tap with explicit clamping
-        const uint32_t x0 = (blockIdx.x * 32u + threadIdx.x) * 4u;
-        const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 8u;
-        for (uint32_t r = r0; r < min(r0 + 8u, h); ++r)
-            for (uint32_t x = x0; x < min(x0 + 4u, w); ++x) {
+        HRow hr[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            uint32_t lb = __shfl_up_sync(0xffffffffu, wd[k].w >> 24, 1);
+            uint32_t rb = __shfl_down_sync(0xffffffffu, wd[k].x & 0xffu, 1);
+            if (lane == 0) lb = x16 > 0 ? le[k] : (wd[k].x & 0xffu);             // clamp at the left edge
+            if (x16 + 16 >= w) rb = wd[k].w >> 24;                                // clamp at the right edge
+            else if (lane == 31) rb = re[k];
+            hr[k] = hsum16(wd[k], lb, rb);
+        }
+        if (!active) return;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (r0 + k < h) {
+                uint32_t o[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t ve = hr[k].ev[q] + 2u * hr[k + 1].ev[q] + hr[k + 2].ev[q];
+                    const uint32_t vo = hr[k].od[q] + 2u * hr[k + 1].od[q] + hr[k + 2].od[q];
+                    o[q] = ((ve >> 4) & 0x00ff00ffu) | (((vo >> 4) & 0x00ff00ffu) << 8);
+                }
+                *reinterpret_cast<uint4*>(out + (size_t)(r0 + k) * w + x16) = make_uint4(o[0], o[1], o[2], o[3]);
+            }
+        }
+    } else {  // ragged width (rows are not 16-byte aligned): per-pixel 9-tap with explicit clamping over the same tile
+        const uint32_t x0 = (blockIdx.x * 32u + threadIdx.x) * 16u;
+        for (uint32_t r = r0; r < min(r0 + 4u, h); ++r)
+            for (uint32_t x = x0; x < min(x0 + 16u, w); ++x) {
                 int acc = 0;
 #pragma unroll
                 for (int dy = -1; dy <= 1; ++dy)
@@ -196,6 +217,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t
 // ------------------------------------------------------------------------------------------------------------
 extern "C" __global__ void __launch_bounds__(256) set_k_hist256_u8(const uint8_t* __restrict__ p, uint32_t* __restrict__ hist,
                                                                    uint32_t w, uint32_t h) {
+    set_pdl_sync();
     const uint32_t n = w * h;
     __shared__ uint32_t sh[8][256];
     const int tid = threadIdx.x, wid = tid >> 5;

@@ -13,9 +13,11 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <condition_variable>
 #include <deque>
 #include <memory>
 #include <mutex>
+#include <thread>
 #include <vector>
 
 #include "../../include/set.h"
@@ -143,8 +145,15 @@ struct set_ctx final : public Backend {
     // baseline state (single caller thread)
     std::vector<JobDesc> batch;
     uint64_t base_ticket = 0;
-    std::mutex mq_mu;                 // SET_MODE_MUTEX_QUEUE: the global issue queue's lock
+    // SET_MODE_MUTEX_QUEUE: one global issue queue behind a mutex; a worker thread scans all
+    // b slots every round (O(b) cudaEventQuery calls), and feeds each free slot from the queue.
+    std::mutex mq_mu;
+    std::condition_variable mq_cv;
     std::deque<JobDesc> mq_queue;
+    std::thread mq_thread;
+    std::atomic<bool> mq_stop{false};
+    std::atomic<uint64_t> mq_queries{0};
+    void mq_loop();
 
     // ------------------------------------------------------------------ errors
     int fail(int code, const char* fmt, ...) {
@@ -753,6 +762,17 @@ int set_ctx::baseline_submit(const JobDesc& job) {
             copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
             break;
         }
+        case SET_MODE_MUTEX_QUEUE: {
+            if (cfg.io == SET_IO_HOST && (!is_pinned(job.in) || !is_pinned(job.out)))
+                return fail(SET_ERR_INVALID, "baseline modes need pinned host buffers");
+            std::unique_lock<std::mutex> g(mq_mu);
+            mq_cv.wait(g, [&] { return (int)mq_queue.size() < b * q || err.load() != 0; });  // bounded like SET's queues
+            if (int e = err.load()) return e;
+            mq_queue.push_back(job);
+            g.unlock();
+            mq_cv.notify_all();
+            break;
+        }
         default:
             return fail(SET_ERR_INVALID, "mode %d not implemented", cfg.mode);
     }
@@ -761,10 +781,78 @@ int set_ctx::baseline_submit(const JobDesc& job) {
     return rc;
 }
 
+void set_ctx::mq_loop() {
+    bind_thread();
+    std::vector<char> busy((size_t)b, 0);
+    std::vector<JobDesc> running((size_t)b);
+    while (!mq_stop.load(std::memory_order_acquire)) {
+        bool progressed = false;
+        for (int w = 0; w < b; ++w) {  // O(b) host-side completion queries per round
+            if (busy[w]) {
+                cudaError_t e = cudaEventQuery(slots[w].done);
+                mq_queries.fetch_add(1, std::memory_order_relaxed);
+                if (e == cudaErrorNotReady) continue;
+                if (e != cudaSuccess) cuda_fail(e, "cudaEventQuery", __LINE__);
+                finish(w * epp, w, running[w]);
+                busy[w] = 0;
+                base_completed.fetch_add(1, std::memory_order_release);
+                progressed = true;
+                mq_cv.notify_all();
+            }
+            JobDesc j;
+            {
+                std::lock_guard<std::mutex> g(mq_mu);  // the shared queue's lock, taken for every dispatch
+                if (mq_queue.empty()) continue;
+                j = mq_queue.front();
+                mq_queue.pop_front();
+            }
+            mq_cv.notify_all();
+            uint64_t t0 = now_ns();
+            bool dummy;
+            int rc = err.load() ? err.load() : bind(w * epp, w, j, &dummy);
+            if (rc == 0) {
+                cudaError_t e = cudaGraphLaunch(execs[w * epp].exec, streams[w % S]);
+                if (e == cudaSuccess) e = cudaEventRecord(slots[w].done, streams[w % S]);
+                if (e != cudaSuccess) rc = cuda_fail(e, "graph launch (queue model)", __LINE__);
+            }
+            base_ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+            if (rc != 0) {  // keep the books balanced so that drain returns
+                base_completed.fetch_add(1, std::memory_order_release);
+                mq_cv.notify_all();
+                continue;
+            }
+            running[w] = j;
+            busy[w] = 1;
+            base_launched.fetch_add(1, std::memory_order_relaxed);
+            kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
+            copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
+            progressed = true;
+        }
+        if (!progressed) {
+            bool any = false;
+            for (int w = 0; w < b; ++w) any = any || busy[w];
+            if (!any) {  // nothing in flight and nothing queued: sleep until a submit arrives
+                std::unique_lock<std::mutex> g(mq_mu);
+                mq_cv.wait_for(g, std::chrono::milliseconds(1), [&] { return !mq_queue.empty() || mq_stop.load(); });
+            } else {
+                cpu_relax();
+            }
+        }
+    }
+}
+
 int set_ctx::baseline_drain() {
     bind_thread();
     if (cfg.mode == SET_MODE_BATCH_SYNC)
         if (int rc = baseline_flush()) return rc;
+    if (cfg.mode == SET_MODE_MUTEX_QUEUE) {
+        uint64_t t0 = now_ns();
+        std::unique_lock<std::mutex> g(mq_mu);
+        while (base_completed.load(std::memory_order_acquire) < base_submitted.load() && err.load() == 0)
+            mq_cv.wait_for(g, std::chrono::microseconds(200));
+        ns_sync.fetch_add(now_ns() - t0, std::memory_order_relaxed);
+        return err.load();
+    }
     uint64_t t0 = now_ns();
     for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
     ns_sync.fetch_add(now_ns() - t0, std::memory_order_relaxed);
@@ -856,7 +944,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
         memset(c->flags_host, 0, bytes);
         c->flag_poll = true;
     }
-    if (cfg.mode == SET_MODE_SET || cfg.mode == SET_MODE_MUTEX_QUEUE)
+    if (cfg.mode == SET_MODE_SET)
         c->sched.reset(new Scheduler(c, c->S, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
     *out = c;
     return SET_OK;
@@ -981,10 +1069,10 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     if (int rc = c->build_graph()) return rc;
 
     // ---- bounded pool of graph executables: q+1 per slot, each re-bound to its slot's M_w
-    int nexec = (c->cfg.mode == SET_MODE_SET || c->cfg.mode == SET_MODE_MUTEX_QUEUE) ? c->b * c->epp : c->b * c->epp;
+    int nexec = c->b * c->epp;
     c->execs.resize(nexec);
     for (int e = 0; e < nexec; ++e) {
-        bool needed = (c->cfg.mode == SET_MODE_SET || c->cfg.mode == SET_MODE_MUTEX_QUEUE) || (e % c->epp == 0);
+        bool needed = c->cfg.mode == SET_MODE_SET || (e % c->epp == 0);
         if (c->cfg.mode == SET_MODE_PLAIN_STREAMS) needed = false;
         if (!needed) continue;
         cudaError_t er = cudaGraphInstantiate(&c->execs[e].exec, c->graph, 0);
@@ -1006,6 +1094,7 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     c->host_rebinds.store(0);
     c->ns_bind.store(0);
     c->registered = true;
+    if (c->cfg.mode == SET_MODE_MUTEX_QUEUE) c->mq_thread = std::thread([c] { c->mq_loop(); });
     return SET_OK;
 }
 
@@ -1054,6 +1143,11 @@ set_status set_destroy(set_ctx* c) {
     cudaSetDevice(c->device);
     if (c->registered && c->err.load() == 0) set_drain(c);
     if (c->sched) c->sched->stop();
+    if (c->mq_thread.joinable()) {
+        c->mq_stop.store(true);
+        c->mq_cv.notify_all();
+        c->mq_thread.join();
+    }
     for (auto s : c->streams) cudaStreamSynchronize(s);
     for (auto s : c->notify) cudaStreamSynchronize(s);  // host functions have returned after this
     for (auto& es : c->execs) {

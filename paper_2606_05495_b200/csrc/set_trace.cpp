@@ -71,6 +71,16 @@ int load_cupti() {
 
 constexpr size_t kBufBytes = 8u << 20;
 
+// kernel names seen, for the optional raw dump (SET_TRACE_DUMP=<file>: one CSV line per record)
+std::vector<std::string> g_names{""};
+uint32_t name_id(const char* n) {
+    if (!n) return 0;
+    for (size_t i = 1; i < g_names.size(); ++i)
+        if (g_names[i] == n) return (uint32_t)i;
+    g_names.emplace_back(n);
+    return (uint32_t)g_names.size() - 1;
+}
+
 void CUPTIAPI buffer_requested(uint8_t** buffer, size_t* size, size_t* max_records) {
     void* p = nullptr;
     if (posix_memalign(&p, 8, kBufBytes) != 0) p = nullptr;
@@ -92,6 +102,7 @@ void CUPTIAPI buffer_completed(CUcontext ctx, uint32_t stream_id, uint8_t* buffe
                     r.stream = k->streamId;
                     r.job = k->correlationId;
                     r.kind = (k->name && strstr(k->name, "set_k_signal")) ? 1u : 0u;
+                    r.reserved = name_id(k->name);
                     r.start_ns = k->start;
                     r.end_ns = k->end;
                     break;
@@ -177,7 +188,7 @@ extern "C" int set_trace_reduce(const set_trace_rec* recs, uint64_t n, set_trace
         const set_trace_rec& p = v[i - 1];
         double gap = r.start_ns > p.end_ns ? (double)(r.start_ns - p.end_ns) * 1e-3 : 0.0;
         any.push_back(gap);
-        if (p.kind == 0 && r.kind == 0) kk.push_back(gap);
+        if (p.kind == 0 && r.kind == 0 && p.job == r.job) kk.push_back(gap);
         (p.job == r.job ? intra : inter).push_back(gap);
     }
     // union of all activity intervals, over all streams
@@ -244,6 +255,15 @@ extern "C" int set_trace_stop(set_trace_stats* out) {
         std::lock_guard<std::mutex> lk(g_mu);
         recs.swap(g_recs);
         dropped = g_dropped;
+    }
+    if (const char* path = getenv("SET_TRACE_DUMP")) {
+        if (FILE* f = fopen(path, "a")) {
+            fprintf(f, "# stream,job,kind,start_ns,end_ns,name\n");
+            for (auto& r : recs)
+                fprintf(f, "%u,%u,%u,%llu,%llu,%s\n", r.stream, r.job, r.kind, (unsigned long long)r.start_ns, (unsigned long long)r.end_ns,
+                        r.reserved < g_names.size() ? g_names[r.reserved].c_str() : "");
+            fclose(f);
+        }
     }
     int rc = set_trace_reduce(recs.data(), recs.size(), out);
     if (rc == 0 && out) out->dropped = dropped;

@@ -101,7 +101,7 @@ def test_parity_small(libset, config):
 
 
 @pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
-@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 def test_baseline_models_compute_the_same(libset, config, mode):
     from paper_2606_05495_b200.workloads import small_workload
     wl = small_workload(config)
@@ -142,7 +142,7 @@ def test_config3_ragged_shapes(libset, m, n, k):
     check(libset, Workload(3, (m, n, k), jobs=3, num_streams=2, max_inflight=4), list(range(3)))
 
 
-@pytest.mark.parametrize("size", [(1, 1), (5, 4), (7, 3), (128, 64), (132, 65), (644, 9)])
+@pytest.mark.parametrize("size", [(1, 1), (5, 4), (7, 3), (128, 64), (132, 65), (644, 9), (16, 1), (512, 33), (528, 40), (1040, 37), (1920, 3)])
 def test_config4_ragged_frames(libset, size):
     from paper_2606_05495_b200.workloads import Workload
     wl = Workload(4, (1920, 1080), jobs=3, num_streams=2, max_inflight=4, extra={"size": size})

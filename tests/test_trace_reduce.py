@@ -52,8 +52,8 @@ def test_streams_are_separate_and_overlap_counts_once(trace):
     # stream 1: [0,10] [20,30]; stream 2: [5,25]  -> union [0,30] is fully busy, yet stream 1 has a 10 us gap
     st = trace.reduce([(1, 1, K, 0, 10_000), (1, 2, K, 20_000, 30_000), (2, 3, K, 5_000, 25_000)])
     assert st["streams"] == 2 and st["busy_us"] == 30.0 and st["idle_frac"] == 0.0 and st["sum_op_us"] == 40.0
-    assert st["kernel_kernel"]["count"] == 1 and st["kernel_kernel"]["mean_us"] == 10.0
-    assert st["inter_job"]["count"] == 1 and st["intra_job"]["count"] == 0
+    assert st["kernel_kernel"]["count"] == 0               # the two kernels of stream 1 belong to different jobs
+    assert st["inter_job"]["count"] == 1 and st["inter_job"]["mean_us"] == 10.0 and st["intra_job"]["count"] == 0
 
 
 def test_overlapping_ops_on_one_stream_give_zero_gap_and_empty_input(trace):
@@ -68,7 +68,7 @@ def test_percentiles(trace):
     K = trace.KIND_KERNEL
     recs, t = [], 0
     for i in range(101):                                    # gaps 0,1,...,99 us between 1 us kernels
-        recs.append((3, i, K, t, t + 1000))
+        recs.append((3, 9, K, t, t + 1000))               # one job: kernel->kernel gaps are counted inside a job only
         t += 1000 + i * 1000
     kk = trace.reduce(recs)["kernel_kernel"]
     assert kk["count"] == 100 and kk["p50_us"] == 50.0 and kk["p99_us"] == 98.0 and kk["max_us"] == 99.0 and kk["mean_us"] == 49.5
