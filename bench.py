@@ -463,6 +463,30 @@ def gap_pass(setlib, wl, ids, all_configs: bool, warmup: int):
     return out
 
 
+def batch_sweep(setlib, wl, ids, flush, trace_ok: bool):
+    """SURVEY.md 8(f)2 / PAPER.md:274-288 (Fig. 5-6): throughput of SET and of the batch-synchronous baseline against the
+    batch size b = max_inflight, streams fixed at the workload's S (b < S: b streams).  End to end, pinned host buffers."""
+    import copy
+    out = {"workload": wl.name, "jobs": min(len(ids), 4000), "b": {}}
+    job_ids = ids[:out["jobs"]]
+    p, r = LAYOUT[wl.config]
+    for b in (1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024):
+        w = copy.copy(wl)
+        w.max_inflight, w.num_streams = b, min(b, wl.num_streams)
+        row = {}
+        for mode in ("set", "batch_sync_graphs"):
+            try:
+                res = run_arm(setlib, w, job_ids, mode, False, 3, 2, p, max(r, 0), verify=0, flush=flush)
+                row[mode] = round(res["jobs_per_s"], 1)
+            except Exception as e:
+                row[mode] = {"error": str(e)[:120]}
+        if all(isinstance(v, float) for v in row.values()):
+            row["speedup"] = round(row["set"] / row["batch_sync_graphs"], 3)
+        out["b"][str(b)] = row
+        log(f"[bench]   sweep b={b:5d} S={w.num_streams}: {row}")
+    return out
+
+
 def workload_for(config, jobs_override=None):
     from paper_2606_05495_b200.workloads import baseline_workload
     wl = baseline_workload(config)
@@ -522,6 +546,7 @@ def main():
     ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
     ap.add_argument("--sm-copy", type=int, default=0, help="set_config.sm_copy_max_bytes: 0 = library default, -1 = copy engines only")
     ap.add_argument("--pdl", type=int, default=1, help="1: programmatic-dependent-launch edges between kernel nodes (default), 0: plain edges")
+    ap.add_argument("--sweep", action="store_true", help="also sweep the batch size b (PAPER.md Fig. 5-6) on the headline workload")
     ap.add_argument("--out", default=None, help="also write the JSON line to this file")
     args = ap.parse_args()
     OPTS["sm_copy_max_bytes"], OPTS["pdl"] = args.sm_copy, bool(args.pdl)
@@ -643,6 +668,8 @@ def main():
                     others[f"config{c}"] = {"error": str(e)[:300]}
                     log(f"[bench] config {c} failed: {e}")
             extra["workloads"] = others
+    if world == 1 and args.sweep:
+        extra["batch_sweep"] = batch_sweep(setlib, wl, ids, flush, not args.no_gaps)
     sampler.stop()
     clocks = sampler.summary(windows)
     if world == 1 and not args.no_gaps:

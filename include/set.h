@@ -180,9 +180,7 @@ typedef struct set_config {
     int32_t sm_copy_max_bytes;/* H2D/D2H copies of a fixed size up to this many bytes become kernel nodes
                                  (SET_K_COPY: the SMs read/write pinned host memory over the link) instead of
                                  copy-engine memcpy nodes; 0 => default (262144 under SET_IO_HOST, never under
-                                 SET_IO_DEVICE), -1 => never.  One D2H copy
-                                 done this way also carries the SET_CB_FLAG_POLL completion signal.
-                                 DESIGN.md "SM copies"                                                  */
+                                 SET_IO_DEVICE), -1 => never.                    */
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */
@@ -305,9 +303,8 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_HIST256_U8     12  /* (const uint8* p, uint32* hist, uint32 w, uint32 h)  hist must be zeroed  */
 #define SET_K_SPIN           13  /* (uint32* scratch, uint32 ns)  debug delay stage (busy-waits ns)          */
 #define SET_K_SIGNAL         14  /* (uint32* flag)  *flag = 1 in mapped pinned HOST memory (SET_CB_FLAG_POLL) */
-#define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes, uint32* ctr, uint32* flag)
-                                    copy by the SMs; src/dst may be pinned HOST or DEVICE memory; flag != NULL:
-                                    the last block stores *flag = 1 after every block's data is visible       */
+#define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes)  copy by the SMs; src / dst may be
+                                    pinned HOST or DEVICE memory                                              */
 
 /* HOST address usable as set_stage_desc.func, or NULL for an unknown id. */
 const void *set_builtin_kernel(int kernel_id);

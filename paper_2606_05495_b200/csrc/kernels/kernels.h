@@ -19,7 +19,7 @@ __global__ void set_k_blur3x3_u8(const uint8_t* g, uint8_t* out, uint32_t w, uin
 __global__ void set_k_hist256_u8(const uint8_t* p, uint32_t* hist, uint32_t w, uint32_t h);
 __global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
 __global__ void set_k_signal(uint32_t* flag);
-__global__ void set_k_copy(const void* src, void* dst, uint32_t bytes, uint32_t* done_ctr, uint32_t* flag);
+__global__ void set_k_copy(const void* src, void* dst, uint32_t bytes);
 }
 
 // Programmatic dependent launch (SET_STAGE_PDL edges of the job graph): let the next kernel node be scheduled now,

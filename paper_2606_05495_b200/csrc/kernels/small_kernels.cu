@@ -179,9 +179,16 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_block_sum_f32(const flo
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     float acc = 0.0f;
     const uint32_t n4 = n / 4;
-    for (uint32_t i = tid; i < n4; i += 1024) {
-        float4 v = reinterpret_cast<const float4*>(y)[i];
-        acc = __fadd_rn(acc, __fadd_rn(__fadd_rn(v.x, v.y), __fadd_rn(v.z, v.w)));
+    // four strided float4 loads in flight per thread; the adds keep the order i = tid, tid + 1024, ... so the tree (and
+    // the result, bit for bit) is the one a plain loop gives
+    for (uint32_t i = tid; i < n4; i += 4096) {
+        float4 v[4];
+#pragma unroll
+        for (uint32_t k = 0; k < 4; ++k)
+            v[k] = (i + k * 1024u < n4) ? reinterpret_cast<const float4*>(y)[i + k * 1024u] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (uint32_t k = 0; k < 4; ++k)
+            if (i + k * 1024u < n4) acc = __fadd_rn(acc, __fadd_rn(__fadd_rn(v[k].x, v[k].y), __fadd_rn(v[k].z, v[k].w)));
     }
     for (uint32_t i = n4 * 4 + tid; i < n; i += 1024) acc = __fadd_rn(acc, y[i]);
 #pragma unroll
@@ -207,12 +214,15 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
     if (scratch) scratch[0] = (uint32_t)(t - t0);
 }
 
-// K14: completion signal of SET_CB_FLAG_POLL.  Last node of the job graph (it depends on every D2H copy node, so
-// the job's output is already in host memory): one thread stores 1 to the slot's word in mapped pinned host
-// memory, which the dispatcher thread is watching.  The fence orders the store after everything this GPU wrote.
+// K14: completion signal of SET_CB_FLAG_POLL.  Last node of the job graph: it depends on every D2H copy node (memcpy
+// node or SET_K_COPY kernel node), so when this grid starts the job's output has been performed at system scope --
+// grid completion orders a grid's writes before everything a dependent grid does.  One thread stores 1 to the slot's
+// word in mapped pinned host memory, which the dispatcher thread is watching.  No __threadfence_system(): measured on
+// B200 a system fence costs 2.5 us idle and more under load even in a thread with no stores of its own (config 1 end
+// to end: 201 K jobs/s with the fence here, 190 K with the signal fused into the copy kernel behind a fence, 217 K
+// without; profiles/r1_bench.md), and the dependency edge already gives the ordering.
 extern "C" __global__ void set_k_signal(uint32_t* flag) {
     set_pdl_sync();
-    __threadfence_system();
     *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
 }
 
@@ -221,37 +231,27 @@ extern "C" __global__ void set_k_signal(uint32_t* flag) {
 // copies up to set_config.sm_copy_max_bytes are kernel nodes instead: the SMs read pinned host memory directly
 // over the link (H2D) or store into it (D2H).  Each thread moves two 128-bit words, both loads issued before the
 // first store so that 8 KB per block are in flight; unaligned operands or sizes fall back to a byte loop.
-// With flag != NULL this is also the completion signal of SET_CB_FLAG_POLL: every block fences its stores
-// system-wide and bumps the slot's counter; the last block resets the counter and stores the slot's word.
-extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes,
-                                                             uint32_t* done_ctr, uint32_t* flag) {
+extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes) {
     set_pdl_sync();
     const uint32_t tid = threadIdx.x;
-    const uint32_t base = blockIdx.x * (uint32_t)kCopyBytesPerBlock;
-    if (aligned16(src, dst)) {
-        const uint32_t o0 = base + tid * 16u, o1 = o0 + 256u * 16u;
-        uint4 a = make_uint4(0, 0, 0, 0), b = a;
-        const bool f0 = o0 + 16u <= bytes, f1 = o1 + 16u <= bytes;
-        if (f0) a = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o0);
-        if (f1) b = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o1);
-        if (f0) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o0) = a;
-        if (f1) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o1) = b;
-        // ragged tail (< 16 bytes), by the thread whose word would have covered it
-        if (!f0 && o0 < bytes)
-            for (uint32_t k = o0; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
-        if (!f1 && o1 < bytes)
-            for (uint32_t k = o1; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
-    } else {
-        const uint32_t end = min(base + (uint32_t)kCopyBytesPerBlock, bytes);
-        for (uint32_t k = base + tid; k < end; k += 256u) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
-    }
-    if (flag) {
-        __threadfence_system();  // this thread's stores are visible system-wide before anything it does next
-        __syncthreads();
-        if (tid == 0 && atomicAdd(done_ctr, 1u) == gridDim.x - 1) {
-            *done_ctr = 0;  // ready for the slot's next job (which starts only after the host has seen the flag)
-            __threadfence_system();
-            *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+    const bool vec = aligned16(src, dst);
+    for (uint32_t base = blockIdx.x * (uint32_t)kCopyBytesPerBlock; base < bytes; base += gridDim.x * (uint32_t)kCopyBytesPerBlock) {
+        if (vec) {
+            const uint32_t o0 = base + tid * 16u, o1 = o0 + 256u * 16u;
+            uint4 a = make_uint4(0, 0, 0, 0), b = a;
+            const bool f0 = o0 + 16u <= bytes, f1 = o1 + 16u <= bytes;
+            if (f0) a = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o0);
+            if (f1) b = *reinterpret_cast<const uint4*>(static_cast<const char*>(src) + o1);
+            if (f0) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o0) = a;
+            if (f1) *reinterpret_cast<uint4*>(static_cast<char*>(dst) + o1) = b;
+            // ragged tail (< 16 bytes), by the thread whose word would have covered it
+            if (!f0 && o0 < bytes)
+                for (uint32_t k = o0; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
+            if (!f1 && o1 < bytes)
+                for (uint32_t k = o1; k < bytes; ++k) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
+        } else {
+            const uint32_t end = min(base + (uint32_t)kCopyBytesPerBlock, bytes);
+            for (uint32_t k = base + tid; k < end; k += 256u) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
         }
     }
 }

@@ -103,9 +103,7 @@ struct set_ctx final : public Backend {
     // SM copies (set_config.sm_copy_max_bytes): h2d_nodes[i] / d2h_nodes[i] are SET_K_COPY kernel nodes where set
     bool h2d_sm[SET_MAX_BUFFERS] = {}, d2h_sm[SET_MAX_BUFFERS] = {};
     int n_sm_copies = 0;
-    int fused_signal_buf = -1;                 // the one D2H SM copy that also stores the completion word, or -1
     bool pdl = false;                          // some stage asked for SET_STAGE_PDL: kernel-to-kernel edges are programmatic
-    uint32_t* ctrs_dev = nullptr;              // per-slot block counters of the fused copy+signal node (DEVICE)
     uint32_t* flags_host = nullptr;            // b words, kFlagStride apart, mapped pinned host memory
     uint32_t* flags_dev = nullptr;             // the device's address of the same memory
     bool flag_poll = false;
@@ -194,9 +192,7 @@ struct set_ctx final : public Backend {
         const void* src;
         void* dst;
         uint32_t bytes;
-        uint32_t* ctr;
-        uint32_t* flag;
-        void* ptrs[5];
+        void* ptrs[3];
         cudaKernelNodeParams kp;
     };
     void copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims);
@@ -279,24 +275,18 @@ void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const v
         ca.src = (const char*)host + eval(bd.h2d_host_off, dims);
         ca.dst = (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, dims);
         ca.bytes = (uint32_t)eval(bd.h2d_bytes, dims);
-        ca.ctr = nullptr;
-        ca.flag = nullptr;
     } else {
         ca.src = (const char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, dims);
         ca.dst = (char*)host + eval(bd.d2h_host_off, dims);
         ca.bytes = (uint32_t)eval(bd.d2h_bytes, dims);
-        bool sig = fused_signal_buf == i;
-        ca.ctr = sig ? ctrs_dev + (size_t)slot * kFlagStride : nullptr;
-        ca.flag = sig ? flags_dev + (size_t)slot * kFlagStride : nullptr;
     }
     ca.ptrs[0] = &ca.src;
     ca.ptrs[1] = &ca.dst;
     ca.ptrs[2] = &ca.bytes;
-    ca.ptrs[3] = &ca.ctr;
-    ca.ptrs[4] = &ca.flag;
     ca.kp = cudaKernelNodeParams{};
     ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
-    ca.kp.gridDim = dim3((ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK);
+    uint32_t pieces = (ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK;
+    ca.kp.gridDim = dim3(pieces ? pieces : 1);
     ca.kp.blockDim = dim3(256);
     ca.kp.kernelParams = ca.ptrs;
 }
@@ -454,8 +444,14 @@ int set_ctx::build_graph() {
             leaves.push_back(d2h_nodes[i]);
         }
     }
-    if (flag_poll && fused_signal_buf < 0) {  // completion signal: runs after every D2H copy of the job has finished
-        if (leaves.empty()) leaves.push_back(prev);
+    if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished (kernels.cu K14)
+        std::vector<bool> leaf_is_kernel;
+        for (size_t i = 0; i < bufs.size(); ++i)
+            if (!expr_is_zero(bufs[i].d2h_bytes)) leaf_is_kernel.push_back(d2h_sm[i]);
+        if (leaves.empty()) {
+            leaves.push_back(prev);
+            leaf_is_kernel.push_back(true);
+        }
         uint32_t* flag = flags_dev;
         void* args[1] = {&flag};
         cudaKernelNodeParams kp{};
@@ -463,7 +459,8 @@ int set_ctx::build_graph() {
         kp.gridDim = dim3(1);
         kp.blockDim = dim3(1);
         kp.kernelParams = args;
-        CK(cudaGraphAddKernelNode(&signal_node, graph, leaves.data(), leaves.size(), &kp));
+        CK(cudaGraphAddKernelNode(&signal_node, graph, nullptr, 0, &kp));
+        for (size_t l = 0; l < leaves.size(); ++l) CK(depend(leaves[l], signal_node, pdl && leaves.size() == 1 && leaf_is_kernel[l]));
     }
     return 0;
 }
@@ -688,8 +685,6 @@ int set_ctx::plain_job(int slot, const JobDesc& job) {
             if (d2h_sm[i]) {
                 CopyArgs ca;
                 copy_params(ca, slot, (int)i, false, job.out, job.dims);
-                ca.ctr = nullptr;  // no completion word outside SET mode
-                ca.flag = nullptr;
                 CK(cudaLaunchKernel(ca.kp.func, ca.kp.gridDim, ca.kp.blockDim, ca.ptrs, 0, st));
             } else {
                 CK(cudaMemcpyAsync((char*)job.out + eval(bd.d2h_host_off, job.dims), (char*)sm.buf[i] + eval(bd.d2h_dev_off, job.dims),
@@ -1046,25 +1041,14 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
         // default: 256 KiB across the host link; off for SET_IO_DEVICE, where a D2D memcpy node runs on a copy engine
         // beside the kernels while an SM copy would lengthen the stream's kernel chain (measured, profiles/r1_bench.md)
         int64_t lim = c->cfg.sm_copy_max_bytes != 0 ? c->cfg.sm_copy_max_bytes : (c->cfg.io == SET_IO_DEVICE ? -1 : 262144);
-        int n_d2h = 0, last_sm = -1;
         for (size_t i = 0; i < c->bufs.size(); ++i) {
             const set_buffer_desc& bd = c->bufs[i];
             auto small = [&](const set_size_expr& e) { return e.per_unit == 0 && e.fixed > 0 && (int64_t)e.fixed <= lim; };
             c->h2d_sm[i] = small(bd.h2d_bytes);
             c->d2h_sm[i] = small(bd.d2h_bytes);
             c->n_sm_copies += (int)c->h2d_sm[i] + (int)c->d2h_sm[i];
-            if (!expr_is_zero(bd.d2h_bytes)) ++n_d2h;
-            if (c->d2h_sm[i]) last_sm = (int)i;
         }
-        if (c->flag_poll && n_d2h == 1 && last_sm >= 0) c->fused_signal_buf = last_sm;
         for (auto& st : c->stages) c->pdl = c->pdl || (st.flags & SET_STAGE_PDL);
-        if (c->fused_signal_buf >= 0) {
-            size_t bytes = (size_t)c->b * kFlagStride * sizeof(uint32_t);
-            if (cudaMalloc((void**)&c->ctrs_dev, bytes) != cudaSuccess || cudaMemset(c->ctrs_dev, 0, bytes) != cudaSuccess) {
-                cudaGetLastError();
-                return c->fail(SET_ERR_NOMEM, "counter allocation failed");
-            }
-        }
     }
     if (int rc = c->build_graph()) return rc;
 
@@ -1165,7 +1149,6 @@ set_status set_destroy(set_ctx* c) {
     if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
     if (c->flags_host) cudaFreeHost(c->flags_host);
-    if (c->ctrs_dev) cudaFree(c->ctrs_dev);
     for (int s = 0; s < c->S; ++s) {
         if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
         if (c->notify[s]) cudaStreamDestroy(c->notify[s]);

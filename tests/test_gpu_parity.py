@@ -207,8 +207,7 @@ def test_every_completion_mode_delivers_every_job(libset, cb, disp):
     for config in (0, 4):
         wl = small_workload(config)
         st = check(libset, wl, list(range(wl.jobs)), callback_mode=cb, num_dispatchers=disp)
-        # config 0: its one D2H copy is an SM copy node that carries the completion word itself; config 4 has two D2H copies
-        assert st["signal_nodes"] == (wl.jobs if cb == 3 and config == 4 else 0)
+        assert st["signal_nodes"] == (wl.jobs if cb == 3 else 0)
         assert st["copy_nodes"] == wl.jobs * (2 if config == 0 else 1)
         assert st["max_inflight_seen"] <= wl.max_inflight
 
@@ -233,12 +232,13 @@ def test_sm_copies_with_unaligned_pinned_pointers(libset, misalign):
     check(libset, Workload(0, (1001,), jobs=12, num_streams=2, max_inflight=4), list(range(12)), misalign=misalign, pdl=True)
 
 
-def test_sm_copy_completion_signal_survives_many_jobs_per_slot(libset):
-    """The fused copy+signal node counts its blocks in a per-slot device word that the last block resets: 600 jobs over
-    4 slots, outputs of three blocks each (config 0 with n = 5000 -> 20,256 bytes)."""
+def test_completion_word_never_overtakes_the_output(libset):
+    """The signal node stores the slot's word without a system fence: the graph edge from the D2H copy node orders the
+    output before it.  600 jobs over 4 slots with sentinel-filled outputs of three copy blocks each (config 0 with
+    n = 5000 -> 20,256 bytes): a word seen early would release the slot and the check would read sentinel bytes."""
     from paper_2606_05495_b200.workloads import Workload
     st = check(libset, Workload(0, (5000,), jobs=600, num_streams=2, max_inflight=4), list(range(600)), pdl=True)
-    assert st["signal_nodes"] == 0 and st["copy_nodes"] == 1200
+    assert st["signal_nodes"] == 600 and st["copy_nodes"] == 1200
 
 
 def test_submit_before_register_and_double_register(libset):
