@@ -367,8 +367,26 @@ def kernel_rooflines(setlib, wl, pk, dims=None):
         else:
             m["achieved"] = round(m["algorithmic"] / (m["avg_us"] * 1e-6) / 1e12, 2)
         m["frac"] = round(m["achieved"] / m["peak"], 4)
+        m["traffic"] = NCU_TRAFFIC.get("set_k_" + m["kernel"], {}).get(wl_key(wl))
         out.append(m)
     return out
+
+
+def wl_key(wl):
+    return f"config{wl.config}"
+
+
+def _load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+    (profiles/ncu_traffic.json, written from the .ncu-rep files; the file names the capture it came from)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get("kernels", {})
+    except Exception:
+        return {}
+
+
+NCU_TRAFFIC = _load_traffic()
 
 
 def pipeline_roofline(wl, in_bytes_job, out_bytes_job, link, pk, dims):
@@ -417,8 +435,29 @@ def cpu_baseline(wl, job_ids, budget_s=15.0, passes=10):
         secs += s
         if secs >= budget_s:
             break
-    return {"value": round(total / secs, 2), "unit": "jobs/s", "cores": 1, "kind": "oracle",
-            "sample": f"{total} jobs of the workload (first {n} job inputs, repeated) in {secs:.1f} s, single thread, oracle/*.c -O2"}
+    out = {"value": round(total / secs, 2), "unit": "jobs/s", "cores": 1, "kind": "oracle",
+           "sample": f"{total} jobs of the workload (first {n} job inputs, repeated) in {secs:.1f} s, single thread, oracle/*.c -O2"}
+    # the same oracle, job-parallel over the box's cores (jobs are independent; ctypes releases the GIL inside the C call)
+    try:
+        from concurrent.futures import ThreadPoolExecutor
+        cores = len(os.sched_getaffinity(0))
+        if cores > 1:
+            chunks = [(images[i::cores], dims[i::cores]) for i in range(cores)]
+            def worker(c, budget=4.0):
+                n_done, t_used = 0, 0.0
+                while t_used < budget and c[0]:
+                    d, t = oracle_pass(wl, c[0], c[1], budget - t_used)
+                    n_done, t_used = n_done + d, t_used + t
+                return n_done
+
+            t0 = time.perf_counter()
+            with ThreadPoolExecutor(cores) as ex:
+                done = sum(ex.map(worker, chunks))
+            dt = time.perf_counter() - t0
+            out["all_cores"] = {"value": round(done / dt, 2), "cores": cores, "sample": f"{done} jobs in {dt:.1f} s, one thread per core"}
+    except Exception as e:
+        out["all_cores"] = {"error": str(e)[:120]}
+    return out
 
 
 # ------------------------------------------------------------------------------------------------ main
@@ -622,7 +661,7 @@ def main():
             extra["completion_modes"] = dict(cm, flag_poll_e2e={"jobs_per_s": round(e2e_value, 1)})
             gv = {}
             for name, o in (("ce_copies_plain_edges", {"sm_copy_max_bytes": -1, "pdl": False}), ("ce_copies_pdl", {"sm_copy_max_bytes": -1, "pdl": True}),
-                            ("sm_copies_plain_edges", {"sm_copy_max_bytes": 0, "pdl": False}), ("sm_copies_pdl", {"sm_copy_max_bytes": 0, "pdl": True})):
+                            ("sm_copies_plain_edges", {"sm_copy_max_bytes": 262144, "pdl": False}), ("sm_copies_pdl", {"sm_copy_max_bytes": 262144, "pdl": True})):
                 p_, r_ = LAYOUT[wl.config]
                 for io_device in (False, True):
                     r = run_arm(setlib, wl, ids, "set", io_device, steps, warmup, p_, r_, verify=2, flush=flush, opts=o)
@@ -641,6 +680,14 @@ def main():
             extra["baselines"] = base
             extra["speedup_vs_batch_sync_graphs"] = {"e2e": round(e2e_value / base["batch_sync_graphs_e2e"]["jobs_per_s"], 3),
                                                      "device": round(value / base["batch_sync_graphs_device"]["jobs_per_s"], 3)}
+            # host scheduling overhead per job (BASELINE.json:metric): time the host spends updating, launching, completing
+            # and -- in the batch model -- blocked in synchronisation, per job, end to end
+            hs, hb = e2e_arm["host_us_per_job"], base["batch_sync_graphs_e2e"]["host_us_per_job"]
+            so_set = hs["bind"] + hs["launch"] + hs["callback"]
+            so_batch = hb["bind"] + hb["launch"] + hb["sync"]
+            extra["sched_overhead_us_per_job"] = {"set": round(so_set, 3), "batch_sync_graphs": round(so_batch, 3),
+                                                  "reduction": round(1.0 - so_set / so_batch, 3) if so_batch > 0 else None,
+                                                  "how": "set: bind + launch + callback; batch: bind + launch + host sync wait; e2e arms"}
         if args.suite == "all":
             others = {}
             for c in range(5):
@@ -680,7 +727,7 @@ def main():
         roof = None
         if dom:
             roof = {"bound": dom["bound"], "achieved": dom["achieved"], "peak": dom["peak"], "unit": dom["unit"], "frac": dom["frac"],
-                    "traffic": None, "kernel": dom["kernel"], "avg_us": dom["avg_us"], "algorithmic_per_launch": dom["algorithmic"],
+                    "traffic": dom.get("traffic"), "kernel": dom["kernel"], "avg_us": dom["avg_us"], "algorithmic_per_launch": dom["algorithmic"],
                     "peak_source": pk["source"],
                     "how": "set_time_stage: the stage kernel alone, a chain of launches bracketed by CUDA events on the launching stream"}
         line = {"metric": "jobs/s", "value": round(value, 1), "unit": "jobs/s", "n_gpus": world, "steps": steps, "warmup": warmup,
