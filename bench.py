@@ -734,8 +734,8 @@ def main():
                 "ms_per_step": round(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": wl.dtype, "data": "synthetic",
                 "config": {"workload": wl.name, "jobs_per_step_per_gpu": len(ids), "num_streams": wl.num_streams,
-                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or "library default: 262144 for host buffers, copy engines for device-resident I/O", "pdl_edges": OPTS["pdl"],
-                           "max_inflight": wl.max_inflight, "io": "value: inputs/outputs resident in HBM (D2D copy nodes); e2e: pinned host buffers",
+                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or 262144, "pdl_edges": OPTS["pdl"],
+                           "max_inflight": wl.max_inflight, "io": "value: inputs/outputs resident in HBM (the copy nodes move HBM to HBM); e2e: pinned host buffers",
                            "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer rewritten between timed steps; distinct job inputs "
                                  f"{dev_arm['in_bytes'] / 1e6:.0f} MB per step"},
                 "clocks": clocks,

@@ -179,8 +179,7 @@ typedef struct set_config {
     int32_t spin_us;          /* dispatcher/drain spin time before sleeping; 0 => default (50)     */
     int32_t sm_copy_max_bytes;/* H2D/D2H copies of a fixed size up to this many bytes become kernel nodes
                                  (SET_K_COPY: the SMs read/write pinned host memory over the link) instead of
-                                 copy-engine memcpy nodes; 0 => default (262144 under SET_IO_HOST, never under
-                                 SET_IO_DEVICE), -1 => never.                    */
+                                 copy-engine memcpy nodes; 0 => default (262144), -1 => never.                    */
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */

@@ -1038,9 +1038,9 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     }
     // ---- which copies become SET_K_COPY kernel nodes: fixed size (the grid never changes), at most sm_copy_max_bytes
     {
-        // default: 256 KiB across the host link; off for SET_IO_DEVICE, where a D2D memcpy node runs on a copy engine
-        // beside the kernels while an SM copy would lengthen the stream's kernel chain (measured, profiles/r1_bench.md)
-        int64_t lim = c->cfg.sm_copy_max_bytes != 0 ? c->cfg.sm_copy_max_bytes : (c->cfg.io == SET_IO_DEVICE ? -1 : 262144);
+        // default 256 KiB: below that a copy-engine node costs more in engine hand-off than the copy itself, across the
+        // host link and (SET_IO_DEVICE) inside HBM alike (profiles/r1_bench.md, graph_variants)
+        int64_t lim = c->cfg.sm_copy_max_bytes != 0 ? c->cfg.sm_copy_max_bytes : 262144;
         for (size_t i = 0; i < c->bufs.size(); ++i) {
             const set_buffer_desc& bd = c->bufs[i];
             auto small = [&](const set_size_expr& e) { return e.per_unit == 0 && e.fixed > 0 && (int64_t)e.fixed <= lim; };
