@@ -194,7 +194,7 @@ MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3
 
 
 # graph-shape options of every arm (SET and the in-run baselines share the job graph): --sm-copy / --pdl
-OPTS = {"sm_copy_max_bytes": 0, "pdl": True}
+OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0}
 
 
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
@@ -204,7 +204,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
     import torch
     o = dict(OPTS, **(opts or {}))
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=MODES[mode], io=setlib.IO_DEVICE if io_device else setlib.IO_HOST,
-                         sm_copy_max_bytes=o["sm_copy_max_bytes"], **(ctx_kw or {}))
+                         sm_copy_max_bytes=o["sm_copy_max_bytes"], **dict({"num_dispatchers": o["num_dispatchers"]}, **(ctx_kw or {})))
     try:
         ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=o["pdl"])
         js = build_jobs(setlib, ctx, wl, job_ids, io_device, pool, out_ring)
@@ -584,11 +584,12 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
     ap.add_argument("--sm-copy", type=int, default=0, help="set_config.sm_copy_max_bytes: 0 = library default, -1 = copy engines only")
+    ap.add_argument("--dispatchers", type=int, default=0, help="set_config.num_dispatchers (0 = library default, 1)")
     ap.add_argument("--pdl", type=int, default=1, help="1: programmatic-dependent-launch edges between kernel nodes (default), 0: plain edges")
     ap.add_argument("--sweep", action="store_true", help="also sweep the batch size b (PAPER.md Fig. 5-6) on the headline workload")
     ap.add_argument("--out", default=None, help="also write the JSON line to this file")
     args = ap.parse_args()
-    OPTS["sm_copy_max_bytes"], OPTS["pdl"] = args.sm_copy, bool(args.pdl)
+    OPTS["sm_copy_max_bytes"], OPTS["pdl"], OPTS["num_dispatchers"] = args.sm_copy, bool(args.pdl), args.dispatchers
 
     from paper_2606_05495_b200 import multi
     if args.impl == "reference":

@@ -281,3 +281,30 @@ def test_device_resident_io(libset):
     for j in range(40):
         compare(wl, d_out[j].cpu().numpy(), oracle_out(wl, ins[j], (1, 1, 1, 1)))
     ctx.close()
+
+
+@pytest.mark.parametrize("config", [0, 1, 4])
+def test_device_slot_padding_is_never_written(libset, config):
+    """Canary bytes on the device: the slot buffers live in a caller-owned torch arena pre-filled with a sentinel; each
+    buffer is padded to a multiple of 1024 bytes (set.h: set_register_pipeline), and neither the padding, nor the space
+    in front of the first slot, nor the space after the last one may change while jobs run at full depth."""
+    import torch
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(config)
+    _, _, bufs, nb, _, _ = libset.builtin_pipeline(wl.config, wl.variant, list(wl.params))
+    sizes = [int(bufs[i].bytes) for i in range(nb)]
+    up = lambda v: (v + 1023) & ~1023
+    per_slot = sum(up(b) for b in sizes)
+    arena = torch.full((per_slot * wl.max_inflight + 4096,), SENTINEL, dtype=torch.uint8, device="cuda")
+    check(libset, wl, list(range(min(wl.jobs, 64))), device_arena=arena.data_ptr(), device_arena_bytes=arena.numel(), pdl=True)
+    torch.cuda.synchronize()
+    host = arena.cpu().numpy()
+    first = up(arena.data_ptr()) - arena.data_ptr()
+    pad = np.ones(host.size, bool)                      # True = must still hold the sentinel
+    for w in range(wl.max_inflight):
+        off = first + w * per_slot
+        for b in sizes:
+            pad[off:off + b] = False
+            off += up(b)
+    assert pad.sum() > 0
+    assert np.all(host[pad] == SENTINEL), "a kernel or copy wrote outside its slot buffer"
