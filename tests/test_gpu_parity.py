@@ -308,3 +308,37 @@ def test_device_slot_padding_is_never_written(libset, config):
             off += up(b)
     assert pad.sum() > 0
     assert np.all(host[pad] == SENTINEL), "a kernel or copy wrote outside its slot buffer"
+
+
+def test_full_size_config2_bit_exact(libset):
+    """BASELINE.json:configs[2] at its full per-job size (4096 x 4096 fp32, 10 sweeps, 4 streams, 8 in flight), every
+    element of every output against the oracle."""
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(2)
+    st = check(libset, wl, list(range(3)), io_check=False)
+    assert st["kernel_nodes"] == 3 * 10
+
+
+def test_full_size_config3_sampled_entries(libset):
+    """BASELINE.json:configs[3] at its full per-job size (2048^3, 4 streams, 8 in flight, 10 jobs so that slots are
+    reused): the naive-loop oracle takes minutes per job at this size, so 4096 seeded (m, n) entries per job are
+    computed one by one (oracle_config3_sampled) and compared; tile corners and edges are always among them."""
+    import oracle
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(3)
+    M, N, K = wl.params
+    ids = list(range(10))
+    outs, ins, _, st = run_jobs(libset, wl, ids, io_check=False)
+    assert st["completed"] == len(ids)
+    fixed = [(0, 0), (M - 1, N - 1), (127, 255), (128, 256), (127, 256), (128, 255), (M - 1, 0), (0, N - 1), (1023, 1024), (1024, 1023)]
+    for k, j in enumerate(ids):
+        a = ins[k][:2 * M * K].view(np.uint16).reshape(M, K)
+        b = ins[k][2 * M * K:2 * M * K + 2 * K * N].view(np.uint16).reshape(K, N)
+        bias = ins[k][2 * M * K + 2 * K * N:].view(np.float32)
+        r = inputgen.uniform24(1234, j, 7, 2 * 4096)
+        ms = np.concatenate([np.array([f[0] for f in fixed]), r[:4096] % M]).astype(np.int64)
+        ns = np.concatenate([np.array([f[1] for f in fixed]), r[4096:] % N]).astype(np.int64)
+        ref = inputgen.bf16_bits_to_f64(oracle.config3_sampled(a, b, bias, ms, ns))
+        got = inputgen.bf16_bits_to_f64(outs[k].view(np.uint16).reshape(M, N)[ms, ns])
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 2e-2
+        assert np.abs(got - ref).max() <= 0.05 * max(1.0, np.abs(ref).max())
