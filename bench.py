@@ -194,7 +194,7 @@ MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3
 
 
 # graph-shape options of every arm (SET and the in-run baselines share the job graph): --sm-copy / --pdl
-OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0}
+OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0, "submitters": 1}
 
 
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
@@ -210,9 +210,24 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
         js = build_jobs(setlib, ctx, wl, job_ids, io_device, pool, out_ring)
         n = js.n
 
-        def step():
-            ctx.submit_batch(js.ins, js.outs, js.dims)
-            ctx.drain()
+        # SET takes submissions from several caller threads (Algorithm 1 claims jobs with an atomic); the
+        # baseline models are single-caller by definition
+        nsub = max(1, min(int(o["submitters"]), n)) if mode == "set" else 1
+        pool_ex = None
+        if nsub > 1:
+            from concurrent.futures import ThreadPoolExecutor
+            pool_ex = ThreadPoolExecutor(nsub)
+            cuts = [n * t // nsub for t in range(nsub + 1)]
+
+            def step():
+                futs = [pool_ex.submit(ctx.submit_batch_slice, js.ins, js.outs, js.dims, cuts[t], cuts[t + 1]) for t in range(nsub)]
+                for f in futs:
+                    f.result()
+                ctx.drain()
+        else:
+            def step():
+                ctx.submit_batch(js.ins, js.outs, js.dims)
+                ctx.drain()
 
         for _ in range(warmup):
             step()
@@ -269,6 +284,8 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
         js.keep.clear()
         return out
     finally:
+        if "pool_ex" in locals() and pool_ex is not None:
+            pool_ex.shutdown()
         ctx.close()
 
 
@@ -278,6 +295,20 @@ def time_stages(setlib, wl, dims=None, iters=50):
     with setlib.Context(1, 1) as ctx:
         ctx.register_builtin(wl.config, wl.variant, list(wl.params))
         return [ctx.time_stage(s, dims, warmup=5, iters=iters) for s in range(ctx.num_stages)]
+
+
+_FLOOR = {}
+
+
+def launch_floor_us(setlib):
+    """Duration of a kernel node that does nothing (the debug delay stage with a 0 ns wait), timed like the stages: what
+    one node of a job graph costs on this GPU whatever its work.  SURVEY.md 8(d): the latency-class kernels of configs
+    0, 1 and 4 are judged against this floor rather than against the HBM roofline."""
+    if "us" not in _FLOOR:
+        with setlib.Context(1, 1) as ctx:
+            ctx.register_builtin(0, setlib.VARIANT_SPIN, [64])
+            _FLOOR["us"] = round(ctx.time_stage(ctx.num_stages - 1, (1, 1, 1, 0), warmup=5, iters=50), 3)
+    return _FLOOR["us"]
 
 
 def link_bandwidth():
@@ -368,6 +399,7 @@ def kernel_rooflines(setlib, wl, pk, dims=None):
             m["achieved"] = round(m["algorithmic"] / (m["avg_us"] * 1e-6) / 1e12, 2)
         m["frac"] = round(m["achieved"] / m["peak"], 4)
         m["traffic"] = NCU_TRAFFIC.get("set_k_" + m["kernel"], {}).get(wl_key(wl))
+        m["launch_floor_us"] = launch_floor_us(setlib)
         out.append(m)
     return out
 
@@ -584,12 +616,14 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
     ap.add_argument("--sm-copy", type=int, default=0, help="set_config.sm_copy_max_bytes: 0 = library default, -1 = copy engines only")
+    ap.add_argument("--submitters", type=int, default=1, help="caller threads that submit a step's jobs to SET (baselines: always 1); measured on B200: no gain beyond 1, the driver serialises graph updates and launches")
     ap.add_argument("--dispatchers", type=int, default=0, help="set_config.num_dispatchers (0 = library default, 1)")
     ap.add_argument("--pdl", type=int, default=1, help="1: programmatic-dependent-launch edges between kernel nodes (default), 0: plain edges")
     ap.add_argument("--sweep", action="store_true", help="also sweep the batch size b (PAPER.md Fig. 5-6) on the headline workload")
     ap.add_argument("--out", default=None, help="also write the JSON line to this file")
     args = ap.parse_args()
     OPTS["sm_copy_max_bytes"], OPTS["pdl"], OPTS["num_dispatchers"] = args.sm_copy, bool(args.pdl), args.dispatchers
+    OPTS["submitters"] = args.submitters
 
     from paper_2606_05495_b200 import multi
     if args.impl == "reference":
@@ -735,7 +769,7 @@ def main():
                 "ms_per_step": round(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": wl.dtype, "data": "synthetic",
                 "config": {"workload": wl.name, "jobs_per_step_per_gpu": len(ids), "num_streams": wl.num_streams,
-                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or 262144, "pdl_edges": OPTS["pdl"],
+                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or 262144, "pdl_edges": OPTS["pdl"], "submitter_threads": OPTS["submitters"],
                            "max_inflight": wl.max_inflight, "io": "value: inputs/outputs resident in HBM (the copy nodes move HBM to HBM); e2e: pinned host buffers",
                            "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer rewritten between timed steps; distinct job inputs "
                                  f"{dev_arm['in_bytes'] / 1e6:.0f} MB per step"},

@@ -235,6 +235,15 @@ class Context:
             d = dims if isinstance(dims, C.Array) else (C.c_uint32 * (4 * n))(*dims)
         self._check(self._lib.set_submit_batch(self._h, n, first_id, None, ins, outs, d), "set_submit_batch")
 
+    def submit_batch_slice(self, ins, outs, dims, lo: int, hi: int):
+        """Jobs lo..hi-1 of pre-built ctypes arrays (no copies): several caller threads can share one job list --
+        set_submit* is thread-safe (set.h), and ctypes releases the GIL for the duration of the call."""
+        vp = C.c_void_p
+        pi = C.cast(C.byref(ins, lo * C.sizeof(vp)), C.POINTER(vp))
+        po = C.cast(C.byref(outs, lo * C.sizeof(vp)), C.POINTER(vp))
+        pd = C.cast(C.byref(dims, lo * 16), C.POINTER(C.c_uint32)) if dims is not None else None
+        self._check(self._lib.set_submit_batch(self._h, hi - lo, lo, None, pi, po, pd), "set_submit_batch")
+
     def drain(self):
         self._check(self._lib.set_drain(self._h), "set_drain")
 

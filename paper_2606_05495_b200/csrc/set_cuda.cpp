@@ -309,21 +309,25 @@ int set_ctx::check_sizes(const uint32_t* dims) {
 // ---------------------------------------------------------------------------------------------------------
 // pinned-memory test: known ranges first, one driver query per unknown allocation
 // ---------------------------------------------------------------------------------------------------------
+// pinned_ranges is kept sorted by start address (ranges never overlap: they are whole allocations), so the test is a
+// binary search however many buffers the caller has allocated
 void set_ctx::add_pinned_range(const void* p, size_t n) {
+    PinnedRange r{(uintptr_t)p, (uintptr_t)p + n};
     range_lock.lock();
-    pinned_ranges.push_back({(uintptr_t)p, (uintptr_t)p + n});
+    auto it = std::upper_bound(pinned_ranges.begin(), pinned_ranges.end(), r.lo,
+                               [](uintptr_t a, const PinnedRange& b) { return a < b.lo; });
+    pinned_ranges.insert(it, r);
     range_lock.unlock();
 }
 
 bool set_ctx::is_pinned(const void* p) {
     uintptr_t a = (uintptr_t)p;
     range_lock.lock();
-    for (auto& r : pinned_ranges)
-        if (a >= r.lo && a < r.hi) {
-            range_lock.unlock();
-            return true;
-        }
+    auto it = std::upper_bound(pinned_ranges.begin(), pinned_ranges.end(), a,
+                               [](uintptr_t x, const PinnedRange& b) { return x < b.lo; });
+    bool hit = it != pinned_ranges.begin() && a < (it - 1)->hi;
     range_lock.unlock();
+    if (hit) return true;
     cudaPointerAttributes at;
     if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
         cudaGetLastError();
