@@ -687,7 +687,7 @@ def main():
         extra["kernels"] = kr
         if not args.no_baselines:
             cm = {}
-            for name, cb in (("hostfunc_notify_stream", 1), ("hostfunc_work_stream", 2)):
+            for name, cb in (("hostfunc_notify_stream", 1), ("hostfunc_work_stream", 2), ("graph_host_node", 4)):
                 p_, r_ = LAYOUT[wl.config]
                 r = run_arm(setlib, wl, ids, "set", False, steps, warmup, p_, r_, verify=2, ctx_kw={"callback_mode": cb}, flush=flush)
                 log(f"[bench]   {wl.config} set/{name:24s} host   {r['jobs_per_s']:12.1f} jobs/s  host us/job {r['host_us_per_job']}")

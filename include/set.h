@@ -165,6 +165,10 @@ typedef struct set_buffer_desc {
                                   thread, no extra API call per job; measured 8x lower completion
                                   latency than cudaLaunchHostFunc on B200, profiles/)             */
 
+#define SET_CB_HOST_NODE     4 /* the job graph ends in a host node (cudaGraphAddHostNode) that runs Algorithm 3 on the
+                                  driver's callback thread: no API call per job beyond cudaGraphLaunch, but the
+                                  stream waits for the host round trip like SET_CB_WORK_STREAM                */
+
 typedef struct set_config {
     uint32_t struct_bytes;    /* = sizeof(set_config), for forward compatibility                   */
     int32_t num_streams;      /* S >= 1                                                            */

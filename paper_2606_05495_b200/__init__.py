@@ -23,7 +23,7 @@ SET_MAX_STAGES, SET_MAX_BUFFERS, SET_MAX_ARGS, SET_MAX_DIMS = 16, 8, 12, 4
 MODE_SET, MODE_PLAIN_STREAMS, MODE_BATCH_SYNC, MODE_SINGLE_GRAPH, MODE_MUTEX_QUEUE = 0, 1, 2, 3, 4
 IO_HOST, IO_DEVICE = 0, 1
 STEAL_SWAP, STEAL_RETARGET = 0, 1
-CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL = 0, 1, 2, 3
+CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL, CB_HOST_NODE = 0, 1, 2, 3, 4
 ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D = 0, 1, 2, 3, 4
 STAGE_PDL = 1
 K_COPY = 15

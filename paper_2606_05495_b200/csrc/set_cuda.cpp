@@ -100,6 +100,7 @@ struct set_ctx final : public Backend {
     std::vector<cudaGraphNode_t> kern_nodes;
     cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
     cudaGraphNode_t signal_node = nullptr;     // SET_CB_FLAG_POLL: last node, stores the slot's completion word
+    cudaGraphNode_t host_node = nullptr;       // SET_CB_HOST_NODE: last node, runs Algorithm 3 on the driver's callback thread
     // SM copies (set_config.sm_copy_max_bytes): h2d_nodes[i] / d2h_nodes[i] are SET_K_COPY kernel nodes where set
     bool h2d_sm[SET_MAX_BUFFERS] = {}, d2h_sm[SET_MAX_BUFFERS] = {};
     int n_sm_copies = 0;
@@ -364,6 +365,8 @@ bool set_ctx::is_pinned(const void* p) {
 // A2: job-as-graph.  [memset] / H2D roots -> kernel chain -> D2H leaves, built by explicit construction
 // with slot 0's buffers and placeholder host operands; every exec is then re-bound.
 // ---------------------------------------------------------------------------------------------------------
+static void CUDART_CB set_completion_cb(void* arg);
+
 int set_ctx::build_graph() {
     const uint32_t unit[4] = {1, 1, 1, 1};
     cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -466,6 +469,13 @@ int set_ctx::build_graph() {
         CK(cudaGraphAddKernelNode(&signal_node, graph, nullptr, 0, &kp));
         for (size_t l = 0; l < leaves.size(); ++l) CK(depend(leaves[l], signal_node, pdl && leaves.size() == 1 && leaf_is_kernel[l]));
     }
+    if (cfg.mode == SET_MODE_SET && cfg.callback_mode == SET_CB_HOST_NODE) {
+        if (leaves.empty()) leaves.push_back(prev);
+        cudaHostNodeParams hp{};
+        hp.fn = set_completion_cb;
+        hp.userData = &cbargs[0];
+        CK(cudaGraphAddHostNode(&host_node, graph, leaves.data(), leaves.size(), &hp));
+    }
     return 0;
 }
 
@@ -554,6 +564,12 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             kp.kernelParams = args;
             CK(cudaGraphExecKernelNodeSetParams(es.exec, signal_node, &kp));
         }
+        if (host_node && es.bound_slot != slot) {
+            cudaHostNodeParams hp{};
+            hp.fn = set_completion_cb;
+            hp.userData = &cbargs[slot];
+            CK(cudaGraphExecHostNodeSetParams(es.exec, host_node, &hp));
+        }
         full_rebinds.fetch_add(1, std::memory_order_relaxed);
     } else {
         host_rebinds.fetch_add(1, std::memory_order_relaxed);
@@ -608,7 +624,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     SpinLock& lk = stream_locks[s];
     lk.lock();
     cudaError_t e = cudaGraphLaunch(execs[exec].exec, streams[s]);
-    if (e == cudaSuccess && !flag_poll) {
+    if (e == cudaSuccess && !flag_poll && !host_node) {
         if (cfg.callback_mode == SET_CB_WORK_STREAM) {
             e = cudaLaunchHostFunc(streams[s], set_completion_cb, &cbargs[slot]);
         } else {
@@ -877,7 +893,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.queue_capacity == 0) cfg.queue_capacity = 2;
     if (cfg.num_dispatchers == 0) cfg.num_dispatchers = 1;
     if (cfg.spin_us == 0) cfg.spin_us = 50;
-    if (cfg.callback_mode < SET_CB_DEFAULT || cfg.callback_mode > SET_CB_FLAG_POLL) return SET_ERR_INVALID;
+    if (cfg.callback_mode < SET_CB_DEFAULT || cfg.callback_mode > SET_CB_HOST_NODE) return SET_ERR_INVALID;
     if (cfg.callback_mode == SET_CB_DEFAULT) cfg.callback_mode = SET_CB_FLAG_POLL;
     if (cfg.mode == SET_MODE_SINGLE_GRAPH) {  // one worker, one stream, one exec by definition
         cfg.num_streams = 1;

@@ -198,11 +198,12 @@ def test_same_inputs_twice_give_identical_bits(libset):
             assert np.array_equal(x, y)
 
 
-@pytest.mark.parametrize("cb", [1, 2, 3])
+@pytest.mark.parametrize("cb", [1, 2, 3, 4])
 @pytest.mark.parametrize("disp", [1, 2])
 def test_every_completion_mode_delivers_every_job(libset, cb, disp):
     """A6/A7: event chain + cudaLaunchHostFunc on a notify stream (1), host function on the work stream (2, PAPER.md:203
-    literally) and the GPU-written flag watched by the dispatcher (3) all release each slot exactly once."""
+    literally), the GPU-written flag watched by the dispatcher (3) and a host node at the end of the job graph (4) all release
+    each slot exactly once."""
     from paper_2606_05495_b200.workloads import small_workload
     for config in (0, 4):
         wl = small_workload(config)
