@@ -204,7 +204,8 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
     import torch
     o = dict(OPTS, **(opts or {}))
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=MODES[mode], io=setlib.IO_DEVICE if io_device else setlib.IO_HOST,
-                         sm_copy_max_bytes=o["sm_copy_max_bytes"], **dict({"num_dispatchers": o["num_dispatchers"]}, **(ctx_kw or {})))
+                         sm_copy_max_bytes=o["sm_copy_max_bytes"], timestamps=bool(o.get("timestamps")),
+                         **dict({"num_dispatchers": o["num_dispatchers"]}, **(ctx_kw or {})))
     try:
         ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=o["pdl"])
         js = build_jobs(setlib, ctx, wl, job_ids, io_device, pool, out_ring)
@@ -258,6 +259,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
             if clock_windows is not None:
                 clock_windows.append((t0, t1))
         st = ctx.stats()
+        gap_stats = ctx.gap_stats() if o.get("timestamps") else None
         bad = 0
         if verify:
             sys.path.insert(0, os.path.join(ROOT, "tests"))
@@ -279,6 +281,8 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
                "d2h_bytes": 0 if io_device else js.out_bytes, "in_bytes": js.in_bytes, "out_bytes": js.out_bytes,
                "kernel_launches": st["kernel_nodes"] + st["copy_nodes"] + st["signal_nodes"], "verified": len(picks) if verify else 0, "mismatches": bad,
                "stats": st}
+        if gap_stats is not None:
+            out["device_gaps"] = gap_stats
         jobs_total = max(1, st["submitted"])
         out["host_us_per_job"] = {k: st["ns_" + k] / jobs_total / 1e3 for k in ("submit", "bind", "launch", "callback", "sync")}
         js.keep.clear()
@@ -558,6 +562,35 @@ def batch_sweep(setlib, wl, ids, flush, trace_ok: bool):
     return out
 
 
+def device_gap_pass(setlib, wl, ids, all_configs: bool, flush):
+    """Gaps between consecutive jobs of a stream from the GPU's own clock (set_config.timestamps, include/set.h
+    set_get_gap_stats): two one-thread stamp nodes per job graph, no profiler attached, full speed.  For SET, the
+    batch-synchronous baseline and the mutex-queue model; the jobs/s of these arms is reported beside the gaps to show
+    what the stamps cost."""
+    from paper_2606_05495_b200.workloads import baseline_workload
+    out = {"how": "set_config.timestamps=1: %globaltimer at graph start (root node) and end (signal / last node); gap = start(next job on "
+                  "the stream) - end(previous), 3 timed steps per arm"}
+    todo = [(wl, ids)] + ([(baseline_workload(c), None) for c in range(5) if c != wl.config] if all_configs else [])
+    for w, job_ids in todo:
+        job_ids = list(range(w.jobs)) if job_ids is None else job_ids
+        p, r = LAYOUT[w.config]
+        res = {}
+        for mode in ("set", "batch_sync_graphs", "mutex_queue"):
+            for io_device in (False, True):
+                key = f"{mode}_{'device' if io_device else 'e2e'}"
+                try:
+                    a = run_arm(setlib, w, job_ids, mode, io_device, 3, 2, p, r, verify=0, flush=flush, opts={"timestamps": True})
+                    res[key] = dict(a["device_gaps"], jobs_per_s=round(a["jobs_per_s"], 1))
+                    g = res[key]
+                    log(f"[bench]   device gaps config{w.config} {key:28s} inter-job mean {g['gap_mean_us']:.2f} us p50 {g['gap_p50_us']:.2f} p99 "
+                        f"{g['gap_p99_us']:.2f}  job chain {g['job_mean_us']:.2f} us  streams busy {g['stream_busy_frac']:.3f}  {g['jobs_per_s']:.0f} jobs/s")
+                except Exception as e:
+                    res[key] = {"error": str(e)[:200]}
+                    log(f"[bench]   device gaps config{w.config} {key} failed: {e}")
+        out[f"config{w.config}"] = res
+    return out
+
+
 def workload_for(config, jobs_override=None):
     from paper_2606_05495_b200.workloads import baseline_workload
     wl = baseline_workload(config)
@@ -750,6 +783,8 @@ def main():
                     others[f"config{c}"] = {"error": str(e)[:300]}
                     log(f"[bench] config {c} failed: {e}")
             extra["workloads"] = others
+    if world == 1 and not args.no_gaps:
+        extra["device_gaps"] = device_gap_pass(setlib, wl, ids, args.suite == "all", flush)
     if world == 1 and args.sweep:
         extra["batch_sweep"] = batch_sweep(setlib, wl, ids, flush, not args.no_gaps)
     sampler.stop()

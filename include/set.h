@@ -184,6 +184,12 @@ typedef struct set_config {
     int32_t sm_copy_max_bytes;/* H2D/D2H copies of a fixed size up to this many bytes become kernel nodes
                                  (SET_K_COPY: the SMs read/write pinned host memory over the link) instead of
                                  copy-engine memcpy nodes; 0 => default (262144), -1 => never.                    */
+    int32_t timestamps;       /* 1: every job graph gets two extra one-thread kernel nodes that store the GPU's
+                                 %globaltimer when the graph starts (a root node beside the first copy) and when it
+                                 ends (the completion-signal node, or a last node of its own): the device-side gap
+                                 between consecutive jobs of a stream, measured at full speed without a profiler
+                                 attached; read with set_get_gap_stats.  0 (default): no such nodes.            */
+    int32_t reserved1;
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */
@@ -274,6 +280,21 @@ void set_host_free(set_ctx *ctx, void *p);
 set_status set_get_stats(set_ctx *ctx, set_stats *out);
 set_status set_reset_stats(set_ctx *ctx);
 
+/* Device-side timing of the jobs completed since create / set_reset_stats, from the timestamp nodes of
+ * set_config.timestamps = 1 (all zero otherwise).  A gap is  start(job k+1) - end(job k)  of two jobs that ran
+ * one after the other on the same stream (negative differences count as 0): the idle "white space" between
+ * jobs of PAPER.md:15-17 as the GPU saw it.  Collected in SET, batch-synchronous and mutex-queue modes.
+ * Single caller, drained context.  out: HOST. */
+typedef struct set_gap_stats {
+    uint64_t jobs;          /* jobs with both timestamps                                            */
+    uint64_t gaps;          /* job pairs                                                            */
+    double gap_mean_us, gap_p50_us, gap_p99_us, gap_max_us;
+    double job_mean_us;     /* mean of end - start of one job (its chain on the device)             */
+    double span_us;         /* last end - first start over all jobs                                 */
+    double stream_busy_frac;/* sum of job durations / (span * streams): how full the streams were   */
+} set_gap_stats;
+set_status set_get_gap_stats(set_ctx *ctx, set_gap_stats *out);
+
 /* HOST, NUL-terminated text of the first error on this context ("" if none).  Valid until destroy. */
 const char *set_last_error(set_ctx *ctx);
 
@@ -305,7 +326,9 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_BLUR3X3_U8     11  /* (const uint8* g, uint8* out, uint32 w, uint32 h)  clamp-to-edge          */
 #define SET_K_HIST256_U8     12  /* (const uint8* p, uint32* hist, uint32 w, uint32 h)  hist must be zeroed  */
 #define SET_K_SPIN           13  /* (uint32* scratch, uint32 ns)  debug delay stage (busy-waits ns)          */
-#define SET_K_SIGNAL         14  /* (uint32* flag)  *flag = 1 in mapped pinned HOST memory (SET_CB_FLAG_POLL) */
+#define SET_K_SIGNAL         14  /* (uint32* flag, uint64* stamp)  *flag = 1 in mapped pinned HOST memory
+                                    (SET_CB_FLAG_POLL); stamp != NULL: *stamp = %globaltimer first            */
+#define SET_K_STAMP          16  /* (uint64* stamp)  *stamp = %globaltimer (set_config.timestamps)               */
 #define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes)  copy by the SMs; src / dst may be
                                     pinned HOST or DEVICE memory                                              */
 

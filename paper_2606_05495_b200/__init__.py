@@ -72,7 +72,7 @@ class Config(C.Structure):
     _fields_ = [("struct_bytes", C.c_uint32), ("num_streams", C.c_int32), ("max_inflight", C.c_int32), ("mode", C.c_int32),
                 ("io", C.c_int32), ("queue_capacity", C.c_int32), ("num_dispatchers", C.c_int32), ("steal_policy", C.c_int32),
                 ("callback_mode", C.c_int32), ("device", C.c_int32), ("spin_us", C.c_int32), ("sm_copy_max_bytes", C.c_int32),
-                ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64)]
+                ("timestamps", C.c_int32), ("reserved1", C.c_int32), ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64)]
 
 
 class Stats(C.Structure):
@@ -85,9 +85,18 @@ class Stats(C.Structure):
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if n != "reserved"}
 
 
+class GapStats(C.Structure):
+    _fields_ = [("jobs", C.c_uint64), ("gaps", C.c_uint64), ("gap_mean_us", C.c_double), ("gap_p50_us", C.c_double),
+                ("gap_p99_us", C.c_double), ("gap_max_us", C.c_double), ("job_mean_us", C.c_double), ("span_us", C.c_double),
+                ("stream_busy_frac", C.c_double)]
+
+    def as_dict(self):
+        return {n: (int(getattr(self, n)) if n in ("jobs", "gaps") else round(float(getattr(self, n)), 4)) for n, _ in self._fields_}
+
+
 # every symbol include/set.h declares -- tests/test_abi.py checks the list against the header
 EXPORTS = ["set_create", "set_create_ex", "set_register_pipeline", "set_submit", "set_submit_dims", "set_submit_batch",
-           "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_get_stats", "set_reset_stats",
+           "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_get_stats", "set_reset_stats", "set_get_gap_stats",
            "set_last_error", "set_get_geometry", "set_time_stage", "set_builtin_kernel", "set_builtin_pipeline",
            "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler"]
 
@@ -118,6 +127,7 @@ def load():
     lib.set_host_free.restype = None
     lib.set_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.set_reset_stats.argtypes = [vp]
+    lib.set_get_gap_stats.argtypes = [vp, C.POINTER(GapStats)]
     lib.set_last_error.argtypes = [vp]
     lib.set_last_error.restype = C.c_char_p
     lib.set_get_geometry.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
@@ -160,7 +170,7 @@ class Context:
     def __init__(self, num_streams: int, max_inflight: int, mode: int = MODE_SET, io: int = IO_HOST, queue_capacity: int = 0,
                  num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_DEFAULT,
                  device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0,
-                 sm_copy_max_bytes: int = 0):
+                 sm_copy_max_bytes: int = 0, timestamps: bool = False):
         self._lib = load()
         self._h = C.c_void_p(None)
         cfg = Config()
@@ -169,6 +179,7 @@ class Context:
         cfg.queue_capacity, cfg.num_dispatchers, cfg.steal_policy = queue_capacity, num_dispatchers, steal_policy
         cfg.callback_mode, cfg.device, cfg.spin_us = callback_mode, device, spin_us
         cfg.sm_copy_max_bytes = sm_copy_max_bytes
+        cfg.timestamps = 1 if timestamps else 0
         self._streams_arr = None
         if streams is not None:
             self._streams_arr = (C.c_void_p * len(streams))(*[int(s) for s in streams])
@@ -261,6 +272,11 @@ class Context:
         s = Stats()
         self._check(self._lib.set_get_stats(self._h, C.byref(s)), "set_get_stats")
         return s.as_dict()
+
+    def gap_stats(self) -> dict:
+        g = GapStats()
+        self._check(self._lib.set_get_gap_stats(self._h, C.byref(g)), "set_get_gap_stats")
+        return g.as_dict()
 
     def reset_stats(self):
         self._lib.set_reset_stats(self._h)

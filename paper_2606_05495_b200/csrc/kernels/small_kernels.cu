@@ -221,9 +221,24 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
 // B200 a system fence costs 2.5 us idle and more under load even in a thread with no stores of its own (config 1 end
 // to end: 201 K jobs/s with the fence here, 190 K with the signal fused into the copy kernel behind a fence, 217 K
 // without; profiles/r1_bench.md), and the dependency edge already gives the ordering.
-extern "C" __global__ void set_k_signal(uint32_t* flag) {
+extern "C" __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp) {
     set_pdl_sync();
+    if (stamp) {  // set_config.timestamps: when the job ended on the device
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        *reinterpret_cast<volatile unsigned long long*>(stamp) = t;
+    }
     *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+}
+
+// K16: timestamp node of set_config.timestamps.  As a root of the job graph it runs when the graph starts (beside the
+// first copy); as the last node (modes without a signal node) when it ends.  One thread, one 8-byte store to mapped
+// pinned host memory.
+extern "C" __global__ void set_k_stamp(unsigned long long* stamp) {
+    set_pdl_sync();
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    *reinterpret_cast<volatile unsigned long long*>(stamp) = t;
 }
 
 // K15: copy node executed by the SMs.  A job of configs 0-1 moves 16-128 KB per direction;

@@ -93,6 +93,7 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_SPIN: return (const void*)set_k_spin;
         case SET_K_SIGNAL: return (const void*)set_k_signal;
         case SET_K_COPY: return (const void*)set_k_copy;
+        case SET_K_STAMP: return (const void*)set_k_stamp;
         default: return nullptr;
     }
 }

@@ -101,6 +101,17 @@ struct set_ctx final : public Backend {
     cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
     cudaGraphNode_t signal_node = nullptr;     // SET_CB_FLAG_POLL: last node, stores the slot's completion word
     cudaGraphNode_t host_node = nullptr;       // SET_CB_HOST_NODE: last node, runs Algorithm 3 on the driver's callback thread
+    // set_config.timestamps: per slot one 64-byte line of mapped pinned memory, [0] = %globaltimer at graph start, [1] = at end
+    bool stamps = false;
+    unsigned long long* ts_host = nullptr;
+    unsigned long long* ts_dev = nullptr;
+    cudaGraphNode_t stamp_start_node = nullptr, stamp_end_node = nullptr;
+    struct StampRec {
+        uint32_t stream;
+        uint64_t start, end;
+    };
+    SpinLock stamp_lock;
+    std::vector<StampRec> stamp_recs;  // one per completed job, reduced by set_get_gap_stats
     // SM copies (set_config.sm_copy_max_bytes): h2d_nodes[i] / d2h_nodes[i] are SET_K_COPY kernel nodes where set
     bool h2d_sm[SET_MAX_BUFFERS] = {}, d2h_sm[SET_MAX_BUFFERS] = {};
     int n_sm_copies = 0;
@@ -409,6 +420,16 @@ int set_ctx::build_graph() {
             root_is_kernel.push_back(h2d_sm[i]);
         }
     }
+    if (stamps) {  // a root of its own, beside the first copies: runs when the graph starts, nothing waits for it
+        unsigned long long* p = ts_dev;
+        void* args[1] = {&p};
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void*>(set_builtin_kernel(SET_K_STAMP));
+        kp.gridDim = dim3(1);
+        kp.blockDim = dim3(1);
+        kp.kernelParams = args;
+        CK(cudaGraphAddKernelNode(&stamp_start_node, graph, nullptr, 0, &kp));
+    }
     kern_nodes.resize(stages.size());
     cudaGraphNode_t prev = nullptr;
     for (size_t s = 0; s < stages.size(); ++s) {
@@ -460,7 +481,8 @@ int set_ctx::build_graph() {
             leaf_is_kernel.push_back(true);
         }
         uint32_t* flag = flags_dev;
-        void* args[1] = {&flag};
+        unsigned long long* stamp = stamps ? ts_dev + 1 : nullptr;
+        void* args[2] = {&flag, &stamp};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
         kp.gridDim = dim3(1);
@@ -468,6 +490,20 @@ int set_ctx::build_graph() {
         kp.kernelParams = args;
         CK(cudaGraphAddKernelNode(&signal_node, graph, nullptr, 0, &kp));
         for (size_t l = 0; l < leaves.size(); ++l) CK(depend(leaves[l], signal_node, pdl && leaves.size() == 1 && leaf_is_kernel[l]));
+        // the start stamp is a root nothing else waits for; this edge only makes sure it has run before the end stamp
+        if (stamps) CK(depend(stamp_start_node, signal_node, false));
+    } else if (stamps) {  // no signal node in this mode: the end timestamp gets a last node of its own
+        if (leaves.empty()) leaves.push_back(prev);
+        unsigned long long* p = ts_dev + 1;
+        void* args[1] = {&p};
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void*>(set_builtin_kernel(SET_K_STAMP));
+        kp.gridDim = dim3(1);
+        kp.blockDim = dim3(1);
+        kp.kernelParams = args;
+        leaves.push_back(stamp_start_node);  // not on the critical path: it only has to have run before the end stamp
+        CK(cudaGraphAddKernelNode(&stamp_end_node, graph, leaves.data(), leaves.size(), &kp));
+        leaves.assign(1, stamp_end_node);
     }
     if (cfg.mode == SET_MODE_SET && cfg.callback_mode == SET_CB_HOST_NODE) {
         if (leaves.empty()) leaves.push_back(prev);
@@ -556,13 +592,30 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             }
         if (signal_node && es.bound_slot != slot) {
             uint32_t* flag = flags_dev + (size_t)slot * kFlagStride;
-            void* args[1] = {&flag};
+            unsigned long long* stamp = stamps ? ts_dev + (size_t)slot * 8 + 1 : nullptr;
+            void* args[2] = {&flag, &stamp};
             cudaKernelNodeParams kp{};
             kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
             kp.gridDim = dim3(1);
             kp.blockDim = dim3(1);
             kp.kernelParams = args;
             CK(cudaGraphExecKernelNodeSetParams(es.exec, signal_node, &kp));
+        }
+        if (stamps && es.bound_slot != slot) {
+            unsigned long long* p0 = ts_dev + (size_t)slot * 8;
+            unsigned long long* p1 = p0 + 1;
+            cudaKernelNodeParams kp{};
+            kp.func = const_cast<void*>(set_builtin_kernel(SET_K_STAMP));
+            kp.gridDim = dim3(1);
+            kp.blockDim = dim3(1);
+            void* a0[1] = {&p0};
+            kp.kernelParams = a0;
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, stamp_start_node, &kp));
+            if (stamp_end_node) {
+                void* a1[1] = {&p1};
+                kp.kernelParams = a1;
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, stamp_end_node, &kp));
+            }
         }
         if (host_node && es.bound_slot != slot) {
             cudaHostNodeParams hp{};
@@ -650,7 +703,16 @@ int set_ctx::poll() {
     return 0;
 }
 
-void set_ctx::finish(int exec, int, const JobDesc&) {
+void set_ctx::finish(int exec, int slot, const JobDesc&) {
+    if (stamps) {
+        StampRec r{(uint32_t)(slot % S), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
+                   __atomic_load_n(&ts_host[(size_t)slot * 8 + 1], __ATOMIC_ACQUIRE)};
+        if (r.start != 0 && r.end >= r.start) {
+            stamp_lock.lock();
+            if (stamp_recs.size() < (1u << 22)) stamp_recs.push_back(r);
+            stamp_lock.unlock();
+        }
+    }
     ExecState& es = execs[exec];
     if (es.staged) {  // staged D2H: pinned ring -> caller's pageable memory, on the callback thread
         memcpy(es.user_out, es.stage_out, es.out_bytes);
@@ -959,6 +1021,18 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
         memset(c->flags_host, 0, bytes);
         c->flag_poll = true;
     }
+    if (cfg.timestamps) {
+        size_t bytes = (size_t)c->b * 8 * sizeof(unsigned long long);
+        if (cudaHostAlloc((void**)&c->ts_host, bytes, cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess ||
+            cudaHostGetDevicePointer((void**)&c->ts_dev, c->ts_host, 0) != cudaSuccess) {
+            cudaGetLastError();
+            delete c;
+            return SET_ERR_CUDA;
+        }
+        memset(c->ts_host, 0, bytes);
+        c->stamps = true;
+        c->stamp_recs.reserve(1 << 16);
+    }
     if (cfg.mode == SET_MODE_SET)
         c->sched.reset(new Scheduler(c, c->S, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
     *out = c;
@@ -1169,6 +1243,7 @@ set_status set_destroy(set_ctx* c) {
     if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
     if (c->flags_host) cudaFreeHost(c->flags_host);
+    if (c->ts_host) cudaFreeHost(c->ts_host);
     for (int s = 0; s < c->S; ++s) {
         if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
         if (c->notify[s]) cudaStreamDestroy(c->notify[s]);
@@ -1255,7 +1330,50 @@ set_status set_reset_stats(set_ctx* c) {
         st.ns_submit = 0; st.ns_launch = 0; st.ns_callback = 0; st.max_inflight = 0;
     }
     c->base_submitted = 0; c->base_completed = 0; c->base_launched = 0; c->base_ns_submit = 0; c->base_ns_launch = 0;
-    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->copy_nodes = 0; c->ns_bind = 0; c->ns_sync = 0;
+    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->copy_nodes = 0;
+    c->stamp_lock.lock();
+    c->stamp_recs.clear();
+    c->stamp_lock.unlock(); c->ns_bind = 0; c->ns_sync = 0;
+    return SET_OK;
+}
+
+set_status set_get_gap_stats(set_ctx* c, set_gap_stats* out) {
+    if (!c || !out) return SET_ERR_INVALID;
+    memset(out, 0, sizeof(*out));
+    c->stamp_lock.lock();
+    std::vector<set_ctx::StampRec> v = c->stamp_recs;
+    c->stamp_lock.unlock();
+    if (v.empty()) return SET_OK;
+    // jobs of one stream ran one after the other: order them by start time, whatever order their completions were seen in
+    std::sort(v.begin(), v.end(), [](const set_ctx::StampRec& a, const set_ctx::StampRec& b) {
+        return a.stream != b.stream ? a.stream < b.stream : a.start < b.start;
+    });
+    std::vector<double> gaps;
+    gaps.reserve(v.size());
+    double job_sum = 0;
+    uint64_t t0 = UINT64_MAX, t1 = 0;
+    for (size_t i = 0; i < v.size(); ++i) {
+        job_sum += (double)(v[i].end - v[i].start) * 1e-3;
+        t0 = std::min(t0, v[i].start);
+        t1 = std::max(t1, v[i].end);
+        if (i > 0 && v[i - 1].stream == v[i].stream)
+            gaps.push_back(v[i].start > v[i - 1].end ? (double)(v[i].start - v[i - 1].end) * 1e-3 : 0.0);
+    }
+    out->jobs = v.size();
+    out->gaps = gaps.size();
+    out->job_mean_us = job_sum / (double)v.size();
+    out->span_us = (double)(t1 - t0) * 1e-3;
+    out->stream_busy_frac = out->span_us > 0 ? job_sum / (out->span_us * (double)c->S) : 0.0;
+    if (!gaps.empty()) {
+        std::sort(gaps.begin(), gaps.end());
+        double sum = 0;
+        for (double g : gaps) sum += g;
+        auto q = [&](double p) { return gaps[std::min(gaps.size() - 1, (size_t)(p * (double)(gaps.size() - 1) + 0.5))]; };
+        out->gap_mean_us = sum / (double)gaps.size();
+        out->gap_p50_us = q(0.50);
+        out->gap_p99_us = q(0.99);
+        out->gap_max_us = gaps.back();
+    }
     return SET_OK;
 }
 

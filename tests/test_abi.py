@@ -18,7 +18,7 @@ def _declared_symbols():
 def test_library_exports_every_declared_symbol(libset):
     lib = libset.load()
     declared = _declared_symbols()
-    assert len(declared) >= 18
+    assert len(declared) >= 19
     for name in declared:
         assert hasattr(lib, name), f"{name} declared in include/set.h but not exported by libset.so"
     assert sorted(libset.EXPORTS) == declared
@@ -66,7 +66,8 @@ def test_struct_sizes_match_header(libset):
     assert C.sizeof(libset.SizeExpr) == 24 and C.sizeof(libset.GridRule) == 32 and C.sizeof(libset.Tmap2D) == 40
     assert C.sizeof(libset.ArgDesc) == 8 + 24 + 8 + 40
     assert C.sizeof(libset.Stats) == 20 * 8
-    assert C.sizeof(libset.Config) == 12 * 4 + 8 + 8 + 8
+    assert C.sizeof(libset.Config) == 14 * 4 + 8 + 8 + 8
+    assert C.sizeof(libset.GapStats) == 9 * 8
 
 
 def test_invalid_arguments_are_rejected_without_a_device(libset):

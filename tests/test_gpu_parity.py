@@ -343,3 +343,51 @@ def test_full_size_config3_sampled_entries(libset):
         got = inputgen.bf16_bits_to_f64(outs[k].view(np.uint16).reshape(M, N)[ms, ns])
         assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 2e-2
         assert np.abs(got - ref).max() <= 0.05 * max(1.0, np.abs(ref).max())
+
+
+@pytest.mark.parametrize("mode", [0, 2, 4])
+@pytest.mark.parametrize("config", [1, 4])
+def test_device_timestamps_give_per_stream_gaps(libset, config, mode):
+    """set_config.timestamps: two stamp nodes per job graph, gaps between consecutive jobs of a stream from the GPU's own
+    clock.  The results stay the oracle's, every job is stamped, and the numbers are sane."""
+    from paper_2606_05495_b200.workloads import PinnedArena, small_workload
+    wl = small_workload(config)
+    n = min(wl.jobs, 96)
+    ctx = libset.Context(wl.num_streams, wl.max_inflight, mode=mode, timestamps=True)
+    try:
+        ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=True)
+        ins = [wl.make_input(j) for j in range(n)]
+        dims = [wl.dims(j) for j in range(n)]
+        arena = PinnedArena(ctx, sum(wl.in_bytes(d) + wl.out_bytes(d) + 1024 for d in dims))
+        outs = []
+        for j in range(n):
+            a_in, v_in = arena.take(wl.in_bytes(dims[j]))
+            v_in[:] = ins[j]
+            a_out, v_out = arena.take(wl.out_bytes(dims[j]))
+            v_out[:] = SENTINEL
+            outs.append(v_out)
+            ctx.submit(j, a_in, a_out, dims[j] if config == 4 else None)
+        ctx.drain()
+        for j in range(n):
+            compare(wl, np.array(outs[j], copy=True), oracle_out(wl, ins[j], dims[j]))
+        g = ctx.gap_stats()
+        assert g["jobs"] == n
+        assert n - wl.num_streams <= g["gaps"] <= n - 1
+        assert 1.0 < g["job_mean_us"] < 5000.0 and 0.0 <= g["gap_mean_us"] <= g["gap_max_us"] < 1e6
+        assert g["gap_p50_us"] <= g["gap_p99_us"] <= g["gap_max_us"] and 0.0 < g["stream_busy_frac"] <= 1.0001
+        ctx.reset_stats()
+        assert ctx.gap_stats()["jobs"] == 0
+        outs = None
+        arena.free()
+    finally:
+        ctx.close()
+
+
+def test_gap_stats_are_zero_without_timestamps(libset):
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(0)
+    ctx = libset.Context(wl.num_streams, wl.max_inflight)
+    ctx.register_builtin(0)
+    assert ctx.gap_stats() == {"jobs": 0, "gaps": 0, "gap_mean_us": 0.0, "gap_p50_us": 0.0, "gap_p99_us": 0.0, "gap_max_us": 0.0,
+                               "job_mean_us": 0.0, "span_us": 0.0, "stream_busy_frac": 0.0}
+    ctx.close()
