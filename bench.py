@@ -573,8 +573,9 @@ def device_gap_pass(setlib, wl, ids, all_configs: bool, flush):
     todo = [(wl, ids)] + ([(baseline_workload(c), None) for c in range(5) if c != wl.config] if all_configs else [])
     for w, job_ids in todo:
         job_ids = list(range(w.jobs)) if job_ids is None else job_ids
+        job_ids = job_ids[:{0: 256, 1: 10000, 2: 64, 3: 200, 4: 1024}[w.config]]  # keeps the default run within minutes
         p, r = LAYOUT[w.config]
-        res = {}
+        res = {"jobs_per_step": len(job_ids)}
         for mode in ("set", "batch_sync_graphs", "mutex_queue"):
             for io_device in (False, True):
                 key = f"{mode}_{'device' if io_device else 'e2e'}"
