@@ -391,3 +391,41 @@ def test_gap_stats_are_zero_without_timestamps(libset):
     assert ctx.gap_stats() == {"jobs": 0, "gaps": 0, "gap_mean_us": 0.0, "gap_p50_us": 0.0, "gap_p99_us": 0.0, "gap_max_us": 0.0,
                                "job_mean_us": 0.0, "span_us": 0.0, "stream_busy_frac": 0.0}
     ctx.close()
+
+
+def test_every_output_is_there_when_the_completion_word_is_seen(libset):
+    """Full-rate check of the fence-free signal node: 30,000 config-1 jobs at the bench geometry (8 streams, 32
+    in flight, SM copies, PDL edges), every 4-byte output pre-filled with a sentinel pattern and read as soon as
+    set_drain returns.  A completion word that reached the host before its job's output would release the slot early
+    and leave sentinel bytes (or a neighbour's result) behind."""
+    import ctypes as C
+    from paper_2606_05495_b200.workloads import PinnedArena, baseline_workload
+    wl = baseline_workload(1)
+    n, npool = 30000, 128
+    ctx = libset.Context(wl.num_streams, wl.max_inflight)
+    try:
+        ctx.register_builtin(1, 0, list(wl.params), pdl=True)
+        ins = [wl.make_input(j) for j in range(npool)]
+        want = np.array([oracle_out(wl, x, (1, 1, 1, 1)).view(np.float32)[0] for x in ins], np.float32)
+        arena = PinnedArena(ctx, npool * (wl.in_bytes() + 256) + 4 * n + 4096)
+        in_ptrs = []
+        for x in ins:
+            a, v = arena.take(wl.in_bytes())
+            v[:] = x
+            in_ptrs.append(a)
+        a_out, v_out = arena.take(4 * n)
+        out_f = v_out.view(np.float32)
+        pi = (C.c_void_p * n)(*[in_ptrs[k % npool] for k in range(n)])
+        po = (C.c_void_p * n)(*[a_out + 4 * k for k in range(n)])
+        for rep in range(3):
+            v_out[:] = SENTINEL
+            ctx.submit_batch(pi, po)
+            ctx.drain()
+            got = np.array(out_f, copy=True)
+            ref = want[np.arange(n) % npool]
+            bad = np.nonzero(np.abs(got - ref) > 1e-6 * np.abs(ref))[0]
+            assert bad.size == 0, f"rep {rep}: {bad.size} outputs wrong, first job {bad[0]}: {got[bad[0]]} vs {ref[bad[0]]}"
+        out_f = v_out = None
+        arena.free()
+    finally:
+        ctx.close()
