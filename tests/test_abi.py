@@ -50,6 +50,10 @@ def test_builtin_descriptors_roundtrip_struct_layout(libset):
     assert ns == 3 and nb == 3 and st[2].args[1].kind == libset.ARG_DIM and st[2].args[1].index == 3
     with pytest.raises(libset.SetError):
         libset.builtin_pipeline(7)
+    # degenerate sizes are rejected when the descriptors are built (an empty job has no graph)
+    for config, params in ((0, [0]), (1, [0]), (2, [0, 16, 1]), (2, [16, 16, 0]), (2, [16, 16, 17]), (3, [0, 8, 8]), (3, [8, 12, 8]), (4, [0, 4])):
+        with pytest.raises(libset.SetError):
+            libset.builtin_pipeline(config, params=params)
     assert libset.load().set_builtin_kernel(99) is None
 
 

@@ -429,3 +429,12 @@ def test_every_output_is_there_when_the_completion_word_is_seen(libset):
         arena.free()
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("n", [32768, 32772])
+def test_config1_around_the_sm_copy_limit(libset, n):
+    """8n = 262,144 bytes is the largest H2D copy the SMs do by default; 4 floats more and the same copy becomes a
+    copy-engine memcpy node.  Both sides of the limit compute the same thing."""
+    from paper_2606_05495_b200.workloads import Workload
+    st = check(libset, Workload(1, (n,), jobs=12, num_streams=2, max_inflight=4), list(range(12)), pdl=True)
+    assert st["copy_nodes"] == 12 * (2 if n == 32768 else 1)
