@@ -38,6 +38,6 @@ constexpr int kJacobiRows = 16;        // rows per block
 constexpr int kJacobiCols = 1024;      // columns per block (256 threads x float4)
 constexpr unsigned kJacobiUnroll = 4;  // rows whose loads are in flight together
 constexpr int kGrayPixPerBlock = 256 * 16;
-constexpr int kBlurTileW = 512, kBlurTileH = 32;  // 32 lanes x 16 pixels, 8 warps x 4 rows
-constexpr int kHistPixPerBlock = 256 * 16 * 4;
+constexpr int kBlurTileW = 512, kBlurTileH = 16;  // 32 lanes x 16 pixels, 4 warps x 4 rows (a 1280 x 720 frame: 135 blocks)
+constexpr int kHistPixPerBlock = 256 * 16;  // one 128-bit load per thread; a 1280 x 720 frame: 225 blocks
 constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words

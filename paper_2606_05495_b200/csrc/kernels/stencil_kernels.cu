@@ -124,7 +124,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_rgb2gray_u8(const uint8_
 // ------------------------------------------------------------------------------------------------------------
 // K11: 3x3 blur [1 2 1; 2 4 2; 1 2 1] >> 4, clamp-to-edge.  Evaluated separably -- horizontal [1 2 1] sums per
 // row (<= 1020), then vertical [1 2 1] (<= 4080) and ONE final >> 4 -- which is exactly the 2-D form in integers.
-// blockDim = (32, 8), tile = 512 pixels x 32 rows: a lane owns 16 pixels (one 128-bit word) of 4 consecutive rows.
+// blockDim = (32, 4), tile = 512 pixels x 16 rows: a lane owns 16 pixels (one 128-bit word) of 4 consecutive rows.
 // All six input rows of a lane (4 + the row above and below) are loaded before the first add, so 96 bytes per
 // thread are in flight; horizontal neighbours come from the adjacent lanes by shuffle.  Sums are kept as two 16-bit
 // halves per register (even pixels / odd pixels of a 32-bit word): every partial sum fits 16 bits, so packed adds
@@ -218,18 +218,20 @@ extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t
 extern "C" __global__ void __launch_bounds__(256) set_k_hist256_u8(const uint8_t* __restrict__ p, uint32_t* __restrict__ hist,
                                                                    uint32_t w, uint32_t h) {
     set_pdl_sync();
+    static_assert(kHistPixPerBlock == 256 * 16, "one 128-bit load per thread");
     const uint32_t n = w * h;
     __shared__ uint32_t sh[8][256];
     const int tid = threadIdx.x, wid = tid >> 5;
+    const uint32_t end = min((blockIdx.x + 1u) * (uint32_t)kHistPixPerBlock, n);
+    const uint32_t i = blockIdx.x * (uint32_t)kHistPixPerBlock + tid * 16u;
+    const bool full = i + 15 < end;
+    uint4 v = make_uint4(0, 0, 0, 0);
+    if (full) v = __ldg(reinterpret_cast<const uint4*>(p + i));  // in flight while the histograms are cleared
     for (int k = tid; k < 8 * 256; k += 256) (&sh[0][0])[k] = 0;
     __syncthreads();
-    const uint32_t base = blockIdx.x * (uint32_t)kHistPixPerBlock;
-    const uint32_t end = min(base + (uint32_t)kHistPixPerBlock, n);
     uint32_t* my = sh[wid];
-    uint32_t i = base + tid * 16u;
-    for (; i + 15 < end; i += 256u * 16u) {
-        uint4 v = __ldg(reinterpret_cast<const uint4*>(p + i));
-        uint32_t wds[4] = {v.x, v.y, v.z, v.w};
+    if (full) {
+        const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             atomicAdd(&my[wds[k] & 0xff], 1u);
@@ -237,8 +239,9 @@ extern "C" __global__ void __launch_bounds__(256) set_k_hist256_u8(const uint8_t
             atomicAdd(&my[(wds[k] >> 16) & 0xff], 1u);
             atomicAdd(&my[wds[k] >> 24], 1u);
         }
+    } else {
+        for (uint32_t j = i; j < end; ++j) atomicAdd(&my[p[j]], 1u);  // ragged tail of the image
     }
-    for (uint32_t j = i; j < end && j < i + 16; ++j) atomicAdd(&my[p[j]], 1u);  // ragged tail of this block's range
     __syncthreads();
     uint32_t s = 0;
 #pragma unroll

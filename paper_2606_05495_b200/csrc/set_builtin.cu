@@ -203,7 +203,7 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             nb = 4;
             st[ns++] = stage(SET_K_RGB2GRAY_U8, grid_div(scaled(1, WH), kGrayPixPerBlock), grid_fixed(1), 256, 1, 0,
                              {arg_buf(0), arg_buf(1), arg_dim(0), arg_dim(1)});
-            st[ns++] = stage(SET_K_BLUR3X3_U8, grid_div(scaled(1, 0x1), kBlurTileW), grid_div(scaled(1, 0x2), kBlurTileH), 32, 8, 0,
+            st[ns++] = stage(SET_K_BLUR3X3_U8, grid_div(scaled(1, 0x1), kBlurTileW), grid_div(scaled(1, 0x2), kBlurTileH), 32, 4, 0,
                              {arg_buf(1), arg_buf(2), arg_dim(0), arg_dim(1)});
             st[ns++] = stage(SET_K_HIST256_U8, grid_div(scaled(1, WH), kHistPixPerBlock), grid_fixed(1), 256, 1, 0,
                              {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});

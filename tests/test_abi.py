@@ -45,7 +45,7 @@ def test_builtin_descriptors_roundtrip_struct_layout(libset):
     st, ns, bf, nb, hin, hout = libset.builtin_pipeline(4)
     assert (ns, nb, hin, hout) == (3, 4, 6220800, 2073600 + 1024)
     assert bf[0].h2d_bytes.per_unit == 3 and bf[0].h2d_bytes.dim_mask == 3 and bf[3].flags == libset.BUF_ZERO
-    assert bf[3].d2h_host_off.per_unit == 1 and st[1].block[0] == 32 and st[1].block[1] == 8
+    assert bf[3].d2h_host_off.per_unit == 1 and st[1].block[0] == 32 and st[1].block[1] == 4
     st, ns, bf, nb, _, _ = libset.builtin_pipeline(0, variant=libset.VARIANT_SPIN)
     assert ns == 3 and nb == 3 and st[2].args[1].kind == libset.ARG_DIM and st[2].args[1].index == 3
     with pytest.raises(libset.SetError):
