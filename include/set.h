@@ -312,8 +312,8 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
  * Built-in stage kernels (hand-written sm_100a CUDA, csrc/kernels/) and the five pipelines of
  * BASELINE.json:configs[0..4].  Operation definitions: DESIGN.md §"Stage kernels".
  */
-#define SET_K_SCAN_I32        1  /* (const int32* in, int32* out, uint32 n)  inclusive prefix sum, 1 block   */
-#define SET_K_HIST_MOD64      2  /* (const int32* in, uint32* hist, uint32 n) 64 bins of v mod 64, 1 block   */
+#define SET_K_SCAN_I32        1  /* (const int32* in, int32* out, uint32 n)  inclusive prefix sum, 1 block of 1024 */
+#define SET_K_HIST_MOD64      2  /* (const int32* in, uint32* hist, uint32 n) 64 bins of v mod 64, 1 block of 256 */
 #define SET_K_AFFINE_F32      3  /* (const float* x, float* y, uint32 n)  y = fl(fl(2.5x)+0.1)               */
 #define SET_K_ADD_BIAS_F32    4  /* (float* y, const float* bias, uint32 n)  y = fl(y + bias)                */
 #define SET_K_RELU_F32        5  /* (float* y, uint32 n)  y = max(y,0)                                       */

@@ -77,30 +77,46 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t*
     }
 }
 
-// K2: hist[b] = #{i : v[i] mod 64 == b}, v >= 0 (reading C0-3), one block of 1024 threads.
-// One private 64-bin histogram per warp in shared memory (32 x 64 counters) keeps atomic contention inside a
-// warp; the 32 copies are then summed, one bin per thread.
-extern "C" __global__ void __launch_bounds__(1024) set_k_hist_mod64(const int32_t* __restrict__ in, uint32_t* __restrict__ hist,
-                                                                    uint32_t n) {
+// K2: hist[b] = #{i : v[i] mod 64 == b}, v >= 0 (reading C0-3), one block of 256 threads.
+// Every thread's first four 128-bit loads are issued before the shared histograms are cleared.  One private 64-bin
+// histogram per warp in shared memory (8 x 64 counters) keeps atomic contention inside a warp; the 8 copies are then
+// summed, one bin per thread.
+extern "C" __global__ void __launch_bounds__(256) set_k_hist_mod64(const int32_t* __restrict__ in, uint32_t* __restrict__ hist,
+                                                                   uint32_t n) {
     set_pdl_sync();
-    __shared__ uint32_t h[32][64 + 1];
+    __shared__ uint32_t h[8][64 + 1];
     const int tid = threadIdx.x, wid = tid >> 5;
-    for (int k = tid; k < 32 * 65; k += 1024) (&h[0][0])[k] = 0;
-    __syncthreads();
     const uint32_t n4 = n / 4;
-    for (uint32_t i = tid; i < n4; i += 1024) {
+    int4 first[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t i = tid + 256u * k;
+        first[k] = i < n4 ? reinterpret_cast<const int4*>(in)[i] : make_int4(0, 0, 0, 0);
+    }
+    for (int k = tid; k < 8 * 65; k += 256) (&h[0][0])[k] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (tid + 256u * k < n4) {
+            atomicAdd(&h[wid][first[k].x & 63], 1u);
+            atomicAdd(&h[wid][first[k].y & 63], 1u);
+            atomicAdd(&h[wid][first[k].z & 63], 1u);
+            atomicAdd(&h[wid][first[k].w & 63], 1u);
+        }
+    }
+    for (uint32_t i = tid + 1024u; i < n4; i += 256) {
         int4 v = reinterpret_cast<const int4*>(in)[i];
         atomicAdd(&h[wid][v.x & 63], 1u);
         atomicAdd(&h[wid][v.y & 63], 1u);
         atomicAdd(&h[wid][v.z & 63], 1u);
         atomicAdd(&h[wid][v.w & 63], 1u);
     }
-    for (uint32_t i = n4 * 4 + tid; i < n; i += 1024) atomicAdd(&h[wid][in[i] & 63], 1u);
+    for (uint32_t i = n4 * 4 + tid; i < n; i += 256) atomicAdd(&h[wid][in[i] & 63], 1u);
     __syncthreads();
     if (tid < 64) {
         uint32_t s = 0;
 #pragma unroll
-        for (int w = 0; w < 32; ++w) s += h[w][tid];
+        for (int w = 0; w < 8; ++w) s += h[w][tid];
         hist[tid] = s;
     }
 }

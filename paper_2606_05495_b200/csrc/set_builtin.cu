@@ -119,7 +119,7 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[1].d2h_bytes = fixed(out_bytes);
             nb = 2;
             st[ns++] = stage(SET_K_SCAN_I32, grid_fixed(1), grid_fixed(1), 1024, 1, 0, {arg_buf(0), arg_buf(1), arg_u32(n)});
-            st[ns++] = stage(SET_K_HIST_MOD64, grid_fixed(1), grid_fixed(1), 1024, 1, 0,
+            st[ns++] = stage(SET_K_HIST_MOD64, grid_fixed(1), grid_fixed(1), 256, 1, 0,
                              {variant == 1 ? arg_buf(0) : arg_buf(1), arg_buf(1, fixed(4ull * n)), arg_u32(n)});
             break;
         }

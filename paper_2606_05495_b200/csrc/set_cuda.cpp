@@ -707,6 +707,11 @@ void set_ctx::finish(int exec, int slot, const JobDesc&) {
     if (stamps) {
         StampRec r{(uint32_t)(slot % S), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
                    __atomic_load_n(&ts_host[(size_t)slot * 8 + 1], __ATOMIC_ACQUIRE)};
+        // The signal thread stores the end stamp and then the completion word, unfenced: the two stores may reach host
+        // memory in either order (seen on B200, rarely -- the reason the job's OUTPUT is never written by
+        // the grid that stores the word).  An end stamp older than the start stamp is the previous job's: wait for ours.
+        for (uint64_t t0 = now_ns(); r.end < r.start && now_ns() - t0 < 200000;)
+            r.end = __atomic_load_n(&ts_host[(size_t)slot * 8 + 1], __ATOMIC_ACQUIRE);
         if (r.start != 0 && r.end >= r.start) {
             stamp_lock.lock();
             if (stamp_recs.size() < (1u << 22)) stamp_recs.push_back(r);

@@ -29,7 +29,7 @@ def test_builtin_descriptors_roundtrip_struct_layout(libset):
     # these fields would come back as garbage
     st, ns, bf, nb, hin, hout = libset.builtin_pipeline(0)
     assert (ns, nb, hin, hout) == (2, 2, 16384, 16640)
-    assert st[0].block[0] == 1024 and st[0].num_args == 3 and st[0].args[2].kind == libset.ARG_IMM32 and st[0].args[2].imm == 4096
+    assert st[0].block[0] == 1024 and st[1].block[0] == 256 and st[0].num_args == 3 and st[0].args[2].kind == libset.ARG_IMM32 and st[0].args[2].imm == 4096
     assert st[1].args[1].kind == libset.ARG_BUFFER and st[1].args[1].index == 1 and st[1].args[1].offset.fixed == 16384
     assert bf[0].h2d_bytes.fixed == 16384 and bf[1].d2h_bytes.fixed == 16640 and bf[1].bytes == 16640
     assert st[0].func == libset.load().set_builtin_kernel(1) and st[0].func
