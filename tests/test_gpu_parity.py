@@ -439,3 +439,42 @@ def test_config1_around_the_sm_copy_limit(libset, n):
     from paper_2606_05495_b200.workloads import Workload
     st = check(libset, Workload(1, (n,), jobs=12, num_streams=2, max_inflight=4), list(range(12)), pdl=True)
     assert st["copy_nodes"] == 12 * (2 if n == 32768 else 1)
+
+
+def test_config3_gelu_epilogue_within_one_bf16_ulp(libset):
+    """K9 evaluates erfc by a branch-free formula (C3-3) instead of calling erff.  With A = 0 the output is
+    bf16(GELU(bias)) exactly, so the epilogue alone is compared with the oracle's double-precision erf: over biases from -9
+    to 9 the two bf16 results may differ by at most one unit in the last place where |GELU| >= 1e-3 (almost all must be
+    identical) and by at most 4e-6 (one bf16 ulp at 1e-3) in the far negative tail."""
+    from paper_2606_05495_b200.workloads import PinnedArena, Workload
+    M, N, K = 128, 2048, 64
+    wl = Workload(3, (M, N, K), jobs=1, num_streams=1, max_inflight=1)
+    a = np.zeros((M, K), np.uint16)
+    b = inputgen.f32_to_bf16_bits(inputgen.gaussian(3, 0, 1, K * N).astype(np.float32)).reshape(K, N)
+    bias = np.linspace(-9.0, 9.0, N).astype(np.float32)
+    image = inputgen.config3_pack(a, b, bias)
+    ctx = libset.Context(1, 1)
+    try:
+        ctx.register_builtin(3, 0, [M, N, K])
+        arena = PinnedArena(ctx, image.size + 2 * M * N + 4096)
+        a_in, v_in = arena.take(image.size)
+        v_in[:] = image
+        a_out, v_out = arena.take(2 * M * N)
+        ctx.submit(0, a_in, a_out)
+        ctx.drain()
+        got = np.array(v_out, copy=True).view(np.uint16).reshape(M, N)
+        ref = oracle_out(wl, image, (1, 1, 1, 1)).view(np.uint16).reshape(M, N)
+        v_in = v_out = None
+        arena.free()
+    finally:
+        ctx.close()
+    assert np.array_equal(got, np.broadcast_to(got[0], got.shape))          # every row sees the same bias
+    # where GELU is not negligible: bf16 bit patterns of equal sign are ordered like the values, compare in units in the
+    # last place; in the far negative tail (|GELU| < 1e-3) the formula's absolute error bound applies instead
+    g, r = inputgen.bf16_bits_to_f64(got), inputgen.bf16_bits_to_f64(ref)
+    big = np.abs(r) >= 1e-3
+    assert np.all(((got >> 15) == (ref >> 15))[big])
+    ulp = np.abs((got & 0x7fff).astype(np.int32) - (ref & 0x7fff).astype(np.int32))
+    assert ulp[big].max() <= 1
+    assert (ulp[big] == 0).mean() > 0.98
+    assert np.abs(g - r)[~big].max() <= 4e-6              # one bf16 ulp just below 1e-3 is 3.8e-6
