@@ -149,6 +149,7 @@ struct set_ctx final : public Backend {
     // SET_DRIVER_LOCK=1 (environment, read at create): every graph update and graph launch takes this one lock.
     // Only for runs under Nsight Compute 2025.2, whose injection library double-frees when one thread updates a
     // graph executable while another thread is inside cudaGraphLaunch (profiles/r1_ncu.md); never set for timing.
+    uint32_t copy_max_blocks = 0;  // SET_COPY_MAX_BLOCKS (environment): blocks per SM copy that reads host memory; 0 = default (8)
     bool driver_lock = false;
     std::mutex driver_mu;
 
@@ -298,6 +299,14 @@ void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const v
     ca.kp = cudaKernelNodeParams{};
     ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
     uint32_t pieces = (ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK;
+    // Reads of pinned host memory share the link with the GPU's own fetches of launch commands: eight streams that each
+    // put 128 KB of reads in flight at once delay the start of every stream's next graph (measured: 15 us between graphs
+    // with 16 blocks per copy, 12 us with 4; profiles/r1_bench.md).  Eight blocks per H2D copy (64 KB in flight, the kernel
+    // strides over the rest) gave the best jobs/s; stores to host memory and HBM-to-HBM copies are not capped.
+    if (to_device && cfg.io == SET_IO_HOST) {
+        const uint32_t cap = copy_max_blocks ? copy_max_blocks : 8u;
+        if (pieces > cap) pieces = cap;
+    }
     ca.kp.gridDim = dim3(pieces ? pieces : 1);
     ca.kp.blockDim = dim3(256);
     ca.kp.kernelParams = ca.ptrs;
@@ -981,6 +990,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     c->cfg = cfg;
     c->device = dev;
     if (const char* dlk = getenv("SET_DRIVER_LOCK")) c->driver_lock = dlk[0] == '1';
+    if (const char* cmb = getenv("SET_COPY_MAX_BLOCKS")) c->copy_max_blocks = (uint32_t)atoi(cmb);
     c->S = cfg.num_streams;
     c->b = ((cfg.max_inflight + c->S - 1) / c->S) * c->S;
     c->q = cfg.queue_capacity;
