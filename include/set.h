@@ -11,6 +11,13 @@
  * (PAPER.md:110); here slot w runs on stream  w mod num_streams  and there are max_inflight slots, so a
  * stream carries max_inflight/num_streams jobs back to back.
  *
+ * Environment (read once, at set_create / set_create_ex):
+ *   SET_DRIVER_LOCK=1       take one mutex around every graph update and graph launch.  Only for runs under Nsight
+ *                           Compute 2025.2, whose injection library is not safe against one thread updating a graph
+ *                           executable while another launches one (profiles/r1_ncu.md).  Never set for timing.
+ *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 8: 64 KB in flight per
+ *                           copy; more delays the GPU's own command fetches over the same link).
+ *
  * Conventions
  *   - Plain C, opaque handle, no exceptions cross the ABI, the library never aborts the process.
  *   - Every pointer argument says HOST or DEVICE.  No torch / C++ types appear in any signature.

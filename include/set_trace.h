@@ -9,6 +9,9 @@
  * Tracing costs throughput (CUPTI serialises part of the launch path), so bench.py times jobs/s WITHOUT
  * this library loaded and measures gaps in a second pass.  libset.so does not depend on this library.
  *
+ * Environment: SET_TRACE_DUMP=<file> makes set_trace_stop append one CSV line per activity record
+ * (stream, job, kind, start_ns, end_ns, kernel name) before reducing them.
+ *
  * All pointers are HOST.  Calls are single-caller.  Return 0 on success, negative on failure
  * (text in set_trace_error()).  The library never aborts.
  */
