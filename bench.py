@@ -817,6 +817,22 @@ def main():
                 "host_us_per_job": {"device": dev_arm["host_us_per_job"], "e2e": e2e_arm["host_us_per_job"]},
                 "sched_stats": {k: e2e_arm["stats"][k] for k in ("steals", "submit_stalls", "dispatcher_sleeps", "max_inflight_seen",
                                                                   "full_rebinds", "host_rebinds")}}
+        # BASELINE.json:metric in one place: jobs/s; mean inter-kernel gap; scheduling overhead against batched graphs
+        try:
+            dg, cg = extra.get("device_gaps", {}).get(f"config{wl.config}", {}), extra.get("gaps", {}).get(f"config{wl.config}", {})
+            line["headline_metrics"] = {
+                "jobs_per_s": {"set_e2e": round(e2e_value, 1), "set_device_resident": round(value, 1),
+                               "batch_sync_graphs_e2e": extra.get("baselines", {}).get("batch_sync_graphs_e2e", {}).get("jobs_per_s")},
+                "mean_gap_between_kernels_of_a_job_us": {k: cg[k]["kernel_kernel"]["mean_us"] for k in ("set_e2e", "batch_sync_graphs_e2e")
+                                                         if isinstance(cg.get(k), dict) and "kernel_kernel" in cg[k]},
+                "gap_between_jobs_on_a_stream_at_full_speed_us": {k: {"mean": dg[k]["gap_mean_us"], "p99": dg[k]["gap_p99_us"]}
+                                                                  for k in ("set_e2e", "batch_sync_graphs_e2e", "mutex_queue_e2e")
+                                                                  if isinstance(dg.get(k), dict) and "gap_mean_us" in dg[k]},
+                "device_idle_fraction_traced": {k: cg[k]["idle_frac"] for k in ("set_e2e", "batch_sync_graphs_e2e")
+                                                if isinstance(cg.get(k), dict) and "idle_frac" in cg[k]},
+                "host_sched_overhead_us_per_job": extra.get("sched_overhead_us_per_job")}
+        except Exception as e:  # a summary must never cost the line
+            line["headline_metrics"] = {"error": str(e)[:120]}
         if roof:
             line["roofline"] = roof
         if world == 1 and not args.no_cpu:
