@@ -569,7 +569,7 @@ def device_gap_pass(setlib, wl, ids, all_configs: bool, flush):
     what the stamps cost."""
     from paper_2606_05495_b200.workloads import baseline_workload
     out = {"how": "set_config.timestamps=1: %globaltimer at graph start (root node) and end (signal / last node); gap = start(next job on "
-                  "the stream) - end(previous), 3 timed steps per arm"}
+                  "the stream) - end(previous), 2-3 timed steps per arm"}
     todo = [(wl, ids)] + ([(baseline_workload(c), None) for c in range(5) if c != wl.config] if all_configs else [])
     for w, job_ids in todo:
         job_ids = list(range(w.jobs)) if job_ids is None else job_ids
@@ -577,10 +577,13 @@ def device_gap_pass(setlib, wl, ids, all_configs: bool, flush):
         p, r = LAYOUT[w.config]
         res = {"jobs_per_step": len(job_ids)}
         for mode in ("set", "batch_sync_graphs", "mutex_queue"):
+            if mode == "mutex_queue" and w.config != wl.config:
+                continue  # the queue model is traced on the headline workload only (keeps the default run short)
             for io_device in (False, True):
                 key = f"{mode}_{'device' if io_device else 'e2e'}"
                 try:
-                    a = run_arm(setlib, w, job_ids, mode, io_device, 3, 2, p, r, verify=0, flush=flush, opts={"timestamps": True})
+                    a = run_arm(setlib, w, job_ids, mode, io_device, 3 if w.config == wl.config else 2, 2, p, r, verify=0, flush=flush,
+                                opts={"timestamps": True})
                     res[key] = dict(a["device_gaps"], jobs_per_s=round(a["jobs_per_s"], 1))
                     g = res[key]
                     log(f"[bench]   device gaps config{w.config} {key:28s} inter-job mean {g['gap_mean_us']:.2f} us p50 {g['gap_p50_us']:.2f} p99 "
