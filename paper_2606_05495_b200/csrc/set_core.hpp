@@ -146,6 +146,8 @@ class Scheduler {
             free_execs_[w].r.init((size_t)epp_ * 2);  // room for migrated execs under kRetarget
             for (int k = 0; k < epp_; ++k) free_execs_[w].r.push(w * epp_ + k);
         }
+        launched_.reset(new StreamOrder[S_]);
+        for (int s = 0; s < S_; ++s) launched_[s].q.init((size_t)b_ + 1);
         pool_.init((size_t)b_ + 1);
         // the main thread initialises all workers; all of them start idle.
         for (int w = 0; w < b_; ++w) pool_.push(w);
@@ -282,23 +284,40 @@ class Scheduler {
     struct alignas(kCacheLine) PaddedRing {
         Ring<T> r;
     };
+    // Slots in the order their jobs were launched on one stream.  A stream completes its graphs in launch order, so a
+    // polling dispatcher only has to watch the OLDEST in-flight slot of each stream: O(S) words per look instead of O(b).
+    struct alignas(kCacheLine) StreamOrder {
+        std::atomic_flag launching = ATOMIC_FLAG_INIT;  // held around launch + push: list order == stream order
+        std::atomic_flag polling = ATOMIC_FLAG_INIT;    // one dispatcher at a time walks a stream's list
+        Ring<int> q;
+    };
     struct alignas(kCacheLine) Running {
         int exec = -1;
         std::atomic<int> state{0};  // 0 idle, 1 in flight, 2 completion claimed by a polling dispatcher
         JobDesc job;
     };
 
-    // Flag-polled completion: scan the in-flight slots' words; whoever wins the 1 -> 2 claim runs Algorithm 3.
+    // Flag-polled completion: look at the oldest in-flight slot of every stream; whoever wins the 1 -> 2 claim runs
+    // Algorithm 3, then the stream's next slot becomes the oldest.
     bool poll_flags() {
         bool any = false;
-        for (int w = 0; w < b_; ++w) {
-            Running& r = running_[w];
-            if (r.state.load(std::memory_order_acquire) != 1) continue;
-            if (__atomic_load_n(&flags_[w * kFlagStride], __ATOMIC_ACQUIRE) == 0) continue;
-            int one = 1;
-            if (!r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) continue;
-            on_complete(w);
-            any = true;
+        for (int s = 0; s < S_; ++s) {
+            StreamOrder& so = launched_[s];
+            if (so.q.empty_approx()) continue;
+            if (so.polling.test_and_set(std::memory_order_acquire)) continue;  // another dispatcher is on this stream
+            int w;
+            while (so.q.try_peek(w)) {
+                Running& r = running_[w];
+                if (r.state.load(std::memory_order_acquire) != 1) break;  // still being set up by the launching thread
+                if (__atomic_load_n(&flags_[w * kFlagStride], __ATOMIC_ACQUIRE) == 0) break;
+                int one = 1;
+                if (!r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) break;
+                int popped;
+                so.q.try_pop(popped);
+                on_complete(w);
+                any = true;
+            }
+            so.polling.clear(std::memory_order_release);
         }
         return any;
     }
@@ -354,7 +373,17 @@ class Scheduler {
             __atomic_store_n(&flags_[w * kFlagStride], 0u, __ATOMIC_RELAXED);
             r.state.store(1, std::memory_order_release);
         }
-        if (rc == 0) rc = be_->launch(exec, w, p.job);  // GraphLaunch + AddCallback
+        if (rc == 0) {
+            if (flags_) {
+                StreamOrder& so = launched_[w % S_];
+                while (so.launching.test_and_set(std::memory_order_acquire)) cpu_relax();
+                rc = be_->launch(exec, w, p.job);  // GraphLaunch
+                if (rc == 0) so.q.push(w);         // room is guaranteed: at most b slots are in flight
+                so.launching.clear(std::memory_order_release);
+            } else {
+                rc = be_->launch(exec, w, p.job);  // GraphLaunch + AddCallback
+            }
+        }
         stats_.launched.fetch_add(1, std::memory_order_relaxed);
         stats_.ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
         if (rc != 0) {  // keep the books balanced so that drain returns; the error is sticky
@@ -413,6 +442,7 @@ class Scheduler {
     std::unique_ptr<PaddedRing<Prepared>[]> queues_;
     std::unique_ptr<PaddedRing<int>[]> free_execs_;
     std::unique_ptr<Running[]> running_;
+    std::unique_ptr<StreamOrder[]> launched_;
     Ring<int> pool_;
     alignas(kCacheLine) std::atomic<uint64_t> c_next_{0};
     alignas(kCacheLine) std::atomic<uint64_t> c_submitted_{0};

@@ -119,6 +119,16 @@ class Ring {
         }
     }
 
+    // Look at the oldest entry without taking it.  Only meaningful while the caller is the ring's sole consumer
+    // (producers may push concurrently): used for the per-stream launch-order lists the polling dispatcher walks.
+    bool try_peek(T& out) const {
+        const uint64_t pos = head_.load(std::memory_order_relaxed);
+        const Cell& c = cells_[pos & mask_];
+        if (c.seq.load(std::memory_order_acquire) != pos + 1) return false;
+        out = c.value;
+        return true;
+    }
+
     // Racy size estimate (exact when quiescent).
     size_t size_approx() const {
         uint64_t t = tail_.load(std::memory_order_relaxed), h = head_.load(std::memory_order_relaxed);
