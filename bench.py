@@ -1,7 +1,11 @@
 #!/usr/bin/env python
-"""bench.py -- jobs/s of the SET hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+"""bench.py -- jobs/s of the SET hot path on B200 (BASELINE.json metric).  The LAST line of stdout is one compact JSON
+object (< 2 KB: the contract keys plus roofline, cpu_baseline, e2e, headline_metrics and one scalar per side workload);
+everything else -- per-arm statistics, per-kernel tables, baselines, gaps, sweeps -- goes to a detail file (--out, default
+bench_detail.json beside this script) and, as progress lines, to stderr.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--suite headline|all] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--suite headline|default|all] [--sweep]
+                    [--impl reference] [--out FILE]
 
 A *step* is one pass of the whole hot path over one batch of synthetic input: every job of the workload
 (BASELINE.json:configs[C], default C = 1: 10,000 jobs of the short-lived-kernel pipeline, 8 streams, 32 in
@@ -112,6 +116,16 @@ class JobSet:
         self.pool_inputs = []   # distinct input images (numpy), index = job % len
 
 
+_INPUTS = {}  # (config, params, variant, first job id, count) -> list of input images: generated once, reused by every arm
+
+
+def job_inputs(wl, job_ids, npool):
+    key = (wl.config, tuple(wl.params), wl.variant, job_ids[0] if len(job_ids) else 0, npool)
+    if key not in _INPUTS:
+        _INPUTS[key] = [wl.make_input(job_ids[k]) for k in range(npool)]
+    return _INPUTS[key]
+
+
 def build_jobs(setlib, ctx, wl, job_ids, io_device: bool, pool: int, out_ring: int):
     """Place the jobs' inputs in pinned host memory (or HBM) and give every job an output slot.
     pool     : number of DISTINCT input images generated (job k uses image k mod pool); 0 = all distinct.
@@ -126,7 +140,7 @@ def build_jobs(setlib, ctx, wl, job_ids, io_device: bool, pool: int, out_ring: i
     dims = [wl.dims(j) for j in job_ids]
     if wl.config == 4:
         js.dims = (C.c_uint32 * (4 * n))(*[v for d in dims for v in d])
-    images = [wl.make_input(job_ids[k]) for k in range(npool)]
+    images = job_inputs(wl, job_ids, npool)
     js.pool_inputs = images
     pool_dims = dims[:npool]
     in_sz = [wl.in_bytes(d) for d in pool_dims]
@@ -194,7 +208,7 @@ MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3
 
 
 # graph-shape options of every arm (SET and the in-run baselines share the job graph): --sm-copy / --pdl
-OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0, "submitters": 1}
+OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0, "submitters": 1, "streams_per_lane": 0, "completion_fence": 0}
 
 
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
@@ -205,6 +219,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
     o = dict(OPTS, **(opts or {}))
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=MODES[mode], io=setlib.IO_DEVICE if io_device else setlib.IO_HOST,
                          sm_copy_max_bytes=o["sm_copy_max_bytes"], timestamps=bool(o.get("timestamps")),
+                         streams_per_lane=o["streams_per_lane"], completion_fence=o["completion_fence"],
                          **dict({"num_dispatchers": o["num_dispatchers"]}, **(ctx_kw or {})))
     try:
         ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=o["pdl"])
@@ -242,7 +257,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
             g = trace.stop()
             js.keep.clear()
             return {"mode": mode, "io": "device" if io_device else "host", "jobs": n, "gaps": g}
-        ev_ms, wall_ms = [], []
+        ev_ms, wall_ms, per_step_gaps, st_sum = [], [], [], None
         for _ in range(steps):
             if flush is not None:
                 flush.add_(1)  # rewrite a buffer larger than L2 between timed steps
@@ -258,13 +273,19 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
             wall_ms.append((t1 - t0) * 1e3)
             if clock_windows is not None:
                 clock_windows.append((t0, t1))
-        st = ctx.stats()
-        gap_stats = ctx.gap_stats() if o.get("timestamps") else None
+            if o.get("timestamps"):
+                # one reduction per step: the span of a step's stamps must not include the pause between steps
+                g = ctx.gap_stats()
+                g["overhead_frac"] = max(0.0, 1.0 - g["busy_union_us"] / (ev_ms[-1] * 1e3))
+                per_step_gaps.append(g)
+                stp = ctx.stats()
+                st_sum = stp if st_sum is None else {k: (max(st_sum[k], v) if k == "max_inflight_seen" else st_sum[k] + v) for k, v in stp.items()}
+                ctx.reset_stats()
+        st = st_sum if st_sum is not None else ctx.stats()
+        gap_stats = merge_gap_stats(per_step_gaps) if per_step_gaps else None
         bad = 0
         if verify:
-            sys.path.insert(0, os.path.join(ROOT, "tests"))
-            from oracle_map import oracle_out          # the oracle is only touched for this spot check
-            from test_gpu_parity import compare
+            from checker import compare, oracle_out          # the oracle is only touched for this spot check
             picks = sorted(set(np.linspace(0, n - 1, verify).astype(int).tolist()))
             # with an output ring only the last writer of a slot is still there
             picks = [k for k in picks if k + js.nring >= n] or [n - 1]
@@ -291,6 +312,23 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
         if "pool_ex" in locals() and pool_ex is not None:
             pool_ex.shutdown()
         ctx.close()
+
+
+def merge_gap_stats(per_step):
+    """Job-weighted mean of the per-step device-stamp statistics (p99 / max: the worst step's)."""
+    out = {}
+    w = [g["jobs"] for g in per_step]
+    tot = max(1, sum(w))
+    for k in per_step[0]:
+        if k in ("jobs", "gaps"):
+            out[k] = int(sum(g[k] for g in per_step))
+        elif k in ("gap_p99_us", "gap_max_us"):
+            out[k] = round(max(g[k] for g in per_step), 4)
+        elif k in ("span_us", "busy_union_us"):
+            out[k] = round(sum(g[k] for g in per_step), 3)
+        else:
+            out[k] = round(sum(g[k] * n for g, n in zip(per_step, w)) / tot, 4)
+    return out
 
 
 def time_stages(setlib, wl, dims=None, iters=50):
@@ -449,8 +487,7 @@ def pipeline_roofline(wl, in_bytes_job, out_bytes_job, link, pk, dims):
 def oracle_pass(wl, images, dims_list, budget_s: float):
     """Time the oracle, as it stands, single-threaded, over the given job images until `budget_s` of CPU work is done
     or every job has been processed once.  Returns (jobs done, seconds)."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from oracle_map import oracle_out
+    from checker import oracle_out
     done, t0 = 0, time.perf_counter()
     for img, d in zip(images, dims_list):
         oracle_out(wl, img, d)
@@ -460,9 +497,13 @@ def oracle_pass(wl, images, dims_list, budget_s: float):
     return done, time.perf_counter() - t0
 
 
-def cpu_baseline(wl, job_ids, budget_s=15.0, passes=10):
-    n = min(len(job_ids), 2048 if wl.config != 1 else len(job_ids))
-    images = [wl.make_input(j) for j in job_ids[:n]]
+def cpu_baseline(wl, job_ids, budget_s=12.0, passes=10, all_cores_s=4.0):
+    """The oracle, as it stands, timed on this box's host cores over a bounded sample of the workload's jobs."""
+    cap = {0: 256, 1: 2048, 2: 2, 3: 1, 4: 24}[wl.config]      # distinct inputs prepared for the sample
+    n = min(len(job_ids), cap)
+    if wl.config == 3 and budget_s < 60:
+        return cpu_baseline_config3_sampled(wl, job_ids, budget_s)
+    images = job_inputs(wl, job_ids, n)
     dims = [wl.dims(j) for j in job_ids[:n]]
     total, secs = 0, 0.0
     for _ in range(passes):
@@ -477,9 +518,9 @@ def cpu_baseline(wl, job_ids, budget_s=15.0, passes=10):
     try:
         from concurrent.futures import ThreadPoolExecutor
         cores = len(os.sched_getaffinity(0))
-        if cores > 1:
+        if cores > 1 and all_cores_s > 0:
             chunks = [(images[i::cores], dims[i::cores]) for i in range(cores)]
-            def worker(c, budget=4.0):
+            def worker(c, budget=all_cores_s):
                 n_done, t_used = 0, 0.0
                 while t_used < budget and c[0]:
                     d, t = oracle_pass(wl, c[0], c[1], budget - t_used)
@@ -496,103 +537,118 @@ def cpu_baseline(wl, job_ids, budget_s=15.0, passes=10):
     return out
 
 
+
+
+def cpu_baseline_config3_sampled(wl, job_ids, budget_s):
+    """Config 3: one full 2048^3 job takes the naive-loop oracle minutes, so the bounded sample is a set of output entries
+    of one job computed one by one (oracle_config3_sampled, the same arithmetic per entry) and the per-job figure is
+    extrapolated from the entry rate -- labelled as such (SURVEY.md 8(d) "Oracle timing")."""
+    import oracle
+    m, n, k = wl.params
+    img = job_inputs(wl, job_ids, 1)[0]
+    a = img[:2 * m * k].view(np.uint16).reshape(m, k)
+    b = img[2 * m * k:2 * m * k + 2 * k * n].view(np.uint16).reshape(k, n)
+    bias = img[2 * m * k + 2 * k * n:].view(np.float32)
+    per, done, t0 = 4096, 0, time.perf_counter()
+    while time.perf_counter() - t0 < budget_s:
+        r = np.arange(done, done + per, dtype=np.int64)
+        oracle.config3_sampled(a, b, bias, (r * 7919) % m, (r * 104729) % n)
+        done += per
+    secs = time.perf_counter() - t0
+    return {"value": round(done / secs / (m * n), 6), "unit": "jobs/s", "cores": 1, "kind": "oracle", "extrapolated": True,
+            "sample": f"{done} output entries of one job ({m}x{n}x{k}) in {secs:.1f} s, single thread; per-job rate = entry rate / {m * n}"}
 # ------------------------------------------------------------------------------------------------ main
 # distinct-input pool / output ring per config (0 = one per job).  Rings are >= b*(q+1) outstanding jobs.
-LAYOUT = {0: (0, 0), 1: (0, 0), 2: (16, 32), 3: (8, 64), 4: (96, 128)}
-GAP_JOBS = {0: 256, 1: 2000, 2: 64, 3: 200, 4: 512}  # jobs traced per arm in the gap pass (records stay in host memory)
+LAYOUT = {0: (0, 0), 1: (0, 0), 2: (16, 32), 3: (8, 64), 4: (96, 128), 5: (64, 0), 6: (96, 128)}
+GAP_JOBS = {0: 256, 1: 2000, 2: 64, 3: 200, 4: 512, 5: 256, 6: 512}  # jobs traced per arm in the CUPTI pass (records stay in host memory)
+SIDE_STEPS, SIDE_WARMUP = 2, 2                                       # side workloads and secondary arms: fixed, small
 
 
 def gap_pass(setlib, wl, ids, all_configs: bool, warmup: int):
-    """Inter-kernel gaps and device idle fraction from CUPTI activity records (include/set_trace.h), for SET and for the
+    """Kernel-level gaps and device idle fraction from CUPTI activity records (include/set_trace.h), for SET and for the
     batch-synchronous-graph baseline on the same jobs.  Runs after every timed arm: tracing slows the launch path, so no
     throughput figure comes from here."""
-    out = {"how": "one step per arm under CUPTI activity tracing (kernel, memcpy, memset records), after all timed arms; "
-                  "gap = start(next) - end(previous) of operations consecutive on one stream; idle_frac = 1 - |union of "
-                  "activity| / wall (DESIGN.md reading S12)"}
+    out = {"how": "one step per arm under CUPTI activity tracing (kernel, memcpy, memset records), after all timed arms; records are "
+                  "grouped into jobs by the correlation id of their cudaGraphLaunch and jobs into work streams by the stream of the job's "
+                  "first stage kernel; kernel->kernel gaps are signed (negative = PDL overlap); idle_frac = 1 - |union of activity| / wall"}
     try:
         from paper_2606_05495_b200 import trace
         trace.load()
     except Exception as e:
         return {"unavailable": str(e)[:200]}
-    from paper_2606_05495_b200.workloads import baseline_workload
     todo = [(wl, ids)]
     if all_configs:
-        todo += [(baseline_workload(c), None) for c in range(5) if c != wl.config]
+        todo += [(workload_for(c), None) for c in range(5) if c != wl.config]
     for w, job_ids in todo:
         job_ids = list(range(w.jobs)) if job_ids is None else job_ids
         job_ids = job_ids[:GAP_JOBS[w.config]]
         p, r = LAYOUT[w.config]
         res = {"jobs": len(job_ids)}
         for mode in ("set", "batch_sync_graphs"):
-            for io_device in (True, False):
-                key = f"{mode}_{'device' if io_device else 'e2e'}"
-                try:
-                    g = run_arm(setlib, w, job_ids, mode, io_device, 1, max(1, min(warmup, 2)), p, r, trace=trace)["gaps"]
-                    res[key] = g
-                    log(f"[bench]   gaps config{w.config} {key:28s} kernel->kernel mean {g['kernel_kernel']['mean_us']:.2f} us "
-                        f"p99 {g['kernel_kernel']['p99_us']:.2f}  inter-job mean {g['inter_job']['mean_us']:.2f} us  idle {g['idle_frac']:.3f}")
-                except Exception as e:
-                    res[key] = {"error": str(e)[:200]}
-                    log(f"[bench]   gaps config{w.config} {key} failed: {e}")
+            key = f"{mode}_e2e"
+            try:
+                g = run_arm(setlib, w, job_ids, mode, False, 1, max(1, min(warmup, 2)), p, r, trace=trace)["gaps"]
+                res[key] = g
+                log(f"[bench]   cupti config{w.config} {key:28s} kernel->kernel mean {g['kernel_kernel']['mean_us']:.2f} us "
+                    f"p99 {g['kernel_kernel']['p99_us']:.2f}  inter-job mean {g['inter_job']['mean_us']:.2f} us  idle {g['idle_frac']:.3f}")
+            except Exception as e:
+                res[key] = {"error": str(e)[:200]}
+                log(f"[bench]   cupti config{w.config} {key} failed: {e}")
         out[f"config{w.config}"] = res
     return out
 
 
-def batch_sweep(setlib, wl, ids, flush, trace_ok: bool):
-    """SURVEY.md 8(f)2 / PAPER.md:274-288 (Fig. 5-6): throughput of SET and of the batch-synchronous baseline against the
-    batch size b = max_inflight, streams fixed at the workload's S (b < S: b streams).  End to end, pinned host buffers."""
+SWEEP_B = (1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096)
+
+
+def batch_sweep(setlib, wl, ids, flush):
+    """SURVEY.md 8(f)2 / PAPER.md:274-288 (Fig. 5-6): for b = max_inflight from 1 to 4096 and the three models the paper
+    draws (SET, batching, queue) -- throughput, the scheduling-overhead fraction (1 - |union of job intervals| / T, reading
+    S12, from the device stamps) and the mean device-side gap between consecutive jobs of a stream.  End to end, pinned host
+    buffers, streams fixed at the workload's S (b < S: b streams)."""
     import copy
-    out = {"workload": wl.name, "jobs": min(len(ids), 4000), "b": {}}
+    out = {"workload": wl.name, "jobs": min(len(ids), 8192), "b": {},
+           "how": "3 timed steps per point with set_config.timestamps=1 (two stamp nodes per job); overhead_frac = 1 - busy_union / step time"}
     job_ids = ids[:out["jobs"]]
     p, r = LAYOUT[wl.config]
-    for b in (1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1024):
+    for b in SWEEP_B:
         w = copy.copy(wl)
         w.max_inflight, w.num_streams = b, min(b, wl.num_streams)
         row = {}
-        for mode in ("set", "batch_sync_graphs"):
+        for mode in ("set", "batch_sync_graphs", "mutex_queue"):
             try:
-                res = run_arm(setlib, w, job_ids, mode, False, 3, 2, p, max(r, 0), verify=0, flush=flush)
-                row[mode] = round(res["jobs_per_s"], 1)
+                res = run_arm(setlib, w, job_ids, mode, False, 3, 2, p, max(r, 0), verify=0, flush=flush, opts={"timestamps": True})
+                g = res["device_gaps"]
+                row[mode] = {"jobs_per_s": round(res["jobs_per_s"], 1), "overhead_frac": round(g["overhead_frac"], 4),
+                             "gap_mean_us": round(g["gap_mean_us"], 2), "host_us_per_job": round(sum(res["host_us_per_job"][k] for k in ("submit", "launch", "callback")), 3)}
             except Exception as e:
                 row[mode] = {"error": str(e)[:120]}
-        if all(isinstance(v, float) for v in row.values()):
-            row["speedup"] = round(row["set"] / row["batch_sync_graphs"], 3)
+        if all("jobs_per_s" in v for v in row.values()):
+            row["set_over_batch"] = round(row["set"]["jobs_per_s"] / row["batch_sync_graphs"]["jobs_per_s"], 3)
+            row["set_over_queue"] = round(row["set"]["jobs_per_s"] / row["mutex_queue"]["jobs_per_s"], 3)
         out["b"][str(b)] = row
         log(f"[bench]   sweep b={b:5d} S={w.num_streams}: {row}")
     return out
 
 
-def device_gap_pass(setlib, wl, ids, all_configs: bool, flush):
-    """Gaps between consecutive jobs of a stream from the GPU's own clock (set_config.timestamps, include/set.h
-    set_get_gap_stats): two one-thread stamp nodes per job graph, no profiler attached, full speed.  For SET, the
-    batch-synchronous baseline and the mutex-queue model; the jobs/s of these arms is reported beside the gaps to show
-    what the stamps cost."""
-    from paper_2606_05495_b200.workloads import baseline_workload
-    out = {"how": "set_config.timestamps=1: %globaltimer at graph start (root node) and end (signal / last node); gap = start(next job on "
-                  "the stream) - end(previous), 2-3 timed steps per arm"}
-    todo = [(wl, ids)] + ([(baseline_workload(c), None) for c in range(5) if c != wl.config] if all_configs else [])
-    for w, job_ids in todo:
-        job_ids = list(range(w.jobs)) if job_ids is None else job_ids
-        job_ids = job_ids[:{0: 256, 1: 10000, 2: 64, 3: 200, 4: 1024}[w.config]]  # keeps the default run within minutes
-        p, r = LAYOUT[w.config]
-        res = {"jobs_per_step": len(job_ids)}
-        for mode in ("set", "batch_sync_graphs", "mutex_queue"):
-            if mode == "mutex_queue" and w.config != wl.config:
-                continue  # the queue model is traced on the headline workload only (keeps the default run short)
-            for io_device in (False, True):
-                key = f"{mode}_{'device' if io_device else 'e2e'}"
-                try:
-                    a = run_arm(setlib, w, job_ids, mode, io_device, 3 if w.config == wl.config else 2, 2, p, r, verify=0, flush=flush,
-                                opts={"timestamps": True})
-                    res[key] = dict(a["device_gaps"], jobs_per_s=round(a["jobs_per_s"], 1))
-                    g = res[key]
-                    log(f"[bench]   device gaps config{w.config} {key:28s} inter-job mean {g['gap_mean_us']:.2f} us p50 {g['gap_p50_us']:.2f} p99 "
-                        f"{g['gap_p99_us']:.2f}  job chain {g['job_mean_us']:.2f} us  streams busy {g['stream_busy_frac']:.3f}  {g['jobs_per_s']:.0f} jobs/s")
-                except Exception as e:
-                    res[key] = {"error": str(e)[:200]}
-                    log(f"[bench]   device gaps config{w.config} {key} failed: {e}")
-        out[f"config{w.config}"] = res
-    return out
+def device_gap_arms(setlib, w, job_ids, modes, flush, steps=3):
+    """Gaps between consecutive jobs of a stream and the overhead fraction from the GPU's own clock (set_config.timestamps,
+    set_get_gap_stats): two one-thread stamp nodes per job graph, no profiler attached, full speed, end to end."""
+    p, r = LAYOUT[w.config]
+    res = {"jobs_per_step": len(job_ids)}
+    for mode in modes:
+        key = f"{mode}_e2e"
+        try:
+            a = run_arm(setlib, w, job_ids, mode, False, steps, 2, p, r, verify=0, flush=flush, opts={"timestamps": True})
+            res[key] = dict(a["device_gaps"], jobs_per_s=round(a["jobs_per_s"], 1),
+                            host_us_per_job={k: round(v, 3) for k, v in a["host_us_per_job"].items()})
+            g = res[key]
+            log(f"[bench]   stamps config{w.config} {key:24s} inter-job gap mean {g['gap_mean_us']:.2f} us p99 {g['gap_p99_us']:.2f}  job chain "
+                f"{g['job_mean_us']:.2f} us  overhead frac {g['overhead_frac']:.4f}  {g['jobs_per_s']:.0f} jobs/s")
+        except Exception as e:
+            res[key] = {"error": str(e)[:200]}
+            log(f"[bench]   stamps config{w.config} {key} failed: {e}")
+    return res
 
 
 def workload_for(config, jobs_override=None):
@@ -604,7 +660,7 @@ def workload_for(config, jobs_override=None):
 
 
 def mean_dims(wl, job_ids):
-    if wl.config != 4:
+    if wl.config not in (4, 6):
         return (1, 1, 1, 1)
     return (1280, 720, 1, 1)
 
@@ -640,6 +696,78 @@ def reference_main(args, rank, world):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ the compact line
+REQUIRED_KEYS = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+                 "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline")
+
+
+def _r(x, nd=1):
+    return None if x is None else round(float(x), nd)
+
+
+def compact_line(wl, world, steps, warmup, n_jobs, ms_dev, value, ms_e2e, e2e_value, dev_arm, e2e_arm, clocks, detail, detail_path, pk):
+    """The one stdout line (driver contract + tier additions), built from the measured arms and the detail dict.  Pure host
+    arithmetic: tests/test_bench_helpers.py feeds it fake arms and checks the keys and the size bound."""
+    kr = detail.get("kernels") or []
+    dom = max(kr, key=lambda r: r.get("total_us", 0)) if kr else None
+    roof = None
+    if dom:
+        roof = {"bound": dom["bound"], "achieved": dom["achieved"], "peak": dom["peak"], "unit": dom["unit"], "frac": dom["frac"],
+                "traffic": dom.get("traffic"), "kernel": dom["kernel"], "avg_us": dom["avg_us"], "peak_source": pk["source"].split(" ")[0],
+                "floor_us": dom.get("launch_floor_us")}  # floor_us: an empty kernel node; avg_us near it = latency-class kernel
+    line = {"metric": "jobs/s", "value": _r(value), "unit": "jobs/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": _r(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype,
+            "data": "synthetic",
+            "config": {"workload": wl.name, "jobs_per_step_per_gpu": n_jobs, "num_streams": wl.num_streams, "max_inflight": wl.max_inflight,
+                       "streams_per_lane": detail.get("streams_per_lane"), "io": "value: HBM-resident I/O; e2e: pinned host",
+                       "l2": f"{L2_FLUSH_BYTES >> 20} MiB flush/step; {dev_arm['in_bytes'] / 1e6:.0f} MB inputs/step"},
+            "clocks": clocks,
+            "e2e": {"value": _r(e2e_value), "unit": "jobs/s", "h2d_bytes_per_step": int(e2e_arm["h2d_bytes"] * world),
+                    "d2h_bytes_per_step": int(e2e_arm["d2h_bytes"] * world), "ms_per_step": _r(ms_e2e, 4)},
+            "gpu_launches": int(dev_arm["kernel_launches"] * world),
+            "mismatches": int(dev_arm["mismatches"] + e2e_arm["mismatches"] + detail.get("side_mismatches", 0)),
+            "roofline": roof, "cpu_baseline": None}
+    cb = detail.get("cpu_baseline")
+    if cb:  # the line carries the contract's five fields; the job-parallel figure stays in the detail file
+        line["cpu_baseline"] = {"value": cb["value"], "unit": cb["unit"], "cores": cb["cores"], "kind": cb["kind"], "sample": cb["sample"][:90]}
+    # BASELINE.json:metric in one object, e2e first: jobs/s; gap between jobs of a stream; scheduling overhead vs batched graphs
+    base = detail.get("baselines", {})
+    dg = detail.get("device_gaps", {}).get(f"config{wl.config}", {})
+
+    def pick(key, field, nd=3):
+        v = dg.get(key, {})
+        return _r(v.get(field), nd) if isinstance(v, dict) and field in v else None
+
+    bs = base.get("batch_sync_graphs_e2e", {}).get("jobs_per_s")
+    hm = {"set_e2e_jobs_per_s": _r(e2e_value), "batch_sync_e2e_jobs_per_s": _r(bs),
+          "set_over_batch_sync_e2e": _r(e2e_value / bs, 3) if bs else None,
+          "gap_between_jobs_us": {"set": pick("set_e2e", "gap_mean_us", 2), "batch_sync": pick("batch_sync_graphs_e2e", "gap_mean_us", 2),
+                                  "set_p99": pick("set_e2e", "gap_p99_us", 2), "batch_sync_p99": pick("batch_sync_graphs_e2e", "gap_p99_us", 2)},
+          "sched_overhead_frac": {"set": pick("set_e2e", "overhead_frac", 4), "batch_sync": pick("batch_sync_graphs_e2e", "overhead_frac", 4)},
+          "host_us_per_job": {"set": _r(sum(e2e_arm["host_us_per_job"][k] for k in ("submit", "launch", "callback")), 3),
+                              "batch_sync": _r(sum(base["batch_sync_graphs_e2e"]["host_us_per_job"][k] for k in ("submit", "launch")), 3)
+                              if "batch_sync_graphs_e2e" in base else None}}
+    pr = detail.get("pipeline_roofline")
+    if pr:
+        hm["pipeline_roofline"] = {"bound_by": pr["e2e_bound_by"], "e2e_bound_jobs_per_s": pr["e2e_bound_jobs_per_s"], "e2e_frac": pr["e2e_frac"]}
+    line["headline_metrics"] = hm
+    side = {}
+    for k, v in (detail.get("workloads") or {}).items():
+        side[k] = {"e2e": v.get("e2e"), "frac": (v.get("pipeline_roofline") or {}).get("e2e_frac"), "vs_batch": v.get("speedup_vs_batch_sync_e2e")} \
+            if "error" not in v else {"error": v["error"][:60]}
+    if side:
+        line["workloads"] = side
+    kroofs = {}
+    for k, v in (detail.get("workloads") or {}).items():
+        for row in v.get("kernels", []) if isinstance(v, dict) else []:
+            if row["kernel"] in ("jacobi5_f32", "gemm_bias_gelu_bf16"):
+                kroofs[row["kernel"]] = {"frac": row["frac"], "avg_us": row["avg_us"], "bound": row["bound"]}
+    if kroofs:
+        line["kernel_rooflines"] = kroofs
+    line["detail"] = os.path.basename(detail_path) if detail_path else None
+    return line
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -647,20 +775,25 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json:configs index of the headline workload")
     ap.add_argument("--jobs", type=int, default=None, help="override the job count (debugging only)")
-    ap.add_argument("--suite", default="all", choices=["headline", "all"], help="all: also run configs 0,2,3,4 (N=1 only)")
+    ap.add_argument("--suite", default="default", choices=["headline", "default", "all"],
+                    help="headline: the headline workload, its batch-sync baseline, rooflines, CPU oracle; default: + the other four "
+                         "configs (2 steps each) and the device-stamp gap pass; all: + completion modes, graph variants, every "
+                         "baseline model, per-config CPU oracle timing and the CUPTI gap pass (N=1 only)")
     ap.add_argument("--impl", default="set", choices=["set", "reference"])
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-gaps", action="store_true", help="skip the CUPTI gap pass (run last, after every timed arm)")
+    ap.add_argument("--no-gaps", action="store_true", help="skip the gap passes")
     ap.add_argument("--sm-copy", type=int, default=0, help="set_config.sm_copy_max_bytes: 0 = library default, -1 = copy engines only")
-    ap.add_argument("--submitters", type=int, default=1, help="caller threads that submit a step's jobs to SET (baselines: always 1); measured on B200: no gain beyond 1, the driver serialises graph updates and launches")
+    ap.add_argument("--submitters", type=int, default=1, help="caller threads that submit a step's jobs to SET (baselines: always 1)")
     ap.add_argument("--dispatchers", type=int, default=0, help="set_config.num_dispatchers (0 = library default, 1)")
+    ap.add_argument("--lanes", type=int, default=0, help="set_config.streams_per_lane (0 = library default)")
+    ap.add_argument("--fence", type=int, default=0, help="set_config.completion_fence: 0 default, 1 system fence, 2 none")
     ap.add_argument("--pdl", type=int, default=1, help="1: programmatic-dependent-launch edges between kernel nodes (default), 0: plain edges")
-    ap.add_argument("--sweep", action="store_true", help="also sweep the batch size b (PAPER.md Fig. 5-6) on the headline workload")
-    ap.add_argument("--out", default=None, help="also write the JSON line to this file")
+    ap.add_argument("--sweep", action="store_true", help="also sweep the batch size b = 1..4096 (PAPER.md Fig. 5-6) on the headline workload")
+    ap.add_argument("--out", default=os.path.join(ROOT, "bench_detail.json"), help="detail file (everything that is not on the stdout line)")
     args = ap.parse_args()
     OPTS["sm_copy_max_bytes"], OPTS["pdl"], OPTS["num_dispatchers"] = args.sm_copy, bool(args.pdl), args.dispatchers
-    OPTS["submitters"] = args.submitters
+    OPTS["submitters"], OPTS["streams_per_lane"], OPTS["completion_fence"] = args.submitters, args.lanes, args.fence
 
     from paper_2606_05495_b200 import multi
     if args.impl == "reference":
@@ -679,8 +812,8 @@ def main():
     multi.barrier(dev)
     import paper_2606_05495_b200 as setlib
     setlib.load()
-    from paper_2606_05495_b200.workloads import baseline_workload
 
+    t_start = time.perf_counter()
     steps, warmup = args.steps, max(args.warmup, 0)
     pk = peaks()
     flush = torch.zeros(L2_FLUSH_BYTES // 4, dtype=torch.int32, device=dev)
@@ -690,165 +823,144 @@ def main():
 
     wl = workload_for(args.config, args.jobs)
     ids = list(multi.shard_jobs(wl.jobs, rank, world, "weak"))
-    pool, ring = LAYOUT[wl.config]
-    log(f"[bench] rank {rank}/{world} headline {wl.name}: {len(ids)} jobs/step, {steps} steps, {warmup} warm-up")
+    log(f"[bench] rank {rank}/{world} headline {wl.name}: {len(ids)} jobs/step, {steps} steps, {warmup} warm-up, suite {args.suite}")
 
-    def arm(w, job_ids, mode, io_device, k=steps, wu=warmup, verify=4, win=None):
+    def arm(w, job_ids, mode, io_device, k=steps, wu=warmup, verify=4, win=None, **kw):
         p, r = LAYOUT[w.config]
         multi.barrier(dev)
         torch.cuda.synchronize()
-        res = run_arm(setlib, w, job_ids, mode, io_device, k, wu, p, r, verify=verify, flush=flush, clock_windows=win)
+        res = run_arm(setlib, w, job_ids, mode, io_device, k, wu, p, r, verify=verify, flush=flush, clock_windows=win, **kw)
         torch.cuda.synchronize()
         multi.barrier(dev)
         log(f"[bench]   {w.config} {mode:18s} {'device' if io_device else 'host  '} {res['jobs_per_s']:12.1f} jobs/s "
-            f"{res['ms_per_step']:9.3f} ms/step  host us/job {res['host_us_per_job']}  mismatches {res['mismatches']}")
+            f"{res['ms_per_step']:9.3f} ms/step  host us/job { {k_: round(v, 3) for k_, v in res['host_us_per_job'].items()} }  mismatches {res['mismatches']}")
         return res
 
-    dev_arm = arm(wl, ids, "set", True, win=windows)
+    def brief(r):
+        return {"jobs_per_s": round(r["jobs_per_s"], 1), "ms_per_step": round(r["ms_per_step"], 3), "mismatches": r["mismatches"],
+                "host_us_per_job": {k: round(v, 3) for k, v in r["host_us_per_job"].items()}}
+
+    # ---- the headline arms first: whatever happens later, these numbers exist
     e2e_arm = arm(wl, ids, "set", False, win=windows)
+    dev_arm = arm(wl, ids, "set", True, win=windows)
     ms_dev, units = multi.aggregate(dev_arm["ms_per_step"], dev_arm["jobs"], dev)
     ms_e2e, _ = multi.aggregate(e2e_arm["ms_per_step"], e2e_arm["jobs"], dev)
     value, e2e_value = units / (ms_dev * 1e-3), units / (ms_e2e * 1e-3)
 
-    extra = {}
+    detail = {"argv": sys.argv[1:], "suite": args.suite, "peaks": pk}
+    detail["streams_per_lane"] = e2e_arm["stats"].get("cuda_streams", 0) // max(1, wl.num_streams)
+    detail["set_e2e"], detail["set_device"] = dict(brief(e2e_arm), stats=e2e_arm["stats"], step_ms=e2e_arm["step_ms"]), dict(brief(dev_arm), stats=dev_arm["stats"], step_ms=dev_arm["step_ms"])
+    side_bad = 0
     if world == 1:
         link = link_bandwidth()
-        extra["link_gbs"] = link
+        detail["link_gbs"] = link
         d = mean_dims(wl, ids)
         in_job, out_job = e2e_arm["in_bytes"] / e2e_arm["jobs"], e2e_arm["out_bytes"] / e2e_arm["jobs"]
         pr = pipeline_roofline(wl, in_job, out_job, link, pk, d)
         pr["e2e_frac"] = round(e2e_value / pr["e2e_bound_jobs_per_s"], 4)
         pr["device_frac"] = round(value / pr["device_bound_jobs_per_s"], 4)
-        extra["pipeline_roofline"] = pr
-        kr = kernel_rooflines(setlib, wl, pk, d if wl.config == 4 else None)
-        extra["kernels"] = kr
+        detail["pipeline_roofline"] = pr
+        detail["kernels"] = kernel_rooflines(setlib, wl, pk, d if wl.config in (4, 6) else None)
+        ks = min(steps, 10)
         if not args.no_baselines:
+            base = {}
+            modes = ("batch_sync_graphs",) if args.suite != "all" else ("batch_sync_graphs", "plain_streams", "single_graph", "mutex_queue")
+            for mode in modes:
+                for io_device in (False, True):
+                    base[f"{mode}_{'device' if io_device else 'e2e'}"] = brief(arm(wl, ids, mode, io_device, ks, min(warmup, 3), verify=2))
+            detail["baselines"] = base
+            detail["speedup_vs_batch_sync_graphs"] = {"e2e": round(e2e_value / base["batch_sync_graphs_e2e"]["jobs_per_s"], 3),
+                                                      "device": round(value / base["batch_sync_graphs_device"]["jobs_per_s"], 3)}
+        if not args.no_gaps:
+            gm = ("set", "batch_sync_graphs") if args.suite == "headline" else ("set", "batch_sync_graphs", "mutex_queue")
+            detail["device_gaps"] = {"how": "set_config.timestamps=1: %globaltimer at graph start (root node) and end (signal / last node); gap = "
+                                            "start(next job on the CUDA stream) - end(previous); overhead_frac = 1 - |union of job intervals| / step time "
+                                            "(PAPER.md:81-90, :253, reading S12), per step; e2e arms",
+                                     f"config{wl.config}": device_gap_arms(setlib, wl, ids, gm, flush)}
+        if args.suite == "all" and not args.no_baselines:
             cm = {}
             for name, cb in (("hostfunc_notify_stream", 1), ("hostfunc_work_stream", 2), ("graph_host_node", 4)):
-                p_, r_ = LAYOUT[wl.config]
-                r = run_arm(setlib, wl, ids, "set", False, steps, warmup, p_, r_, verify=2, ctx_kw={"callback_mode": cb}, flush=flush)
-                log(f"[bench]   {wl.config} set/{name:24s} host   {r['jobs_per_s']:12.1f} jobs/s  host us/job {r['host_us_per_job']}")
-                cm[name + "_e2e"] = {"jobs_per_s": round(r["jobs_per_s"], 1), "ms_per_step": round(r["ms_per_step"], 3),
-                                     "host_us_per_job": r["host_us_per_job"], "mismatches": r["mismatches"]}
-            extra["completion_modes"] = dict(cm, flag_poll_e2e={"jobs_per_s": round(e2e_value, 1)})
+                cm[name + "_e2e"] = brief(arm(wl, ids, "set", False, ks, min(warmup, 3), verify=2, ctx_kw={"callback_mode": cb}))
+            for name, f in (("flag_poll_system_fence", 1), ("flag_poll_no_fence", 2)):
+                cm[name + "_e2e"] = brief(arm(wl, ids, "set", False, ks, min(warmup, 3), verify=2, opts={"completion_fence": f}))
+            detail["completion_modes"] = cm
             gv = {}
             for name, o in (("ce_copies_plain_edges", {"sm_copy_max_bytes": -1, "pdl": False}), ("ce_copies_pdl", {"sm_copy_max_bytes": -1, "pdl": True}),
                             ("sm_copies_plain_edges", {"sm_copy_max_bytes": 262144, "pdl": False}), ("sm_copies_pdl", {"sm_copy_max_bytes": 262144, "pdl": True})):
-                p_, r_ = LAYOUT[wl.config]
                 for io_device in (False, True):
-                    r = run_arm(setlib, wl, ids, "set", io_device, steps, warmup, p_, r_, verify=2, flush=flush, opts=o)
-                    gv[f"{name}_{'device' if io_device else 'e2e'}"] = {"jobs_per_s": round(r["jobs_per_s"], 1), "mismatches": r["mismatches"],
-                                                                        "host_us_per_job": r["host_us_per_job"]}
-                    log(f"[bench]   {wl.config} set/{name:24s} {'device' if io_device else 'host  '} {r['jobs_per_s']:12.1f} jobs/s")
-            extra["graph_variants"] = gv
-            base = {}
-            for mode in ("batch_sync_graphs", "plain_streams", "single_graph", "mutex_queue"):
-                for io_device in (False, True):
-                    r = arm(wl, ids, mode, io_device, verify=2)
-                    base[f"{mode}_{'device' if io_device else 'e2e'}"] = {"jobs_per_s": round(r["jobs_per_s"], 1),
-                                                                         "ms_per_step": round(r["ms_per_step"], 3),
-                                                                         "host_us_per_job": r["host_us_per_job"],
-                                                                         "mismatches": r["mismatches"]}
-            extra["baselines"] = base
-            extra["speedup_vs_batch_sync_graphs"] = {"e2e": round(e2e_value / base["batch_sync_graphs_e2e"]["jobs_per_s"], 3),
-                                                     "device": round(value / base["batch_sync_graphs_device"]["jobs_per_s"], 3)}
-            # host scheduling overhead per job (BASELINE.json:metric): time the host spends updating, launching, completing
-            # and -- in the batch model -- blocked in synchronisation, per job, end to end
-            hs, hb = e2e_arm["host_us_per_job"], base["batch_sync_graphs_e2e"]["host_us_per_job"]
-            so_set = hs["bind"] + hs["launch"] + hs["callback"]
-            so_batch = hb["bind"] + hb["launch"] + hb["sync"]
-            extra["sched_overhead_us_per_job"] = {"set": round(so_set, 3), "batch_sync_graphs": round(so_batch, 3),
-                                                  "reduction": round(1.0 - so_set / so_batch, 3) if so_batch > 0 else None,
-                                                  "how": "set: bind + launch + callback; batch: bind + launch + host sync wait; e2e arms"}
-        if args.suite == "all":
+                    gv[f"{name}_{'device' if io_device else 'e2e'}"] = brief(arm(wl, ids, "set", io_device, ks, min(warmup, 3), verify=2, opts=o))
+            detail["graph_variants"] = gv
+            lv = {}
+            for lanes in (1, 2, 4):
+                for mode in ("set", "batch_sync_graphs"):
+                    lv[f"{mode}_lanes{lanes}_e2e"] = brief(arm(wl, ids, mode, False, ks, min(warmup, 3), verify=2, opts={"streams_per_lane": lanes}))
+            detail["streams_per_lane_variants"] = lv
+        if args.suite in ("default", "all"):
             others = {}
-            for c in range(5):
+            for c in SIDE_CONFIGS:
                 if c == wl.config:
                     continue
-                w2 = baseline_workload(c)
+                w2 = workload_for(c)
                 ids2 = list(range(w2.jobs))
-                k2, wu2 = (3, 3)
                 try:
-                    a_dev = arm(w2, ids2, "set", True, k2, wu2, verify=2)
-                    a_e2e = arm(w2, ids2, "set", False, k2, wu2, verify=2)
-                    b_e2e = arm(w2, ids2, "batch_sync_graphs", False, k2, wu2, verify=0)
-                    b_dev = arm(w2, ids2, "batch_sync_graphs", True, k2, wu2, verify=0)
+                    a_e2e = arm(w2, ids2, "set", False, SIDE_STEPS, SIDE_WARMUP, verify=2)
+                    b_e2e = arm(w2, ids2, "batch_sync_graphs", False, SIDE_STEPS, SIDE_WARMUP, verify=0)
+                    a_dev = arm(w2, ids2, "set", True, SIDE_STEPS, SIDE_WARMUP, verify=2)
                     d2 = mean_dims(w2, ids2)
                     pr2 = pipeline_roofline(w2, a_e2e["in_bytes"] / a_e2e["jobs"], a_e2e["out_bytes"] / a_e2e["jobs"], link, pk, d2)
-                    others[f"config{c}"] = {
-                        "workload": w2.name, "value": round(a_dev["jobs_per_s"], 1), "e2e": round(a_e2e["jobs_per_s"], 1),
-                        "batch_sync_graphs_e2e": round(b_e2e["jobs_per_s"], 1), "batch_sync_graphs_device": round(b_dev["jobs_per_s"], 1),
-                        "speedup_vs_batch_sync_e2e": round(a_e2e["jobs_per_s"] / b_e2e["jobs_per_s"], 3),
-                        "speedup_vs_batch_sync_device": round(a_dev["jobs_per_s"] / b_dev["jobs_per_s"], 3),
-                        "host_us_per_job": a_e2e["host_us_per_job"], "mismatches": a_dev["mismatches"] + a_e2e["mismatches"],
-                        "pipeline_roofline": dict(pr2, e2e_frac=round(a_e2e["jobs_per_s"] / pr2["e2e_bound_jobs_per_s"], 4)),
-                        "kernels": kernel_rooflines(setlib, w2, pk, d2 if c == 4 else None)}
+                    row = {"workload": w2.name, "e2e": round(a_e2e["jobs_per_s"], 1), "value": round(a_dev["jobs_per_s"], 1),
+                           "batch_sync_graphs_e2e": round(b_e2e["jobs_per_s"], 1),
+                           "speedup_vs_batch_sync_e2e": round(a_e2e["jobs_per_s"] / b_e2e["jobs_per_s"], 3),
+                           "host_us_per_job": {k: round(v, 3) for k, v in a_e2e["host_us_per_job"].items()},
+                           "mismatches": a_dev["mismatches"] + a_e2e["mismatches"],
+                           "pipeline_roofline": dict(pr2, e2e_frac=round(a_e2e["jobs_per_s"] / pr2["e2e_bound_jobs_per_s"], 4)),
+                           "kernels": kernel_rooflines(setlib, w2, pk, d2 if c in (4, 6) else None)}
+                    side_bad += row["mismatches"]
+                    if args.suite == "all" and not args.no_baselines:
+                        b_dev = arm(w2, ids2, "batch_sync_graphs", True, SIDE_STEPS, SIDE_WARMUP, verify=0)
+                        row["batch_sync_graphs_device"] = round(b_dev["jobs_per_s"], 1)
+                        row["speedup_vs_batch_sync_device"] = round(a_dev["jobs_per_s"] / b_dev["jobs_per_s"], 3)
+                    if not args.no_cpu:
+                        # SURVEY.md 8(d) "Oracle timing": every config, bounded; config 0 is where a CPU core may out-run the PCIe round trip
+                        row["cpu_baseline"] = cpu_baseline(w2, ids2, budget_s=3.0 if args.suite == "default" else 10.0,
+                                                           all_cores_s=0.0 if args.suite == "default" else 3.0)
+                        row["gpu_e2e_over_one_cpu_core"] = round(row["e2e"] / row["cpu_baseline"]["value"], 2) if row["cpu_baseline"]["value"] else None
+                    if args.suite == "all" and not args.no_gaps:
+                        detail["device_gaps"][f"config{c}"] = device_gap_arms(setlib, w2, ids2[:{0: 256, 1: 10000, 2: 64, 3: 200, 4: 1024}.get(c, 256)],
+                                                                              ("set", "batch_sync_graphs"), flush, steps=2)
+                    others[f"config{c}"] = row
                 except Exception as e:  # a failing side workload must not hide the headline number
                     others[f"config{c}"] = {"error": str(e)[:300]}
                     log(f"[bench] config {c} failed: {e}")
-            extra["workloads"] = others
-    if world == 1 and not args.no_gaps:
-        extra["device_gaps"] = device_gap_pass(setlib, wl, ids, args.suite == "all", flush)
-    if world == 1 and args.sweep:
-        extra["batch_sweep"] = batch_sweep(setlib, wl, ids, flush, not args.no_gaps)
+                _INPUTS.clear()  # the side workloads' inputs are large (config 2: 1 GB): keep only what is in use
+            detail["workloads"] = others
+        if args.sweep:
+            detail["batch_sweep"] = batch_sweep(setlib, wl, ids, flush)
+    detail["side_mismatches"] = side_bad
     sampler.stop()
     clocks = sampler.summary(windows)
-    if world == 1 and not args.no_gaps:
-        extra["gaps"] = gap_pass(setlib, wl, ids, args.suite == "all", warmup)
+    if world == 1 and args.suite == "all" and not args.no_gaps:
+        detail["gaps_cupti"] = gap_pass(setlib, wl, ids, True, warmup)
+    if rank == 0 and world == 1 and not args.no_cpu:
+        detail["cpu_baseline"] = cpu_baseline(wl, ids)
+    detail["wall_s"] = round(time.perf_counter() - t_start, 1)
 
     if rank == 0:
-        dom = max(extra.get("kernels", [{"total_us": 0}]), key=lambda r: r.get("total_us", 0)) if extra.get("kernels") else None
-        roof = None
-        if dom:
-            roof = {"bound": dom["bound"], "achieved": dom["achieved"], "peak": dom["peak"], "unit": dom["unit"], "frac": dom["frac"],
-                    "traffic": dom.get("traffic"), "kernel": dom["kernel"], "avg_us": dom["avg_us"], "algorithmic_per_launch": dom["algorithmic"],
-                    "peak_source": pk["source"],
-                    "how": "set_time_stage: the stage kernel alone, a chain of launches bracketed by CUDA events on the launching stream"}
-        line = {"metric": "jobs/s", "value": round(value, 1), "unit": "jobs/s", "n_gpus": world, "steps": steps, "warmup": warmup,
-                "ms_per_step": round(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": wl.dtype, "data": "synthetic",
-                "config": {"workload": wl.name, "jobs_per_step_per_gpu": len(ids), "num_streams": wl.num_streams,
-                           "sm_copy_max_bytes": OPTS["sm_copy_max_bytes"] or 262144, "pdl_edges": OPTS["pdl"], "submitter_threads": OPTS["submitters"],
-                           "max_inflight": wl.max_inflight, "io": "value: inputs/outputs resident in HBM (the copy nodes move HBM to HBM); e2e: pinned host buffers",
-                           "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer rewritten between timed steps; distinct job inputs "
-                                 f"{dev_arm['in_bytes'] / 1e6:.0f} MB per step"},
-                "clocks": clocks,
-                "e2e": {"value": round(e2e_value, 1), "unit": "jobs/s", "h2d_bytes_per_step": int(e2e_arm["h2d_bytes"] * world),
-                        "d2h_bytes_per_step": int(e2e_arm["d2h_bytes"] * world), "ms_per_step": round(ms_e2e, 4)},
-                "gpu_launches": int(dev_arm["kernel_launches"] * world),
-                "mismatches": dev_arm["mismatches"] + e2e_arm["mismatches"],
-                "host_us_per_job": {"device": dev_arm["host_us_per_job"], "e2e": e2e_arm["host_us_per_job"]},
-                "sched_stats": {k: e2e_arm["stats"][k] for k in ("steals", "submit_stalls", "dispatcher_sleeps", "max_inflight_seen",
-                                                                  "full_rebinds", "host_rebinds")}}
-        # BASELINE.json:metric in one place: jobs/s; mean inter-kernel gap; scheduling overhead against batched graphs
+        line = compact_line(wl, world, steps, warmup, len(ids), ms_dev, value, ms_e2e, e2e_value, dev_arm, e2e_arm, clocks, detail, args.out, pk)
+        detail["line"] = line
         try:
-            dg, cg = extra.get("device_gaps", {}).get(f"config{wl.config}", {}), extra.get("gaps", {}).get(f"config{wl.config}", {})
-            line["headline_metrics"] = {
-                "jobs_per_s": {"set_e2e": round(e2e_value, 1), "set_device_resident": round(value, 1),
-                               "batch_sync_graphs_e2e": extra.get("baselines", {}).get("batch_sync_graphs_e2e", {}).get("jobs_per_s")},
-                "mean_gap_between_kernels_of_a_job_us": {k: cg[k]["kernel_kernel"]["mean_us"] for k in ("set_e2e", "batch_sync_graphs_e2e")
-                                                         if isinstance(cg.get(k), dict) and "kernel_kernel" in cg[k]},
-                "gap_between_jobs_on_a_stream_at_full_speed_us": {k: {"mean": dg[k]["gap_mean_us"], "p99": dg[k]["gap_p99_us"]}
-                                                                  for k in ("set_e2e", "batch_sync_graphs_e2e", "mutex_queue_e2e")
-                                                                  if isinstance(dg.get(k), dict) and "gap_mean_us" in dg[k]},
-                "device_idle_fraction_traced": {k: cg[k]["idle_frac"] for k in ("set_e2e", "batch_sync_graphs_e2e")
-                                                if isinstance(cg.get(k), dict) and "idle_frac" in cg[k]},
-                "host_sched_overhead_us_per_job": extra.get("sched_overhead_us_per_job")}
-        except Exception as e:  # a summary must never cost the line
-            line["headline_metrics"] = {"error": str(e)[:120]}
-        if roof:
-            line["roofline"] = roof
-        if world == 1 and not args.no_cpu:
-            line["cpu_baseline"] = cpu_baseline(wl, ids)
-        line.update(extra)
-        s = json.dumps(line)
-        print(s, flush=True)
-        if args.out:
             with open(args.out, "w") as f:
-                f.write(s + "\n")
+                json.dump(detail, f, indent=1)
+            log(f"[bench] detail written to {args.out} ({detail['wall_s']} s)")
+        except OSError as e:
+            log(f"[bench] could not write {args.out}: {e}")
+        s = json.dumps(line, separators=(",", ":"))
+        print(s, flush=True)
     multi.barrier(dev)
     return 0
 
+
+SIDE_CONFIGS = (0, 1, 2, 3, 4)
 
 if __name__ == "__main__":
     sys.exit(main())

@@ -15,6 +15,8 @@
  *   SET_DRIVER_LOCK=1       take one mutex around every graph update and graph launch.  Only for runs under Nsight
  *                           Compute 2025.2, whose injection library is not safe against one thread updating a graph
  *                           executable while another launches one (profiles/r1_ncu.md).  Never set for timing.
+ *                           Turned on by itself when the process runs under a CUDA injection library (CUDA_INJECTION64_PATH
+ *                           or an NV_NSIGHT_INJECTION_* / NV_COMPUTE_PROFILER_* variable is set); SET_DRIVER_LOCK=0 overrides.
  *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 8: 64 KB in flight per
  *                           copy; more delays the GPU's own command fetches over the same link).
  *
@@ -103,9 +105,10 @@ typedef struct set_arg_desc {
 } set_arg_desc;
 
 #define SET_STAGE_PDL 1u   /* connect this stage to the node before it (the previous stage; for the first stage,
-                              an SM copy node) with a programmatic-dependent-launch edge: the kernel must
-                              execute griddepcontrol.wait before it reads or writes job data (every built-in
-                              kernel does).  Ignored where the predecessor is a copy-engine node.           */
+                              an SM copy node) with a programmatic-dependent-launch edge.  By setting the flag the
+                              caller asserts that the kernel executes griddepcontrol.wait before it reads or writes
+                              job data; every built-in kernel does (the tcgen05 GEMM after its barrier / TMEM set-up,
+                              before its first TMA load).  Ignored where the predecessor is a copy-engine node.  */
 
 /* One stage = one kernel node of the job graph ("nodes are initialized with the target
  * function, input arguments, grid and block dimensions").  Stages run in list order. */
@@ -196,12 +199,31 @@ typedef struct set_config {
                                  ends (the completion-signal node, or a last node of its own): the device-side gap
                                  between consecutive jobs of a stream, measured at full speed without a profiler
                                  attached; read with set_get_gap_stats.  0 (default): no such nodes.            */
-    int32_t reserved1;
+    int32_t completion_fence; /* SET_CB_FLAG_POLL: how the signal node publishes the slot's word.  SET_FENCE_DEFAULT (0) =
+                                 the library's choice, SET_FENCE_SYSTEM; SET_FENCE_SYSTEM (1) = fence.acq_rel.sys before
+                                 the store (release at system scope: the job's D2H output, written by an earlier grid, is
+                                 ordered before the word by the PTX memory model); SET_FENCE_NONE (2) = plain volatile
+                                 store, relying on grid completion alone (faster, measured never wrong on B200, but not
+                                 guaranteed by the model).  DESIGN.md 5a.                                           */
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */
     uint64_t device_arena_bytes;
+    int32_t streams_per_lane; /* CUDA streams behind each of the num_streams logical streams ("lanes"): slot w runs on
+                                 lane w mod S, CUDA stream (w / S) mod streams_per_lane of that lane, so consecutive jobs
+                                 of a lane overlap (job k+1's copy-in runs beside job k's kernels and tail) instead of
+                                 queueing behind each other's last node.  The paper's worker owns a stream of its own
+                                 (PAPER.md:110), which is streams_per_lane = max_inflight / num_streams.  0 => default
+                                 (DESIGN.md 5b); forced to 1 when the caller supplies `streams`.                      */
+    uint32_t debug_sentinel;  /* test hook: non-zero => at the moment a job's completion is observed (before the slot is
+                                 released) the first and last 32-bit word of every D2H region of its host_out are compared
+                                 with this value; a match means the completion overtook the output, counted in
+                                 set_stats.early_completions.  The caller pre-fills host_out with the value.  0 = off.  */
 } set_config;
+
+#define SET_FENCE_DEFAULT 0
+#define SET_FENCE_SYSTEM  1
+#define SET_FENCE_NONE    2
 
 typedef struct set_stats {
     uint64_t submitted;        /* jobs accepted by set_submit*                                     */
@@ -222,7 +244,9 @@ typedef struct set_stats {
     uint64_t max_inflight_seen;/* high-water mark of launched-not-completed jobs                   */
     uint64_t signal_nodes;     /* completion-signal kernel launches (SET_CB_FLAG_POLL: one per job)*/
     uint64_t copy_nodes;       /* SET_K_COPY kernel launches (copies done by the SMs)                 */
-    uint64_t reserved[2];
+    uint64_t early_completions;/* set_config.debug_sentinel: jobs whose output still held the sentinel when their completion
+                                  was observed (must stay 0)                                             */
+    uint64_t cuda_streams;     /* CUDA streams the context runs on: num_streams * streams_per_lane (not a counter) */
 } set_stats;
 
 /* ---------------------------------------------------------------------------------------------- *
@@ -283,6 +307,14 @@ set_status set_destroy(set_ctx *ctx);
 void *set_host_alloc(set_ctx *ctx, size_t bytes);
 void set_host_free(set_ctx *ctx, void *p);
 
+/* Tell the library that [p, p + bytes) is pinned HOST memory the caller owns (cudaHostAlloc / cudaHostRegister / torch
+ * pin_memory) so that jobs in it skip the per-job driver query.  The range is checked once (SET_ERR_INVALID if it is
+ * not pinned, or if an SM copy could not dereference it on the device).  The caller must call set_host_unregister
+ * before freeing or unpinning the memory: the library caches only ranges it was told about (its own set_host_alloc
+ * blocks and these); any other pointer is queried at every submit. */
+set_status set_host_register(set_ctx *ctx, const void *p, size_t bytes);
+set_status set_host_unregister(set_ctx *ctx, const void *p);
+
 /* Counters and per-phase host time since create (or since set_reset_stats). out: HOST. */
 set_status set_get_stats(set_ctx *ctx, set_stats *out);
 set_status set_reset_stats(set_ctx *ctx);
@@ -298,7 +330,11 @@ typedef struct set_gap_stats {
     double gap_mean_us, gap_p50_us, gap_p99_us, gap_max_us;
     double job_mean_us;     /* mean of end - start of one job (its chain on the device)             */
     double span_us;         /* last end - first start over all jobs                                 */
-    double stream_busy_frac;/* sum of job durations / (span * streams): how full the streams were   */
+    double stream_busy_frac;/* sum of job durations / (span * CUDA streams): how full the streams were */
+    double busy_union_us;   /* |union over all streams of the jobs' [start, end] intervals|: time during which the
+                               GPU had at least one job in progress                                  */
+    double idle_frac;       /* 1 - busy_union_us / span_us: the timeline's white space, the
+                               t_schedule / T_measured of PAPER.md:81-90, :253 under reading S12, at job granularity */
 } set_gap_stats;
 set_status set_get_gap_stats(set_ctx *ctx, set_gap_stats *out);
 
@@ -333,8 +369,9 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_BLUR3X3_U8     11  /* (const uint8* g, uint8* out, uint32 w, uint32 h)  clamp-to-edge          */
 #define SET_K_HIST256_U8     12  /* (const uint8* p, uint32* hist, uint32 w, uint32 h)  hist must be zeroed  */
 #define SET_K_SPIN           13  /* (uint32* scratch, uint32 ns)  debug delay stage (busy-waits ns)          */
-#define SET_K_SIGNAL         14  /* (uint32* flag, uint64* stamp)  *flag = 1 in mapped pinned HOST memory
-                                    (SET_CB_FLAG_POLL); stamp != NULL: *stamp = %globaltimer first            */
+#define SET_K_SIGNAL         14  /* (uint32* flag, uint64* stamp, uint32 fence)  *flag = 1 in mapped pinned HOST memory
+                                    (SET_CB_FLAG_POLL), behind fence.acq_rel.sys if fence != 0; stamp != NULL:
+                                    *stamp = %globaltimer first                                               */
 #define SET_K_STAMP          16  /* (uint64* stamp)  *stamp = %globaltimer (set_config.timestamps)               */
 #define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes)  copy by the SMs; src / dst may be
                                     pinned HOST or DEVICE memory                                              */

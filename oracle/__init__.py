@@ -28,6 +28,8 @@ _lib.oracle_hist_mod.argtypes = [_p, _i64, C.c_int32, _p]
 _lib.oracle_config0.argtypes = [_p, _i64, C.c_int, _p]
 _lib.oracle_config1.argtypes = [_p, _p, _i64, _p]
 _lib.oracle_config1.restype = C.c_float
+_lib.oracle_config1_chain.argtypes = [_p, _p, _i64, _p, _p, _p, _p]
+_lib.oracle_config1_chain.restype = None
 _lib.oracle_jacobi5_sweep.argtypes = [_p, _i64, _i64, _p]
 _lib.oracle_config2.argtypes = [_p, _i64, _i64, C.c_int, _p, _p]
 _lib.oracle_bf16_to_f64.argtypes = [C.c_uint16]
@@ -78,6 +80,16 @@ def config1(x: np.ndarray, bias: np.ndarray, want_t4: bool = False):
     r = _lib.oracle_config1(_ptr(x), _ptr(bias), x.size, _ptr(t4) if want_t4 else None)
     r = np.float32(r)
     return (r, t4) if want_t4 else r
+
+
+def config1_chain(x: np.ndarray, bias: np.ndarray):
+    """(t1, t2, t3, t4): the four elementwise stages of config 1, every intermediate (reading C1-1)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    bias = np.ascontiguousarray(bias, dtype=np.float32)
+    assert x.size == bias.size
+    t = [np.empty_like(x) for _ in range(4)]
+    _lib.oracle_config1_chain(_ptr(x), _ptr(bias), x.size, *[_ptr(a) for a in t])
+    return tuple(t)
 
 
 # ------------------------------------------------------------------ config 2

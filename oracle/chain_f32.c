@@ -24,3 +24,21 @@ float oracle_config1(const float *x, const float *bias, int64_t n, float *t4_out
     }
     return (float)acc;
 }
+
+/* The same chain with every intermediate written out (any of t1..t4 may be NULL): what the GPU's four elementwise
+ * kernels K3..K6 must reproduce bit for bit, one kernel per line (reading C1-1: every line is one correctly rounded
+ * fp32 operation; reading C1-5: the stages stay unfused).  Same statements as oracle_config1, no sum. */
+void oracle_config1_chain(const float *x, const float *bias, int64_t n, float *t1_out, float *t2_out, float *t3_out,
+                          float *t4_out) {
+    for (int64_t i = 0; i < n; ++i) {
+        float m = 2.5f * x[i];
+        float t1 = m + 0.1f;
+        float t2 = t1 + bias[i];
+        float t3 = t2 > 0.0f ? t2 : 0.0f;
+        float t4 = t3 * t3;
+        if (t1_out) t1_out[i] = t1;
+        if (t2_out) t2_out[i] = t2;
+        if (t3_out) t3_out[i] = t3;
+        if (t4_out) t4_out[i] = t4;
+    }
+}

@@ -31,6 +31,8 @@ void oracle_config0(const int32_t *v, int64_t n, int hist_of_input, void *out);
 
 /* config 1 (configs[1]; readings C1-1..C1-6).  t4 (optional, may be NULL) receives the chain before the sum */
 float oracle_config1(const float *x, const float *bias, int64_t n, float *t4);
+/* the chain's intermediates t1 = affine, t2 = + bias, t3 = relu, t4 = square (each may be NULL): what K3..K6 write */
+void oracle_config1_chain(const float *x, const float *bias, int64_t n, float *t1, float *t2, float *t3, float *t4);
 
 /* config 2 (configs[2]; readings C2-1..C2-4).  u, out: fp32[h][w] row-major; tmp: scratch fp32[h*w] */
 void oracle_jacobi5_sweep(const float *u, int64_t h, int64_t w, float *out);

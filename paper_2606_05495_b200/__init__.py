@@ -26,6 +26,7 @@ STEAL_SWAP, STEAL_RETARGET = 0, 1
 CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL, CB_HOST_NODE = 0, 1, 2, 3, 4
 ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D = 0, 1, 2, 3, 4
 STAGE_PDL = 1
+FENCE_DEFAULT, FENCE_SYSTEM, FENCE_NONE = 0, 1, 2
 K_COPY = 15
 BUF_ZERO = 1
 VARIANT_SPIN = 0x100
@@ -72,14 +73,15 @@ class Config(C.Structure):
     _fields_ = [("struct_bytes", C.c_uint32), ("num_streams", C.c_int32), ("max_inflight", C.c_int32), ("mode", C.c_int32),
                 ("io", C.c_int32), ("queue_capacity", C.c_int32), ("num_dispatchers", C.c_int32), ("steal_policy", C.c_int32),
                 ("callback_mode", C.c_int32), ("device", C.c_int32), ("spin_us", C.c_int32), ("sm_copy_max_bytes", C.c_int32),
-                ("timestamps", C.c_int32), ("reserved1", C.c_int32), ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64)]
+                ("timestamps", C.c_int32), ("completion_fence", C.c_int32), ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64),
+                ("streams_per_lane", C.c_int32), ("debug_sentinel", C.c_uint32)]
 
 
 class Stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in
                 ("submitted", "completed", "launched", "steals", "full_rebinds", "host_rebinds", "staged_jobs", "submit_stalls",
                  "dispatcher_sleeps", "kernel_nodes", "ns_submit", "ns_bind", "ns_launch", "ns_callback", "ns_sync",
-                 "max_inflight_seen", "signal_nodes", "copy_nodes")] + [("reserved", C.c_uint64 * 2)]
+                 "max_inflight_seen", "signal_nodes", "copy_nodes", "early_completions", "cuda_streams")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if n != "reserved"}
@@ -88,7 +90,7 @@ class Stats(C.Structure):
 class GapStats(C.Structure):
     _fields_ = [("jobs", C.c_uint64), ("gaps", C.c_uint64), ("gap_mean_us", C.c_double), ("gap_p50_us", C.c_double),
                 ("gap_p99_us", C.c_double), ("gap_max_us", C.c_double), ("job_mean_us", C.c_double), ("span_us", C.c_double),
-                ("stream_busy_frac", C.c_double)]
+                ("stream_busy_frac", C.c_double), ("busy_union_us", C.c_double), ("idle_frac", C.c_double)]
 
     def as_dict(self):
         return {n: (int(getattr(self, n)) if n in ("jobs", "gaps") else round(float(getattr(self, n)), 4)) for n, _ in self._fields_}
@@ -96,7 +98,7 @@ class GapStats(C.Structure):
 
 # every symbol include/set.h declares -- tests/test_abi.py checks the list against the header
 EXPORTS = ["set_create", "set_create_ex", "set_register_pipeline", "set_submit", "set_submit_dims", "set_submit_batch",
-           "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_get_stats", "set_reset_stats", "set_get_gap_stats",
+           "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_host_register", "set_host_unregister", "set_get_stats", "set_reset_stats", "set_get_gap_stats",
            "set_last_error", "set_get_geometry", "set_time_stage", "set_builtin_kernel", "set_builtin_pipeline",
            "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler"]
 
@@ -125,6 +127,8 @@ def load():
     lib.set_host_alloc.restype = vp
     lib.set_host_free.argtypes = [vp, vp]
     lib.set_host_free.restype = None
+    lib.set_host_register.argtypes = [vp, vp, C.c_size_t]
+    lib.set_host_unregister.argtypes = [vp, vp]
     lib.set_get_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.set_reset_stats.argtypes = [vp]
     lib.set_get_gap_stats.argtypes = [vp, C.POINTER(GapStats)]
@@ -170,7 +174,8 @@ class Context:
     def __init__(self, num_streams: int, max_inflight: int, mode: int = MODE_SET, io: int = IO_HOST, queue_capacity: int = 0,
                  num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_DEFAULT,
                  device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0,
-                 sm_copy_max_bytes: int = 0, timestamps: bool = False):
+                 sm_copy_max_bytes: int = 0, timestamps: bool = False, completion_fence: int = FENCE_DEFAULT,
+                 streams_per_lane: int = 0, debug_sentinel: int = 0):
         self._lib = load()
         self._h = C.c_void_p(None)
         cfg = Config()
@@ -180,6 +185,7 @@ class Context:
         cfg.callback_mode, cfg.device, cfg.spin_us = callback_mode, device, spin_us
         cfg.sm_copy_max_bytes = sm_copy_max_bytes
         cfg.timestamps = 1 if timestamps else 0
+        cfg.completion_fence, cfg.streams_per_lane, cfg.debug_sentinel = completion_fence, streams_per_lane, debug_sentinel
         self._streams_arr = None
         if streams is not None:
             self._streams_arr = (C.c_void_p * len(streams))(*[int(s) for s in streams])
@@ -267,6 +273,12 @@ class Context:
 
     def host_free(self, p: int):
         self._lib.set_host_free(self._h, p)
+
+    def host_register(self, p: int, nbytes: int):
+        self._check(self._lib.set_host_register(self._h, p, nbytes), "set_host_register")
+
+    def host_unregister(self, p: int):
+        self._check(self._lib.set_host_unregister(self._h, p), "set_host_unregister")
 
     def stats(self) -> dict:
         s = Stats()

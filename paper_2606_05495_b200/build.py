@@ -79,5 +79,24 @@ def build_trace(force: bool = False) -> str:
     return TRACE_LIB
 
 
+def build_selftest(sanitizer: str = "thread") -> str:
+    """csrc/selftest_main.cpp + set_selftest.cpp (header-only scheduler core, no CUDA) with -fsanitize=<sanitizer>:
+    the lock-free ring and Algorithms 1-3 against a simulated device under ThreadSanitizer / AddressSanitizer."""
+    os.makedirs(BUILD_DIR, exist_ok=True)
+    exe = os.path.join(BUILD_DIR, f"selftest_{sanitizer.replace(',', '_')}")
+    srcs = [os.path.join(CSRC, "selftest_main.cpp"), os.path.join(CSRC, "set_selftest.cpp")]
+    deps = srcs + [os.path.join(CSRC, h) for h in ("set_core.hpp", "set_ring.hpp")] + [os.path.join(INCLUDE, "set.h")]
+    if _stale(exe, deps):
+        cmd = ["g++", "-O1", "-g", "-std=c++17", f"-fsanitize={sanitizer}", "-pthread", "-I", INCLUDE, "-o", exe] + srcs
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+            raise RuntimeError("building the sanitizer self test failed")
+    return exe
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    if "--selftest" in sys.argv:
+        print(build_selftest(sys.argv[sys.argv.index("--selftest") + 1]))
+    else:
+        print(build(force="--force" in sys.argv, verbose=True))

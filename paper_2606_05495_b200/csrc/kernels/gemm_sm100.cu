@@ -172,6 +172,10 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+    // Programmatic dependent launch (set.h SET_STAGE_PDL): the prologue above (tensor-map prefetch, barrier init, TMEM
+    // allocation) may overlap the node before this one; nothing below may read A, B or bias, or write C, before that
+    // node's writes are visible.  Both instructions do nothing over an ordinary edge.
+    set_pdl_sync();
 
     if (warp == 0) {
         // ===== TMA producer =====

@@ -18,7 +18,7 @@ __global__ void set_k_rgb2gray_u8(const uint8_t* rgb, uint8_t* gray, uint32_t w,
 __global__ void set_k_blur3x3_u8(const uint8_t* g, uint8_t* out, uint32_t w, uint32_t h);
 __global__ void set_k_hist256_u8(const uint8_t* p, uint32_t* hist, uint32_t w, uint32_t h);
 __global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
-__global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp);
+__global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp, uint32_t fence);
 __global__ void set_k_stamp(unsigned long long* stamp);
 __global__ void set_k_copy(const void* src, void* dst, uint32_t bytes);
 }

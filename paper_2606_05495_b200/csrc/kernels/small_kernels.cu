@@ -222,6 +222,7 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_block_sum_f32(const flo
 // K13: debug delay stage (SURVEY.md §5 fault injection): one thread busy-waits `ns` nanoseconds so that job
 // completions reorder and slots stay occupied; scratch[0] receives the waited time.
 extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
+    set_pdl_sync();
     unsigned long long t0, t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
     do {
@@ -231,19 +232,25 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
 }
 
 // K14: completion signal of SET_CB_FLAG_POLL.  Last node of the job graph: it depends on every D2H copy node (memcpy
-// node or SET_K_COPY kernel node), so when this grid starts the job's output has been performed at system scope --
-// grid completion orders a grid's writes before everything a dependent grid does.  One thread stores 1 to the slot's
-// word in mapped pinned host memory, which the dispatcher thread is watching.  No __threadfence_system(): measured on
-// B200 a system fence costs 2.5 us idle and more under load even in a thread with no stores of its own (config 1 end
-// to end: 201 K jobs/s with the fence here, 190 K with the signal fused into the copy kernel behind a fence, 217 K
-// without; profiles/r1_bench.md), and the dependency edge already gives the ordering.
-extern "C" __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp) {
+// node or SET_K_COPY kernel node).  One thread stores 1 to the slot's word in mapped pinned host memory, which the
+// dispatcher thread is watching.
+//   fence != 0 (SET_FENCE_SYSTEM, the default): fence.acq_rel.sys, then the store.  The job's output was written by an
+//     EARLIER grid; its completion (or griddepcontrol.wait) makes those writes visible to this thread, and the system-
+//     scope fence is cumulative, so they are ordered before the word for an observer on the host: a release pattern
+//     the PTX memory model guarantees.  Costs about 2.5 us of the signal node's time on B200, which
+//     set_config.streams_per_lane takes off the job-to-job critical path (the next job of the lane runs on another
+//     CUDA stream and does not wait for this node).
+//   fence == 0 (SET_FENCE_NONE): plain volatile store, relying on grid completion alone to have pushed the output out.
+//     Two unfenced stores of ONE thread were seen to reach host memory out of order on this machine (the stamp and the
+//     word below), so nothing but measurement (profiles/r2_signal_soak.md) backs this variant; it is opt-in.
+extern "C" __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp, uint32_t fence) {
     set_pdl_sync();
     if (stamp) {  // set_config.timestamps: when the job ended on the device
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         *reinterpret_cast<volatile unsigned long long*>(stamp) = t;
     }
+    if (fence) asm volatile("fence.acq_rel.sys;" ::: "memory");
     *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
 }
 

@@ -26,6 +26,7 @@
 using namespace setrt;
 
 #define SET_COPY_BYTES_PER_BLOCK 8192u  // kernels/kernels.h kCopyBytesPerBlock (SET_K_COPY: 256 threads x 2 x 16 B)
+static constexpr int kDefaultStreamsPerLane = 1;  // set_config.streams_per_lane == 0
 
 namespace {
 
@@ -84,6 +85,7 @@ struct PinnedRange {
 struct set_ctx final : public Backend {
     set_config cfg{};
     int S = 0, b = 0, q = 0, epp = 0, device = 0;
+    int L = 1, H = 0;  // set_config.streams_per_lane and the number of CUDA streams H = S * L; slot w runs on streams[w % H]
     std::vector<cudaStream_t> streams, notify;
     bool own_streams = false;
     std::unique_ptr<SpinLock[]> stream_locks;
@@ -130,7 +132,8 @@ struct set_ctx final : public Backend {
     std::vector<CbArg> cbargs;
 
     // counters owned by the backend
-    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0}, signal_nodes{0}, copy_nodes{0};
+    std::atomic<uint64_t> full_rebinds{0}, host_rebinds{0}, staged_jobs{0}, ns_bind{0}, ns_sync{0}, kernel_nodes{0}, signal_nodes{0}, copy_nodes{0},
+        early_completions{0};
     std::atomic<uint64_t> base_submitted{0}, base_completed{0}, base_launched{0}, base_ns_submit{0}, base_ns_launch{0};
 
     // sticky error
@@ -358,26 +361,8 @@ bool set_ctx::is_pinned(const void* p) {
     // SM copies dereference the caller's pointer on the device: registered memory whose device alias differs (or
     // that is not mapped at all) goes through the library's own pinned staging blocks like pageable memory
     if (n_sm_copies && at.devicePointer != p) return false;
-    // remember the whole allocation so that later jobs from the same arena skip the query
-    typedef CUresult (*PFN_getattr)(void*, CUpointer_attribute, CUdeviceptr);
-    static PFN_getattr getattr = [] {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuPointerGetAttribute", &fn, cudaEnableDefault, &qr) != cudaSuccess) fn = nullptr;
-        return (PFN_getattr)fn;
-    }();
-    uintptr_t lo = a, hi = a + 1;
-    if (getattr) {
-        CUdeviceptr start = 0;
-        size_t size = 0;
-        if (getattr(&start, CU_POINTER_ATTRIBUTE_RANGE_START_ADDR, (CUdeviceptr)at.devicePointer) == CUDA_SUCCESS &&
-            getattr(&size, CU_POINTER_ATTRIBUTE_RANGE_SIZE, (CUdeviceptr)at.devicePointer) == CUDA_SUCCESS && size > 0 &&
-            (uintptr_t)at.devicePointer == a) {  // unified addressing: host and device views coincide
-            lo = (uintptr_t)start;
-            hi = lo + size;
-        }
-    }
-    if (hi > lo + 1) add_pinned_range((void*)lo, hi - lo);
+    // Not cached: the library does not own this memory and cannot see it being freed (a stale entry would later send
+    // an SM copy into pageable memory).  Callers with their own pinned buffers declare them with set_host_register.
     return true;
 }
 
@@ -491,7 +476,8 @@ int set_ctx::build_graph() {
         }
         uint32_t* flag = flags_dev;
         unsigned long long* stamp = stamps ? ts_dev + 1 : nullptr;
-        void* args[2] = {&flag, &stamp};
+        uint32_t fence = cfg.completion_fence == SET_FENCE_SYSTEM ? 1u : 0u;
+        void* args[3] = {&flag, &stamp, &fence};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
         kp.gridDim = dim3(1);
@@ -602,7 +588,8 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
         if (signal_node && es.bound_slot != slot) {
             uint32_t* flag = flags_dev + (size_t)slot * kFlagStride;
             unsigned long long* stamp = stamps ? ts_dev + (size_t)slot * 8 + 1 : nullptr;
-            void* args[2] = {&flag, &stamp};
+            uint32_t fence = cfg.completion_fence == SET_FENCE_SYSTEM ? 1u : 0u;
+            void* args[3] = {&flag, &stamp, &fence};
             cudaKernelNodeParams kp{};
             kp.func = const_cast<void*>(set_builtin_kernel(SET_K_SIGNAL));
             kp.gridDim = dim3(1);
@@ -680,7 +667,7 @@ static void CUDART_CB set_completion_cb(void* arg) {
 
 int set_ctx::launch(int exec, int slot, const JobDesc&) {
     bind_thread();
-    int s = slot % S;
+    int s = slot % H;
     std::unique_lock<std::mutex> dl(driver_mu, std::defer_lock);
     if (driver_lock) dl.lock();
     SpinLock& lk = stream_locks[s];
@@ -705,7 +692,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
 
 int set_ctx::poll() {
     bind_thread();
-    for (int s = 0; s < S; ++s) {
+    for (int s = 0; s < H; ++s) {
         cudaError_t e = cudaStreamQuery(streams[s]);
         if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(e, "asynchronous failure on a work stream", __LINE__);
     }
@@ -714,7 +701,7 @@ int set_ctx::poll() {
 
 void set_ctx::finish(int exec, int slot, const JobDesc&) {
     if (stamps) {
-        StampRec r{(uint32_t)(slot % S), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
+        StampRec r{(uint32_t)(slot % H), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
                    __atomic_load_n(&ts_host[(size_t)slot * 8 + 1], __ATOMIC_ACQUIRE)};
         // The signal thread stores the end stamp and then the completion word, unfenced: the two stores may reach host
         // memory in either order (seen on B200, rarely -- the reason the job's OUTPUT is never written by
@@ -728,6 +715,22 @@ void set_ctx::finish(int exec, int slot, const JobDesc&) {
         }
     }
     ExecState& es = execs[exec];
+    if (cfg.debug_sentinel && cfg.io == SET_IO_HOST && es.out) {
+        // test hook (set.h debug_sentinel): this is the moment the job's completion was observed and the slot is about to
+        // be released.  The caller pre-filled host_out with the sentinel; a D2H region whose first or last word still
+        // holds it means the completion overtook the output.
+        bool early = false;
+        for (size_t i = 0; i < bufs.size(); ++i) {
+            const uint64_t n = eval(bufs[i].d2h_bytes, es.dims);
+            if (n < 4) continue;
+            const char* base = (const char*)es.out + eval(bufs[i].d2h_host_off, es.dims);
+            uint32_t first, last;  // host_out need not be 4-byte aligned
+            memcpy(&first, const_cast<const char*>(static_cast<const volatile char*>(base)), 4);
+            memcpy(&last, const_cast<const char*>(static_cast<const volatile char*>(base + ((n - 4) & ~3ull))), 4);
+            early = early || first == cfg.debug_sentinel || last == cfg.debug_sentinel;
+        }
+        if (early) early_completions.fetch_add(1, std::memory_order_relaxed);
+    }
     if (es.staged) {  // staged D2H: pinned ring -> caller's pageable memory, on the callback thread
         memcpy(es.user_out, es.stage_out, es.out_bytes);
         es.staged = false;
@@ -741,7 +744,7 @@ void set_ctx::finish(int exec, int slot, const JobDesc&) {
 // ---------------------------------------------------------------------------------------------------------
 int set_ctx::plain_job(int slot, const JobDesc& job) {
     // "Synchronous model": individual copies and kernel launches, no graph
-    int s = slot % S;
+    int s = slot % H;
     cudaStream_t st = streams[s];
     SlotMem& sm = slots[slot];
     if (sm.used) {  // buffer reuse guarded by event synchronisation
@@ -803,13 +806,13 @@ int set_ctx::baseline_flush() {
         bool dummy;
         int e = (int)i * epp;
         if (int rc = bind(e, (int)i, batch[i], &dummy)) return rc;
-        CK(cudaGraphLaunch(execs[e].exec, streams[i % S]));
+        CK(cudaGraphLaunch(execs[e].exec, streams[i % H]));
     }
     base_launched.fetch_add(batch.size(), std::memory_order_relaxed);
     kernel_nodes.fetch_add(stages.size() * batch.size(), std::memory_order_relaxed);
     copy_nodes.fetch_add((uint64_t)n_sm_copies * batch.size(), std::memory_order_relaxed);
     uint64_t t1 = now_ns();
-    for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
+    for (int s = 0; s < H; ++s) CK(cudaStreamSynchronize(streams[s]));
     uint64_t t2 = now_ns();
     for (size_t i = 0; i < batch.size(); ++i) finish((int)i * epp, (int)i, batch[i]);
     base_completed.fetch_add(batch.size(), std::memory_order_relaxed);
@@ -902,8 +905,8 @@ void set_ctx::mq_loop() {
             bool dummy;
             int rc = err.load() ? err.load() : bind(w * epp, w, j, &dummy);
             if (rc == 0) {
-                cudaError_t e = cudaGraphLaunch(execs[w * epp].exec, streams[w % S]);
-                if (e == cudaSuccess) e = cudaEventRecord(slots[w].done, streams[w % S]);
+                cudaError_t e = cudaGraphLaunch(execs[w * epp].exec, streams[w % H]);
+                if (e == cudaSuccess) e = cudaEventRecord(slots[w].done, streams[w % H]);
                 if (e != cudaSuccess) rc = cuda_fail(e, "graph launch (queue model)", __LINE__);
             }
             base_ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
@@ -945,7 +948,7 @@ int set_ctx::baseline_drain() {
         return err.load();
     }
     uint64_t t0 = now_ns();
-    for (int s = 0; s < S; ++s) CK(cudaStreamSynchronize(streams[s]));
+    for (int s = 0; s < H; ++s) CK(cudaStreamSynchronize(streams[s]));
     ns_sync.fetch_add(now_ns() - t0, std::memory_order_relaxed);
     for (auto& sm : slots) sm.used = false;
     base_completed.store(base_submitted.load());
@@ -971,9 +974,14 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.spin_us == 0) cfg.spin_us = 50;
     if (cfg.callback_mode < SET_CB_DEFAULT || cfg.callback_mode > SET_CB_HOST_NODE) return SET_ERR_INVALID;
     if (cfg.callback_mode == SET_CB_DEFAULT) cfg.callback_mode = SET_CB_FLAG_POLL;
+    if (cfg.completion_fence < SET_FENCE_DEFAULT || cfg.completion_fence > SET_FENCE_NONE) return SET_ERR_INVALID;
+    if (cfg.completion_fence == SET_FENCE_DEFAULT) cfg.completion_fence = SET_FENCE_SYSTEM;
+    if (cfg.streams_per_lane < 0 || cfg.streams_per_lane > 4096) return SET_ERR_INVALID;
+    if (cfg.streams_per_lane == 0) cfg.streams_per_lane = kDefaultStreamsPerLane;
     if (cfg.mode == SET_MODE_SINGLE_GRAPH) {  // one worker, one stream, one exec by definition
         cfg.num_streams = 1;
         cfg.max_inflight = 1;
+        cfg.streams_per_lane = 1;
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -989,18 +997,26 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (!c) return SET_ERR_NOMEM;
     c->cfg = cfg;
     c->device = dev;
+    // Nsight Compute's injection library is not safe against concurrent graph update + launch (profiles/r1_ncu.md):
+    // serialise them whenever a CUDA injection library is present, unless the environment says otherwise
+    for (const char* v : {"CUDA_INJECTION64_PATH", "NV_NSIGHT_INJECTION_PORT_BASE", "NV_NSIGHT_INJECTION_TRANSPORT_TYPE",
+                          "NV_COMPUTE_PROFILER_PERFWORKS_DIR", "NV_COMPUTE_PROFILER_LOCAL_CONNECTION_OVERRIDE"})
+        if (const char* e = getenv(v)) c->driver_lock = c->driver_lock || e[0] != 0;
     if (const char* dlk = getenv("SET_DRIVER_LOCK")) c->driver_lock = dlk[0] == '1';
     if (const char* cmb = getenv("SET_COPY_MAX_BLOCKS")) c->copy_max_blocks = (uint32_t)atoi(cmb);
     c->S = cfg.num_streams;
     c->b = ((cfg.max_inflight + c->S - 1) / c->S) * c->S;
     c->q = cfg.queue_capacity;
     c->epp = c->q + 1;
-    c->streams.resize(c->S);
-    c->notify.resize(c->S);
-    c->stream_locks.reset(new SpinLock[c->S]);
     c->own_streams = cfg.streams == nullptr;
+    // CUDA streams behind each logical stream (set.h streams_per_lane): never more than the lane has slots
+    c->L = c->own_streams ? std::max(1, std::min(cfg.streams_per_lane, c->b / c->S)) : 1;
+    c->H = c->S * c->L;
+    c->streams.resize(c->H);
+    c->notify.resize(c->H);
+    c->stream_locks.reset(new SpinLock[c->H]);
     bool ok = true;
-    for (int s = 0; s < c->S && ok; ++s) {
+    for (int s = 0; s < c->H && ok; ++s) {
         if (c->own_streams)
             ok = cudaStreamCreateWithFlags(&c->streams[s], cudaStreamNonBlocking) == cudaSuccess;
         else
@@ -1049,7 +1065,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
         c->stamp_recs.reserve(1 << 16);
     }
     if (cfg.mode == SET_MODE_SET)
-        c->sched.reset(new Scheduler(c, c->S, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
+        c->sched.reset(new Scheduler(c, c->H, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
     *out = c;
     return SET_OK;
 }
@@ -1259,7 +1275,7 @@ set_status set_destroy(set_ctx* c) {
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
     if (c->flags_host) cudaFreeHost(c->flags_host);
     if (c->ts_host) cudaFreeHost(c->ts_host);
-    for (int s = 0; s < c->S; ++s) {
+    for (int s = 0; s < c->H; ++s) {
         if (c->own_streams && c->streams[s]) cudaStreamDestroy(c->streams[s]);
         if (c->notify[s]) cudaStreamDestroy(c->notify[s]);
     }
@@ -1303,6 +1319,36 @@ void set_host_free(set_ctx* c, void* p) {
         }
 }
 
+set_status set_host_register(set_ctx* c, const void* p, size_t bytes) {
+    if (!c || !p || bytes == 0) return SET_ERR_INVALID;
+    c->bind_thread();
+    // both ends must be pinned host memory that the device addresses at the host's own address (SM copies dereference it)
+    for (const char* q : {(const char*)p, (const char*)p + bytes - 1}) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, q) != cudaSuccess) {
+            cudaGetLastError();
+            return SET_ERR_INVALID;
+        }
+        if (at.type != cudaMemoryTypeHost || at.devicePointer != (const void*)q) return SET_ERR_INVALID;
+    }
+    c->add_pinned_range(p, bytes);
+    return SET_OK;
+}
+
+set_status set_host_unregister(set_ctx* c, const void* p) {
+    if (!c || !p) return SET_ERR_INVALID;
+    set_status rc = SET_ERR_INVALID;
+    c->range_lock.lock();
+    for (size_t k = 0; k < c->pinned_ranges.size(); ++k)
+        if (c->pinned_ranges[k].lo == (uintptr_t)p) {
+            c->pinned_ranges.erase(c->pinned_ranges.begin() + (long)k);
+            rc = SET_OK;
+            break;
+        }
+    c->range_lock.unlock();
+    return rc;
+}
+
 set_status set_get_stats(set_ctx* c, set_stats* out) {
     if (!c || !out) return SET_ERR_INVALID;
     memset(out, 0, sizeof(*out));
@@ -1332,6 +1378,8 @@ set_status set_get_stats(set_ctx* c, set_stats* out) {
     out->kernel_nodes = c->kernel_nodes.load();
     out->signal_nodes = c->signal_nodes.load();
     out->copy_nodes = c->copy_nodes.load();
+    out->early_completions = c->early_completions.load();
+    out->cuda_streams = (uint64_t)c->H;
     out->ns_bind = c->ns_bind.load();
     out->ns_sync = c->ns_sync.load();
     return SET_OK;
@@ -1345,7 +1393,7 @@ set_status set_reset_stats(set_ctx* c) {
         st.ns_submit = 0; st.ns_launch = 0; st.ns_callback = 0; st.max_inflight = 0;
     }
     c->base_submitted = 0; c->base_completed = 0; c->base_launched = 0; c->base_ns_submit = 0; c->base_ns_launch = 0;
-    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->copy_nodes = 0;
+    c->full_rebinds = 0; c->host_rebinds = 0; c->staged_jobs = 0; c->kernel_nodes = 0; c->signal_nodes = 0; c->copy_nodes = 0; c->early_completions = 0;
     c->stamp_lock.lock();
     c->stamp_recs.clear();
     c->stamp_lock.unlock(); c->ns_bind = 0; c->ns_sync = 0;
@@ -1374,11 +1422,30 @@ set_status set_get_gap_stats(set_ctx* c, set_gap_stats* out) {
         if (i > 0 && v[i - 1].stream == v[i].stream)
             gaps.push_back(v[i].start > v[i - 1].end ? (double)(v[i].start - v[i - 1].end) * 1e-3 : 0.0);
     }
+    {  // |union of the jobs' intervals| over all streams: sweep in start order
+        std::vector<std::pair<uint64_t, uint64_t>> iv;
+        iv.reserve(v.size());
+        for (auto& r : v) iv.push_back({r.start, r.end});
+        std::sort(iv.begin(), iv.end());
+        uint64_t busy = 0, lo = iv[0].first, hi = iv[0].second;
+        for (size_t i = 1; i < iv.size(); ++i) {
+            if (iv[i].first > hi) {
+                busy += hi - lo;
+                lo = iv[i].first;
+                hi = iv[i].second;
+            } else if (iv[i].second > hi) {
+                hi = iv[i].second;
+            }
+        }
+        busy += hi - lo;
+        out->busy_union_us = (double)busy * 1e-3;
+    }
     out->jobs = v.size();
     out->gaps = gaps.size();
     out->job_mean_us = job_sum / (double)v.size();
     out->span_us = (double)(t1 - t0) * 1e-3;
-    out->stream_busy_frac = out->span_us > 0 ? job_sum / (out->span_us * (double)c->S) : 0.0;
+    out->stream_busy_frac = out->span_us > 0 ? job_sum / (out->span_us * (double)c->H) : 0.0;
+    out->idle_frac = out->span_us > 0 ? 1.0 - out->busy_union_us / out->span_us : 0.0;
     if (!gaps.empty()) {
         std::sort(gaps.begin(), gaps.end());
         double sum = 0;

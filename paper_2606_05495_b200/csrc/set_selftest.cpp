@@ -95,7 +95,6 @@ class SimBackend : public Backend {
         *pinned = false;
         if (exec_busy_[(size_t)exec].load() != 0) errors.fetch_add(1);  // never update an exec that is in flight
         bound_slot_[(size_t)exec] = slot;
-        bound_job_[exec % 1] = 0;
         (void)job;
         binds.fetch_add(1);
         return 0;
@@ -171,7 +170,6 @@ class SimBackend : public Backend {
     bool polled_ = false;
     std::vector<uint32_t> flags_;
     std::vector<int> bound_slot_;
-    int bound_job_[1] = {0};
     std::vector<std::atomic<int>> exec_busy_, slot_busy_, done_count_;
     std::atomic<int64_t> inflight_{0};
     std::atomic<bool> stop_{false};

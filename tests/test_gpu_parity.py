@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import inputgen
-from oracle_map import oracle_out
+from checker import compare, oracle_out
 
 pytestmark = pytest.mark.gpu
 
@@ -61,26 +61,6 @@ def run_jobs(setlib, wl, job_ids, mode=0, pageable=False, io_check=True, pdl=Fal
         return outs, ins, dims, stats
     finally:
         ctx.close()
-
-
-def compare(wl, out, ref):
-    c = wl.config
-    if c in (0, 4):
-        assert np.array_equal(out, ref)
-    elif c == 1:
-        g, r = float(out.view(np.float32)[0]), float(ref.view(np.float32)[0])
-        assert abs(g - r) <= 1e-6 * abs(r), (g, r)
-    elif c == 2:
-        g, r = out.view(np.float32).astype(np.float64), ref.view(np.float32).astype(np.float64)
-        scale = np.abs(r).max()
-        assert np.abs(g - r).max() <= 1e-6 * scale                      # reading C2-4
-        big = np.abs(r) >= 1e-3 * scale
-        assert np.all(np.abs(g - r)[big] <= 1e-6 * np.abs(r)[big])
-        assert np.array_equal(out, ref)                                  # reading C2-3: same add order -> bit-exact
-    elif c == 3:
-        g, r = inputgen.bf16_bits_to_f64(out.view(np.uint16)), inputgen.bf16_bits_to_f64(ref.view(np.uint16))
-        assert np.linalg.norm(g - r) / np.linalg.norm(r) <= 2e-2
-        assert np.abs(g - r).max() <= 0.05 * max(1.0, np.abs(r).max())  # no wild single entries either
 
 
 def check(setlib, wl, job_ids, **kw):
@@ -478,3 +458,329 @@ def test_config3_gelu_epilogue_within_one_bf16_ulp(libset):
     assert ulp[big].max() <= 1
     assert (ulp[big] == 0).mean() > 0.98
     assert np.abs(g - r)[~big].max() <= 4e-6              # one bf16 ulp just below 1e-3 is 3.8e-6
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# config 1, element by element: K3..K6 are only visible through K7's sum in the built-in pipeline, and a sum at 1e-6
+# cannot see a contracted fma(2.5, x, 0.1) (about 1 ulp per element, random sign).  Reading C1-1 says the four
+# elementwise kernels are bit-exact, so the stage list is registered truncated after K3, K4, K5, K6 in turn -- through
+# set_register_pipeline, with the y buffer copied back instead of the scalar -- and y is compared bit for bit with the
+# oracle's intermediate of the same step (oracle_config1_chain).
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [16384, 16385, 1023, 5])
+@pytest.mark.parametrize("pdl", [False, True])
+@pytest.mark.parametrize("upto", [1, 2, 3, 4])
+def test_config1_elementwise_stages_bit_exact(libset, upto, pdl, n):
+    import oracle
+    from paper_2606_05495_b200.workloads import PinnedArena
+    st, ns, bf, nb, hin, _ = libset.builtin_pipeline(1, 0, [n])
+    assert ns == 5 and nb == 3
+    for i in range(ns):
+        if pdl:
+            st[i].flags |= libset.STAGE_PDL
+    bf[1].d2h_bytes.fixed = 4 * n          # y comes back ...
+    bf[2].d2h_bytes.fixed = 0              # ... the scalar does not (K7 is not part of the truncated chain)
+    jobs = 24
+    ctx = libset.Context(4, 8)
+    try:
+        ctx.register_pipeline(st, upto, bf, nb)
+        ins = [inputgen.config1_job(1000 + j, n) for j in range(jobs)]
+        arena = PinnedArena(ctx, jobs * (hin + 4 * n + 1024) + 4096)
+        outs = []
+        for j, x in enumerate(ins):
+            a_in, v_in = arena.take(hin)
+            v_in[:] = x.view(np.uint8)
+            a_out, v_out = arena.take(4 * n)
+            v_out[:] = SENTINEL
+            outs.append(v_out)
+            ctx.submit(j, a_in, a_out)
+        ctx.drain()
+        for j, x in enumerate(ins):
+            want = oracle.config1_chain(x[:n], x[n:])[upto - 1]
+            got = np.array(outs[j], copy=True).view(np.uint32)
+            bad = np.nonzero(got != want.view(np.uint32))[0]
+            assert bad.size == 0, (f"stage {upto} (pdl={pdl}, n={n}) job {j}: {bad.size} of {n} elements differ, first at {bad[0]}: "
+                                   f"{got.view(np.float32)[bad[0]]!r} vs {want[bad[0]]!r}")
+        outs = None
+        arena.free()
+    finally:
+        ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Parity at the configs' FULL job counts, in the launch configuration bench.py times (BASELINE geometry, SM copies, PDL
+# edges): every output of every job is checked.  Jobs that share a pool input must produce identical bytes, and one
+# representative per distinct input is compared with the oracle -- which together pins every output to the oracle.
+# ---------------------------------------------------------------------------------------------------------------------
+def _full_count(libset, wl, n_jobs, npool, dims_of=None, sampled=None):
+    import ctypes as C
+    from paper_2606_05495_b200.workloads import PinnedArena
+    ctx = libset.Context(wl.num_streams, wl.max_inflight)
+    try:
+        ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=True)
+        ins = [wl.make_input(j) for j in range(npool)]
+        dims = [wl.dims(j) for j in range(npool)]
+        in_sz = [wl.in_bytes(d) for d in dims]
+        out_sz = [wl.out_bytes(dims[k % npool]) for k in range(n_jobs)]
+        arena = PinnedArena(ctx, sum(in_sz) + sum(out_sz) + 256 * (npool + n_jobs + 2))
+        in_ptr = []
+        for x, n in zip(ins, in_sz):
+            a, v = arena.take(n)
+            v[:] = x
+            in_ptr.append(a)
+        out_ptr, out_view = [], []
+        for n in out_sz:
+            a, v = arena.take(n)
+            v[:] = SENTINEL
+            out_ptr.append(a)
+            out_view.append(v)
+        pi = (C.c_void_p * n_jobs)(*[in_ptr[k % npool] for k in range(n_jobs)])
+        po = (C.c_void_p * n_jobs)(*out_ptr)
+        pd = None
+        if wl.config == 4:
+            pd = (C.c_uint32 * (4 * n_jobs))(*[v for k in range(n_jobs) for v in dims[k % npool]])
+        ctx.submit_batch(pi, po, pd)
+        ctx.drain()
+        st = ctx.stats()
+        assert st["completed"] == n_jobs and st["submitted"] == n_jobs and st["max_inflight_seen"] <= wl.max_inflight
+        for p in range(npool):
+            first = np.array(out_view[p], copy=True)
+            if sampled is None:
+                compare(wl, first, oracle_out(wl, ins[p], dims[p]))
+            else:
+                sampled(p, ins[p], first)
+            for k in range(p + npool, n_jobs, npool):     # same input -> same bytes, in its own output slot
+                assert np.array_equal(out_view[k], first), f"job {k} differs from job {p} although both ran input {p}"
+        out_view = None
+        arena.free()
+        return st
+    finally:
+        ctx.close()
+
+
+def test_full_job_count_config0(libset):
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(0)
+    _full_count(libset, wl, wl.jobs, wl.jobs)                       # 256 jobs, all distinct
+
+
+def test_full_job_count_config1(libset):
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(1)
+    _full_count(libset, wl, wl.jobs, wl.jobs)                       # 10,000 jobs, all distinct
+
+
+def test_full_job_count_config4(libset):
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(4)
+    st = _full_count(libset, wl, wl.jobs, 96)                       # 4,096 frames over 96 distinct ones (jittered sizes)
+    assert st["full_rebinds"] > 0                                   # frame sizes change from job to job on a slot
+
+
+def test_slot_reuse_config2_full_size(libset):
+    """Full-size Jacobi jobs, every slot (8) and every exec (3 per slot) reused: 40 jobs over 8 distinct grids."""
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(2)
+    _full_count(libset, wl, 40, 8)
+
+
+def test_slot_reuse_config3_full_size(libset):
+    """Full-size GEMM jobs, 48 jobs over the 8 distinct triples of the bench pool: every slot used >= 4 times.  The oracle is
+    evaluated on 2,048 sampled entries per distinct input (tile corners included); identical inputs must give identical
+    bytes."""
+    import oracle
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(3)
+    M, N, K = wl.params
+    fixed = [(0, 0), (M - 1, N - 1), (127, 255), (128, 256), (127, 256), (128, 255), (M - 1, 0), (0, N - 1), (1023, 1024), (1024, 1023)]
+
+    def sampled(p, image, out):
+        a = image[:2 * M * K].view(np.uint16).reshape(M, K)
+        b = image[2 * M * K:2 * M * K + 2 * K * N].view(np.uint16).reshape(K, N)
+        bias = image[2 * M * K + 2 * K * N:].view(np.float32)
+        r = inputgen.uniform24(4321, p, 7, 2 * 2048)
+        ms = np.concatenate([np.array([f[0] for f in fixed]), r[:2048] % M]).astype(np.int64)
+        ns = np.concatenate([np.array([f[1] for f in fixed]), r[2048:] % N]).astype(np.int64)
+        ref = inputgen.bf16_bits_to_f64(oracle.config3_sampled(a, b, bias, ms, ns))
+        got = inputgen.bf16_bits_to_f64(out.view(np.uint16).reshape(M, N)[ms, ns])
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 2e-2
+        assert np.abs(got - ref).max() <= 0.05 * max(1.0, np.abs(ref).max())
+
+    _full_count(libset, wl, 48, 8, sampled=sampled)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# round 2: PDL edge into the tcgen05 GEMM, completion fence modes with the early-completion hook, CUDA streams per lane,
+# declared pinned ranges, maximum depth
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,sm_copy", [((128, 256, 64), 0), ((384, 512, 256), 1 << 20), ((200, 264, 72), 1 << 20)])
+def test_config3_behind_a_programmatic_edge(libset, shape, sm_copy):
+    """with the whole [A][B][bias] image at or below sm_copy_max_bytes the GEMM's only predecessor is an SM copy
+    node and SET_STAGE_PDL makes the edge programmatic: the kernel must not issue a TMA load or read bias before
+    griddepcontrol.wait.  64 jobs over 4 slots so that every slot's buffers are overwritten while the next GEMM's prologue
+    is already running."""
+    from paper_2606_05495_b200.workloads import Workload
+    st = check(libset, Workload(3, shape, jobs=64, num_streams=2, max_inflight=4), list(range(64)), pdl=True, sm_copy_max_bytes=sm_copy)
+    assert st["copy_nodes"] >= 64          # the copy-in really was a kernel node
+
+
+@pytest.mark.parametrize("fence", [1, 2])
+@pytest.mark.parametrize("lanes", [1, 4])
+def test_no_completion_is_seen_before_its_output(libset, fence, lanes):
+    """set_config.debug_sentinel: inside Algorithm 3, at the moment the dispatcher sees a job's completion word and before
+    the slot is released, the library itself looks at the first and last word of the job's sentinel-filled output.
+    30,000 config-0 jobs (16,640-byte outputs written by an SM copy node) and 30,000 config-1 jobs per repetition at the
+    bench geometry; SET_SOAK_REPS raises the count for a soak run (profiles/r2_signal_soak.md)."""
+    import ctypes as C
+    import os
+    from paper_2606_05495_b200.workloads import PinnedArena, baseline_workload
+    reps = int(os.environ.get("SET_SOAK_REPS", "2"))
+    for config in (1, 0):
+        wl = baseline_workload(config)
+        n, npool = 30000, 64
+        ctx = libset.Context(8, 32, completion_fence=fence, streams_per_lane=lanes, debug_sentinel=0xA5A5A5A5)
+        try:
+            ctx.register_builtin(config, 0, list(wl.params), pdl=True)
+            ins = [wl.make_input(j) for j in range(npool)]
+            want = [oracle_out(wl, x, (1, 1, 1, 1)) for x in ins]
+            ob = wl.out_bytes()
+            arena = PinnedArena(ctx, npool * (wl.in_bytes() + 256) + (ob + 0) * n + 4096)
+            in_ptrs = []
+            for x in ins:
+                a, v = arena.take(wl.in_bytes())
+                v[:] = x
+                in_ptrs.append(a)
+            a_out, v_out = arena.take(ob * n, align=256)
+            pi = (C.c_void_p * n)(*[in_ptrs[k % npool] for k in range(n)])
+            po = (C.c_void_p * n)(*[a_out + ob * k for k in range(n)])
+            for rep in range(reps):
+                v_out[:] = SENTINEL
+                ctx.submit_batch(pi, po)
+                ctx.drain()
+                st = ctx.stats()
+                assert st["early_completions"] == 0, f"config {config} fence {fence} lanes {lanes} rep {rep}: {st['early_completions']} completions overtook their output"
+                got = np.array(v_out, copy=True).reshape(n, ob)
+                for p_ in range(npool):
+                    rows = got[p_::npool]
+                    if config == 1:
+                        g, r = rows.view(np.float32)[:, 0], want[p_].view(np.float32)[0]
+                        assert np.all(np.abs(g - r) <= 1e-6 * abs(r))
+                    else:
+                        assert np.all(rows == want[p_][None, :])
+            assert ctx.stats()["completed"] == n * reps
+            v_out = None
+            arena.free()
+        finally:
+            ctx.close()
+
+
+def test_pageable_staging_at_full_rate(libset):
+    """The one path that reads a job's output the moment its completion is seen: the staged D2H memcpy from the exec's pinned
+    block into the caller's pageable buffer (set_ctx::finish).  6,000 config-0 jobs with pageable buffers, every output checked."""
+    from paper_2606_05495_b200.workloads import baseline_workload
+    wl = baseline_workload(0)
+    n, npool = 6000, 32
+    ctx = libset.Context(8, 32)
+    try:
+        ctx.register_builtin(0, 0, list(wl.params), pdl=True)
+        ins = [np.array(wl.make_input(j), copy=True) for j in range(npool)]
+        want = [oracle_out(wl, x, (1, 1, 1, 1)) for x in ins]
+        outs = np.full((n, wl.out_bytes()), SENTINEL, np.uint8)
+        for k in range(n):
+            ctx.submit(k, ins[k % npool].ctypes.data, outs[k].ctypes.data)
+        ctx.drain()
+        st = ctx.stats()
+        assert st["staged_jobs"] == n and st["completed"] == n
+        for p_ in range(npool):
+            assert np.all(outs[p_::npool] == want[p_][None, :])
+    finally:
+        ctx.close()
+
+
+@pytest.mark.parametrize("config", [0, 1, 4])
+@pytest.mark.parametrize("lanes", [1, 2, 4, 8])
+@pytest.mark.parametrize("mode", [0, 2, 4])
+def test_streams_per_lane_compute_the_same(libset, config, lanes, mode):
+    """set_config.streams_per_lane: consecutive jobs of a logical stream run on different CUDA streams; results, slot
+    safety and the in-flight bound are unchanged, in SET and in the baseline models that share the streams."""
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(config)
+    st = check(libset, wl, list(range(min(wl.jobs, 64))), mode=mode, streams_per_lane=lanes, pdl=True)
+    depth = wl.max_inflight // wl.num_streams
+    assert st["cuda_streams"] == wl.num_streams * min(lanes, depth)
+    assert st["max_inflight_seen"] <= wl.max_inflight
+
+
+def test_declared_pinned_ranges(libset):
+    """set_host_register / set_host_unregister: a torch pinned tensor declared once is used in place; pageable memory and
+    device memory are refused; after unregistering, the pointer is queried per job again (still pinned, still in place)."""
+    import torch
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(0)
+    ctx = libset.Context(wl.num_streams, wl.max_inflight)
+    try:
+        ctx.register_builtin(0)
+        n = 16
+        t_in = torch.empty(n * wl.in_bytes(), dtype=torch.uint8).pin_memory()
+        t_out = torch.full((n * wl.out_bytes(),), SENTINEL, dtype=torch.uint8).pin_memory()
+        ins = [wl.make_input(j) for j in range(n)]
+        for j, x in enumerate(ins):
+            t_in[j * wl.in_bytes():(j + 1) * wl.in_bytes()] = torch.from_numpy(np.array(x, copy=True))
+        ctx.host_register(t_in.data_ptr(), t_in.numel())
+        ctx.host_register(t_out.data_ptr(), t_out.numel())
+        with pytest.raises(libset.SetError):
+            ctx.host_register(np.zeros(4096, np.uint8).ctypes.data, 4096)            # pageable
+        with pytest.raises(libset.SetError):
+            ctx.host_register(torch.zeros(4096, dtype=torch.uint8, device="cuda").data_ptr(), 4096)
+        for rnd in range(2):
+            for j in range(n):
+                ctx.submit(j, t_in.data_ptr() + j * wl.in_bytes(), t_out.data_ptr() + j * wl.out_bytes())
+            ctx.drain()
+            out = t_out.numpy()
+            for j in range(n):
+                compare(wl, np.array(out[j * wl.out_bytes():(j + 1) * wl.out_bytes()], copy=True), oracle_out(wl, ins[j], (1, 1, 1, 1)))
+            if rnd == 0:
+                ctx.host_unregister(t_in.data_ptr())
+                ctx.host_unregister(t_out.data_ptr())
+                with pytest.raises(libset.SetError):
+                    ctx.host_unregister(t_out.data_ptr())
+                t_out.fill_(SENTINEL)
+        assert ctx.stats()["staged_jobs"] == 0
+    finally:
+        ctx.close()
+
+
+def test_maximum_depth_4096_in_flight(libset):
+    """PAPER.md:276 sweeps the batch size to b = 4096: max_inflight = 4096 registers (4096 slots x 2 execs), runs 8,192
+    config-1 jobs and every result is the oracle's."""
+    import ctypes as C
+    from paper_2606_05495_b200.workloads import PinnedArena, Workload
+    wl = Workload(1, (4096,), jobs=8192, num_streams=8, max_inflight=4096)
+    n, npool = 8192, 256
+    ctx = libset.Context(8, 4096, queue_capacity=1)
+    try:
+        ctx.register_builtin(1, 0, list(wl.params), pdl=True)
+        assert ctx.geometry() == (4096, 8, 2)
+        ins = [wl.make_input(j) for j in range(npool)]
+        want = np.array([oracle_out(wl, x, (1, 1, 1, 1)).view(np.float32)[0] for x in ins], np.float32)
+        arena = PinnedArena(ctx, npool * (wl.in_bytes() + 256) + 4 * n + 4096)
+        in_ptrs = []
+        for x in ins:
+            a, v = arena.take(wl.in_bytes())
+            v[:] = x
+            in_ptrs.append(a)
+        a_out, v_out = arena.take(4 * n)
+        v_out[:] = SENTINEL
+        pi = (C.c_void_p * n)(*[in_ptrs[k % npool] for k in range(n)])
+        po = (C.c_void_p * n)(*[a_out + 4 * k for k in range(n)])
+        ctx.submit_batch(pi, po)
+        ctx.drain()
+        st = ctx.stats()
+        assert st["completed"] == n and st["max_inflight_seen"] <= 4096
+        got = np.array(v_out.view(np.float32), copy=True)
+        ref = want[np.arange(n) % npool]
+        assert np.all(np.abs(got - ref) <= 1e-6 * np.abs(ref))
+        v_out = None
+        arena.free()
+    finally:
+        ctx.close()

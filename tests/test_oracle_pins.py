@@ -123,6 +123,30 @@ def test_c1_each_step_is_one_fp32_rounding():
     assert np.count_nonzero(fused != t1) > 100
 
 
+def test_c1_chain_intermediates_each_one_rounding():
+    """oracle_config1_chain (what K3..K6 are compared with element by element): every intermediate against the
+    single-rounding route through double, and t4 against oracle_config1's own t4."""
+    for job in (3, 11):
+        j = inputgen.config1_job(job)
+        x, b = j[:16384], j[16384:]
+        t1, t2, t3, t4 = oracle.config1_chain(x, b)
+        xd, bd = x.astype(np.float64), b.astype(np.float64)
+        m = (2.5 * xd).astype(np.float32)
+        r1 = (m.astype(np.float64) + float(np.float32(0.1))).astype(np.float32)
+        r2 = (r1.astype(np.float64) + bd).astype(np.float32)
+        r3 = np.where(r2 > 0, r2, np.float32(0)).astype(np.float32)
+        r4 = (r3.astype(np.float64) * r3.astype(np.float64)).astype(np.float32)
+        assert np.array_equal(t1, r1) and np.array_equal(t2, r2) and np.array_equal(t3, r3) and np.array_equal(t4, r4)
+        assert np.array_equal(t4, oracle.config1(x, b, want_t4=True)[1])
+        assert (t3 >= 0).all() and np.count_nonzero(t3 == 0) > 1000 and np.count_nonzero(t2 < 0) == np.count_nonzero(t3 == 0) - np.count_nonzero(t2 == 0)
+        # a contracted fma(2.5, x, 0.1) would differ from t1 in many elements (reading C1-1)
+        fused = (2.5 * xd + float(np.float32(0.1))).astype(np.float32)
+        assert np.count_nonzero(fused != t1) > 100
+    # tiny hand case: x = 0.5, bias = -2 -> t1 = fl(1.25 + 0.1f), t2 < 0, t3 = 0, t4 = 0
+    t1, t2, t3, t4 = oracle.config1_chain(np.array([0.5], np.float32), np.array([-2.0], np.float32))
+    assert float(t1[0]) == float(np.float32(1.25) + np.float32(0.1)) and t2[0] < 0 and t3[0] == 0 and t4[0] == 0
+
+
 def test_c1_sum_in_double_vs_independent_double_chain():
     for job in (0, 1, 2):
         j = inputgen.config1_job(job)
