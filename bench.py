@@ -497,7 +497,7 @@ def oracle_pass(wl, images, dims_list, budget_s: float):
     return done, time.perf_counter() - t0
 
 
-def cpu_baseline(wl, job_ids, budget_s=12.0, passes=10, all_cores_s=4.0):
+def cpu_baseline(wl, job_ids, budget_s=12.0, passes=100000, all_cores_s=4.0):
     """The oracle, as it stands, timed on this box's host cores over a bounded sample of the workload's jobs."""
     cap = {0: 256, 1: 2048, 2: 2, 3: 1, 4: 24}[wl.config]      # distinct inputs prepared for the sample
     n = min(len(job_ids), cap)

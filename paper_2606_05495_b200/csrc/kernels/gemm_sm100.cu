@@ -1,32 +1,42 @@
 // gemm_sm100.cu -- K9: C = bf16( GELU( A.B + bias ) ), bf16 operands, fp32 accumulation on the 5th-generation tensor
-// cores (BASELINE.json:configs[3]; readings C3-1..C3-4).  Hand-written for sm_100a: TMA
-// (cp.async.bulk.tensor) stages 128-byte-swizzled operand tiles in shared memory, one elected thread issues
-// tcgen05.mma with the accumulator in tensor memory (TMEM), eight epilogue warps read it back with tcgen05.ld and
-// apply bias + erf-GELU + round-to-nearest-even bf16 and store the tile through TMA.
+// cores (BASELINE.json:configs[3]; readings C3-1..C3-4).  Hand-written for sm_100a: a CTA PAIR (cluster of two
+// CTAs on the two SMs of a TPC) computes one 256 x 256 tile with tcgen05.mma.cta_group::2; TMA (cp.async.bulk.tensor)
+// stages 128-byte-swizzled operand tiles in shared memory, the pair's leader issues the MMAs with the accumulator in
+// tensor memory (TMEM) of both SMs, and eight epilogue warps per CTA read it back with tcgen05.ld, apply bias + erf-GELU +
+// round-to-nearest-even bf16 and store the tile through TMA.
 //
-//   A : bf16 [M][K] row-major  -> K-major operand,  TMA box 64 (K) x 128 (M) = 16 KiB per stage
-//   B : bf16 [K][N] row-major  -> MN-major operand (no host transpose), 4 TMA boxes 64 (N) x 64 (K) = 32 KiB per stage
-//   D : fp32 128 x 256 accumulator = 256 TMEM columns x 128 lanes; one tile per CTA, grid = (N/256, M/128)
+//   A : bf16 [M][K] row-major  -> K-major operand.  CTA r of the pair loads rows m0 + 128 r .. + 127: box 64 (K) x 128 (M) = 16 KiB
+//   B : bf16 [K][N] row-major  -> MN-major operand (no host transpose).  CTA r loads columns n0 + 128 r .. + 127 as two
+//       boxes 64 (N) x 64 (K) = 16 KiB: each SM stages HALF of B and the tensor cores read the other half from the peer's
+//       shared memory, so a 256 x 256 tile costs 64 KiB of L2 -> SM traffic per 64-deep k-block instead of the 96 KiB of
+//       two independent 128 x 256 tiles.  The one-CTA version of this kernel (round 1) moved 192 MB from L2 for 2048^3,
+//       30,000 cycles at the ~6,300 B/cycle the L2 delivers chip-wide against 16,400 cycles of MMA: it was L2-bound.
+//   D : fp32, rows 128 r .. 128 r + 127 of the pair's tile x 256 columns = 256 TMEM columns x 128 lanes in CTA r
 //
-// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..9 = epilogue
-// (warp w may only touch TMEM lanes 32*(w%4) .. 32*(w%4)+31; two warps share each lane quarter and split the 256
-// columns).  The epilogue writes bf16 rows into 128-byte-swizzled shared memory and hands each 32 x 64 piece to the
-// TMA unit (cp.async.bulk.tensor store): C leaves the SM as full 128-byte lines instead of 16 bytes per row.
+// Grid = (2 * ceil(M / 256), ceil(N / 256)), cluster (2, 1, 1): blockIdx.x >> 1 is the pair's row block, %cluster_ctarank
+// the CTA's rank r.  Warp roles (320 threads): warp 0 = TMA producer (both CTAs, each for its own halves, all signalling the
+// LEADER's "full" barrier), warp 1 = TMEM allocator (both CTAs) + MMA issuer (leader only; tcgen05.commit multicasts the
+// "stage empty" / "accumulator full" arrivals to both CTAs), warps 2..9 = epilogue (warp w may only touch TMEM lanes
+// 32*(w%4) .. 32*(w%4)+31; two warps share each lane quarter and split the 256 columns).  The epilogue writes bf16 rows into
+// 128-byte-swizzled shared memory and hands each 32 x 64 piece to the TMA unit (cp.async.bulk.tensor store).
 // Ragged shapes: TMA zero-fills out-of-bounds rows/columns of a load box, so partial tiles in M, N and K contribute
-// zeros, and clips a store box to the matrix (N and K must be multiples of 8: 16-byte TMA pitches).
+// zeros, and clips a store box to the matrix (N and K must be multiples of 8: 16-byte TMA pitches); a box that starts
+// outside the matrix is never requested (its accumulator rows / columns are never stored).
 #include <cuda_bf16.h>
 
 #include "kernels.h"
 
 namespace {
 
-constexpr uint32_t kBlockM = 128, kBlockN = 256, kBlockK = 64, kUmmaK = 16;
-constexpr uint32_t kStages = 4;
+constexpr uint32_t kBlockM = 128, kBlockN = 256, kBlockK = 64, kUmmaK = 16;  // per CTA: 128 rows of the pair's 256 x 256 tile
+constexpr uint32_t kPairM = 2 * kBlockM, kHalfN = kBlockN / 2;
+constexpr uint32_t kStages = 6;
 constexpr uint32_t kABytes = kBlockM * kBlockK * 2;          // 16 KiB
 constexpr uint32_t kBBoxN = 64;                              // one 128-byte swizzle atom of N per box
 constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
-constexpr uint32_t kBBytes = kBBoxBytes * (kBlockN / kBBoxN);  // 32 KiB
-constexpr uint32_t kStageBytes = kABytes + kBBytes;          // 48 KiB
+constexpr uint32_t kBBoxes = kHalfN / kBBoxN;                // 2 boxes: this CTA's half of B
+constexpr uint32_t kBBytes = kBBoxBytes * kBBoxes;           // 16 KiB
+constexpr uint32_t kStageBytes = kABytes + kBBytes;          // 32 KiB
 constexpr uint32_t kCBoxBytes = 64 * 32 * 2;                 // epilogue staging: one TMA store box, 64 columns x 32 rows of bf16
 static_assert(16 * kCBoxBytes <= kStages * kStageBytes, "the epilogue stages its 16 boxes in the idle operand ring");
 constexpr uint32_t kTmemCols = 256;
@@ -51,10 +61,29 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "DONE_%=:\n\t}" ::"r"(bar), "r"(parity)
         : "memory");
 }
+// TMA load into THIS CTA's shared memory whose completion bytes are counted on `bar`, a shared::cluster address that may
+// belong to the other CTA of the pair (the leader's "full" barrier)
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int32_t c_inner, int32_t c_outer) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+    asm volatile("cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
                  "l"(tm), "r"(bar), "r"(c_inner), "r"(c_outer)
                  : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
@@ -80,20 +109,24 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
     return d;
 }
 
-// Instruction descriptor, kind::f16: D fp32, A and B bf16, A K-major, B MN-major, N >> 3, M >> 4.
-constexpr uint32_t kInstrDesc = (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((kBlockN >> 3) << 17) | ((kBlockM >> 4) << 24);
+// Instruction descriptor, kind::f16: D fp32, A and B bf16, A K-major, B MN-major, N >> 3, M >> 4 -- the shape is the
+// PAIR's: M = 256 (128 rows per CTA), N = 256 (128 columns of B staged per CTA).
+constexpr uint32_t kInstrDesc = (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((kBlockN >> 3) << 17) | ((kPairM >> 4) << 24);
 
 __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
         "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate)
         : "memory");
 }
-// Arrives on the mbarrier once every tcgen05.mma issued so far by this thread has completed.
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+// Arrives on the mbarrier at this shared-memory offset in BOTH CTAs of the pair once every tcgen05.mma issued so far by
+// this thread has completed.
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+    const uint16_t both = 3;
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar), "h"(both)
+                 : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
@@ -130,13 +163,16 @@ __device__ __forceinline__ float gelu_erf(float z) {
 
 extern "C" uint32_t set_gemm_smem_bytes(void) { return kSmemBytes; }
 
-extern "C" __global__ void __launch_bounds__(320, 1)
+extern "C" __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                           const __grid_constant__ CUtensorMap tmC, const float* __restrict__ bias, uint32_t M, uint32_t N, uint32_t K) {
     extern __shared__ uint8_t smem_raw[];
+    // Both CTAs of the pair must carve shared memory identically: the MMA reads the peer's operand tiles at the leader's
+    // offsets and tcgen05.commit signals the peer's barriers at the leader's offsets.  The dynamic shared memory base is
+    // the same in every CTA of a launch, so the same rounding gives the same offsets.
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // 128-byte swizzle atoms repeat every 1024 B
     const uint32_t bars = base + kStages * kStageBytes;
-    // barrier block: full[kStages], empty[kStages], accum_full, then the TMEM base address written by tcgen05.alloc
+    // barrier block: full[kStages] (used in the leader only), empty[kStages], accum_full, then the TMEM base address
     auto full_bar = [&](uint32_t s) { return bars + 8u * s; };
     auto empty_bar = [&](uint32_t s) { return bars + 8u * (kStages + s); };
     const uint32_t accum_bar = bars + 8u * (2 * kStages);
@@ -145,30 +181,39 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     auto b_tile = [&](uint32_t s) { return base + s * kStageBytes + kABytes; };
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t m0 = blockIdx.y * kBlockM, n0 = blockIdx.x * kBlockN;
+    const uint32_t rank = cluster_ctarank();             // 0 = leader of the pair
+    const uint32_t mp0 = (blockIdx.x >> 1) * kPairM;     // first row of the pair's tile
+    const uint32_t m0 = mp0 + rank * kBlockM;            // first row of THIS CTA's half
+    const uint32_t n0 = blockIdx.y * kBlockN;            // first column of the pair's tile
     const uint32_t num_kb = (K + kBlockK - 1) / kBlockK;
-    // B boxes of this tile that start inside the matrix (a box that starts at or beyond N is never requested; the
-    // accumulator columns it would feed are never stored)
-    const uint32_t n_boxes = min((N - n0 + kBBoxN - 1) / kBBoxN, kBlockN / kBBoxN);
-    const uint32_t stage_tx = kABytes + n_boxes * kBBoxBytes;
+    // What CTA r stages per k-block: its A box if its rows start inside the matrix, and the B boxes of its column half that
+    // start inside the matrix.  The leader expects the bytes of both CTAs on its "full" barrier.
+    auto a_valid = [&](uint32_t r) { return mp0 + r * kBlockM < M; };
+    auto b_boxes = [&](uint32_t r) {
+        const uint32_t nb = n0 + r * kHalfN;
+        return nb >= N ? 0u : min((N - nb + kBBoxN - 1) / kBBoxN, kBBoxes);
+    };
+    const bool my_a = a_valid(rank);
+    const uint32_t my_boxes = b_boxes(rank);
+    const uint32_t pair_tx = (a_valid(0) ? kABytes : 0u) + (a_valid(1) ? kABytes : 0u) + (b_boxes(0) + b_boxes(1)) * kBBoxBytes;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         for (uint32_t s = 0; s < kStages; ++s) {
-            mbar_init(full_bar(s), 1);
+            mbar_init(full_bar(s), 2);  // the leader's arrive.expect_tx and the peer's remote arrive
             mbar_init(empty_bar(s), 1);
         }
         mbar_init(accum_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {  // TMEM: 256 columns for the 128 x 256 fp32 accumulator
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (warp == 1) {  // TMEM: 256 columns in each CTA for its 128 x 256 fp32 half of the accumulator
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
+    cluster_sync_all();  // barriers initialised and TMEM allocated in BOTH CTAs before anyone signals or issues
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
@@ -178,20 +223,24 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     set_pdl_sync();
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer: every CTA stages its own halves; all bytes are counted on the leader's barrier =====
         if (elect_one()) {
             for (uint32_t kb = 0; kb < num_kb; ++kb) {
                 const uint32_t s = kb % kStages, round = kb / kStages;
                 mbar_wait(empty_bar(s), (round & 1u) ^ 1u);  // first pass over the ring falls through
-                mbar_expect_tx(full_bar(s), stage_tx);
-                tma_load_2d(a_tile(s), &tmA, full_bar(s), (int32_t)(kb * kBlockK), (int32_t)m0);
-                for (uint32_t j = 0; j < n_boxes; ++j)
-                    tma_load_2d(b_tile(s) + j * kBBoxBytes, &tmB, full_bar(s), (int32_t)(n0 + j * kBBoxN), (int32_t)(kb * kBlockK));
+                const uint32_t lead_full = map_to_cta(full_bar(s), 0);
+                if (rank == 0)
+                    mbar_expect_tx(full_bar(s), pair_tx);
+                else
+                    mbar_arrive_cluster(lead_full);
+                if (my_a) tma_load_2d(a_tile(s), &tmA, lead_full, (int32_t)(kb * kBlockK), (int32_t)m0);
+                for (uint32_t j = 0; j < my_boxes; ++j)
+                    tma_load_2d(b_tile(s) + j * kBBoxBytes, &tmB, lead_full, (int32_t)(n0 + rank * kHalfN + j * kBBoxN), (int32_t)(kb * kBlockK));
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer: one thread drives the tensor core for the whole CTA =====
-        if (elect_one()) {
+        // ===== MMA issuer: one thread of the LEADER drives the tensor cores of both SMs =====
+        if (rank == 0 && elect_one()) {
             for (uint32_t kb = 0; kb < num_kb; ++kb) {
                 const uint32_t s = kb % kStages, round = kb / kStages;
                 mbar_wait(full_bar(s), round & 1u);
@@ -200,19 +249,19 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 for (uint32_t k = 0; k < kBlockK / kUmmaK; ++k) {
                     // A: 16 K-elements = 32 bytes further along the swizzled 128-byte row
                     const uint64_t adesc = smem_desc(a_tile(s) + k * kUmmaK * 2u, 16u, 1024u);
-                    // B: 16 K-rows = two 8-row groups = 2048 bytes further
+                    // B: 16 K-rows = two 8-row groups = 2048 bytes further; the next 64 columns are one box on
                     const uint64_t bdesc = smem_desc(b_tile(s) + k * kUmmaK * 128u, kBBoxBytes, 1024u);
                     umma_bf16(tmem_base, adesc, bdesc, (kb | k) != 0u);
                 }
-                umma_commit(empty_bar(s));  // the stage may be refilled once these MMAs have read it
+                umma_commit_pair(empty_bar(s));  // both CTAs may refill the stage once these MMAs have read it
             }
-            umma_commit(accum_bar);  // accumulator complete
+            umma_commit_pair(accum_bar);  // accumulator complete in both CTAs
         }
     } else {
         // ===== epilogue: TMEM -> registers -> bias + GELU -> bf16 -> swizzled smem -> TMA store =====
         // Eight warps: warp w reads TMEM lane quarter q = w % 4 (the only lanes it may touch) and column half
         // h = (w - 2) / 4, i.e. a 32-row x 128-column piece of the tile = two 64-column TMA boxes of 4 KiB.  The
-        // operand ring is idle once accum_bar has fired (every MMA has read it), so the boxes are staged there.
+        // operand ring is idle once accum_bar has fired (every MMA has read it, in both CTAs), so the boxes are staged there.
         mbar_wait(accum_bar, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t q = warp & 3u, h = (warp - 2u) >> 2;
@@ -220,7 +269,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
 #pragma unroll 1
         for (uint32_t j = 0; j < 2; ++j) {  // one 64-column box per round
             const uint32_t c0 = h * 128u + j * 64u;
-            if (n0 + c0 >= N) break;  // warp-uniform: nothing of this box lies inside the matrix
+            if (n0 + c0 >= N || m0 + q * 32u >= M) break;  // warp-uniform: nothing of this box lies inside the matrix
             uint32_t v[64];
             tmem_ld32(tmem_base + ((q * 32u) << 16) + c0, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
             tmem_ld32(tmem_base + ((q * 32u) << 16) + c0 + 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
@@ -251,7 +300,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
             __syncwarp();
-            if (lane == 0 && m0 + q * 32u < M) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
+            if (lane == 0) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
                 asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(&tmC),
                              "r"(stage0 + j * kCBoxBytes), "r"((int32_t)(n0 + c0)), "r"((int32_t)(m0 + q * 32u))
                              : "memory");
@@ -261,9 +310,10 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // stores done before smem goes away
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
-    __syncthreads();
+    // Neither CTA may leave (or free its TMEM) while the other still uses the pair's resources.
+    cluster_sync_all();
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
 }

@@ -178,7 +178,8 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             nb = 2;
             // A: row-major MxK, box = 64 K-elements (128 B) x 128 rows.  B: row-major KxN, box = 64 N-elements x 64 K-rows.
             // C: row-major MxN, store box = 64 N-elements x 32 rows (one epilogue warp's piece).
-            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed((N + 255) / 256), grid_fixed((M + 127) / 128), 320, 1, set_gemm_smem_bytes(),
+            // grid: CTA pairs (cluster 2 x 1 x 1) along x, one pair per 256 x 256 tile -- gemm_sm100.cu
+            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed(2 * ((M + 255) / 256)), grid_fixed((N + 255) / 256), 320, 1, set_gemm_smem_bytes(),
                              {arg_tmap(0, 0, 2, K, M, 64, 128), arg_tmap(0, a_bytes, 2, N, K, 64, 64), arg_tmap(1, 0, 2, N, M, 64, 32),
                               arg_buf(0, fixed(a_bytes + b_bytes)), arg_u32(M), arg_u32(N), arg_u32(K)});
             break;
