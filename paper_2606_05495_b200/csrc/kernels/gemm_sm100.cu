@@ -30,7 +30,10 @@ namespace {
 
 constexpr uint32_t kBlockM = 128, kBlockN = 256, kBlockK = 64, kUmmaK = 16;  // per CTA: 128 rows of the pair's 256 x 256 tile
 constexpr uint32_t kPairM = 2 * kBlockM, kHalfN = kBlockN / 2;
-constexpr uint32_t kStages = 6;
+#ifndef PROBE_STAGES
+#define PROBE_STAGES 6
+#endif
+constexpr uint32_t kStages = PROBE_STAGES;
 constexpr uint32_t kABytes = kBlockM * kBlockK * 2;          // 16 KiB
 constexpr uint32_t kBBoxN = 64;                              // one 128-byte swizzle atom of N per box
 constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
@@ -41,7 +44,8 @@ constexpr uint32_t kCBoxBytes = 64 * 32 * 2;                 // epilogue staging
 static_assert(16 * kCBoxBytes <= kStages * kStageBytes, "the epilogue stages its 16 boxes in the idle operand ring");
 constexpr uint32_t kTmemCols = 256;
 constexpr uint32_t kBarrierBytes = 256;
-constexpr uint32_t kSmemBytes = kStages * kStageBytes + kBarrierBytes + 1024;  // + slack for 1024-byte alignment
+constexpr uint32_t kBiasBytes = kBlockN * 4;  // the tile's 256 bias values, staged by the epilogue warps while the main loop runs
+constexpr uint32_t kSmemBytes = kStages * kStageBytes + kBarrierBytes + kBiasBytes + 1024;  // + slack for 1024-byte alignment
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -80,7 +84,10 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t addr, uint32_t rank) {
     return r;
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+    // no .release.cluster: a cluster-scope release drains the thread's outstanding TMA loads first (measured: the non-leader's
+    // ring then runs one stage at a time, 0.65 us per k-block whatever its depth).  The data itself is published by the TMA
+    // unit's complete_tx on the same barrier; this arrival only balances the barrier's count.
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -141,22 +148,34 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         : "memory");
 }
 
-// GELU, erf form (reading C3-3): 0.5 z (1 + erf(z / sqrt 2)), evaluated in fp32.  The epilogue is issue-bound (32,768
-// elements per CTA through four schedulers), so erf is one branch-free expression instead of erff()'s two diverging
-// paths: erfc(|x|) = (a1 t + ... + a5 t^5) exp(-x^2), t = 1 / (1 + p |x|)  (Abramowitz & Stegun 7.1.26, |error| <=
-// 1.5e-7 absolute -- more than three orders below the bf16 rounding of the output), and 1 + erf(x) = erfc(|x|) for
-// x < 0, 2 - erfc(|x|) otherwise, which also avoids the cancellation of 1 + erf(x) on the negative side.
-__device__ __forceinline__ float gelu_erf(float z) {
-    const float x = z * 0.70710678118654752440f;
-    const float ax = fabsf(x);
-    const float t = __fdividef(1.0f, fmaf(0.3275911f, ax, 1.0f));
-    float p = fmaf(1.061405429f, t, -1.453152027f);
-    p = fmaf(p, t, 1.421413741f);
-    p = fmaf(p, t, -0.284496736f);
-    p = fmaf(p, t, 0.254829592f);
-    const float w = p * t * __expf(-ax * ax);  // erfc(|x|)
-    const float one_plus_erf = x < 0.0f ? w : 2.0f - w;
-    return 0.5f * z * one_plus_erf;
+// GELU, erf form (reading C3-3): 0.5 z (1 + erf(z / sqrt 2)), evaluated in fp32, TWO elements per call.  The epilogue is
+// issue-bound (32,768 elements per CTA through four schedulers; the scalar version compiled to ~30 instructions per
+// element and took 6 us of the kernel's 17), so (1) erf is one branch-free expression instead of erff()'s two diverging
+// paths: erfc(|x|) = (a1 t + ... + a5 t^5) exp(-x^2), t = 1 / (1 + p |x|)  (Abramowitz & Stegun 7.1.26, |error| <= 1.5e-7
+// absolute -- more than three orders below the bf16 rounding of the output), with 1 + erf(x) = erfc(|x|) for x < 0 and
+// 2 - erfc(|x|) otherwise, which also avoids the cancellation of 1 + erf(x) on the negative side; and (2) every multiply
+// and add is a packed f32x2 instruction (sm_100 FFMA2 / FMUL2 / FADD2: two fp32 lanes per issue slot).  The 0.5 is
+// folded into the polynomial's coefficients.  Per pair: 13 packed FP, 4 MUFU, 2 LOP, 2 SEL, 1 bf16x2 convert.
+__device__ __forceinline__ float2 gelu_erf2(float2 z) {
+    const float2 x = __fmul2_rn(z, make_float2(0.70710678118654752440f, 0.70710678118654752440f));
+    const float2 ax = make_float2(fabsf(x.x), fabsf(x.y));
+    const float2 d = __ffma2_rn(make_float2(0.3275911f, 0.3275911f), ax, make_float2(1.0f, 1.0f));
+    float2 t;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(d.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(d.y));
+    float2 p = __ffma2_rn(make_float2(0.5f * 1.061405429f, 0.5f * 1.061405429f), t, make_float2(0.5f * -1.453152027f, 0.5f * -1.453152027f));
+    p = __ffma2_rn(p, t, make_float2(0.5f * 1.421413741f, 0.5f * 1.421413741f));
+    p = __ffma2_rn(p, t, make_float2(0.5f * -0.284496736f, 0.5f * -0.284496736f));
+    p = __ffma2_rn(p, t, make_float2(0.5f * 0.254829592f, 0.5f * 0.254829592f));
+    // exp(-x^2) = 2^(-x^2 log2 e)
+    const float2 u = __fmul2_rn(__fmul2_rn(ax, ax), make_float2(-1.4426950408889634f, -1.4426950408889634f));
+    float2 e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.x) : "f"(u.x));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.y) : "f"(u.y));
+    const float2 w = __fmul2_rn(__fmul2_rn(p, t), e);                          // erfc(|x|) / 2
+    const float2 c = __fadd2_rn(make_float2(1.0f, 1.0f), make_float2(-w.x, -w.y));  // 1 - erfc(|x|) / 2
+    const float2 phi = make_float2(x.x < 0.0f ? w.x : c.x, x.y < 0.0f ? w.y : c.y);  // (1 + erf(x)) / 2
+    return __fmul2_rn(z, phi);
 }
 
 }  // namespace
@@ -177,6 +196,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     auto empty_bar = [&](uint32_t s) { return bars + 8u * (kStages + s); };
     const uint32_t accum_bar = bars + 8u * (2 * kStages);
     const uint32_t tmem_slot = bars + 8u * (2 * kStages + 1);
+    const uint32_t bias_tile = bars + kBarrierBytes;  // float[256]
     auto a_tile = [&](uint32_t s) { return base + s * kStageBytes; };
     auto b_tile = [&](uint32_t s) { return base + s * kStageBytes + kABytes; };
 
@@ -229,6 +249,10 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 const uint32_t s = kb % kStages, round = kb / kStages;
                 mbar_wait(empty_bar(s), (round & 1u) ^ 1u);  // first pass over the ring falls through
                 const uint32_t lead_full = map_to_cta(full_bar(s), 0);
+#ifdef PROBE_SKIP_TMA
+                if (rank == 0) mbar_expect_tx(full_bar(s), 0); else mbar_arrive_cluster(lead_full);
+                continue;
+#endif
                 if (rank == 0)
                     mbar_expect_tx(full_bar(s), pair_tx);
                 else
@@ -251,7 +275,11 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                     const uint64_t adesc = smem_desc(a_tile(s) + k * kUmmaK * 2u, 16u, 1024u);
                     // B: 16 K-rows = two 8-row groups = 2048 bytes further; the next 64 columns are one box on
                     const uint64_t bdesc = smem_desc(b_tile(s) + k * kUmmaK * 128u, kBBoxBytes, 1024u);
+#ifndef PROBE_SKIP_MMA
                     umma_bf16(tmem_base, adesc, bdesc, (kb | k) != 0u);
+#else
+                    (void)adesc; (void)bdesc;
+#endif
                 }
                 umma_commit_pair(empty_bar(s));  // both CTAs may refill the stage once these MMAs have read it
             }
@@ -262,10 +290,23 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         // Eight warps: warp w reads TMEM lane quarter q = w % 4 (the only lanes it may touch) and column half
         // h = (w - 2) / 4, i.e. a 32-row x 128-column piece of the tile = two 64-column TMA boxes of 4 KiB.  The
         // operand ring is idle once accum_bar has fired (every MMA has read it, in both CTAs), so the boxes are staged there.
+        // While the main loop runs these warps have nothing to do: they stage the tile's 256 bias values in shared memory
+        // (zero beyond N), so that the epilogue proper never waits for a global load -- in the first version every
+        // 8-column chunk issued its own two bias loads behind the previous chunk's shared-memory store (the asm memory
+        // clobbers keep them in order), about 600 cycles each, sixteen times per warp: most of the epilogue's 6 us.
+        {
+            const uint32_t t = threadIdx.x - 64u;  // 0 .. 255: one bias value per epilogue thread
+            const float bv = n0 + t < N ? __ldg(bias + n0 + t) : 0.0f;
+            asm volatile("st.shared.f32 [%0], %1;" ::"r"(bias_tile + 4u * t), "f"(bv) : "memory");
+            asm volatile("bar.sync 1, 256;" ::: "memory");  // named barrier: the eight epilogue warps only
+        }
         mbar_wait(accum_bar, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t q = warp & 3u, h = (warp - 2u) >> 2;
         const uint32_t stage0 = base + ((h * 4u + q) * 2u) * kCBoxBytes;
+#ifdef PROBE_SKIP_EPI
+        if (M) goto epi_done;
+#endif
 #pragma unroll 1
         for (uint32_t j = 0; j < 2; ++j) {  // one 64-column box per round
             const uint32_t c0 = h * 128u + j * 64u;
@@ -277,26 +318,21 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
             const uint32_t srow = stage0 + j * kCBoxBytes + lane * 128u;  // this lane's 128-byte row of the box
 #pragma unroll
             for (uint32_t g = 0; g < 8; ++g) {  // 8 columns -> one 16-byte chunk
-                const uint32_t n = n0 + c0 + 8u * g;
-                float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-                if (n < N) {  // N is a multiple of 8: a chunk is inside or outside as a whole
-                    b0 = __ldg(reinterpret_cast<const float4*>(bias + n));
-                    b1 = __ldg(reinterpret_cast<const float4*>(bias + n + 4));
-                }
-                const float z[8] = {__uint_as_float(v[8 * g + 0]) + b0.x, __uint_as_float(v[8 * g + 1]) + b0.y,
-                                    __uint_as_float(v[8 * g + 2]) + b0.z, __uint_as_float(v[8 * g + 3]) + b0.w,
-                                    __uint_as_float(v[8 * g + 4]) + b1.x, __uint_as_float(v[8 * g + 5]) + b1.y,
-                                    __uint_as_float(v[8 * g + 6]) + b1.z, __uint_as_float(v[8 * g + 7]) + b1.w};
+                float4 b0, b1;  // bias of columns c0 + 8g .. + 7 (a broadcast read: every lane reads the same address)
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b0.x), "=f"(b0.y), "=f"(b0.z), "=f"(b0.w) : "r"(bias_tile + 4u * (c0 + 8u * g)));
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b1.x), "=f"(b1.y), "=f"(b1.z), "=f"(b1.w) : "r"(bias_tile + 4u * (c0 + 8u * g + 4u)));
+                const float2 bb[4] = {make_float2(b0.x, b0.y), make_float2(b0.z, b0.w), make_float2(b1.x, b1.y), make_float2(b1.z, b1.w)};
                 uint32_t o[4];
 #pragma unroll
                 for (int t = 0; t < 4; ++t) {
-                    __nv_bfloat162 hh = __floats2bfloat162_rn(gelu_erf(z[2 * t]), gelu_erf(z[2 * t + 1]));
+                    const float2 acc = make_float2(__uint_as_float(v[8 * g + 2 * t]), __uint_as_float(v[8 * g + 2 * t + 1]));
+                    const float2 r = gelu_erf2(__fadd2_rn(acc, bb[t]));
+                    __nv_bfloat162 hh = __floats2bfloat162_rn(r.x, r.y);
                     o[t] = *reinterpret_cast<uint32_t*>(&hh);
                 }
                 // 128-byte swizzle: chunk g of row r lives at chunk position g ^ (r mod 8)
                 asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(srow + ((g ^ (lane & 7u)) << 4)), "r"(o[0]), "r"(o[1]),
-                             "r"(o[2]), "r"(o[3])
-                             : "memory");
+                             "r"(o[2]), "r"(o[3]));
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
             __syncwarp();
@@ -307,10 +343,16 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
         }
-        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // stores done before smem goes away
+#ifdef PROBE_SKIP_EPI
+    epi_done:
+#endif
+        // the staging memory may go away once the TMA unit has READ it; the writes themselves complete before the grid does
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
-    // Neither CTA may leave (or free its TMEM) while the other still uses the pair's resources.
+    // Neither CTA may leave (or free its TMEM) while the other still uses the pair's resources.  The producer and issuer
+    // warps ran their loops in one elected lane: reconverge before the warp-aligned cluster barrier.
+    __syncwarp();
     cluster_sync_all();
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
