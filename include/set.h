@@ -84,6 +84,7 @@ typedef struct set_grid_rule {
                              region of slot buffer `index` starting at value(offset); see tmap     */
 
 #define SET_SWIZZLE_NONE 0
+#define SET_SWIZZLE_64B  2
 #define SET_SWIZZLE_128B 3
 
 typedef struct set_tmap2d {

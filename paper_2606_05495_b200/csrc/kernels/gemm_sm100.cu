@@ -40,9 +40,11 @@ constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
 constexpr uint32_t kBBoxes = kHalfN / kBBoxN;                // 2 boxes: this CTA's half of B
 constexpr uint32_t kBBytes = kBBoxBytes * kBBoxes;           // 16 KiB
 constexpr uint32_t kStageBytes = kABytes + kBBytes;          // 32 KiB
-constexpr uint32_t kCBoxBytes = 64 * 32 * 2;                 // epilogue staging: one TMA store box, 64 columns x 32 rows of bf16
-static_assert(16 * kCBoxBytes <= kStages * kStageBytes, "the epilogue stages its 16 boxes in the idle operand ring");
+constexpr uint32_t kCBoxBytes = 32 * 32 * 2;                 // epilogue staging: one TMA store box, 32 columns x 32 rows of bf16, 64-byte swizzle
+static_assert(32 * kCBoxBytes <= kStages * kStageBytes, "the epilogue stages its 32 boxes in the idle operand ring");
 constexpr uint32_t kTmemCols = 256;
+constexpr uint32_t kEpiWarps = 16;                      // four per TMEM lane quarter, 64 columns (one TMA store box) each
+constexpr uint32_t kThreads = (2 + kEpiWarps) * 32;     // + TMA producer warp + MMA issuer warp = 576
 constexpr uint32_t kBarrierBytes = 256;
 constexpr uint32_t kBiasBytes = kBlockN * 4;  // the tile's 256 bias values, staged by the epilogue warps while the main loop runs
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + kBarrierBytes + kBiasBytes + 1024;  // + slack for 1024-byte alignment
@@ -88,6 +90,11 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
     // ring then runs one stage at a time, 0.65 us per k-block whatever its depth).  The data itself is published by the TMA
     // unit's complete_tx on the same barrier; this arrival only balances the barrier's count.
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// Cluster barrier without memory ordering: for "nobody leaves before everybody is done".  (A releasing arrive waits for the
+// thread's outstanding writes, TMA stores included, to be performed -- a microsecond at the end of the epilogue.)
+__device__ __forceinline__ void cluster_sync_relaxed() {
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -180,12 +187,27 @@ __device__ __forceinline__ float2 gelu_erf2(float2 z) {
 
 }  // namespace
 
+#ifdef PROBE_STAMPS
+__device__ unsigned long long g_stamps[64 * 8];
+__device__ unsigned int g_stamp_launch;
+#define STAMP(i) do { if (threadIdx.x == (i == 3 || i == 4 ? 64u : 0u) && blockIdx.x == 0 && blockIdx.y == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_stamps[(stamp_launch % 64) * 8 + i] = t_; } } while (0)
+#else
+#define STAMP(i)
+#endif
 extern "C" uint32_t set_gemm_smem_bytes(void) { return kSmemBytes; }
+extern "C" uint32_t set_gemm_threads(void) { return kThreads; }
 
-extern "C" __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
+extern "C" __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                           const __grid_constant__ CUtensorMap tmC, const float* __restrict__ bias, uint32_t M, uint32_t N, uint32_t K) {
     extern __shared__ uint8_t smem_raw[];
+#ifdef PROBE_STAMPS
+    __shared__ unsigned int stamp_launch_s;
+    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0) stamp_launch_s = atomicAdd(&g_stamp_launch, 1u);
+    __syncthreads();
+    const unsigned int stamp_launch = stamp_launch_s;
+    STAMP(0);
+#endif
     // Both CTAs of the pair must carve shared memory identically: the MMA reads the peer's operand tiles at the leader's
     // offsets and tcgen05.commit signals the peer's barriers at the leader's offsets.  The dynamic shared memory base is
     // the same in every CTA of a launch, so the same rounding gives the same offsets.
@@ -195,7 +217,8 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     auto full_bar = [&](uint32_t s) { return bars + 8u * s; };
     auto empty_bar = [&](uint32_t s) { return bars + 8u * (kStages + s); };
     const uint32_t accum_bar = bars + 8u * (2 * kStages);
-    const uint32_t tmem_slot = bars + 8u * (2 * kStages + 1);
+    const uint32_t tmem_ready = bars + 8u * (2 * kStages + 1);  // in the leader: TMEM allocated in both CTAs
+    const uint32_t tmem_slot = bars + 8u * (2 * kStages + 2);
     const uint32_t bias_tile = bars + kBarrierBytes;  // float[256]
     auto a_tile = [&](uint32_t s) { return base + s * kStageBytes; };
     auto b_tile = [&](uint32_t s) { return base + s * kStageBytes + kABytes; };
@@ -226,21 +249,28 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
             mbar_init(empty_bar(s), 1);
         }
         mbar_init(accum_bar, 1);
+        mbar_init(tmem_ready, 2);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {  // TMEM: 256 columns in each CTA for its 128 x 256 fp32 half of the accumulator
-        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    cluster_sync_all();  // barriers initialised and TMEM allocated in BOTH CTAs before anyone signals or issues
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    uint32_t tmem_base;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
-    // Programmatic dependent launch (set.h SET_STAGE_PDL): the prologue above (tensor-map prefetch, barrier init, TMEM
-    // allocation) may overlap the node before this one; nothing below may read A, B or bias, or write C, before that
+    cluster_sync_all();  // barriers initialised in BOTH CTAs before anyone signals
+    // Programmatic dependent launch (set.h SET_STAGE_PDL): the prologue above (tensor-map prefetch, barrier init) and the
+    // TMEM allocation below may overlap the node before this one; nothing may read A, B or bias, or write C, before that
     // node's writes are visible.  Both instructions do nothing over an ordinary edge.
     set_pdl_sync();
+    // The producer warp goes straight to its first loads; the TMEM allocation (0.2 - 0.4 us) runs beside their latency.
+    uint32_t tmem_base = 0;
+    if (warp != 0) {
+        if (warp == 1) {  // TMEM: 256 columns in each CTA for its 128 x 256 fp32 half of the accumulator
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+            if (lane == 0) mbar_arrive_cluster(map_to_cta(tmem_ready, 0));  // the leader's issuer waits for both allocations
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        asm volatile("bar.sync 2, %0;" ::"n"((1 + kEpiWarps) * 32) : "memory");  // issuer warp + epilogue warps: the address is in shared memory
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+    }
+    STAMP(1);
 
     if (warp == 0) {
         // ===== TMA producer: every CTA stages its own halves; all bytes are counted on the leader's barrier =====
@@ -265,6 +295,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     } else if (warp == 1) {
         // ===== MMA issuer: one thread of the LEADER drives the tensor cores of both SMs =====
         if (rank == 0 && elect_one()) {
+            mbar_wait(tmem_ready, 0);
             for (uint32_t kb = 0; kb < num_kb; ++kb) {
                 const uint32_t s = kb % kStages, round = kb / kStages;
                 mbar_wait(full_bar(s), round & 1u);
@@ -295,52 +326,76 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         // 8-column chunk issued its own two bias loads behind the previous chunk's shared-memory store (the asm memory
         // clobbers keep them in order), about 600 cycles each, sixteen times per warp: most of the epilogue's 6 us.
         {
-            const uint32_t t = threadIdx.x - 64u;  // 0 .. 255: one bias value per epilogue thread
-            const float bv = n0 + t < N ? __ldg(bias + n0 + t) : 0.0f;
-            asm volatile("st.shared.f32 [%0], %1;" ::"r"(bias_tile + 4u * t), "f"(bv) : "memory");
-            asm volatile("bar.sync 1, 256;" ::: "memory");  // named barrier: the eight epilogue warps only
+            const uint32_t t = threadIdx.x - 64u;  // 0 .. 511: the first 256 epilogue threads load one bias value each
+            if (t < kBlockN) {
+                const float bv = n0 + t < N ? __ldg(bias + n0 + t) : 0.0f;
+                asm volatile("st.shared.f32 [%0], %1;" ::"r"(bias_tile + 4u * t), "f"(bv) : "memory");
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");  // named barrier: the epilogue warps only
         }
         mbar_wait(accum_bar, 0);
+        STAMP(3);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t q = warp & 3u, h = (warp - 2u) >> 2;
-        const uint32_t stage0 = base + ((h * 4u + q) * 2u) * kCBoxBytes;
+        // Sixteen warps: warp w reads TMEM lane quarter q = w % 4 (the only lanes it may touch) and column group cg = (w - 2) / 4,
+        // i.e. a 32-row x 64-column piece of the tile = one TMA store box of 4 KiB.  The operand ring is idle once accum_bar
+        // has fired (every MMA has read it, in both CTAs), so the boxes are staged there.  The arithmetic is a dependent chain of
+        // ~20 instructions per pair of elements: with eight warps the schedulers issued 15 % of the time (ncu), hence sixteen.
+        const uint32_t q = warp & 3u, cg = (warp - 2u) >> 2;
+        const uint32_t box0 = base + (cg * 4u + q) * 2u * kCBoxBytes;  // this warp's two store boxes
 #ifdef PROBE_SKIP_EPI
         if (M) goto epi_done;
 #endif
-#pragma unroll 1
-        for (uint32_t j = 0; j < 2; ++j) {  // one 64-column box per round
-            const uint32_t c0 = h * 128u + j * 64u;
-            if (n0 + c0 >= N || m0 + q * 32u >= M) break;  // warp-uniform: nothing of this box lies inside the matrix
-            uint32_t v[64];
-            tmem_ld32(tmem_base + ((q * 32u) << 16) + c0, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
-            tmem_ld32(tmem_base + ((q * 32u) << 16) + c0 + 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            const uint32_t srow = stage0 + j * kCBoxBytes + lane * 128u;  // this lane's 128-byte row of the box
+        // Two rounds of 32 columns; the TMEM load of the second is issued before the first is computed.
+        if (m0 + q * 32u < M && n0 + cg * 64u < N) {  // warp-uniform: something of this box lies inside the matrix
+            const uint32_t trow = tmem_base + ((q * 32u) << 16) + cg * 64u;
+            uint32_t va[32], vb[32];
+            tmem_ld32(trow, va);
 #pragma unroll
-            for (uint32_t g = 0; g < 8; ++g) {  // 8 columns -> one 16-byte chunk
-                float4 b0, b1;  // bias of columns c0 + 8g .. + 7 (a broadcast read: every lane reads the same address)
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b0.x), "=f"(b0.y), "=f"(b0.z), "=f"(b0.w) : "r"(bias_tile + 4u * (c0 + 8u * g)));
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b1.x), "=f"(b1.y), "=f"(b1.z), "=f"(b1.w) : "r"(bias_tile + 4u * (c0 + 8u * g + 4u)));
-                const float2 bb[4] = {make_float2(b0.x, b0.y), make_float2(b0.z, b0.w), make_float2(b1.x, b1.y), make_float2(b1.z, b1.w)};
-                uint32_t o[4];
+            for (uint32_t r = 0; r < 2; ++r) {
+                const uint32_t c0 = cg * 64u + r * 32u;  // first column of the round inside the tile
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (r == 0) tmem_ld32(trow + 32u, vb);
+                const uint32_t (&v)[32] = r ? vb : va;
+                const uint32_t box = box0 + r * kCBoxBytes;
+                const uint32_t srow = box + lane * 64u;  // this lane's 64-byte row of the box
+#ifdef PROBE_SKIP_MATH
+                if (n0 + c0 < N && M == 1) {
+#else
+                if (n0 + c0 < N) {  // warp-uniform; N is a multiple of 8, so an 8-column chunk is inside or outside as a whole
+#endif
 #pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                    const float2 acc = make_float2(__uint_as_float(v[8 * g + 2 * t]), __uint_as_float(v[8 * g + 2 * t + 1]));
-                    const float2 r = gelu_erf2(__fadd2_rn(acc, bb[t]));
-                    __nv_bfloat162 hh = __floats2bfloat162_rn(r.x, r.y);
-                    o[t] = *reinterpret_cast<uint32_t*>(&hh);
+                    for (uint32_t g = 0; g < 4; ++g) {  // 8 columns -> one 16-byte chunk
+                        float4 b0, b1;  // bias of columns c0 + 8g .. + 7 (a broadcast read: every lane reads the same address)
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b0.x), "=f"(b0.y), "=f"(b0.z), "=f"(b0.w) : "r"(bias_tile + 4u * (c0 + 8u * g)));
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(b1.x), "=f"(b1.y), "=f"(b1.z), "=f"(b1.w) : "r"(bias_tile + 4u * (c0 + 8u * g + 4u)));
+                        const float2 bb[4] = {make_float2(b0.x, b0.y), make_float2(b0.z, b0.w), make_float2(b1.x, b1.y), make_float2(b1.z, b1.w)};
+                        uint32_t o[4];
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) {
+                            const float2 acc = make_float2(__uint_as_float(v[8 * g + 2 * t]), __uint_as_float(v[8 * g + 2 * t + 1]));
+                            const float2 res = gelu_erf2(__fadd2_rn(acc, bb[t]));
+                            __nv_bfloat162 hh = __floats2bfloat162_rn(res.x, res.y);
+                            o[t] = *reinterpret_cast<uint32_t*>(&hh);
+                        }
+                        // 64-byte swizzle (byte-address bits 4-5 ^= bits 7-8): chunk g of row r lives at chunk position g ^ ((r >> 1) & 3)
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(srow + ((g ^ ((lane >> 1) & 3u)) << 4)), "r"(o[0]), "r"(o[1]),
+                                     "r"(o[2]), "r"(o[3]));
+                    }
+                    // The round's 32 x 32 box goes to the TMA unit at once, so that the first store of every warp (half of the
+                    // tile's 64 KiB) drains while the second round is computed.
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
+                    __syncwarp();
+#ifndef PROBE_SKIP_STORE
+                    if (lane == 0) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
+#else
+                    if (lane == 0 && M == 1) {
+#endif
+                        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(&tmC), "r"(box),
+                                     "r"((int32_t)(n0 + c0)), "r"((int32_t)(m0 + q * 32u))
+                                     : "memory");
+                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    }
                 }
-                // 128-byte swizzle: chunk g of row r lives at chunk position g ^ (r mod 8)
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(srow + ((g ^ (lane & 7u)) << 4)), "r"(o[0]), "r"(o[1]),
-                             "r"(o[2]), "r"(o[3]));
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
-            __syncwarp();
-            if (lane == 0) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
-                asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(&tmC),
-                             "r"(stage0 + j * kCBoxBytes), "r"((int32_t)(n0 + c0)), "r"((int32_t)(m0 + q * 32u))
-                             : "memory");
-                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
         }
 #ifdef PROBE_SKIP_EPI
@@ -349,13 +404,16 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         // the staging memory may go away once the TMA unit has READ it; the writes themselves complete before the grid does
         if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        STAMP(4);
     }
+    STAMP(2);
     // Neither CTA may leave (or free its TMEM) while the other still uses the pair's resources.  The producer and issuer
     // warps ran their loops in one elected lane: reconverge before the warp-aligned cluster barrier.
     __syncwarp();
-    cluster_sync_all();
+    cluster_sync_relaxed();
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
+    STAMP(5);
 }

@@ -10,6 +10,7 @@ extern "C" __global__ void set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUt
                                                      const __grid_constant__ CUtensorMap tmC, const float* bias, uint32_t M, uint32_t N,
                                                      uint32_t K);
 extern "C" uint32_t set_gemm_smem_bytes(void);
+extern "C" uint32_t set_gemm_threads(void);
 
 namespace {
 
@@ -35,13 +36,14 @@ set_arg_desc arg_dim(int i) {
     a.index = i;
     return a;
 }
-set_arg_desc arg_tmap(int idx, uint64_t off, uint32_t elem, uint64_t inner, uint64_t outer, uint32_t box_in, uint32_t box_out) {
+set_arg_desc arg_tmap(int idx, uint64_t off, uint32_t elem, uint64_t inner, uint64_t outer, uint32_t box_in, uint32_t box_out,
+                      uint32_t swizzle = SET_SWIZZLE_128B) {
     set_arg_desc a{};
     a.kind = SET_ARG_TMAP2D;
     a.index = idx;
     a.offset = fixed(off);
     a.tmap.elem_bytes = elem;
-    a.tmap.swizzle = SET_SWIZZLE_128B;
+    a.tmap.swizzle = swizzle;
     a.tmap.inner = inner;
     a.tmap.outer = outer;
     a.tmap.pitch_bytes = inner * elem;
@@ -177,10 +179,10 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[1].d2h_bytes = fixed(out_bytes);
             nb = 2;
             // A: row-major MxK, box = 64 K-elements (128 B) x 128 rows.  B: row-major KxN, box = 64 N-elements x 64 K-rows.
-            // C: row-major MxN, store box = 64 N-elements x 32 rows (one epilogue warp's piece).
+            // C: row-major MxN, store box = 32 N-elements x 32 rows (half of one epilogue warp's piece), 64-byte swizzle.
             // grid: CTA pairs (cluster 2 x 1 x 1) along x, one pair per 256 x 256 tile -- gemm_sm100.cu
-            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed(2 * ((M + 255) / 256)), grid_fixed((N + 255) / 256), 320, 1, set_gemm_smem_bytes(),
-                             {arg_tmap(0, 0, 2, K, M, 64, 128), arg_tmap(0, a_bytes, 2, N, K, 64, 64), arg_tmap(1, 0, 2, N, M, 64, 32),
+            st[ns++] = stage(SET_K_GEMM_BIAS_GELU, grid_fixed(2 * ((M + 255) / 256)), grid_fixed((N + 255) / 256), set_gemm_threads(), 1, set_gemm_smem_bytes(),
+                             {arg_tmap(0, 0, 2, K, M, 64, 128), arg_tmap(0, a_bytes, 2, N, K, 64, 64), arg_tmap(1, 0, 2, N, M, 32, 32, SET_SWIZZLE_64B),
                               arg_buf(0, fixed(a_bytes + b_bytes)), arg_u32(M), arg_u32(N), arg_u32(K)});
             break;
         }

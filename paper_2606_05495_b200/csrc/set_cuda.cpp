@@ -262,7 +262,9 @@ int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims
                 cuuint64_t gstride[1] = {t.pitch_bytes};
                 cuuint32_t box[2] = {t.box_inner, t.box_outer};
                 cuuint32_t estr[2] = {1, 1};
-                CUtensorMapSwizzle sw = t.swizzle == SET_SWIZZLE_128B ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
+                CUtensorMapSwizzle sw = t.swizzle == SET_SWIZZLE_128B  ? CU_TENSOR_MAP_SWIZZLE_128B
+                                        : t.swizzle == SET_SWIZZLE_64B ? CU_TENSOR_MAP_SWIZZLE_64B
+                                                                       : CU_TENSOR_MAP_SWIZZLE_NONE;
                 char* base = (char*)slots[slot].buf[d.index] + eval(d.offset, dims);
                 CUresult r = encode_tiled((CUtensorMap*)ap.store[a], dt, 2, base, gdim, gstride, box, estr,
                                           CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
