@@ -214,8 +214,10 @@ typedef struct set_config {
                                  lane w mod S, CUDA stream (w / S) mod streams_per_lane of that lane, so consecutive jobs
                                  of a lane overlap (job k+1's copy-in runs beside job k's kernels and tail) instead of
                                  queueing behind each other's last node.  The paper's worker owns a stream of its own
-                                 (PAPER.md:110), which is streams_per_lane = max_inflight / num_streams.  0 => default
-                                 (DESIGN.md 5b); forced to 1 when the caller supplies `streams`.                      */
+                                 (PAPER.md:110), which is streams_per_lane = max_inflight / num_streams; larger values are
+                                 clamped to that.  0 => default: with SET_IO_HOST as many as the slots allow up to 32 CUDA
+                                 streams in all, with SET_IO_DEVICE 1 (DESIGN.md 5b gives the measurements).  Forced to 1
+                                 when the caller supplies `streams`.  The in-run baseline models use the same streams.  */
     uint32_t debug_sentinel;  /* test hook: non-zero => at the moment a job's completion is observed (before the slot is
                                  released) the first and last 32-bit word of every D2H region of its host_out are compared
                                  with this value; a match means the completion overtook the output, counted in

@@ -120,3 +120,34 @@ def config4_job(job_id: int, size=None) -> np.ndarray:
     n = h * w * 3
     words = raw_u64(4, job_id, 0, (n + 7) // 8)
     return words.view(np.uint8)[:n].reshape(h, w, 3).copy()
+
+
+# ---------------------------------------------------------------- paper workloads 5 (SSSP) and 6 (Sobel chain)
+def sssp_job(job_id: int, v: int = 4096, mean_deg: int = 8) -> np.ndarray:
+    """int32 image [V, E, src, 0][row_ptr[V+1]][col[E]][w[E]] of one synthetic SSSP graph (stands in for the paper's SSSP
+    inputs, which are not available): directed, out-degree uniform in 1 .. 2*mean_deg - 1, targets uniform
+    over the vertices, weights uniform in 1 .. 100, source = vertex 0.  Vertices nobody points at stay unreachable."""
+    deg = 1 + uniform24(5, job_id, 0, v) % (2 * mean_deg - 1)
+    row_ptr = np.zeros(v + 1, dtype=np.int64)
+    np.cumsum(deg, out=row_ptr[1:])
+    e = int(row_ptr[-1])
+    col = (uniform24(5, job_id, 1, e) % v).astype(np.int32)
+    w = (1 + uniform24(5, job_id, 2, e) % 100).astype(np.int32)
+    return np.concatenate([np.array([v, e, 0, 0], np.int32), row_ptr.astype(np.int32), col, w])
+
+
+def sssp_max_edges(v: int, mean_deg: int = 8) -> int:
+    return v * (2 * mean_deg - 1)
+
+
+def sobel_frame(job_id: int, size=None) -> np.ndarray:
+    """uint8[H][W][3] frame for the Sobel chain (stands in for the paper's Sobel images): 16 x 16 blocks of a
+    random colour (high nibble) plus 4 bits of per-pixel noise, so that there are flat areas and sharp edges -- on pure
+    noise (config 4's frames) every pixel is an edge and the threshold stage would be constant.  Sizes as config 4."""
+    w, h = size if size is not None else config4_size(job_id)
+    bw, bh = (w + 15) // 16, (h + 15) // 16
+    blocks = raw_u64(6, job_id, 0, (bw * bh * 3 + 7) // 8).view(np.uint8)[:bw * bh * 3].reshape(bh, bw, 3) & np.uint8(0xF0)
+    full = np.repeat(np.repeat(blocks, 16, axis=0), 16, axis=1)[:h, :w, :]
+    n = h * w * 3
+    noise = raw_u64(6, job_id, 1, (n + 7) // 8).view(np.uint8)[:n].reshape(h, w, 3) & np.uint8(0x0F)
+    return (full | noise).copy()

@@ -46,6 +46,15 @@ _lib.oracle_gray_u8.argtypes = [_p, _i64, _i64, _p]
 _lib.oracle_blur3x3_u8.argtypes = [_p, _i64, _i64, _p]
 _lib.oracle_hist256_u8.argtypes = [_p, _i64, _p]
 _lib.oracle_config4.argtypes = [_p, _i64, _i64, _p, _p]
+_lib.oracle_sssp_frontier_bf.argtypes = [_p, _p, _p, _i64, C.c_int32, _p, _p]
+_lib.oracle_sssp_frontier_bf.restype = C.c_int32
+_lib.oracle_sssp_job.argtypes = [_p, _p, _p]
+_lib.oracle_sssp_job.restype = None
+_lib.oracle_sobel_u8.argtypes = [_p, _i64, _i64, _p]
+_lib.oracle_mean3x3_u8.argtypes = [_p, _i64, _i64, _p]
+_lib.oracle_threshold_u8.argtypes = [_p, _i64, C.c_int32, _p]
+_lib.oracle_blend_u8.argtypes = [_p, _p, _i64, _p]
+_lib.oracle_sobel_chain.argtypes = [_p, _i64, _i64, _p, _p]
 
 
 # ------------------------------------------------------------------ config 0
@@ -183,4 +192,71 @@ def config4(rgb: np.ndarray) -> np.ndarray:
     tmp = np.empty(h * w, dtype=np.uint8)
     out = np.empty(h * w + 1024, dtype=np.uint8)
     _lib.oracle_config4(_ptr(rgb), h, w, _ptr(tmp), _ptr(out))
+    return out
+
+
+# ------------------------------------------------------------------ config 5: SSSP
+SSSP_INF = 0x7FFFFFFF
+
+
+def sssp_frontier_bf(row_ptr, col, w, src: int = 0):
+    """(dist int32[V], rounds): frontier Bellman-Ford with synchronous rounds (readings S5-1..S5-4)."""
+    row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int32)
+    col = np.ascontiguousarray(col, dtype=np.int32)
+    w = np.ascontiguousarray(w, dtype=np.int32)
+    v = row_ptr.size - 1
+    dist = np.empty(max(v, 0), dtype=np.int32)
+    scratch = np.empty(3 * max(v, 1), dtype=np.int32)
+    rounds = _lib.oracle_sssp_frontier_bf(_ptr(row_ptr), _ptr(col), _ptr(w), v, src, _ptr(dist), _ptr(scratch))
+    return dist, int(rounds)
+
+
+def sssp_job(image: np.ndarray, *_params) -> np.ndarray:
+    """Byte image [dist int32[V]][rounds, 0, 0, 0] of one config-5 job; image = [V, E, src, 0][row_ptr][col][w]."""
+    img = np.ascontiguousarray(image).view(np.int32)
+    v = int(img[0])
+    out = np.empty(v + 4, dtype=np.int32)
+    scratch = np.empty(3 * max(v, 1), dtype=np.int32)
+    _lib.oracle_sssp_job(_ptr(img), _ptr(out), _ptr(scratch))
+    return out.view(np.uint8)
+
+
+# ------------------------------------------------------------------ config 6: Sobel chain
+def sobel_u8(n: np.ndarray) -> np.ndarray:
+    n = np.ascontiguousarray(n, dtype=np.uint8)
+    out = np.empty_like(n)
+    _lib.oracle_sobel_u8(_ptr(n), n.shape[0], n.shape[1], _ptr(out))
+    return out
+
+
+def mean3x3_u8(e: np.ndarray) -> np.ndarray:
+    e = np.ascontiguousarray(e, dtype=np.uint8)
+    out = np.empty_like(e)
+    _lib.oracle_mean3x3_u8(_ptr(e), e.shape[0], e.shape[1], _ptr(out))
+    return out
+
+
+def threshold_u8(m: np.ndarray, thresh: int = 64) -> np.ndarray:
+    m = np.ascontiguousarray(m, dtype=np.uint8)
+    out = np.empty_like(m)
+    _lib.oracle_threshold_u8(_ptr(m), m.size, thresh, _ptr(out))
+    return out
+
+
+def blend_u8(t: np.ndarray, n: np.ndarray) -> np.ndarray:
+    t = np.ascontiguousarray(t, dtype=np.uint8)
+    n = np.ascontiguousarray(n, dtype=np.uint8)
+    assert t.size == n.size
+    out = np.empty_like(t)
+    _lib.oracle_blend_u8(_ptr(t), _ptr(n), t.size, _ptr(out))
+    return out
+
+
+def sobel_chain(rgb: np.ndarray) -> np.ndarray:
+    """uint8[h*w]: the blended output of one config-6 frame (flat byte image)."""
+    rgb = np.ascontiguousarray(rgb, dtype=np.uint8)
+    h, w, _ = rgb.shape
+    tmp = np.empty(3 * h * w, dtype=np.uint8)
+    out = np.empty(h * w, dtype=np.uint8)
+    _lib.oracle_sobel_chain(_ptr(rgb), h, w, _ptr(tmp), _ptr(out))
     return out

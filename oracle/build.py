@@ -8,7 +8,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["scan_hist.c", "chain_f32.c", "jacobi.c", "gemm_gelu.c", "image.c"]
+SOURCES = ["scan_hist.c", "chain_f32.c", "jacobi.c", "gemm_gelu.c", "image.c", "sssp.c", "sobel.c"]
 LIB = os.path.join(HERE, "liboracle.so")
 
 

@@ -1,4 +1,4 @@
-/* oracle.h -- CPU oracle for the five SET workloads.  TEST INFRASTRUCTURE, NOT PRODUCT.
+/* oracle.h -- CPU oracle for the SET workloads (configs 0-4 of BASELINE.json and the two paper workloads 5, 6).  TEST INFRASTRUCTURE, NOT PRODUCT.
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * call this.  It shares no code with the CUDA path (paper_2606_05495_b200/csrc) and neither
@@ -55,6 +55,20 @@ void oracle_gray_u8(const uint8_t *rgb, int64_t h, int64_t w, uint8_t *gray);
 void oracle_blur3x3_u8(const uint8_t *g, int64_t h, int64_t w, uint8_t *blur);
 void oracle_hist256_u8(const uint8_t *p, int64_t n, uint32_t *hist);
 void oracle_config4(const uint8_t *rgb, int64_t h, int64_t w, uint8_t *gray_tmp, void *out);
+
+/* config 5: frontier Bellman-Ford SSSP (readings S5-1..S5-4).  Returns the number of synchronous rounds.
+ * scratch: int32[2V] followed by 2V bytes, i.e. at least 3V int32 */
+#define ORACLE_SSSP_INF 0x7fffffff
+int32_t oracle_sssp_frontier_bf(const int32_t *row_ptr, const int32_t *col, const int32_t *w, int64_t V, int32_t src,
+                                int32_t *dist, int32_t *scratch);
+void oracle_sssp_job(const int32_t *image, int32_t *out, int32_t *scratch);
+
+/* config 6: five-stage Sobel chain (readings S6-1..S6-6) */
+void oracle_sobel_u8(const uint8_t *n, int64_t h, int64_t w, uint8_t *e);
+void oracle_mean3x3_u8(const uint8_t *e, int64_t h, int64_t w, uint8_t *m);
+void oracle_threshold_u8(const uint8_t *m, int64_t n, int32_t thresh, uint8_t *t);
+void oracle_blend_u8(const uint8_t *t, const uint8_t *n, int64_t count, uint8_t *out);
+void oracle_sobel_chain(const uint8_t *rgb, int64_t h, int64_t w, uint8_t *tmp, uint8_t *out);
 
 #ifdef __cplusplus
 }

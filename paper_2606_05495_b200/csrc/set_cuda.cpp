@@ -26,7 +26,7 @@
 using namespace setrt;
 
 #define SET_COPY_BYTES_PER_BLOCK 8192u  // kernels/kernels.h kCopyBytesPerBlock (SET_K_COPY: 256 threads x 2 x 16 B)
-static constexpr int kDefaultStreamsPerLane = 1;  // set_config.streams_per_lane == 0
+
 
 namespace {
 
@@ -979,7 +979,12 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.completion_fence < SET_FENCE_DEFAULT || cfg.completion_fence > SET_FENCE_NONE) return SET_ERR_INVALID;
     if (cfg.completion_fence == SET_FENCE_DEFAULT) cfg.completion_fence = SET_FENCE_SYSTEM;
     if (cfg.streams_per_lane < 0 || cfg.streams_per_lane > 4096) return SET_ERR_INVALID;
-    if (cfg.streams_per_lane == 0) cfg.streams_per_lane = kDefaultStreamsPerLane;
+    // Default (measured on B200): with host I/O a job's chain is latency-bound (its copy-in waits on the link),
+    // so every slot gets a CUDA stream of its own -- the paper's worker W_i = (S_i, G_i, M_i), PAPER.md:110 -- and b chains are
+    // in flight instead of S (config 1 end to end 201 K -> 316 K jobs/s, config 0 227 K -> 336 K).  With device-resident I/O
+    // the host's launch rate is the limit and more streams only make each launch dearer (404 K -> 360 K): one per lane.
+    // The default never goes beyond 32 CUDA streams in all (b = 4096 would otherwise ask for 4096 of them).
+    if (cfg.streams_per_lane == 0) cfg.streams_per_lane = cfg.io == SET_IO_HOST ? std::max(1, 32 / cfg.num_streams) : 1;
     if (cfg.mode == SET_MODE_SINGLE_GRAPH) {  // one worker, one stream, one exec by definition
         cfg.num_streams = 1;
         cfg.max_inflight = 1;

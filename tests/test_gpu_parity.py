@@ -352,7 +352,7 @@ def test_device_timestamps_give_per_stream_gaps(libset, config, mode):
             compare(wl, np.array(outs[j], copy=True), oracle_out(wl, ins[j], dims[j]))
         g = ctx.gap_stats()
         assert g["jobs"] == n
-        assert n - wl.num_streams <= g["gaps"] <= n - 1
+        assert n - ctx.stats()["cuda_streams"] <= g["gaps"] <= n - 1      # one gap less than jobs on every CUDA stream that ran any
         assert 1.0 < g["job_mean_us"] < 5000.0 and 0.0 <= g["gap_mean_us"] <= g["gap_max_us"] < 1e6
         assert g["gap_p50_us"] <= g["gap_p99_us"] <= g["gap_max_us"] and 0.0 < g["stream_busy_frac"] <= 1.0001
         ctx.reset_stats()

@@ -415,3 +415,150 @@ def test_inputgen_distributions():
     assert set(sizes) == set(inputgen.FRAME_SIZES)
     f = inputgen.config4_job(0, (32, 16))
     assert f.shape == (16, 32, 3) and f.dtype == np.uint8 and abs(f.mean() - 127.5) < 8
+
+
+# =============================================================== config 5: SSSP, frontier Bellman-Ford
+def _csr(v, edges):
+    """edges: list of (u, t, w) -> row_ptr, col, w in CSR order."""
+    edges = sorted(edges, key=lambda e: e[0])
+    row_ptr = np.zeros(v + 1, np.int32)
+    for u, _, _ in edges:
+        row_ptr[u + 1] += 1
+    row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    return row_ptr, np.array([e[1] for e in edges], np.int32), np.array([e[2] for e in edges], np.int32)
+
+
+def _dijkstra(v, row_ptr, col, w, src):
+    import heapq
+    dist = [oracle.SSSP_INF] * v
+    dist[src] = 0
+    pq = [(0, src)]
+    while pq:
+        d, u = heapq.heappop(pq)
+        if d > dist[u]:
+            continue
+        for e in range(row_ptr[u], row_ptr[u + 1]):
+            nd = d + int(w[e])
+            if nd < dist[col[e]]:
+                dist[col[e]] = nd
+                heapq.heappush(pq, (nd, int(col[e])))
+    return np.array(dist, np.int32)
+
+
+def test_c5_path_graph_closed_form():
+    # 0 -> 1 -> 2 -> ... -> 9 with weight 3: dist[k] = 3k, and the frontier needs one round per hop plus the round that
+    # finds nothing left to improve (reading S5-3)
+    v = 10
+    rp, col, w = _csr(v, [(k, k + 1, 3) for k in range(v - 1)])
+    dist, rounds = oracle.sssp_frontier_bf(rp, col, w, 0)
+    assert dist.tolist() == [3 * k for k in range(v)]
+    assert rounds == v                        # rounds 1..9 settle vertices 1..9, round 10 relaxes the last vertex's (no) edges
+    # started in the middle: everything upstream is unreachable (reading S5-2)
+    dist, _ = oracle.sssp_frontier_bf(rp, col, w, 4)
+    assert dist.tolist() == [oracle.SSSP_INF] * 4 + [0, 3, 6, 9, 12, 15]
+
+
+def test_c5_hand_graph_with_a_shortcut_found_late():
+    # 0 -1-> 1 -1-> 2 -1-> 3 and the direct but dearer edge 0 -10-> 3; 3 -1-> 4.  The direct edge is seen first (round 1:
+    # dist[3] = 10), the three-hop path wins in round 3 (dist[3] = 3) and vertex 4 is corrected in round 4.
+    rp, col, w = _csr(5, [(0, 1, 1), (0, 3, 10), (1, 2, 1), (2, 3, 1), (3, 4, 1)])
+    dist, rounds = oracle.sssp_frontier_bf(rp, col, w, 0)
+    assert dist.tolist() == [0, 1, 2, 3, 4] and rounds == 5
+    # zero-weight edges and a cycle do not loop for ever (weights >= 0, reading S5-1)
+    rp, col, w = _csr(3, [(0, 1, 0), (1, 2, 0), (2, 0, 0)])
+    dist, rounds = oracle.sssp_frontier_bf(rp, col, w, 0)
+    assert dist.tolist() == [0, 0, 0] and rounds == 3
+    # a source without edges: one round that relaxes nothing
+    rp, col, w = _csr(3, [(1, 2, 5)])
+    dist, rounds = oracle.sssp_frontier_bf(rp, col, w, 0)
+    assert dist.tolist() == [0, oracle.SSSP_INF, oracle.SSSP_INF] and rounds == 1
+
+
+def test_c5_against_dijkstra_and_the_triangle_inequality():
+    for job, (v, deg) in enumerate([(50, 2), (300, 3), (2000, 4), (4096, 8)]):
+        img = inputgen.sssp_job(job, v, deg)
+        assert img[0] == v and img[2] == 0
+        e = int(img[1])
+        rp, col, w = img[4:4 + v + 1], img[5 + v:5 + v + e], img[5 + v + e:5 + v + 2 * e]
+        assert rp[0] == 0 and rp[-1] == e and img.size == 4 + v + 1 + 2 * e and w.min() >= 1 and w.max() <= 100
+        dist, rounds = oracle.sssp_frontier_bf(rp, col, w, 0)
+        assert np.array_equal(dist, _dijkstra(v, rp, col, w, 0))            # an independent algorithm (binary heap)
+        # invariant of any correct answer: no edge can still be relaxed, and every finite distance is attained by some edge
+        src_of = np.repeat(np.arange(v), np.diff(rp))
+        fin = dist[src_of] != oracle.SSSP_INF
+        assert np.all(dist[col][fin].astype(np.int64) <= dist[src_of][fin].astype(np.int64) + w[fin])
+        tight = np.zeros(v, bool)
+        tight[col[fin][dist[col][fin].astype(np.int64) == dist[src_of][fin].astype(np.int64) + w[fin]]] = True
+        reach = dist != oracle.SSSP_INF
+        assert np.all(tight[reach][1:] | (np.nonzero(reach)[0][1:] == 0))   # every reached vertex but the source has a tight in-edge
+        assert 1 <= rounds <= v
+        # the whole-job image: [dist][rounds, 0, 0, 0]
+        out = oracle.sssp_job(img).view(np.int32)
+        assert np.array_equal(out[:v], dist) and out[v:].tolist() == [rounds, 0, 0, 0]
+    # unreachable vertices exist in the sparse cases and stay at INF
+    img = inputgen.sssp_job(0, 50, 2)
+    assert (oracle.sssp_job(img).view(np.int32)[:50] == oracle.SSSP_INF).any()
+
+
+# =============================================================== config 6: Sobel chain (PAPER.md:215)
+def _brute_3x3(img, fn):
+    h, w = img.shape
+    out = np.zeros((h, w), np.int64)
+    for y in range(h):
+        for x in range(w):
+            nb = [[int(img[min(max(y + dy, 0), h - 1), min(max(x + dx, 0), w - 1)]) for dx in (-1, 0, 1)] for dy in (-1, 0, 1)]
+            out[y, x] = fn(nb)
+    return out
+
+
+def test_c6_sobel_closed_forms():
+    # constant image: no edges anywhere, borders included (clamp-to-edge keeps it constant)
+    assert not oracle.sobel_u8(np.full((7, 9), 200, np.uint8)).any()
+    # vertical step 0 | 40 between columns 3 and 4: gx = (1 + 2 + 1) * 40 = 160 on both sides of the step, gy = 0
+    img = np.zeros((6, 8), np.uint8)
+    img[:, 4:] = 40
+    e = oracle.sobel_u8(img)
+    assert np.all(e[:, 3] == 160) and np.all(e[:, 4] == 160) and not e[:, :3].any() and not e[:, 5:].any()
+    # a taller step saturates: 4 * 100 = 400 -> 255 (reading S6-2)
+    img[:, 4:] = 100
+    assert np.all(oracle.sobel_u8(img)[:, 3:5] == 255)
+    # horizontal step: the transposed kernel gives the transposed picture
+    assert np.array_equal(oracle.sobel_u8(img.T.copy()), oracle.sobel_u8(img).T)
+    # single bright pixel 10 in the middle: |gx| + |gy| ring 20 / 20 / 20 on the four-neighbours' ... per tap by hand
+    img = np.zeros((5, 5), np.uint8)
+    img[2, 2] = 10
+    want = np.array([[20, 20, 20], [20, 0, 20], [20, 20, 20]])          # corners |±10| + |±10|, edges |±20| + 0
+    assert np.array_equal(oracle.sobel_u8(img)[1:4, 1:4], want)
+
+
+def test_c6_stages_against_per_pixel_brute_force():
+    rng_img = inputgen.sobel_frame(77, (45, 37))                            # (w, h) = (45, 37) RGB frame: blocks + noise
+    n = oracle.gray_u8(rng_img)
+    kx = [[-1, 0, 1], [-2, 0, 2], [-1, 0, 1]]
+    sob = _brute_3x3(n, lambda nb: min(255, abs(sum(kx[i][j] * nb[i][j] for i in range(3) for j in range(3)))
+                                       + abs(sum(kx[j][i] * nb[i][j] for i in range(3) for j in range(3)))))
+    e = oracle.sobel_u8(n)
+    assert np.array_equal(e, sob)
+    m = oracle.mean3x3_u8(e)
+    assert np.array_equal(m, _brute_3x3(e, lambda nb: sum(map(sum, nb)) // 9))
+    t = oracle.threshold_u8(m, 64)
+    assert np.array_equal(t, np.where(m >= 64, 255, 0)) and set(np.unique(t)) <= {0, 255} and 0 < (t == 255).mean() < 1
+    out = oracle.blend_u8(t, n)
+    assert np.array_equal(out, ((128 * t.astype(np.int64) + 128 * n.astype(np.int64)) >> 8))
+    # the chain is the composition of its stages
+    assert np.array_equal(oracle.sobel_chain(rng_img).reshape(n.shape), out)
+
+
+def test_c6_mean_threshold_blend_special_cases():
+    img = np.zeros((5, 5), np.uint8)
+    img[2, 2] = 255
+    m = oracle.mean3x3_u8(img)
+    assert np.all(m[1:4, 1:4] == 255 // 9) and m.sum() == 9 * 28                  # impulse -> 3 x 3 patch of 28
+    assert np.array_equal(oracle.mean3x3_u8(np.full((4, 6), 77, np.uint8)), np.full((4, 6), 77, np.uint8))
+    v = np.arange(256, dtype=np.uint8)
+    assert oracle.threshold_u8(v, 64).tolist() == [0] * 64 + [255] * 192          # >= is inclusive
+    assert np.array_equal(oracle.blend_u8(v, v), v)                                # blending a picture with itself
+    assert oracle.blend_u8(np.array([255], np.uint8), np.array([0], np.uint8))[0] == 127    # (128 * 255) >> 8 truncates
+    # a flat frame has no edges: the mask is empty and the output is the normalised frame at half intensity
+    flat = np.full((6, 7, 3), 90, np.uint8)
+    assert np.all(oracle.sobel_chain(flat) == 45)
