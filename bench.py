@@ -138,14 +138,14 @@ def build_jobs(setlib, ctx, wl, job_ids, io_device: bool, pool: int, out_ring: i
     npool = n if pool == 0 else min(pool, n)
     nring = n if out_ring == 0 else min(out_ring, n)
     dims = [wl.dims(j) for j in job_ids]
-    if wl.config == 4:
+    if wl.config in (4, 5, 6):
         js.dims = (C.c_uint32 * (4 * n))(*[v for d in dims for v in d])
     images = job_inputs(wl, job_ids, npool)
     js.pool_inputs = images
     pool_dims = dims[:npool]
     in_sz = [wl.in_bytes(d) for d in pool_dims]
     # config 4: the job's frame size is that of its pool image
-    if wl.config == 4:
+    if wl.config in (4, 5, 6):
         for k in range(n):
             d = pool_dims[k % npool]
             for i in range(4):

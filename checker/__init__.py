@@ -45,8 +45,14 @@ def compare(wl, out: np.ndarray, ref: np.ndarray) -> None:
     the integer workloads (configs 0, 4, 5, 6) and -- reading C2-3 -- for the Jacobi stencil; 1e-6 relative for the fp32
     scalar of config 1; 2e-2 relative Frobenius error for the bf16 GEMM (config 3)."""
     c = wl.config
-    if c in (0, 4, 5, 6):
+    if c in (0, 4, 6):
         assert out.shape == ref.shape and np.array_equal(out, ref), _first_diff(out, ref)
+    elif c == 5:
+        # what is unique is compared bit for bit (the distances); the round count depends on the relaxation order (reading
+        # S5-4): the GPU relaxes in place, so it needs at least one round and at most the oracle's synchronous count
+        g, r = out.view(np.int32), ref.view(np.int32)
+        assert g.shape == r.shape and np.array_equal(g[:-4], r[:-4]), _first_diff(out[:-16], ref[:-16])
+        assert 1 <= g[-4] <= r[-4] and not g[-3:].any(), (g[-4:].tolist(), r[-4:].tolist())
     elif c == 1:
         g, r = float(out.view(np.float32)[0]), float(ref.view(np.float32)[0])
         assert abs(g - r) <= 1e-6 * abs(r), (g, r)

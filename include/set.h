@@ -80,6 +80,7 @@ typedef struct set_grid_rule {
 #define SET_ARG_IMM32   1 /* 4-byte immediate (low 32 bits of imm)                                 */
 #define SET_ARG_IMM64   2 /* 8-byte immediate                                                      */
 #define SET_ARG_DIM     3 /* uint32 = dims[index] of the job                                       */
+#define SET_ARG_COND    5 /* 8-byte cudaGraphConditionalHandle of the enclosing loop (SET_STAGE_LOOP_BEGIN)  */
 #define SET_ARG_TMAP2D  4 /* 128-byte CUtensorMap (by value, __grid_constant__) over a 2-D row-major
                              region of slot buffer `index` starting at value(offset); see tmap     */
 
@@ -105,6 +106,17 @@ typedef struct set_arg_desc {
     set_tmap2d tmap;       /* TMAP2D only                                                          */
 } set_arg_desc;
 
+#define SET_STAGE_LOOP_BEGIN 2u /* this stage is the first of a data-dependent loop: the stages from here to the next
+                                   SET_STAGE_LOOP_END (inclusive) become the body of a conditional WHILE node of the job graph
+                                   (a workload whose iteration count depends on the data does not fit a fixed
+                                   graph).  The loop is entered unconditionally; a kernel of the body ends it by calling
+                                   cudaGraphSetConditional(handle, 0) with the handle it receives as a SET_ARG_COND argument.
+                                   A pipeline with a loop is bound to its slot for good (CUDA cannot re-point the nodes of a
+                                   loop body one by one): the kernels of the body may not take SET_ARG_DIM arguments or dim-dependent
+                                   offsets / grids (per-job sizes travel in the job's device image instead), a job is never
+                                   retargeted to another slot's executable (a thief without a free executable of its own
+                                   puts the job back), and SET_MODE_PLAIN_STREAMS is refused.  One loop per pipeline.   */
+#define SET_STAGE_LOOP_END   4u
 #define SET_STAGE_PDL 1u   /* connect this stage to the node before it (the previous stage; for the first stage,
                               an SM copy node) with a programmatic-dependent-launch edge.  By setting the flag the
                               caller asserts that the kernel executes griddepcontrol.wait before it reads or writes
@@ -378,14 +390,27 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_STAMP          16  /* (uint64* stamp)  *stamp = %globaltimer (set_config.timestamps)               */
 #define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes)  copy by the SMs; src / dst may be
                                     pinned HOST or DEVICE memory                                              */
+/* the two paper workloads of SURVEY.md 8(f)4 (readings S5-*, S6-*) */
+#define SET_K_SOBEL3X3_U8    17  /* (const uint8* n, uint8* e, uint32 w, uint32 h)  min(255, |gx| + |gy|), clamp-to-edge   */
+#define SET_K_MEAN3X3_U8     18  /* (const uint8* e, uint8* m, uint32 w, uint32 h)  3 x 3 sum / 9, clamp-to-edge          */
+#define SET_K_THRESHOLD_U8   19  /* (const uint8* m, uint8* t, uint32 w, uint32 h, uint32 thresh)  m >= thresh ? 255 : 0  */
+#define SET_K_BLEND_U8       20  /* (const uint8* t, const uint8* n, uint8* out, uint32 w, uint32 h)  (t + n) >> 1        */
+#define SET_K_SSSP_INIT      21  /* (const int32* img, int32* out, uint32* scratch, uint32 maxV)  dist = INF, dist[src] = 0,
+                                    frontier = {src};  img = [V, E, src, 0][row_ptr V+1][col E][w E]               */
+#define SET_K_SSSP_RELAX     22  /* (img, out, scratch, maxV)  one frontier round: atomicMin relaxation of every edge
+                                    out of the frontier, next frontier = vertices whose distance got smaller       */
+#define SET_K_SSSP_CONTROL   23  /* (img, out, scratch, maxV, loop handle)  counts the round and sets the condition of
+                                    the enclosing WHILE node: another round iff some distance changed               */
 
 /* HOST address usable as set_stage_desc.func, or NULL for an unknown id. */
 const void *set_builtin_kernel(int kernel_id);
 
-/* Fill stage/buffer descriptors for BASELINE.json:configs[config] (0..4).
+/* Fill stage/buffer descriptors for BASELINE.json:configs[config] (0..4) or one of the two paper workloads (5, 6).
  *   params : HOST array of uint32 or NULL for the BASELINE sizes:
  *     config 0: {n}            config 1: {n}          config 2: {h, w, sweeps[, alternate = 1]}
  *     config 3: {M, N, K}      config 4: {max_w, max_h}  (dims per job = {w, h, 1, 1})
+ *     config 5 (SSSP): {maxV, maxE}  (dims per job = {E, 1, 1, 1}; V, E, src travel in the job image)
+ *     config 6 (Sobel chain): {max_w, max_h[, thresh = 64]}  (dims per job = {w, h, 1, 1})
  *   variant: 0 = default.  config 0: 1 = histogram of the INPUT values (reading C0-1 alternative).
  * *            any config: bit 8 set = append a SET_K_SPIN delay stage that busy-waits dims[3] nanoseconds.
  *   stages/bufs : HOST arrays with room for SET_MAX_STAGES / SET_MAX_BUFFERS entries.

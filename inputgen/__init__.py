@@ -136,6 +136,11 @@ def sssp_job(job_id: int, v: int = 4096, mean_deg: int = 8) -> np.ndarray:
     return np.concatenate([np.array([v, e, 0, 0], np.int32), row_ptr.astype(np.int32), col, w])
 
 
+def sssp_edges(job_id: int, v: int = 4096, mean_deg: int = 8) -> int:
+    """E of sssp_job(job_id, v, mean_deg) without building the graph."""
+    return int((1 + uniform24(5, job_id, 0, v) % (2 * mean_deg - 1)).sum())
+
+
 def sssp_max_edges(v: int, mean_deg: int = 8) -> int:
     return v * (2 * mean_deg - 1)
 

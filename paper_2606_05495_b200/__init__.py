@@ -24,7 +24,8 @@ MODE_SET, MODE_PLAIN_STREAMS, MODE_BATCH_SYNC, MODE_SINGLE_GRAPH, MODE_MUTEX_QUE
 IO_HOST, IO_DEVICE = 0, 1
 STEAL_SWAP, STEAL_RETARGET = 0, 1
 CB_DEFAULT, CB_NOTIFY_STREAM, CB_WORK_STREAM, CB_FLAG_POLL, CB_HOST_NODE = 0, 1, 2, 3, 4
-ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D = 0, 1, 2, 3, 4
+ARG_BUFFER, ARG_IMM32, ARG_IMM64, ARG_DIM, ARG_TMAP2D, ARG_COND = 0, 1, 2, 3, 4, 5
+STAGE_LOOP_BEGIN, STAGE_LOOP_END = 2, 4
 STAGE_PDL = 1
 FENCE_DEFAULT, FENCE_SYSTEM, FENCE_NONE = 0, 1, 2
 K_COPY = 15

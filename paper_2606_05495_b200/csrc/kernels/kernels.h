@@ -21,6 +21,13 @@ __global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
 __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp, uint32_t fence);
 __global__ void set_k_stamp(unsigned long long* stamp);
 __global__ void set_k_copy(const void* src, void* dst, uint32_t bytes);
+__global__ void set_k_sobel3x3_u8(const uint8_t* n, uint8_t* e, uint32_t w, uint32_t h);
+__global__ void set_k_mean3x3_u8(const uint8_t* e, uint8_t* m, uint32_t w, uint32_t h);
+__global__ void set_k_threshold_u8(const uint8_t* m, uint8_t* t, uint32_t w, uint32_t h, uint32_t thresh);
+__global__ void set_k_blend_u8(const uint8_t* t, const uint8_t* n, uint8_t* out, uint32_t w, uint32_t h);
+__global__ void set_k_sssp_init(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
+__global__ void set_k_sssp_relax(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
+__global__ void set_k_sssp_control(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, cudaGraphConditionalHandle loop);
 }
 
 // Programmatic dependent launch (SET_STAGE_PDL edges of the job graph): let the next kernel node be scheduled now,
@@ -41,3 +48,5 @@ constexpr int kGrayPixPerBlock = 256 * 16;
 constexpr int kBlurTileW = 512, kBlurTileH = 16;  // 32 lanes x 16 pixels, 4 warps x 4 rows (a 1280 x 720 frame: 135 blocks)
 constexpr int kHistPixPerBlock = 256 * 16;  // one 128-bit load per thread; a 1280 x 720 frame: 225 blocks
 constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words
+constexpr int kStencilTileW = 64 * 4, kStencilTileH = 4;  // K17/K18: block (64, 4), 4 pixels per thread
+constexpr int kBytePixPerBlock = 256 * 16;                // K19/K20: one 128-bit word per thread

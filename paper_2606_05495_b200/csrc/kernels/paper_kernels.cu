@@ -1,0 +1,182 @@
+// paper_kernels.cu -- stage kernels of the two paper workloads added in round 2:
+//   config 6, the five-stage Sobel chain:  K10 gray (stencil_kernels.cu) -> K17 sobel -> K18 mean3x3 ->
+//             K19 threshold -> K20 blend, all integer, bit-exact (readings S6-1..S6-6)
+//   config 5, frontier Bellman-Ford SSSP:  K21 init -> WHILE { K22 relax -> K23 control } (readings S5-1..S5-4);
+//             the loop is a conditional WHILE node of the job graph and K23 sets its condition on the device.
+// Hand-written CUDA for sm_100a.  The frames (0.3 - 2 MB) and graphs (~0.6 MB) sit in L2 right after the H2D copy, so
+// these are latency-class kernels like those of configs 0, 1 and 4: coalesced 32- and 128-bit accesses, no shared memory.
+#include "kernels.h"
+
+namespace {
+
+// ---- 3 x 3 neighbourhoods on a byte image, clamp-to-edge: a thread produces 4 horizontally adjacent pixels --------------
+// rows[r][c]: row y-1+r, column x0-1+c, c = 0..5.  Fast path (w % 4 == 0, so every row starts 4-byte aligned and x0 is a
+// multiple of 4): one 32-bit load for the four centre pixels plus one byte on either side.
+__device__ __forceinline__ void load_row6(const uint8_t* __restrict__ row, uint32_t x0, uint32_t w, bool fast, int (&p)[6]) {
+    if (fast) {
+        const uint32_t v = __ldg(reinterpret_cast<const uint32_t*>(row + x0));
+        p[1] = v & 0xff;
+        p[2] = (v >> 8) & 0xff;
+        p[3] = (v >> 16) & 0xff;
+        p[4] = v >> 24;
+        p[0] = x0 ? __ldg(row + x0 - 1) : p[1];
+        p[5] = x0 + 4 < w ? __ldg(row + x0 + 4) : p[4];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            int x = (int)x0 - 1 + c;
+            x = x < 0 ? 0 : (x >= (int)w ? (int)w - 1 : x);
+            p[c] = __ldg(row + x);
+        }
+    }
+}
+
+template <typename F>
+__device__ __forceinline__ void stencil3x3_u8(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, uint32_t w, uint32_t h, F f) {
+    const uint32_t x0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
+    const uint32_t y = blockIdx.y * blockDim.y + threadIdx.y;
+    if (x0 >= w || y >= h) return;
+    const bool fast = (w & 3u) == 0 && (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (reinterpret_cast<uintptr_t>(out) & 3u) == 0;
+    const uint32_t yu = y ? y - 1 : 0, yd = y + 1 < h ? y + 1 : h - 1;
+    int r[3][6];
+    load_row6(in + (size_t)yu * w, x0, w, fast, r[0]);
+    load_row6(in + (size_t)y * w, x0, w, fast, r[1]);
+    load_row6(in + (size_t)yd * w, x0, w, fast, r[2]);
+    uint32_t o[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) o[k] = f(r[0][k], r[0][k + 1], r[0][k + 2], r[1][k], r[1][k + 1], r[1][k + 2], r[2][k], r[2][k + 1], r[2][k + 2]);
+    if (fast) {
+        *reinterpret_cast<uint32_t*>(out + (size_t)y * w + x0) = o[0] | (o[1] << 8) | (o[2] << 16) | (o[3] << 24);
+    } else {
+        for (uint32_t k = 0; k < 4 && x0 + k < w; ++k) out[(size_t)y * w + x0 + k] = (uint8_t)o[k];
+    }
+}
+
+}  // namespace
+
+// K17: e = min(255, |gx| + |gy|), gx = [-1 0 1; -2 0 2; -1 0 1] * n, gy = its transpose (reading S6-2).
+extern "C" __global__ void __launch_bounds__(256) set_k_sobel3x3_u8(const uint8_t* __restrict__ n, uint8_t* __restrict__ e, uint32_t w, uint32_t h) {
+    set_pdl_sync();
+    stencil3x3_u8(n, e, w, h, [](int a, int b, int c, int d, int, int f, int g, int hh, int i) -> uint32_t {
+        const int gx = (c - a) + 2 * (f - d) + (i - g);
+        const int gy = (g - a) + 2 * (hh - b) + (i - c);
+        const int m = abs(gx) + abs(gy);
+        return (uint32_t)(m > 255 ? 255 : m);
+    });
+}
+
+// K18: m = (sum of the 3 x 3 neighbourhood) / 9, integer division (reading S6-3).
+extern "C" __global__ void __launch_bounds__(256) set_k_mean3x3_u8(const uint8_t* __restrict__ e, uint8_t* __restrict__ m, uint32_t w, uint32_t h) {
+    set_pdl_sync();
+    stencil3x3_u8(e, m, w, h, [](int a, int b, int c, int d, int ee, int f, int g, int hh, int i) -> uint32_t {
+        return (uint32_t)(a + b + c + d + ee + f + g + hh + i) / 9u;
+    });
+}
+
+// K19: t = m >= thresh ? 255 : 0 (reading S6-4).  16 pixels per thread: one 128-bit load, one 128-bit store.
+extern "C" __global__ void __launch_bounds__(256) set_k_threshold_u8(const uint8_t* __restrict__ m, uint8_t* __restrict__ t, uint32_t w, uint32_t h,
+                                                                      uint32_t thresh) {
+    set_pdl_sync();
+    const uint32_t npix = w * h;
+    const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
+    const uint32_t th4 = thresh * 0x01010101u;
+    if (p0 + 15 < npix && ((reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(t)) & 15u) == 0) {
+        uint4 v = __ldg(reinterpret_cast<const uint4*>(m + p0));
+        // per-byte unsigned compare: 0xff where m >= thresh
+        v.x = __vcmpgeu4(v.x, th4);
+        v.y = __vcmpgeu4(v.y, th4);
+        v.z = __vcmpgeu4(v.z, th4);
+        v.w = __vcmpgeu4(v.w, th4);
+        *reinterpret_cast<uint4*>(t + p0) = v;
+    } else {
+        for (uint32_t p = p0; p < npix && p < p0 + 16; ++p) t[p] = m[p] >= thresh ? 255 : 0;
+    }
+}
+
+// K20: out = (128 t + 128 n) >> 8 = (t + n) >> 1 per byte (reading S6-5): the halving add without rounding.
+extern "C" __global__ void __launch_bounds__(256) set_k_blend_u8(const uint8_t* __restrict__ t, const uint8_t* __restrict__ n, uint8_t* __restrict__ out,
+                                                                  uint32_t w, uint32_t h) {
+    set_pdl_sync();
+    const uint32_t npix = w * h;
+    const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
+    if (p0 + 15 < npix && ((reinterpret_cast<uintptr_t>(t) | reinterpret_cast<uintptr_t>(n) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0) {
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(t + p0)), b = __ldg(reinterpret_cast<const uint4*>(n + p0));
+        uint4 o;
+        o.x = __vhaddu4(a.x, b.x);
+        o.y = __vhaddu4(a.y, b.y);
+        o.z = __vhaddu4(a.z, b.z);
+        o.w = __vhaddu4(a.w, b.w);
+        *reinterpret_cast<uint4*>(out + p0) = o;
+    } else {
+        for (uint32_t p = p0; p < npix && p < p0 + 16; ++p) out[p] = (uint8_t)(((uint32_t)t[p] + (uint32_t)n[p]) >> 1);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// SSSP.  Device image of a job (mirrors host_in): int32 [V, E, src, 0][row_ptr V+1][col E][w E].
+// out: int32 [dist V][rounds, 0, 0, 0] (mirrors host_out).  scratch: uint32 flags[2][maxV] then ctrl[4] = {changed, round, -, -}.
+// The frontier is a flag per vertex, double-buffered by the parity of the round, so that a round never clears a flag
+// another thread of the same round is setting.  Distances are relaxed IN PLACE with atomicMin: a vertex may pick up a
+// distance lowered earlier in the same round, so the GPU needs at most as many rounds as the oracle's synchronous rounds
+// and ends on the same, unique, distances (reading S5-4).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kSsspInf = 0x7fffffff;
+
+extern "C" __global__ void __launch_bounds__(256) set_k_sssp_init(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
+                                                                  uint32_t max_v) {
+    set_pdl_sync();
+    const uint32_t V = min((uint32_t)img[0], max_v), src = (uint32_t)img[2];
+    uint32_t* f0 = scratch;
+    uint32_t* f1 = scratch + max_v;
+    for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < V; v += gridDim.x * blockDim.x) {
+        out[v] = v == src ? 0 : kSsspInf;
+        f0[v] = v == src ? 1u : 0u;
+        f1[v] = 0u;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 4) {
+        scratch[2 * (size_t)max_v + threadIdx.x] = 0u;  // changed = 0, round = 0
+        out[V + threadIdx.x] = 0;
+    }
+}
+
+extern "C" __global__ void __launch_bounds__(256) set_k_sssp_relax(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
+                                                                   uint32_t max_v) {
+    set_pdl_sync();
+    const uint32_t V = min((uint32_t)img[0], max_v);
+    const int32_t* row_ptr = img + 4;
+    const int32_t* col = row_ptr + V + 1;
+    const int32_t* wgt = col + img[1];
+    uint32_t* ctrl = scratch + 2 * (size_t)max_v;
+    const uint32_t round = ctrl[1];
+    uint32_t* fin = scratch + (round & 1u) * (size_t)max_v;
+    uint32_t* fout = scratch + ((round + 1u) & 1u) * (size_t)max_v;
+    bool any = false;
+    for (uint32_t u = blockIdx.x * blockDim.x + threadIdx.x; u < V; u += gridDim.x * blockDim.x) {
+        if (!fin[u]) continue;
+        fin[u] = 0u;
+        const int32_t du = *reinterpret_cast<volatile int32_t*>(out + u);  // finite: u entered the frontier by getting a distance
+        const int32_t e1 = __ldg(row_ptr + u + 1);
+        for (int32_t e = __ldg(row_ptr + u); e < e1; ++e) {
+            const int32_t v = __ldg(col + e), nd = du + __ldg(wgt + e);
+            if (nd < atomicMin(out + v, nd)) {
+                fout[v] = 1u;
+                any = true;
+            }
+        }
+    }
+    if (any) ctrl[0] = 1u;
+}
+
+// K23: the loop's condition.  One thread: count the round, report it, and keep the WHILE node going while the round
+// just finished lowered some distance (at most V rounds: Bellman-Ford's bound with non-negative weights).
+extern "C" __global__ void set_k_sssp_control(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch, uint32_t max_v,
+                                              cudaGraphConditionalHandle loop) {
+    set_pdl_sync();
+    const uint32_t V = min((uint32_t)img[0], max_v);
+    uint32_t* ctrl = scratch + 2 * (size_t)max_v;
+    const uint32_t changed = ctrl[0], round = ctrl[1] + 1u;
+    ctrl[0] = 0u;
+    ctrl[1] = round;
+    out[V] = (int32_t)round;
+    cudaGraphSetConditional(loop, (changed != 0u && round <= V) ? 1u : 0u);
+}

@@ -30,6 +30,11 @@ set_arg_desc arg_u32(uint32_t v) {
     a.imm = v;
     return a;
 }
+set_arg_desc arg_cond() {
+    set_arg_desc a{};
+    a.kind = SET_ARG_COND;
+    return a;
+}
 set_arg_desc arg_dim(int i) {
     set_arg_desc a{};
     a.kind = SET_ARG_DIM;
@@ -96,6 +101,13 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_SIGNAL: return (const void*)set_k_signal;
         case SET_K_COPY: return (const void*)set_k_copy;
         case SET_K_STAMP: return (const void*)set_k_stamp;
+        case SET_K_SOBEL3X3_U8: return (const void*)set_k_sobel3x3_u8;
+        case SET_K_MEAN3X3_U8: return (const void*)set_k_mean3x3_u8;
+        case SET_K_THRESHOLD_U8: return (const void*)set_k_threshold_u8;
+        case SET_K_BLEND_U8: return (const void*)set_k_blend_u8;
+        case SET_K_SSSP_INIT: return (const void*)set_k_sssp_init;
+        case SET_K_SSSP_RELAX: return (const void*)set_k_sssp_relax;
+        case SET_K_SSSP_CONTROL: return (const void*)set_k_sssp_control;
         default: return nullptr;
     }
 }
@@ -210,6 +222,50 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
                              {arg_buf(1), arg_buf(2), arg_dim(0), arg_dim(1)});
             st[ns++] = stage(SET_K_HIST256_U8, grid_div(scaled(1, WH), kHistPixPerBlock), grid_fixed(1), 256, 1, 0,
                              {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});
+            break;
+        }
+        case 5: {  // SSSP by frontier Bellman-Ford: init -> WHILE { relax -> control }   (readings S5-1..S5-4)
+            uint32_t maxv = P(0, 4096), maxe = P(1, 15 * 4096);
+            if (maxv == 0 || maxe == 0) return SET_ERR_INVALID;
+            const uint64_t head = 16ull + 4ull * (maxv + 1);  // [V, E, src, 0][row_ptr]; then col and w, 8 bytes per edge
+            in_bytes = head + 8ull * maxe;
+            out_bytes = 4ull * maxv + 16;                      // [dist][rounds, 0, 0, 0]
+            bf[0] = buffer(in_bytes);
+            bf[0].h2d_bytes = set_size_expr{head, 8, 0x1, 0};  // dims[0] = E of the job
+            bf[1] = buffer(out_bytes);
+            bf[1].d2h_bytes = fixed(out_bytes);
+            bf[2] = buffer(8ull * maxv + 16);                  // frontier flags [2][maxV], ctrl[4]
+            nb = 3;
+            const set_grid_rule g = grid_fixed((maxv + 255) / 256);
+            st[ns++] = stage(SET_K_SSSP_INIT, g, grid_fixed(1), 256, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
+            st[ns] = stage(SET_K_SSSP_RELAX, g, grid_fixed(1), 256, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
+            st[ns++].flags = SET_STAGE_LOOP_BEGIN;
+            st[ns] = stage(SET_K_SSSP_CONTROL, grid_fixed(1), grid_fixed(1), 1, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv), arg_cond()});
+            st[ns++].flags = SET_STAGE_LOOP_END;
+            break;
+        }
+        case 6: {  // Sobel chain: gray -> sobel -> mean3x3 -> threshold -> blend; dims = {w, h}   (readings S6-1..S6-6)
+            uint32_t mw = P(0, 1920), mh = P(1, 1080), thresh = P(2, 64);
+            if (mw == 0 || mh == 0) return SET_ERR_INVALID;
+            uint64_t maxpix = (uint64_t)mw * mh;
+            in_bytes = 3 * maxpix;
+            out_bytes = maxpix;
+            const uint32_t WH = 0x3;  // dims[0]*dims[1]
+            bf[0] = buffer(3 * maxpix);
+            bf[0].h2d_bytes = scaled(3, WH);
+            bf[1] = buffer(maxpix);  // n: normalised intensity, kept for the blend
+            bf[2] = buffer(maxpix);  // ping
+            bf[3] = buffer(maxpix);  // pong; the blended output ends here
+            bf[3].d2h_bytes = scaled(1, WH);
+            nb = 4;
+            const set_grid_rule gx = grid_div(scaled(1, 0x1), kStencilTileW), gy = grid_div(scaled(1, 0x2), kStencilTileH);
+            const set_grid_rule gp = grid_div(scaled(1, WH), kBytePixPerBlock);
+            st[ns++] = stage(SET_K_RGB2GRAY_U8, grid_div(scaled(1, WH), kGrayPixPerBlock), grid_fixed(1), 256, 1, 0,
+                             {arg_buf(0), arg_buf(1), arg_dim(0), arg_dim(1)});
+            st[ns++] = stage(SET_K_SOBEL3X3_U8, gx, gy, 64, 4, 0, {arg_buf(1), arg_buf(2), arg_dim(0), arg_dim(1)});
+            st[ns++] = stage(SET_K_MEAN3X3_U8, gx, gy, 64, 4, 0, {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});
+            st[ns++] = stage(SET_K_THRESHOLD_U8, gp, grid_fixed(1), 256, 1, 0, {arg_buf(3), arg_buf(2), arg_dim(0), arg_dim(1), arg_u32(thresh)});
+            st[ns++] = stage(SET_K_BLEND_U8, gp, grid_fixed(1), 256, 1, 0, {arg_buf(2), arg_buf(1), arg_buf(3), arg_dim(0), arg_dim(1)});
             break;
         }
         default:

@@ -165,6 +165,10 @@ class Scheduler {
         dispatchers_.clear();
     }
 
+    // Executables that cannot leave their slot (a job graph with a conditional loop is built per slot): a thief may only
+    // use an executable of its OWN slot; if it has none free at this instant it hands the job back to the victim's queue.
+    void set_slot_bound(bool v) { slot_bound_.store(v, std::memory_order_release); }
+
     int slots() const { return b_; }
     int execs_per_slot() const { return epp_; }
     CoreStats& stats() { return stats_; }
@@ -340,12 +344,28 @@ class Scheduler {
     }
 
     // ---- Algorithm 2: LaunchJob -------------------------------------------
-    void launch_job(Prepared p, int w, bool stolen) {
+    // Returns false if the job could not be taken by slot w after all (slot-bound executables): the caller releases w.
+    bool launch_job(Prepared p, int w, bool stolen) {
         uint64_t t0 = now_ns();
         bool pinned = (p.home & kPinnedBit) != 0;
         int exec = p.exec;
         int rc = 0;
-        if (stolen) {
+        if (stolen && slot_bound_.load(std::memory_order_acquire)) {
+            int mine = -1;
+            bool dummy = false;
+            if (pinned || !free_execs_[w].r.try_pop(mine)) {
+                // staged data lives with the victim's executable, or every executable of w is in a submitter's hands right
+                // now: un-steal (there is room: the entry was just popped from that queue; jobs are independent, so order is free)
+                queues_[p.home & ~kPinnedBit].r.push(p);
+                n_queued_.fetch_add(1, std::memory_order_seq_cst);
+                return false;
+            }
+            stats_.steals.fetch_add(1, std::memory_order_relaxed);
+            rc = be_->bind(mine, w, p.job, &dummy);
+            free_execs_[exec / epp_].r.push(exec);
+            space_ec_.notify_all();
+            exec = mine;
+        } else if (stolen) {
             stats_.steals.fetch_add(1, std::memory_order_relaxed);
             int mine = -1;
             bool dummy = false;
@@ -391,6 +411,7 @@ class Scheduler {
             int one = 1;
             if (!flags_ || r.state.compare_exchange_strong(one, 2, std::memory_order_acq_rel)) on_complete(w);
         }
+        return true;
     }
 
     // ---- Algorithm 2: dispatcher main loop ----------------------------------------------
@@ -411,7 +432,11 @@ class Scheduler {
                 bool stolen = false;
                 if (find_job(w, p, stolen)) {
                     n_queued_.fetch_sub(1, std::memory_order_seq_cst);
-                    launch_job(p, w, stolen);
+                    if (!launch_job(p, w, stolen)) {  // slot-bound executables and none of w's free: w goes back to the pool
+                        pool_.push(w);
+                        n_free_.fetch_add(1, std::memory_order_seq_cst);
+                        idle.pause();
+                    }
                 } else {  // Alg. 2 l.7: no job -> the worker goes back to the pool
                     pool_.push(w);
                     n_free_.fetch_add(1, std::memory_order_seq_cst);
@@ -452,6 +477,7 @@ class Scheduler {
     alignas(kCacheLine) std::atomic<int64_t> inflight_{0};
     EventCount work_ec_, space_ec_, done_ec_;
     std::atomic<bool> stop_{false};
+    std::atomic<bool> slot_bound_{false};
     std::atomic<int> err_{0};
     CoreStats stats_;
     std::vector<std::thread> dispatchers_;

@@ -98,16 +98,29 @@ struct set_ctx final : public Backend {
     std::vector<SlotMem> slots;
     std::vector<ExecState> execs;
     std::vector<void*> owned_dev;
-    cudaGraph_t graph = nullptr;
-    std::vector<cudaGraphNode_t> kern_nodes;
-    cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
-    cudaGraphNode_t signal_node = nullptr;     // SET_CB_FLAG_POLL: last node, stores the slot's completion word
-    cudaGraphNode_t host_node = nullptr;       // SET_CB_HOST_NODE: last node, runs Algorithm 3 on the driver's callback thread
+    // One job graph and the handles of its nodes.  Ordinarily there is ONE template, built on slot 0's buffers, and every
+    // executable is instantiated from it and re-bound to its slot node by node.  A graph that holds a conditional node can be
+    // instantiated only ONCE (a second cudaGraphInstantiate returns cudaErrorNotSupported, CUDA 12.9), so a pipeline with a
+    // data-dependent loop (SET_STAGE_LOOP_BEGIN) gets one graph PER EXECUTABLE, built directly on its slot's buffers -- and
+    // its executables never leave their slot.
+    struct NodeSet {
+        cudaGraph_t graph = nullptr;
+        std::vector<cudaGraphNode_t> kern_nodes;
+        cudaGraphNode_t memset_nodes[SET_MAX_BUFFERS] = {}, h2d_nodes[SET_MAX_BUFFERS] = {}, d2h_nodes[SET_MAX_BUFFERS] = {};
+        cudaGraphNode_t signal_node = nullptr;  // SET_CB_FLAG_POLL: last node, stores the slot's completion word
+        cudaGraphNode_t host_node = nullptr;    // SET_CB_HOST_NODE: last node, runs Algorithm 3 on the driver's callback thread
+        cudaGraphNode_t stamp_start_node = nullptr, stamp_end_node = nullptr;
+        cudaGraphNode_t loop_node = nullptr;    // the conditional WHILE node, if the pipeline has a loop
+    };
+    std::vector<NodeSet> nsets;
+    bool slot_graphs = false;                  // the pipeline has a loop: nsets[e] belongs to executable e (slot e / epp)
+    std::vector<char> stage_in_loop;           // per stage: inside the WHILE body
+    bool has_signal = false, has_host_node = false;
+    NodeSet& nodes_of_exec(int exec) { return nsets[slot_graphs ? (size_t)exec : 0]; }
     // set_config.timestamps: per slot one 64-byte line of mapped pinned memory, [0] = %globaltimer at graph start, [1] = at end
     bool stamps = false;
     unsigned long long* ts_host = nullptr;
     unsigned long long* ts_dev = nullptr;
-    cudaGraphNode_t stamp_start_node = nullptr, stamp_end_node = nullptr;
     struct StampRec {
         uint32_t stream;
         uint64_t start, end;
@@ -202,7 +215,7 @@ struct set_ctx final : public Backend {
     int poll() override;
     volatile uint32_t* done_flags() override { return flag_poll ? flags_host : nullptr; }
 
-    int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid);
+    int build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid, unsigned long long cond = 0);
     // SET_K_COPY node parameters for buffer i of `slot`: H2D (host_or_dev = job input) or D2H (job output)
     struct CopyArgs {
         const void* src;
@@ -215,7 +228,7 @@ struct set_ctx final : public Backend {
     int check_sizes(const uint32_t* dims);
     bool is_pinned(const void* p);
     void add_pinned_range(const void* p, size_t n);
-    int build_graph();
+    int build_graph(int slot, int set_index);
     int plain_job(int slot, const JobDesc& job);
     int baseline_submit(const JobDesc& job);
     int baseline_flush();
@@ -231,7 +244,7 @@ struct set_ctx final : public Backend {
 // ---------------------------------------------------------------------------------------------------------
 // kernel arguments: placeholders -> concrete values for (slot, dims)
 // ---------------------------------------------------------------------------------------------------------
-int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid) {
+int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims, ArgPack& ap, dim3& grid, unsigned long long cond) {
     for (int a = 0; a < st.num_args; ++a) {
         const set_arg_desc& d = st.args[a];
         ap.ptrs[a] = ap.store[a];
@@ -251,6 +264,9 @@ int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims
                 break;
             case SET_ARG_DIM:
                 memcpy(ap.store[a], &dims[d.index], 4);
+                break;
+            case SET_ARG_COND:  // cudaGraphConditionalHandle of the enclosing loop (0 outside a job graph)
+                memcpy(ap.store[a], &cond, 8);
                 break;
             case SET_ARG_TMAP2D: {
                 if (!encode_tiled) return fail(SET_ERR_CUDA, "cuTensorMapEncodeTiled entry point unavailable");
@@ -374,65 +390,96 @@ bool set_ctx::is_pinned(const void* p) {
 // ---------------------------------------------------------------------------------------------------------
 static void CUDART_CB set_completion_cb(void* arg);
 
-int set_ctx::build_graph() {
+int set_ctx::build_graph(int slot, int set_index) {
+    NodeSet& g = nsets[(size_t)set_index];
     const uint32_t unit[4] = {1, 1, 1, 1};
     cudaMemcpyKind kin = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     // dependency helper: a programmatic (PDL) edge where both ends are kernel nodes and the pipeline asked for it
-    auto depend = [&](cudaGraphNode_t from, cudaGraphNode_t to, bool programmatic) -> cudaError_t {
-        if (!programmatic) return cudaGraphAddDependencies(graph, &from, &to, 1);
+    auto depend_in = [&](cudaGraph_t gr, cudaGraphNode_t from, cudaGraphNode_t to, bool programmatic) -> cudaError_t {
+        if (!programmatic) return cudaGraphAddDependencies(gr, &from, &to, 1);
         cudaGraphEdgeData ed{};
         ed.from_port = cudaGraphKernelNodePortProgrammatic;
         ed.to_port = 0;
         ed.type = cudaGraphDependencyTypeProgrammatic;
-        return cudaGraphAddDependencies_v2(graph, &from, &to, &ed, 1);
+        return cudaGraphAddDependencies_v2(gr, &from, &to, &ed, 1);
     };
-    CK(cudaGraphCreate(&graph, 0));
+    auto depend = [&](cudaGraphNode_t from, cudaGraphNode_t to, bool programmatic) { return depend_in(g.graph, from, to, programmatic); };
+    CK(cudaGraphCreate(&g.graph, 0));
     std::vector<cudaGraphNode_t> roots;
     std::vector<bool> root_is_kernel;
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
         if (bd.flags & SET_BUF_ZERO) {
             cudaMemsetParams mp{};
-            mp.dst = (char*)slots[0].buf[i] + eval(bd.zero_off, unit);
+            mp.dst = (char*)slots[slot].buf[i] + eval(bd.zero_off, unit);
             mp.elementSize = 1;
             mp.width = eval(bd.zero_bytes, unit);
             mp.height = 1;
             mp.value = 0;
-            CK(cudaGraphAddMemsetNode(&memset_nodes[i], graph, nullptr, 0, &mp));
-            roots.push_back(memset_nodes[i]);
+            CK(cudaGraphAddMemsetNode(&g.memset_nodes[i], g.graph, nullptr, 0, &mp));
+            roots.push_back(g.memset_nodes[i]);
             root_is_kernel.push_back(false);
         }
         if (!expr_is_zero(bd.h2d_bytes)) {
             if (h2d_sm[i]) {
                 CopyArgs ca;
-                copy_params(ca, 0, (int)i, true, ph_in, unit);
-                CK(cudaGraphAddKernelNode(&h2d_nodes[i], graph, nullptr, 0, &ca.kp));
+                copy_params(ca, slot, (int)i, true, ph_in, unit);
+                CK(cudaGraphAddKernelNode(&g.h2d_nodes[i], g.graph, nullptr, 0, &ca.kp));
             } else {
-                CK(cudaGraphAddMemcpyNode1D(&h2d_nodes[i], graph, nullptr, 0, (char*)slots[0].buf[i] + eval(bd.h2d_dev_off, unit),
+                CK(cudaGraphAddMemcpyNode1D(&g.h2d_nodes[i], g.graph, nullptr, 0, (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, unit),
                                             (char*)ph_in + eval(bd.h2d_host_off, unit), eval(bd.h2d_bytes, unit), kin));
             }
-            roots.push_back(h2d_nodes[i]);
+            roots.push_back(g.h2d_nodes[i]);
             root_is_kernel.push_back(h2d_sm[i]);
         }
     }
     if (stamps) {  // a root of its own, beside the first copies: runs when the graph starts, nothing waits for it
-        unsigned long long* p = ts_dev;
+        unsigned long long* p = ts_dev + (size_t)slot * 8;
         void* args[1] = {&p};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void*>(set_builtin_kernel(SET_K_STAMP));
         kp.gridDim = dim3(1);
         kp.blockDim = dim3(1);
         kp.kernelParams = args;
-        CK(cudaGraphAddKernelNode(&stamp_start_node, graph, nullptr, 0, &kp));
+        CK(cudaGraphAddKernelNode(&g.stamp_start_node, g.graph, nullptr, 0, &kp));
     }
-    kern_nodes.resize(stages.size());
-    cudaGraphNode_t prev = nullptr;
+    g.kern_nodes.assign(stages.size(), nullptr);
+    cudaGraphNode_t prev = nullptr;       // last node of the top-level chain
+    cudaGraph_t body = nullptr;           // body graph of the loop being filled, if any
+    cudaGraphNode_t body_prev = nullptr;
+    cudaGraphConditionalHandle cond = 0;
+    // first node of the top-level chain hangs off every root; a kernel may have at most one programmatic predecessor worth
+    // having: use it only for a lone SM-copy root
+    auto attach_top = [&](cudaGraphNode_t node, bool node_is_kernel, bool want_pdl) -> int {
+        if (!prev) {
+            for (size_t r = 0; r < roots.size(); ++r)
+                CK(depend(roots[r], node, node_is_kernel && want_pdl && roots.size() == 1 && root_is_kernel[r]));
+        } else {
+            CK(depend(prev, node, node_is_kernel && want_pdl && prev != g.loop_node));
+        }
+        prev = node;
+        return 0;
+    };
     for (size_t s = 0; s < stages.size(); ++s) {
         const set_stage_desc& st = stages[s];
+        if (st.flags & SET_STAGE_LOOP_BEGIN) {
+            // PAPER.md:220 / SURVEY.md 8(f)4: the iteration count depends on the data, so the stages up to SET_STAGE_LOOP_END
+            // become the body of a conditional WHILE node; the body's control kernel sets the condition on the device.
+            CK(cudaGraphConditionalHandleCreate(&cond, g.graph, 1, cudaGraphCondAssignDefault));
+            cudaGraphNodeParams np{};
+            np.type = cudaGraphNodeTypeConditional;
+            np.conditional.handle = cond;
+            np.conditional.type = cudaGraphCondTypeWhile;
+            np.conditional.size = 1;
+            CK(cudaGraphAddNode(&g.loop_node, g.graph, nullptr, 0, &np));
+            if (int rc = attach_top(g.loop_node, false, false)) return rc;
+            body = np.conditional.phGraph_out[0];
+            body_prev = nullptr;
+        }
         ArgPack ap;
         dim3 grid;
-        if (int rc = build_args(st, 0, unit, ap, grid)) return rc;
+        if (int rc = build_args(st, slot, unit, ap, grid, (unsigned long long)cond)) return rc;
         if (st.smem_bytes > 48 * 1024)
             CK(cudaFuncSetAttribute(st.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st.smem_bytes));
         cudaKernelNodeParams kp{};
@@ -441,31 +488,35 @@ int set_ctx::build_graph() {
         kp.blockDim = dim3(st.block[0], st.block[1] ? st.block[1] : 1, st.block[2] ? st.block[2] : 1);
         kp.sharedMemBytes = st.smem_bytes;
         kp.kernelParams = ap.ptrs;
-        CK(cudaGraphAddKernelNode(&kern_nodes[s], graph, nullptr, 0, &kp));
         const bool want_pdl = (st.flags & SET_STAGE_PDL) != 0;
-        if (s == 0) {
-            // a kernel may have at most one programmatic predecessor worth having: use it only for a lone SM-copy root
-            for (size_t r = 0; r < roots.size(); ++r)
-                CK(depend(roots[r], kern_nodes[s], want_pdl && roots.size() == 1 && root_is_kernel[r]));
+        if (body) {
+            CK(cudaGraphAddKernelNode(&g.kern_nodes[s], body, nullptr, 0, &kp));
+            // always a plain edge inside a loop body: with a programmatic edge between the relaxation and the control kernel
+            // 16 or more concurrent WHILE graphs ended in cudaErrorLaunchFailure on B200 (CUDA 12.9); SET_STAGE_PDL is ignored here
+            if (body_prev) CK(depend_in(body, body_prev, g.kern_nodes[s], false));
+            (void)want_pdl;
+            body_prev = g.kern_nodes[s];
+            if (st.flags & SET_STAGE_LOOP_END) body = nullptr;
         } else {
-            CK(depend(prev, kern_nodes[s], want_pdl));
+            CK(cudaGraphAddKernelNode(&g.kern_nodes[s], g.graph, nullptr, 0, &kp));
+            if (int rc = attach_top(g.kern_nodes[s], true, want_pdl)) return rc;
         }
-        prev = kern_nodes[s];
     }
+    const bool prev_is_kernel = prev != g.loop_node;
     std::vector<cudaGraphNode_t> leaves;
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
         if (!expr_is_zero(bd.d2h_bytes)) {
             if (d2h_sm[i]) {
                 CopyArgs ca;
-                copy_params(ca, 0, (int)i, false, ph_out, unit);
-                CK(cudaGraphAddKernelNode(&d2h_nodes[i], graph, nullptr, 0, &ca.kp));
-                CK(depend(prev, d2h_nodes[i], pdl));
+                copy_params(ca, slot, (int)i, false, ph_out, unit);
+                CK(cudaGraphAddKernelNode(&g.d2h_nodes[i], g.graph, nullptr, 0, &ca.kp));
+                CK(depend(prev, g.d2h_nodes[i], pdl && prev_is_kernel));
             } else {
-                CK(cudaGraphAddMemcpyNode1D(&d2h_nodes[i], graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
-                                            (char*)slots[0].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
+                CK(cudaGraphAddMemcpyNode1D(&g.d2h_nodes[i], g.graph, &prev, 1, (char*)ph_out + eval(bd.d2h_host_off, unit),
+                                            (char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, unit), eval(bd.d2h_bytes, unit), kout));
             }
-            leaves.push_back(d2h_nodes[i]);
+            leaves.push_back(g.d2h_nodes[i]);
         }
     }
     if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished (kernels.cu K14)
@@ -474,10 +525,10 @@ int set_ctx::build_graph() {
             if (!expr_is_zero(bufs[i].d2h_bytes)) leaf_is_kernel.push_back(d2h_sm[i]);
         if (leaves.empty()) {
             leaves.push_back(prev);
-            leaf_is_kernel.push_back(true);
+            leaf_is_kernel.push_back(prev_is_kernel);
         }
-        uint32_t* flag = flags_dev;
-        unsigned long long* stamp = stamps ? ts_dev + 1 : nullptr;
+        uint32_t* flag = flags_dev + (size_t)slot * kFlagStride;
+        unsigned long long* stamp = stamps ? ts_dev + (size_t)slot * 8 + 1 : nullptr;
         uint32_t fence = cfg.completion_fence == SET_FENCE_SYSTEM ? 1u : 0u;
         void* args[3] = {&flag, &stamp, &fence};
         cudaKernelNodeParams kp{};
@@ -485,29 +536,31 @@ int set_ctx::build_graph() {
         kp.gridDim = dim3(1);
         kp.blockDim = dim3(1);
         kp.kernelParams = args;
-        CK(cudaGraphAddKernelNode(&signal_node, graph, nullptr, 0, &kp));
-        for (size_t l = 0; l < leaves.size(); ++l) CK(depend(leaves[l], signal_node, pdl && leaves.size() == 1 && leaf_is_kernel[l]));
+        CK(cudaGraphAddKernelNode(&g.signal_node, g.graph, nullptr, 0, &kp));
+        for (size_t l = 0; l < leaves.size(); ++l) CK(depend(leaves[l], g.signal_node, pdl && leaves.size() == 1 && leaf_is_kernel[l]));
         // the start stamp is a root nothing else waits for; this edge only makes sure it has run before the end stamp
-        if (stamps) CK(depend(stamp_start_node, signal_node, false));
+        if (stamps) CK(depend(g.stamp_start_node, g.signal_node, false));
+        has_signal = true;
     } else if (stamps) {  // no signal node in this mode: the end timestamp gets a last node of its own
         if (leaves.empty()) leaves.push_back(prev);
-        unsigned long long* p = ts_dev + 1;
+        unsigned long long* p = ts_dev + (size_t)slot * 8 + 1;
         void* args[1] = {&p};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void*>(set_builtin_kernel(SET_K_STAMP));
         kp.gridDim = dim3(1);
         kp.blockDim = dim3(1);
         kp.kernelParams = args;
-        leaves.push_back(stamp_start_node);  // not on the critical path: it only has to have run before the end stamp
-        CK(cudaGraphAddKernelNode(&stamp_end_node, graph, leaves.data(), leaves.size(), &kp));
-        leaves.assign(1, stamp_end_node);
+        leaves.push_back(g.stamp_start_node);  // not on the critical path: it only has to have run before the end stamp
+        CK(cudaGraphAddKernelNode(&g.stamp_end_node, g.graph, leaves.data(), leaves.size(), &kp));
+        leaves.assign(1, g.stamp_end_node);
     }
     if (cfg.mode == SET_MODE_SET && cfg.callback_mode == SET_CB_HOST_NODE) {
         if (leaves.empty()) leaves.push_back(prev);
         cudaHostNodeParams hp{};
         hp.fn = set_completion_cb;
-        hp.userData = &cbargs[0];
-        CK(cudaGraphAddHostNode(&host_node, graph, leaves.data(), leaves.size(), &hp));
+        hp.userData = &cbargs[slot];
+        CK(cudaGraphAddHostNode(&g.host_node, g.graph, leaves.data(), leaves.size(), &hp));
+        has_host_node = true;
     }
     return 0;
 }
@@ -523,8 +576,11 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
     std::unique_lock<std::mutex> dl(driver_mu, std::defer_lock);
     if (driver_lock) dl.lock();
     ExecState& es = execs[exec];
+    NodeSet& g = nodes_of_exec(exec);
     bool dims_changed = memcmp(es.dims, job.dims, sizeof(es.dims)) != 0;
     bool full = es.bound_slot != slot || dims_changed;
+    if (slot_graphs && es.bound_slot != slot)
+        return fail(SET_ERR_STATE, "an executable of a pipeline with a loop cannot move from slot %d to slot %d", es.bound_slot, slot);
     if (dims_changed)
         if (int rc = check_sizes(job.dims)) return rc;
 
@@ -566,6 +622,8 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
     cudaMemcpyKind kout = cfg.io == SET_IO_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (full) {
         for (size_t s = 0; s < stages.size(); ++s) {
+            // nodes inside a loop body cannot be re-pointed one by one; register made sure they do not depend on the job
+            if (slot_graphs && stage_in_loop[s]) continue;
             ArgPack ap;
             dim3 grid;
             if (int rc = build_args(stages[s], slot, job.dims, ap, grid)) return rc;
@@ -576,7 +634,7 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
                                stages[s].block[2] ? stages[s].block[2] : 1);
             kp.sharedMemBytes = stages[s].smem_bytes;
             kp.kernelParams = ap.ptrs;
-            CK(cudaGraphExecKernelNodeSetParams(es.exec, kern_nodes[s], &kp));
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, g.kern_nodes[s], &kp));
         }
         for (size_t i = 0; i < bufs.size(); ++i)
             if (bufs[i].flags & SET_BUF_ZERO) {
@@ -585,9 +643,9 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
                 mp.elementSize = 1;
                 mp.width = eval(bufs[i].zero_bytes, job.dims);
                 mp.height = 1;
-                CK(cudaGraphExecMemsetNodeSetParams(es.exec, memset_nodes[i], &mp));
+                CK(cudaGraphExecMemsetNodeSetParams(es.exec, g.memset_nodes[i], &mp));
             }
-        if (signal_node && es.bound_slot != slot) {
+        if (g.signal_node && es.bound_slot != slot) {
             uint32_t* flag = flags_dev + (size_t)slot * kFlagStride;
             unsigned long long* stamp = stamps ? ts_dev + (size_t)slot * 8 + 1 : nullptr;
             uint32_t fence = cfg.completion_fence == SET_FENCE_SYSTEM ? 1u : 0u;
@@ -597,7 +655,7 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             kp.gridDim = dim3(1);
             kp.blockDim = dim3(1);
             kp.kernelParams = args;
-            CK(cudaGraphExecKernelNodeSetParams(es.exec, signal_node, &kp));
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, g.signal_node, &kp));
         }
         if (stamps && es.bound_slot != slot) {
             unsigned long long* p0 = ts_dev + (size_t)slot * 8;
@@ -608,18 +666,18 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             kp.blockDim = dim3(1);
             void* a0[1] = {&p0};
             kp.kernelParams = a0;
-            CK(cudaGraphExecKernelNodeSetParams(es.exec, stamp_start_node, &kp));
-            if (stamp_end_node) {
+            CK(cudaGraphExecKernelNodeSetParams(es.exec, g.stamp_start_node, &kp));
+            if (g.stamp_end_node) {
                 void* a1[1] = {&p1};
                 kp.kernelParams = a1;
-                CK(cudaGraphExecKernelNodeSetParams(es.exec, stamp_end_node, &kp));
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, g.stamp_end_node, &kp));
             }
         }
-        if (host_node && es.bound_slot != slot) {
+        if (g.host_node && es.bound_slot != slot) {
             cudaHostNodeParams hp{};
             hp.fn = set_completion_cb;
             hp.userData = &cbargs[slot];
-            CK(cudaGraphExecHostNodeSetParams(es.exec, host_node, &hp));
+            CK(cudaGraphExecHostNodeSetParams(es.exec, g.host_node, &hp));
         }
         full_rebinds.fetch_add(1, std::memory_order_relaxed);
     } else {
@@ -631,9 +689,9 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             if (h2d_sm[i]) {
                 CopyArgs ca;
                 copy_params(ca, slot, (int)i, true, in, job.dims);
-                CK(cudaGraphExecKernelNodeSetParams(es.exec, h2d_nodes[i], &ca.kp));
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, g.h2d_nodes[i], &ca.kp));
             } else {
-                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
+                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, g.h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
                                                       (const char*)in + eval(bd.h2d_host_off, job.dims), eval(bd.h2d_bytes, job.dims), kin));
             }
         }
@@ -641,9 +699,9 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
             if (d2h_sm[i]) {
                 CopyArgs ca;
                 copy_params(ca, slot, (int)i, false, out, job.dims);
-                CK(cudaGraphExecKernelNodeSetParams(es.exec, d2h_nodes[i], &ca.kp));
+                CK(cudaGraphExecKernelNodeSetParams(es.exec, g.d2h_nodes[i], &ca.kp));
             } else {
-                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, d2h_nodes[i], (char*)out + eval(bd.d2h_host_off, job.dims),
+                CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, g.d2h_nodes[i], (char*)out + eval(bd.d2h_host_off, job.dims),
                                                       (char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, job.dims), eval(bd.d2h_bytes, job.dims), kout));
             }
         }
@@ -675,7 +733,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     SpinLock& lk = stream_locks[s];
     lk.lock();
     cudaError_t e = cudaGraphLaunch(execs[exec].exec, streams[s]);
-    if (e == cudaSuccess && !flag_poll && !host_node) {
+    if (e == cudaSuccess && !flag_poll && !has_host_node) {
         if (cfg.callback_mode == SET_CB_WORK_STREAM) {
             e = cudaLaunchHostFunc(streams[s], set_completion_cb, &cbargs[slot]);
         } else {
@@ -688,7 +746,7 @@ int set_ctx::launch(int exec, int slot, const JobDesc&) {
     if (e != cudaSuccess) return cuda_fail(e, "graph launch / event chain", __LINE__);
     kernel_nodes.fetch_add(stages.size(), std::memory_order_relaxed);
     if (n_sm_copies) copy_nodes.fetch_add((uint64_t)n_sm_copies, std::memory_order_relaxed);
-    if (signal_node) signal_nodes.fetch_add(1, std::memory_order_relaxed);
+    if (has_signal) signal_nodes.fetch_add(1, std::memory_order_relaxed);
     return 0;
 }
 
@@ -1102,10 +1160,38 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
         if ((uint64_t)st.block[0] * (st.block[1] ? st.block[1] : 1) * (st.block[2] ? st.block[2] : 1) > 1024) return SET_ERR_INVALID;
         for (int a = 0; a < st.num_args; ++a) {
             const set_arg_desc& d = st.args[a];
-            if (d.kind < SET_ARG_BUFFER || d.kind > SET_ARG_TMAP2D) return SET_ERR_INVALID;
+            if (d.kind < SET_ARG_BUFFER || d.kind > SET_ARG_COND) return SET_ERR_INVALID;
             if ((d.kind == SET_ARG_BUFFER || d.kind == SET_ARG_TMAP2D) && (d.index < 0 || d.index >= num_bufs)) return SET_ERR_INVALID;
             if (d.kind == SET_ARG_DIM && (d.index < 0 || d.index >= SET_MAX_DIMS)) return SET_ERR_INVALID;
         }
+    }
+    {  // loop structure (set.h SET_STAGE_LOOP_BEGIN): at most one loop, properly closed; a loop pipeline is bound to its
+       // slot, so no kernel of it may depend on the job's dims; SET_ARG_COND only inside the loop
+        bool any_loop = false, in_loop = false, closed = false;
+        for (int s = 0; s < num_stages; ++s) any_loop = any_loop || (stages[s].flags & SET_STAGE_LOOP_BEGIN);
+        for (int s = 0; s < num_stages; ++s) {
+            const set_stage_desc& st = stages[s];
+            if (st.flags & SET_STAGE_LOOP_BEGIN) {
+                if (in_loop || closed) return SET_ERR_INVALID;
+                in_loop = true;
+            }
+            auto dim_free = [](const set_size_expr& e) { return e.per_unit == 0 || e.dim_mask == 0; };
+            for (int a = 0; a < st.num_args; ++a) {
+                const set_arg_desc& d = st.args[a];
+                if (d.kind == SET_ARG_COND && !in_loop) return SET_ERR_INVALID;
+                if (in_loop && (d.kind == SET_ARG_DIM || !dim_free(d.offset))) return SET_ERR_INVALID;
+            }
+            if (in_loop)
+                for (int k = 0; k < 3; ++k)
+                    if (!dim_free(st.grid[k].count)) return SET_ERR_INVALID;
+            if (st.flags & SET_STAGE_LOOP_END) {
+                if (!in_loop) return SET_ERR_INVALID;
+                in_loop = false;
+                closed = true;
+            }
+        }
+        if (in_loop) return SET_ERR_INVALID;
+        if (any_loop && c->cfg.mode == SET_MODE_SET && c->cfg.steal_policy == SET_STEAL_RETARGET) return SET_ERR_INVALID;
     }
     for (int i = 0; i < num_bufs; ++i) {
         if (bufs[i].bytes == 0) return SET_ERR_INVALID;
@@ -1182,7 +1268,21 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
         }
         for (auto& st : c->stages) c->pdl = c->pdl || (st.flags & SET_STAGE_PDL);
     }
-    if (int rc = c->build_graph()) return rc;
+    {
+        bool in_loop = false;
+        for (auto& st : c->stages) {
+            c->slot_graphs = c->slot_graphs || (st.flags & SET_STAGE_LOOP_BEGIN);
+            in_loop = in_loop || (st.flags & SET_STAGE_LOOP_BEGIN);
+            c->stage_in_loop.push_back(in_loop ? 1 : 0);
+            if (st.flags & SET_STAGE_LOOP_END) in_loop = false;
+        }
+    }
+    if (c->slot_graphs && c->cfg.mode == SET_MODE_PLAIN_STREAMS)
+        return c->fail(SET_ERR_INVALID, "a pipeline with a loop needs a job graph: SET_MODE_PLAIN_STREAMS cannot run it");
+    if (c->slot_graphs && c->sched) c->sched->set_slot_bound(true);
+    c->nsets.resize(c->slot_graphs ? (size_t)c->b * c->epp : 1);
+    if (!c->slot_graphs)
+        if (int rc = c->build_graph(0, 0)) return rc;
 
     // ---- bounded pool of graph executables: q+1 per slot, each re-bound to its slot's M_w
     int nexec = c->b * c->epp;
@@ -1191,13 +1291,15 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
         bool needed = c->cfg.mode == SET_MODE_SET || (e % c->epp == 0);
         if (c->cfg.mode == SET_MODE_PLAIN_STREAMS) needed = false;
         if (!needed) continue;
-        cudaError_t er = cudaGraphInstantiate(&c->execs[e].exec, c->graph, 0);
+        int slot = e / c->epp;
+        if (c->slot_graphs)
+            if (int rc = c->build_graph(slot, e)) return rc;
+        cudaError_t er = cudaGraphInstantiate(&c->execs[e].exec, c->nodes_of_exec(e).graph, 0);
         if (er != cudaSuccess) return c->cuda_fail(er, "cudaGraphInstantiate", __LINE__);
-        c->execs[e].bound_slot = 0;  // the template was built on slot 0's buffers
+        c->execs[e].bound_slot = c->slot_graphs ? slot : 0;  // the template was built on slot 0's buffers (or on this slot's)
         c->execs[e].in = c->ph_in;
         c->execs[e].out = c->ph_out;
-        int slot = e / c->epp;
-        if (slot != 0) {
+        if (slot != 0 && !c->slot_graphs) {
             JobDesc j;
             j.in = c->ph_in;
             j.out = c->ph_out;
@@ -1271,7 +1373,8 @@ set_status set_destroy(set_ctx* c) {
         if (es.stage_in) cudaFreeHost(es.stage_in);
         if (es.stage_out) cudaFreeHost(es.stage_out);
     }
-    if (c->graph) cudaGraphDestroy(c->graph);
+    for (auto& ns : c->nsets)
+        if (ns.graph) cudaGraphDestroy(ns.graph);
     for (auto& sm : c->slots) {
         if (sm.done) cudaEventDestroy(sm.done);
         if (sm.t0) cudaEventDestroy(sm.t0);
@@ -1490,6 +1593,8 @@ set_status set_time_stage(set_ctx* c, int stage, const uint32_t* dims, int warmu
     if (!dims) dims = unit;
     if (c->check_sizes(dims)) return SET_ERR_SIZE;
     const set_stage_desc& sd = c->stages[stage];
+    for (int a = 0; a < sd.num_args; ++a)
+        if (sd.args[a].kind == SET_ARG_COND) return SET_ERR_INVALID;  // a loop's control kernel means nothing outside its WHILE node
     ArgPack ap;
     dim3 grid;
     if (int rc = c->build_args(sd, 0, dims, ap, grid)) return rc;

@@ -29,9 +29,11 @@ class Workload:
 
     # ---- per-job host images
     def dims(self, job_id: int):
-        if self.config == 4:
+        if self.config in (4, 6):
             w, h = inputgen.config4_size(job_id) if "size" not in self.extra else self.extra["size"]
             return (w, h, 1, 1)
+        if self.config == 5:  # dims[0] = E of the job's graph (the copy-in size depends on it)
+            return (inputgen.sssp_edges(job_id, self.params[0], self.extra.get("mean_deg", 8)), 1, 1, 1)
         return (1, 1, 1, 1)
 
     def in_bytes(self, dims=None) -> int:
@@ -40,7 +42,8 @@ class Workload:
         if c == 1: return 8 * p[0]
         if c == 2: return 4 * p[0] * p[1]
         if c == 3: return 2 * p[0] * p[2] + 2 * p[2] * p[1] + 4 * p[1]
-        if c == 4: return 3 * dims[0] * dims[1]
+        if c in (4, 6): return 3 * dims[0] * dims[1]
+        if c == 5: return 16 + 4 * (p[0] + 1) + 8 * dims[0]
         raise ValueError(c)
 
     def out_bytes(self, dims=None) -> int:
@@ -50,6 +53,8 @@ class Workload:
         if c == 2: return 4 * p[0] * p[1]
         if c == 3: return 2 * p[0] * p[1]
         if c == 4: return dims[0] * dims[1] + 1024
+        if c == 5: return 4 * p[0] + 16
+        if c == 6: return dims[0] * dims[1]
         raise ValueError(c)
 
     def make_input(self, job_id: int) -> np.ndarray:
@@ -62,6 +67,10 @@ class Workload:
         if c == 4:
             d = self.dims(job_id)
             return inputgen.config4_job(job_id, (d[0], d[1])).reshape(-1)
+        if c == 5: return inputgen.sssp_job(job_id, p[0], self.extra.get("mean_deg", 8)).view(np.uint8)
+        if c == 6:
+            d = self.dims(job_id)
+            return inputgen.sobel_frame(job_id, (d[0], d[1])).reshape(-1)
         raise ValueError(c)
 
 
@@ -82,6 +91,13 @@ def baseline_workload(config: int) -> Workload:
     if config == 4:
         return Workload(4, (1920, 1080), jobs=4096, num_streams=8, max_inflight=32,
                         name="config4 RGB frames gray->blur->hist256, jittered sizes (4096 jobs)", dtype="u8", kernels_per_job=3)
+    if config == 5:  # paper workload 6; SURVEY.md 8(f)4
+        return Workload(5, (4096, inputgen.sssp_max_edges(4096, 8)), jobs=2048, num_streams=8, max_inflight=32,
+                        name="config5 SSSP frontier Bellman-Ford, 4096 vertices, mean out-degree 8, WHILE node (2048 jobs)", dtype="int32",
+                        kernels_per_job=3, extra={"mean_deg": 8})
+    if config == 6:  # paper workload 1; SURVEY.md 8(f)4
+        return Workload(6, (1920, 1080), jobs=4096, num_streams=8, max_inflight=32,
+                        name="config6 Sobel chain gray->sobel->mean->threshold->blend, jittered sizes (4096 jobs)", dtype="u8", kernels_per_job=5)
     raise ValueError(config)
 
 
@@ -92,6 +108,8 @@ def small_workload(config: int) -> Workload:
     if config == 2: return Workload(2, (300, 2052, 10), jobs=12, num_streams=4, max_inflight=8, dtype="f32", kernels_per_job=10)
     if config == 3: return Workload(3, (384, 512, 256), jobs=8, num_streams=4, max_inflight=8, dtype="bf16", kernels_per_job=1)
     if config == 4: return Workload(4, (1920, 1080), jobs=48, num_streams=8, max_inflight=32, dtype="u8", kernels_per_job=3)
+    if config == 5: return Workload(5, (1000, inputgen.sssp_max_edges(1000, 4)), jobs=48, num_streams=4, max_inflight=8, dtype="int32", kernels_per_job=3, extra={"mean_deg": 4})
+    if config == 6: return Workload(6, (1920, 1080), jobs=48, num_streams=8, max_inflight=32, dtype="u8", kernels_per_job=5)
     raise ValueError(config)
 
 
