@@ -350,6 +350,8 @@ typedef struct set_gap_stats {
                                GPU had at least one job in progress                                  */
     double idle_frac;       /* 1 - busy_union_us / span_us: the timeline's white space, the
                                t_schedule / T_measured of PAPER.md:81-90, :253 under reading S12, at job granularity */
+    double idle_gaps;       /* number of intervals inside the span during which NO job was in progress on any stream */
+    double idle_gap_mean_us;/* their mean length: the device-wide gap between jobs (0 if there is none)             */
 } set_gap_stats;
 set_status set_get_gap_stats(set_ctx *ctx, set_gap_stats *out);
 

@@ -24,8 +24,9 @@
 extern "C" {
 #endif
 
-/* A gap is  start(next op) - end(previous op)  between two operations that are CONSECUTIVE ON ONE STREAM
- * (ordered by start time); negative values (overlapping copies and kernels of one graph) count as 0. */
+/* Records are grouped into JOBS by the correlation id of their cudaGraphLaunch (CUPTI gives the parallel branches of a job
+ * graph stream ids of their own, so the id is no guide to which work stream an operation belongs to); a job's work stream
+ * is the id most of its kernels ran under.  Gaps are in microseconds. */
 typedef struct set_gap_summary {
     uint64_t count;
     double mean_us, p50_us, p99_us, max_us;
@@ -35,18 +36,21 @@ typedef struct set_trace_stats {
     uint64_t kernels;          /* kernel records (completion-signal kernels included)                  */
     uint64_t signal_kernels;   /* of those, set_k_signal (SET_CB_FLAG_POLL's one-thread end node)      */
     uint64_t memcpys, memsets;
-    uint64_t streams;          /* distinct streams seen                                                */
+    uint64_t streams;          /* distinct work streams (see above)                                    */
     uint64_t dropped;          /* records CUPTI reported as dropped                                    */
+    uint64_t jobs;             /* distinct correlation ids                                             */
+    uint64_t kernel_kernel_overlapped; /* kernel_kernel gaps that are negative (PDL overlap)           */
     double wall_us;            /* T: last end - first start over all records                           */
     double busy_us;            /* |union of activity intervals| over all streams                       */
     double idle_frac;          /* t_schedule / T = 1 - busy/wall                                       */
     double kernel_mean_us;     /* mean duration of the stage kernels (signal kernels excluded)         */
     double sum_op_us;          /* sum of all op durations (> busy_us when streams overlap)             */
-    set_gap_summary kernel_kernel; /* stage kernel -> next stage kernel of the SAME job, nothing else between them:
-                                      the "inter-kernel gap" of BASELINE.json:metric                   */
-    set_gap_summary intra_job; /* consecutive ops of ONE job (same launch correlation id)              */
-    set_gap_summary inter_job; /* last op of a job -> first op of the next job on that stream          */
-    set_gap_summary any_op;    /* every consecutive pair                                               */
+    set_gap_summary kernel_kernel; /* stage kernel -> next stage kernel of the SAME job with no copy or memset between them,
+                                      start(next) - end(previous), SIGNED: negative when a programmatic edge lets the next
+                                      kernel start early.  The "inter-kernel gap" of BASELINE.json:metric.              */
+    set_gap_summary intra_job; /* consecutive ops of ONE job in start order: start(next) - latest end so far, >= 0      */
+    set_gap_summary inter_job; /* end of a job (its last op) -> start of the next job on the same work stream, >= 0     */
+    set_gap_summary any_op;    /* every consecutive pair under one CUPTI stream id, >= 0 (the raw view)                 */
 } set_trace_stats;
 
 /* Enable kernel / memcpy / memset activity collection for the process.  Records accumulate in host

@@ -91,7 +91,8 @@ class Stats(C.Structure):
 class GapStats(C.Structure):
     _fields_ = [("jobs", C.c_uint64), ("gaps", C.c_uint64), ("gap_mean_us", C.c_double), ("gap_p50_us", C.c_double),
                 ("gap_p99_us", C.c_double), ("gap_max_us", C.c_double), ("job_mean_us", C.c_double), ("span_us", C.c_double),
-                ("stream_busy_frac", C.c_double), ("busy_union_us", C.c_double), ("idle_frac", C.c_double)]
+                ("stream_busy_frac", C.c_double), ("busy_union_us", C.c_double), ("idle_frac", C.c_double),
+                ("idle_gaps", C.c_double), ("idle_gap_mean_us", C.c_double)]
 
     def as_dict(self):
         return {n: (int(getattr(self, n)) if n in ("jobs", "gaps") else round(float(getattr(self, n)), 4)) for n, _ in self._fields_}

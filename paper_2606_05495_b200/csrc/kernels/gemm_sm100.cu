@@ -14,11 +14,15 @@
 //   D : fp32, rows 128 r .. 128 r + 127 of the pair's tile x 256 columns = 256 TMEM columns x 128 lanes in CTA r
 //
 // Grid = (2 * ceil(M / 256), ceil(N / 256)), cluster (2, 1, 1): blockIdx.x >> 1 is the pair's row block, %cluster_ctarank
-// the CTA's rank r.  Warp roles (320 threads): warp 0 = TMA producer (both CTAs, each for its own halves, all signalling the
+// the CTA's rank r.  Warp roles (576 threads): warp 0 = TMA producer (both CTAs, each for its own halves, all signalling the
 // LEADER's "full" barrier), warp 1 = TMEM allocator (both CTAs) + MMA issuer (leader only; tcgen05.commit multicasts the
-// "stage empty" / "accumulator full" arrivals to both CTAs), warps 2..9 = epilogue (warp w may only touch TMEM lanes
-// 32*(w%4) .. 32*(w%4)+31; two warps share each lane quarter and split the 256 columns).  The epilogue writes bf16 rows into
-// 128-byte-swizzled shared memory and hands each 32 x 64 piece to the TMA unit (cp.async.bulk.tensor store).
+// "stage empty" / "accumulator full" arrivals to both CTAs), warps 2..17 = epilogue (warp w may only touch TMEM lanes
+// 32*(w%4) .. 32*(w%4)+31; four warps share each lane quarter and take 64 of the 256 columns each).  The epilogue stages the
+// tile's bias values in shared memory while the main loop runs, then per 32-column round: tcgen05.ld (the next round's load
+// already in flight), packed-f32x2 bias + GELU, bf16 rows into 64-byte-swizzled shared memory, and the 32 x 32 box goes to the
+// TMA unit at once (cp.async.bulk.tensor store) so that it drains under the next round's arithmetic.
+// What was measured on B200 at 2048^3 (one wave of 64 pairs on 74 TPCs; profiles/r2_k9.md): kernel entry -> first MMA 0.6 us,
+// main loop 10.0 us (L2-bound: 128 MB at ~12.8 TB/s; the MMAs alone need 8.3 us), epilogue 3.2 us, kernel-to-kernel 1.9 us.
 // Ragged shapes: TMA zero-fills out-of-bounds rows/columns of a load box, so partial tiles in M, N and K contribute
 // zeros, and clips a store box to the matrix (N and K must be multiples of 8: 16-byte TMA pitches); a box that starts
 // outside the matrix is never requested (its accumulator rows / columns are never stored).
@@ -30,10 +34,7 @@ namespace {
 
 constexpr uint32_t kBlockM = 128, kBlockN = 256, kBlockK = 64, kUmmaK = 16;  // per CTA: 128 rows of the pair's 256 x 256 tile
 constexpr uint32_t kPairM = 2 * kBlockM, kHalfN = kBlockN / 2;
-#ifndef PROBE_STAGES
-#define PROBE_STAGES 6
-#endif
-constexpr uint32_t kStages = PROBE_STAGES;
+constexpr uint32_t kStages = 6;
 constexpr uint32_t kABytes = kBlockM * kBlockK * 2;          // 16 KiB
 constexpr uint32_t kBBoxN = 64;                              // one 128-byte swizzle atom of N per box
 constexpr uint32_t kBBoxBytes = kBBoxN * kBlockK * 2;        // 8 KiB
@@ -187,13 +188,6 @@ __device__ __forceinline__ float2 gelu_erf2(float2 z) {
 
 }  // namespace
 
-#ifdef PROBE_STAMPS
-__device__ unsigned long long g_stamps[64 * 8];
-__device__ unsigned int g_stamp_launch;
-#define STAMP(i) do { if (threadIdx.x == (i == 3 || i == 4 ? 64u : 0u) && blockIdx.x == 0 && blockIdx.y == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_stamps[(stamp_launch % 64) * 8 + i] = t_; } } while (0)
-#else
-#define STAMP(i)
-#endif
 extern "C" uint32_t set_gemm_smem_bytes(void) { return kSmemBytes; }
 extern "C" uint32_t set_gemm_threads(void) { return kThreads; }
 
@@ -201,13 +195,6 @@ extern "C" __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads,
 set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                           const __grid_constant__ CUtensorMap tmC, const float* __restrict__ bias, uint32_t M, uint32_t N, uint32_t K) {
     extern __shared__ uint8_t smem_raw[];
-#ifdef PROBE_STAMPS
-    __shared__ unsigned int stamp_launch_s;
-    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0) stamp_launch_s = atomicAdd(&g_stamp_launch, 1u);
-    __syncthreads();
-    const unsigned int stamp_launch = stamp_launch_s;
-    STAMP(0);
-#endif
     // Both CTAs of the pair must carve shared memory identically: the MMA reads the peer's operand tiles at the leader's
     // offsets and tcgen05.commit signals the peer's barriers at the leader's offsets.  The dynamic shared memory base is
     // the same in every CTA of a launch, so the same rounding gives the same offsets.
@@ -270,7 +257,6 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
     }
-    STAMP(1);
 
     if (warp == 0) {
         // ===== TMA producer: every CTA stages its own halves; all bytes are counted on the leader's barrier =====
@@ -279,10 +265,6 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 const uint32_t s = kb % kStages, round = kb / kStages;
                 mbar_wait(empty_bar(s), (round & 1u) ^ 1u);  // first pass over the ring falls through
                 const uint32_t lead_full = map_to_cta(full_bar(s), 0);
-#ifdef PROBE_SKIP_TMA
-                if (rank == 0) mbar_expect_tx(full_bar(s), 0); else mbar_arrive_cluster(lead_full);
-                continue;
-#endif
                 if (rank == 0)
                     mbar_expect_tx(full_bar(s), pair_tx);
                 else
@@ -306,11 +288,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                     const uint64_t adesc = smem_desc(a_tile(s) + k * kUmmaK * 2u, 16u, 1024u);
                     // B: 16 K-rows = two 8-row groups = 2048 bytes further; the next 64 columns are one box on
                     const uint64_t bdesc = smem_desc(b_tile(s) + k * kUmmaK * 128u, kBBoxBytes, 1024u);
-#ifndef PROBE_SKIP_MMA
                     umma_bf16(tmem_base, adesc, bdesc, (kb | k) != 0u);
-#else
-                    (void)adesc; (void)bdesc;
-#endif
                 }
                 umma_commit_pair(empty_bar(s));  // both CTAs may refill the stage once these MMAs have read it
             }
@@ -334,7 +312,6 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
             asm volatile("bar.sync 1, %0;" ::"n"(kEpiWarps * 32) : "memory");  // named barrier: the epilogue warps only
         }
         mbar_wait(accum_bar, 0);
-        STAMP(3);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // Sixteen warps: warp w reads TMEM lane quarter q = w % 4 (the only lanes it may touch) and column group cg = (w - 2) / 4,
         // i.e. a 32-row x 64-column piece of the tile = one TMA store box of 4 KiB.  The operand ring is idle once accum_bar
@@ -342,9 +319,6 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         // ~20 instructions per pair of elements: with eight warps the schedulers issued 15 % of the time (ncu), hence sixteen.
         const uint32_t q = warp & 3u, cg = (warp - 2u) >> 2;
         const uint32_t box0 = base + (cg * 4u + q) * 2u * kCBoxBytes;  // this warp's two store boxes
-#ifdef PROBE_SKIP_EPI
-        if (M) goto epi_done;
-#endif
         // Two rounds of 32 columns; the TMEM load of the second is issued before the first is computed.
         if (m0 + q * 32u < M && n0 + cg * 64u < N) {  // warp-uniform: something of this box lies inside the matrix
             const uint32_t trow = tmem_base + ((q * 32u) << 16) + cg * 64u;
@@ -358,11 +332,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 const uint32_t (&v)[32] = r ? vb : va;
                 const uint32_t box = box0 + r * kCBoxBytes;
                 const uint32_t srow = box + lane * 64u;  // this lane's 64-byte row of the box
-#ifdef PROBE_SKIP_MATH
-                if (n0 + c0 < N && M == 1) {
-#else
                 if (n0 + c0 < N) {  // warp-uniform; N is a multiple of 8, so an 8-column chunk is inside or outside as a whole
-#endif
 #pragma unroll
                     for (uint32_t g = 0; g < 4; ++g) {  // 8 columns -> one 16-byte chunk
                         float4 b0, b1;  // bias of columns c0 + 8g .. + 7 (a broadcast read: every lane reads the same address)
@@ -385,11 +355,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                     // tile's 64 KiB) drains while the second round is computed.
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the TMA engine
                     __syncwarp();
-#ifndef PROBE_SKIP_STORE
                     if (lane == 0) {  // rows >= M and columns >= N of the box are clipped by the TMA unit
-#else
-                    if (lane == 0 && M == 1) {
-#endif
                         asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(&tmC), "r"(box),
                                      "r"((int32_t)(n0 + c0)), "r"((int32_t)(m0 + q * 32u))
                                      : "memory");
@@ -398,15 +364,10 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
                 }
             }
         }
-#ifdef PROBE_SKIP_EPI
-    epi_done:
-#endif
         // the staging memory may go away once the TMA unit has READ it; the writes themselves complete before the grid does
         if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        STAMP(4);
     }
-    STAMP(2);
     // Neither CTA may leave (or free its TMEM) while the other still uses the pair's resources.  The producer and issuer
     // warps ran their loops in one elected lane: reconverge before the warp-aligned cluster barrier.
     __syncwarp();
@@ -415,5 +376,4 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
-    STAMP(5);
 }

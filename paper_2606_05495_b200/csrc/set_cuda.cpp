@@ -1537,9 +1537,11 @@ set_status set_get_gap_stats(set_ctx* c, set_gap_stats* out) {
         iv.reserve(v.size());
         for (auto& r : v) iv.push_back({r.start, r.end});
         std::sort(iv.begin(), iv.end());
-        uint64_t busy = 0, lo = iv[0].first, hi = iv[0].second;
+        uint64_t busy = 0, lo = iv[0].first, hi = iv[0].second, idle = 0, nidle = 0;
         for (size_t i = 1; i < iv.size(); ++i) {
             if (iv[i].first > hi) {
+                idle += iv[i].first - hi;
+                nidle += 1;
                 busy += hi - lo;
                 lo = iv[i].first;
                 hi = iv[i].second;
@@ -1549,6 +1551,8 @@ set_status set_get_gap_stats(set_ctx* c, set_gap_stats* out) {
         }
         busy += hi - lo;
         out->busy_union_us = (double)busy * 1e-3;
+        out->idle_gaps = (double)nidle;
+        out->idle_gap_mean_us = nidle ? (double)idle * 1e-3 / (double)nidle : 0.0;
     }
     out->jobs = v.size();
     out->gaps = gaps.size();

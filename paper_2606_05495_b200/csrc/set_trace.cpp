@@ -160,18 +160,11 @@ extern "C" int set_trace_reduce(const set_trace_rec* recs, uint64_t n, set_trace
     memset(out, 0, sizeof(*out));
     if (n == 0) return 0;
     std::vector<set_trace_rec> v(recs, recs + n);
-    // per stream, by start time (ties: by end)
-    std::sort(v.begin(), v.end(), [](const set_trace_rec& a, const set_trace_rec& b) {
-        if (a.stream != b.stream) return a.stream < b.stream;
-        if (a.start_ns != b.start_ns) return a.start_ns < b.start_ns;
-        return a.end_ns < b.end_ns;
-    });
     std::vector<double> kk, intra, inter, any;
     uint64_t t_first = UINT64_MAX, t_last = 0;
     double ksum = 0, opsum = 0;
     uint64_t nk = 0;
-    for (size_t i = 0; i < v.size(); ++i) {
-        const set_trace_rec& r = v[i];
+    for (auto& r : v) {
         t_first = std::min(t_first, r.start_ns);
         t_last = std::max(t_last, r.end_ns);
         opsum += (double)(r.end_ns - r.start_ns) * 1e-3;
@@ -181,15 +174,72 @@ extern "C" int set_trace_reduce(const set_trace_rec* recs, uint64_t n, set_trace
             case 2: out->memcpys++; break;
             default: out->memsets++; break;
         }
-        if (i == 0 || v[i - 1].stream != r.stream) {
+    }
+    // ---- every consecutive pair on one CUPTI stream id (the raw view; negative = overlap = 0)
+    std::sort(v.begin(), v.end(), [](const set_trace_rec& a, const set_trace_rec& b) {
+        if (a.stream != b.stream) return a.stream < b.stream;
+        if (a.start_ns != b.start_ns) return a.start_ns < b.start_ns;
+        return a.end_ns < b.end_ns;
+    });
+    for (size_t i = 1; i < v.size(); ++i)
+        if (v[i - 1].stream == v[i].stream)
+            any.push_back(v[i].start_ns > v[i - 1].end_ns ? (double)(v[i].start_ns - v[i - 1].end_ns) * 1e-3 : 0.0);
+    // ---- jobs: the records of one graph launch share its correlation id.  CUPTI gives the parallel branches of a job graph
+    // (memset || H2D, two D2H leaves) stream ids of their own, so a job's WORK STREAM is the id most of its kernels ran under,
+    // and everything below is per job, not per CUPTI stream id.
+    std::sort(v.begin(), v.end(), [](const set_trace_rec& a, const set_trace_rec& b) {
+        if (a.job != b.job) return a.job < b.job;
+        if (a.start_ns != b.start_ns) return a.start_ns < b.start_ns;
+        return a.end_ns < b.end_ns;
+    });
+    struct Job {
+        uint32_t stream;
+        uint64_t start, end;
+    };
+    std::vector<Job> jobs;
+    for (size_t a = 0; a < v.size();) {
+        size_t b = a;
+        while (b < v.size() && v[b].job == v[a].job) ++b;
+        Job jb{v[a].stream, v[a].start_ns, v[a].end_ns};
+        std::map<uint32_t, int> votes;
+        uint64_t reach = v[a].end_ns;      // latest end among the job's ops so far
+        const set_trace_rec* last_kernel = nullptr;
+        for (size_t i = a; i < b; ++i) {
+            const set_trace_rec& r = v[i];
+            jb.end = std::max(jb.end, r.end_ns);
+            if (r.kind <= 1) votes[r.stream]++;
+            if (i > a) intra.push_back(r.start_ns > reach ? (double)(r.start_ns - reach) * 1e-3 : 0.0);
+            reach = std::max(reach, r.end_ns);
+            if (r.kind == 0) {
+                // stage kernel -> next stage kernel of the same job, SIGNED: a programmatic (PDL) edge lets the next kernel
+                // start before its predecessor has ended, which shows as a negative gap instead of a flat zero
+                if (last_kernel) {
+                    double g = ((double)r.start_ns - (double)last_kernel->end_ns) * 1e-3;
+                    kk.push_back(g);
+                    if (g < 0) out->kernel_kernel_overlapped++;
+                }
+                last_kernel = &r;
+            } else if (r.kind != 1) {
+                last_kernel = nullptr;  // a copy or memset in between: not a kernel-to-kernel hand-off
+            }
+        }
+        int best = 0;
+        for (auto& kv : votes)
+            if (kv.second > best) {
+                best = kv.second;
+                jb.stream = kv.first;
+            }
+        jobs.push_back(jb);
+        a = b;
+    }
+    out->jobs = jobs.size();
+    std::sort(jobs.begin(), jobs.end(), [](const Job& a, const Job& b) { return a.stream != b.stream ? a.stream < b.stream : a.start < b.start; });
+    for (size_t i = 0; i < jobs.size(); ++i) {
+        if (i == 0 || jobs[i - 1].stream != jobs[i].stream) {
             out->streams++;
             continue;
         }
-        const set_trace_rec& p = v[i - 1];
-        double gap = r.start_ns > p.end_ns ? (double)(r.start_ns - p.end_ns) * 1e-3 : 0.0;
-        any.push_back(gap);
-        if (p.kind == 0 && r.kind == 0 && p.job == r.job) kk.push_back(gap);
-        (p.job == r.job ? intra : inter).push_back(gap);
+        inter.push_back(jobs[i].start > jobs[i - 1].end ? (double)(jobs[i].start - jobs[i - 1].end) * 1e-3 : 0.0);
     }
     // union of all activity intervals, over all streams
     std::vector<std::pair<uint64_t, uint64_t>> iv;

@@ -24,7 +24,7 @@ class GapSummary(C.Structure):
 
 class TraceStats(C.Structure):
     _fields_ = [("kernels", C.c_uint64), ("signal_kernels", C.c_uint64), ("memcpys", C.c_uint64), ("memsets", C.c_uint64),
-                ("streams", C.c_uint64), ("dropped", C.c_uint64), ("wall_us", C.c_double), ("busy_us", C.c_double),
+                ("streams", C.c_uint64), ("dropped", C.c_uint64), ("jobs", C.c_uint64), ("kernel_kernel_overlapped", C.c_uint64), ("wall_us", C.c_double), ("busy_us", C.c_double),
                 ("idle_frac", C.c_double), ("kernel_mean_us", C.c_double), ("sum_op_us", C.c_double),
                 ("kernel_kernel", GapSummary), ("intra_job", GapSummary), ("inter_job", GapSummary), ("any_op", GapSummary)]
 

@@ -71,7 +71,7 @@ def test_struct_sizes_match_header(libset):
     assert C.sizeof(libset.ArgDesc) == 8 + 24 + 8 + 40
     assert C.sizeof(libset.Stats) == 20 * 8
     assert C.sizeof(libset.Config) == 14 * 4 + 8 + 8 + 8 + 8
-    assert C.sizeof(libset.GapStats) == 11 * 8
+    assert C.sizeof(libset.GapStats) == 13 * 8
 
 
 def test_invalid_arguments_are_rejected_without_a_device(libset):

@@ -65,7 +65,7 @@ def test_stdout_line_is_compact_and_complete():
               "baselines": {"batch_sync_graphs_e2e": {"jobs_per_s": 193000.0, "host_us_per_job": _fake_arm(1, "host")["host_us_per_job"]}},
               "device_gaps": {"how": "...", "config1": {"set_e2e": gaps, "batch_sync_graphs_e2e": dict(gaps, gap_mean_us=22.1), "mutex_queue_e2e": gaps}},
               "pipeline_roofline": {"e2e_bound_by": "link", "e2e_bound_jobs_per_s": 380868.2, "e2e_frac": 0.5703},
-              "workloads": {f"config{c}": dict(side) for c in (0, 2, 3, 4)},
+              "workloads": {f"config{c}": dict(side) for c in (0, 2, 3, 4, 5, 6)},
               "cpu_baseline": {"value": 9943.12, "unit": "jobs/s", "cores": 1, "kind": "oracle",
                                "sample": "99431 jobs of the workload (first 2048 job inputs, repeated) in 10.0 s, single thread, oracle/*.c -O2",
                                "all_cores": {"value": 43460.0, "cores": 16, "sample": "s" * 40}},
@@ -86,7 +86,8 @@ def test_stdout_line_is_compact_and_complete():
     assert hm["set_over_batch_sync_e2e"] == round(217224.4 / 193000.0, 3)
     assert hm["sched_overhead_frac"] == {"set": 0.0312, "batch_sync": 0.0312} and hm["gap_between_jobs_us"]["batch_sync"] == 22.1
     assert back["kernel_rooflines"]["jacobi5_f32"]["frac"] == 0.9351 and back["kernel_rooflines"]["gemm_bias_gelu_bf16"]["frac"] == 0.7123
-    assert set(back["workloads"]) == {"config0", "config2", "config3", "config4"} and back["workloads"]["config2"]["frac"] == 0.9412
+    side_line = back["workloads_e2e_frac_vsbatch"]
+    assert set(side_line) == {"config0", "config2", "config3", "config4", "config5", "config6"} and side_line["config2"] == [812.3, 0.9412, 1.031]
     assert back["detail"] == "bench_detail.json"
     # world > 1: no side passes ran, the line is still complete
     line2 = bench.compact_line(wl, 8, 20, 5, 10000, 24.8, 3.2e6, 46.0, 1.7e6, _fake_arm(402503.2, "device"), _fake_arm(217224.4, "host"),

@@ -369,7 +369,8 @@ def test_gap_stats_are_zero_without_timestamps(libset):
     ctx = libset.Context(wl.num_streams, wl.max_inflight)
     ctx.register_builtin(0)
     assert ctx.gap_stats() == {"jobs": 0, "gaps": 0, "gap_mean_us": 0.0, "gap_p50_us": 0.0, "gap_p99_us": 0.0, "gap_max_us": 0.0,
-                               "job_mean_us": 0.0, "span_us": 0.0, "stream_busy_frac": 0.0, "busy_union_us": 0.0, "idle_frac": 0.0}
+                               "job_mean_us": 0.0, "span_us": 0.0, "stream_busy_frac": 0.0, "busy_union_us": 0.0, "idle_frac": 0.0,
+                               "idle_gaps": 0.0, "idle_gap_mean_us": 0.0}
     ctx.close()
 
 

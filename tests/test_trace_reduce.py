@@ -23,7 +23,7 @@ def test_trace_library_exports_every_declared_symbol(trace):
     assert declared == ["set_trace_error", "set_trace_reduce", "set_trace_start", "set_trace_stop"]
     for name in declared:
         assert hasattr(trace.load(), name)
-    assert C.sizeof(trace.GapSummary) == 40 and C.sizeof(trace.TraceStats) == 6 * 8 + 5 * 8 + 4 * 40 and C.sizeof(trace.TraceRec) == 32
+    assert C.sizeof(trace.GapSummary) == 40 and C.sizeof(trace.TraceStats) == 8 * 8 + 5 * 8 + 4 * 40 and C.sizeof(trace.TraceRec) == 32
 
 
 def test_one_stream_two_jobs(trace):
@@ -72,3 +72,25 @@ def test_percentiles(trace):
         t += 1000 + i * 1000
     kk = trace.reduce(recs)["kernel_kernel"]
     assert kk["count"] == 100 and kk["p50_us"] == 50.0 and kk["p99_us"] == 98.0 and kk["max_us"] == 99.0 and kk["mean_us"] == 49.5
+
+
+def test_jobs_are_grouped_by_launch_not_by_cupti_stream_id(trace):
+    """CUPTI labels the parallel branches of a job graph with stream ids of their own (round 1 saw 200 'streams' on an
+    8-stream context): jobs are rebuilt from the correlation id, the work stream is the id most of a job's kernels ran
+    under, and a PDL overlap shows as a NEGATIVE kernel-to-kernel gap."""
+    K, S, M, Z = trace.KIND_KERNEL, trace.KIND_SIGNAL, trace.KIND_MEMCPY, trace.KIND_MEMSET
+    us = 1000
+    recs = [  # job 1 on work stream 7: memset on an internal id 901 beside the H2D on 7; kernels on 7; second D2H leaf on 902
+        (901, 1, Z, 0, 1 * us), (7, 1, M, 0, 10 * us), (7, 1, K, 11 * us, 14 * us), (7, 1, K, 13 * us, 16 * us), (7, 1, K, 18 * us, 19 * us),
+        (7, 1, M, 20 * us, 30 * us), (902, 1, M, 20 * us, 22 * us), (7, 1, S, 31 * us, 32 * us),
+        # job 2 on the same work stream, 4 us after job 1's last op; its memset again on another internal id
+        (903, 2, Z, 36 * us, 37 * us), (7, 2, M, 36 * us, 46 * us), (7, 2, K, 47 * us, 49 * us), (7, 2, S, 50 * us, 51 * us),
+        # job 3 on work stream 8, overlapping both
+        (8, 3, M, 5 * us, 15 * us), (8, 3, K, 16 * us, 40 * us), (8, 3, S, 41 * us, 42 * us)]
+    st = trace.reduce(recs)
+    assert st["jobs"] == 3 and st["streams"] == 2                      # not 5
+    kk = st["kernel_kernel"]                                           # job 1: 13 - 14 = -1 (PDL overlap), 18 - 16 = +2
+    assert kk["count"] == 2 and st["kernel_kernel_overlapped"] == 1 and kk["mean_us"] == 0.5 and kk["max_us"] == 2.0
+    assert st["inter_job"] == {"count": 1, "mean_us": 4.0, "p50_us": 4.0, "p99_us": 4.0, "max_us": 4.0}    # 36 - 32 on work stream 7
+    # intra-job gaps never count a parallel branch as idle time: job 1 has 1 (10->11), 2 (16->18), 1, 1 and zeros
+    assert st["intra_job"]["max_us"] == 2.0
