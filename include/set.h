@@ -216,8 +216,10 @@ typedef struct set_config {
                                  the library's choice, SET_FENCE_SYSTEM; SET_FENCE_SYSTEM (1) = fence.acq_rel.sys before
                                  the store (release at system scope: the job's D2H output, written by an earlier grid, is
                                  ordered before the word by the PTX memory model); SET_FENCE_NONE (2) = plain volatile
-                                 store, relying on grid completion alone (faster, measured never wrong on B200, but not
-                                 guaranteed by the model).  DESIGN.md 5a.                                           */
+                                 store, relying on grid completion alone.  UNSAFE, a measurement arm only: about 10 % faster,
+                                 not guaranteed by the model, and caught on B200 with several CUDA streams per lane -- about
+                                 one completion in 30,000 is seen before its output (profiles/r2_signal_soak.md).  Outputs are
+                                 still complete once set_drain has returned.  DESIGN.md 5a.                          */
     void *const *streams;     /* HOST array of num_streams cudaStream_t owned by the caller (e.g.
                                  torch.cuda.Stream.cuda_stream), or NULL: the library creates them */
     void *device_arena;       /* DEVICE memory owned by the caller for all slot buffers, or NULL   */

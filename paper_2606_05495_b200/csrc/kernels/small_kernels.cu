@@ -242,7 +242,8 @@ extern "C" __global__ void set_k_spin(uint32_t* scratch, uint32_t ns) {
 //     CUDA stream and does not wait for this node).
 //   fence == 0 (SET_FENCE_NONE): plain volatile store, relying on grid completion alone to have pushed the output out.
 //     Two unfenced stores of ONE thread were seen to reach host memory out of order on this machine (the stamp and the
-//     word below), so nothing but measurement (profiles/r2_signal_soak.md) backs this variant; it is opt-in.
+//     word below), and with several CUDA streams per lane the library's own hook caught the word overtaking a job's
+//     output about once in 30,000 jobs (profiles/r2_signal_soak.md): unsafe, kept as a measurement arm only.
 extern "C" __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp, uint32_t fence) {
     set_pdl_sync();
     if (stamp) {  // set_config.timestamps: when the job ended on the device

@@ -629,17 +629,16 @@ def test_config3_behind_a_programmatic_edge(libset, shape, sm_copy):
     assert st["copy_nodes"] >= 64          # the copy-in really was a kernel node
 
 
-@pytest.mark.parametrize("fence", [1, 2])
-@pytest.mark.parametrize("lanes", [1, 4])
-def test_no_completion_is_seen_before_its_output(libset, fence, lanes):
-    """set_config.debug_sentinel: inside Algorithm 3, at the moment the dispatcher sees a job's completion word and before
-    the slot is released, the library itself looks at the first and last word of the job's sentinel-filled output.
-    30,000 config-0 jobs (16,640-byte outputs written by an SM copy node) and 30,000 config-1 jobs per repetition at the
-    bench geometry; SET_SOAK_REPS raises the count for a soak run (profiles/r2_signal_soak.md)."""
+def _completion_soak(libset, fence, lanes):
+    """30,000 config-1 jobs and 30,000 config-0 jobs per repetition at the bench geometry with set_config.debug_sentinel: inside
+    Algorithm 3, at the moment the dispatcher sees a job's completion word and before the slot is released, the library itself
+    looks at the first and last word of the job's sentinel-filled output.  Returns the number of early completions; every output
+    is checked after set_drain regardless.  SET_SOAK_REPS raises the repetition count for a soak run."""
     import ctypes as C
     import os
     from paper_2606_05495_b200.workloads import PinnedArena, baseline_workload
     reps = int(os.environ.get("SET_SOAK_REPS", "2"))
+    early = 0
     for config in (1, 0):
         wl = baseline_workload(config)
         n, npool = 30000, 64
@@ -649,7 +648,7 @@ def test_no_completion_is_seen_before_its_output(libset, fence, lanes):
             ins = [wl.make_input(j) for j in range(npool)]
             want = [oracle_out(wl, x, (1, 1, 1, 1)) for x in ins]
             ob = wl.out_bytes()
-            arena = PinnedArena(ctx, npool * (wl.in_bytes() + 256) + (ob + 0) * n + 4096)
+            arena = PinnedArena(ctx, npool * (wl.in_bytes() + 256) + ob * n + 4096)
             in_ptrs = []
             for x in ins:
                 a, v = arena.take(wl.in_bytes())
@@ -662,21 +661,40 @@ def test_no_completion_is_seen_before_its_output(libset, fence, lanes):
                 v_out[:] = SENTINEL
                 ctx.submit_batch(pi, po)
                 ctx.drain()
-                st = ctx.stats()
-                assert st["early_completions"] == 0, f"config {config} fence {fence} lanes {lanes} rep {rep}: {st['early_completions']} completions overtook their output"
                 got = np.array(v_out, copy=True).reshape(n, ob)
-                for p_ in range(npool):
+                for p_ in range(npool):                       # after set_drain every output is there, whatever the fence mode
                     rows = got[p_::npool]
                     if config == 1:
                         g, r = rows.view(np.float32)[:, 0], want[p_].view(np.float32)[0]
                         assert np.all(np.abs(g - r) <= 1e-6 * abs(r))
                     else:
                         assert np.all(rows == want[p_][None, :])
-            assert ctx.stats()["completed"] == n * reps
+            st = ctx.stats()
+            assert st["completed"] == n * reps
+            early += st["early_completions"]
             v_out = None
             arena.free()
         finally:
             ctx.close()
+    return early
+
+
+@pytest.mark.parametrize("lanes", [1, 4])
+def test_no_completion_is_seen_before_its_output(libset, lanes):
+    """The default completion store (SET_FENCE_SYSTEM: fence.acq_rel.sys, then the word): no completion may ever be observed
+    before its job's output is in host memory."""
+    assert _completion_soak(libset, libset.FENCE_SYSTEM, lanes) == 0
+
+
+@pytest.mark.parametrize("lanes", [1, 4])
+def test_fence_free_completion_is_only_a_measurement_arm(libset, lanes):
+    """SET_FENCE_NONE (round 1's default) relies on grid completion alone.  Round 2 caught it in the act: with four CUDA
+    streams per lane about one completion in 30,000 overtakes its output (profiles/r2_signal_soak.md), so the mode is opt-in,
+    documented as unsafe for anything that reads the output on completion, and this test only requires what still holds --
+    every output is correct once set_drain has returned -- and prints what the hook counted."""
+    early = _completion_soak(libset, libset.FENCE_NONE, lanes)
+    print(f"SET_FENCE_NONE, {lanes} CUDA stream(s) per lane: {early} early completions")
+    assert early >= 0
 
 
 def test_pageable_staging_at_full_rate(libset):
