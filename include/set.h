@@ -19,6 +19,10 @@
  *                           or an NV_NSIGHT_INJECTION_* / NV_COMPUTE_PROFILER_* variable is set); SET_DRIVER_LOCK=0 overrides.
  *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 8: 64 KB in flight per
  *                           copy; more delays the GPU's own command fetches over the same link).
+ *   SET_FORWARD_OUT=0       turn output-address forwarding off (read at set_register_pipeline; for A/B measurements).  By default,
+ *                           where a job graph has an SM copy-in node and SM copy-out nodes, the copy-in node carries the job's
+ *                           host_out address into a per-slot device word and the copy-out nodes take their destination from
+ *                           there, so that binding a job updates ONE graph node instead of two.
  *
  * Conventions
  *   - Plain C, opaque handle, no exceptions cross the ABI, the library never aborts the process.
@@ -232,6 +236,10 @@ typedef struct set_config {
                                  clamped to that.  0 => default: with SET_IO_HOST as many as the slots allow up to 32 CUDA
                                  streams in all, with SET_IO_DEVICE 1 (DESIGN.md 5b gives the measurements).  Forced to 1
                                  when the caller supplies `streams`.  The in-run baseline models use the same streams.  */
+    int32_t completion_thread;/* SET_CB_FLAG_POLL: 1 = a thread of its own watches the completion words and runs Algorithm 3, the
+                                 dispatcher(s) only find and launch jobs; 2 = the dispatcher(s) poll between launches (round 1);
+                                 0 => default (1).  DESIGN.md 5d.                                                   */
+    int32_t reserved2;
     uint32_t debug_sentinel;  /* test hook: non-zero => at the moment a job's completion is observed (before the slot is
                                  released) the first and last 32-bit word of every D2H region of its host_out are compared
                                  with this value; a match means the completion overtook the output, counted in
@@ -392,8 +400,11 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
                                     (SET_CB_FLAG_POLL), behind fence.acq_rel.sys if fence != 0; stamp != NULL:
                                     *stamp = %globaltimer first                                               */
 #define SET_K_STAMP          16  /* (uint64* stamp)  *stamp = %globaltimer (set_config.timestamps)               */
-#define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes)  copy by the SMs; src / dst may be
-                                    pinned HOST or DEVICE memory                                              */
+#define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes, void** fwd_slot, void* fwd_value)  copy by the
+                                    SMs; src / dst may be pinned HOST or DEVICE memory; fwd_slot != NULL: also stores
+                                    fwd_value (the job's output address) into that DEVICE word                */
+#define SET_K_COPY_OUT       24  /* (const void* src, void* const* dst_slot, uint64 dst_off, uint32 bytes)  copy by the SMs
+                                    to *dst_slot + dst_off: the address the job's copy-in node forwarded       */
 /* the two paper workloads of SURVEY.md 8(f)4 (readings S5-*, S6-*) */
 #define SET_K_SOBEL3X3_U8    17  /* (const uint8* n, uint8* e, uint32 w, uint32 h)  min(255, |gx| + |gy|), clamp-to-edge   */
 #define SET_K_MEAN3X3_U8     18  /* (const uint8* e, uint8* m, uint32 w, uint32 h)  3 x 3 sum / 9, clamp-to-edge          */
@@ -440,7 +451,8 @@ int64_t set_selftest_ring(int capacity, int producers, int consumers, int64_t it
  * CUDA driver's callback thread and finish launched jobs after a pseudo-random delay.  Checks: every
  * job completes exactly once, never more than b in flight, no slot runs two jobs at once, a stolen
  * job is bound to the thief's slot.  seed bit 0 selects SET_STEAL_RETARGET, seed bit 1 flag-polled completion
- * (the completers store the slot's word instead of calling Algorithm 3).  Returns 0 or a negative error code. */
+ * (the completers store the slot's word instead of calling Algorithm 3), seed bit 2 a completion thread of its own
+ * (set_config.completion_thread).  Returns 0 or a negative error code. */
 int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capacity, int num_dispatchers,
                                int submitters, int64_t jobs, uint32_t seed, uint64_t *out_steals);
 

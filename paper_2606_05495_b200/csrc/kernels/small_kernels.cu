@@ -270,8 +270,8 @@ extern "C" __global__ void set_k_stamp(unsigned long long* stamp) {
 // copies up to set_config.sm_copy_max_bytes are kernel nodes instead: the SMs read pinned host memory directly
 // over the link (H2D) or store into it (D2H).  Each thread moves two 128-bit words, both loads issued before the
 // first store so that 8 KB per block are in flight; unaligned operands or sizes fall back to a byte loop.
-extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes) {
-    set_pdl_sync();
+namespace {
+__device__ __forceinline__ void copy_bytes(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes) {
     const uint32_t tid = threadIdx.x;
     const bool vec = aligned16(src, dst);
     for (uint32_t base = blockIdx.x * (uint32_t)kCopyBytesPerBlock; base < bytes; base += gridDim.x * (uint32_t)kCopyBytesPerBlock) {
@@ -293,4 +293,24 @@ extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restr
             for (uint32_t k = base + tid; k < end; k += 256u) static_cast<char*>(dst)[k] = static_cast<const char*>(src)[k];
         }
     }
+}
+}  // namespace
+
+// fwd_slot != NULL: the copy-in node also carries the job's OUTPUT address into the slot's device word, from which the
+// copy-out node (K25) takes its destination -- so that a job costs ONE graph-node update instead of two (the update and the
+// launch go through the same driver lock, about 0.5 us per node: DESIGN.md 5d).
+extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes, void** fwd_slot,
+                                                             void* fwd_value) {
+    set_pdl_sync();
+    if (fwd_slot && blockIdx.x == 0 && threadIdx.x == 0) *fwd_slot = fwd_value;
+    copy_bytes(src, dst, bytes);
+}
+
+// K25: copy-out whose destination is *dst_slot + dst_off: the address the job's copy-in node left in the slot's device word.
+// Every kernel between the two is ordered behind its predecessor (plain edge or griddepcontrol.wait), so the word is visible.
+extern "C" __global__ void __launch_bounds__(256) set_k_copy_out(const void* __restrict__ src, void* const* __restrict__ dst_slot, unsigned long long dst_off,
+                                                                 uint32_t bytes) {
+    set_pdl_sync();
+    char* dst = static_cast<char*>(*reinterpret_cast<void* const volatile*>(dst_slot)) + dst_off;
+    copy_bytes(src, dst, bytes);
 }

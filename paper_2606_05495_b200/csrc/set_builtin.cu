@@ -100,6 +100,7 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_SPIN: return (const void*)set_k_spin;
         case SET_K_SIGNAL: return (const void*)set_k_signal;
         case SET_K_COPY: return (const void*)set_k_copy;
+        case SET_K_COPY_OUT: return (const void*)set_k_copy_out;
         case SET_K_STAMP: return (const void*)set_k_stamp;
         case SET_K_SOBEL3X3_U8: return (const void*)set_k_sobel3x3_u8;
         case SET_K_MEAN3X3_U8: return (const void*)set_k_mean3x3_u8;

@@ -221,10 +221,19 @@ struct set_ctx final : public Backend {
         const void* src;
         void* dst;
         uint32_t bytes;
-        void* ptrs[3];
+        void** fwd_slot;               // SET_K_COPY: where the copy-in node leaves the job's output address (or NULL)
+        void* fwd_value;
+        unsigned long long dst_off;    // SET_K_COPY_OUT: byte offset behind the forwarded address
+        void* ptrs[5];
         cudaKernelNodeParams kp;
     };
-    void copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims);
+    // `host` is the job's input (to_device) or output image; `fwd_out` the job's output image, forwarded by copy-in node fwd_buf
+    void copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims, const void* fwd_out = nullptr);
+    // Output-address forwarding: SM copy-out nodes take their destination from a per-slot device word that the
+    // job's first SM copy-in node fills, so a job in the steady state costs one graph-node update, not two.
+    int fwd_buf = -1;                  // buffer whose H2D SM-copy node forwards; -1 = off
+    bool d2h_ind[SET_MAX_BUFFERS] = {};
+    void** fwd_dev = nullptr;          // b device words
     int check_sizes(const uint32_t* dims);
     bool is_pinned(const void* p);
     void add_pinned_range(const void* p, size_t n);
@@ -303,22 +312,41 @@ int set_ctx::build_args(const set_stage_desc& st, int slot, const uint32_t* dims
     return 0;
 }
 
-void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims) {
+void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const void* host, const uint32_t* dims, const void* fwd_out) {
     const set_buffer_desc& bd = bufs[i];
+    ca.kp = cudaKernelNodeParams{};
+    ca.fwd_slot = nullptr;
+    ca.fwd_value = nullptr;
+    ca.dst_off = 0;
     if (to_device) {
         ca.src = (const char*)host + eval(bd.h2d_host_off, dims);
         ca.dst = (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, dims);
         ca.bytes = (uint32_t)eval(bd.h2d_bytes, dims);
+        if (i == fwd_buf) {
+            ca.fwd_slot = fwd_dev + slot;
+            ca.fwd_value = const_cast<void*>(fwd_out);
+        }
     } else {
         ca.src = (const char*)slots[slot].buf[i] + eval(bd.d2h_dev_off, dims);
         ca.dst = (char*)host + eval(bd.d2h_host_off, dims);
         ca.bytes = (uint32_t)eval(bd.d2h_bytes, dims);
+        ca.dst_off = eval(bd.d2h_host_off, dims);
     }
-    ca.ptrs[0] = &ca.src;
-    ca.ptrs[1] = &ca.dst;
-    ca.ptrs[2] = &ca.bytes;
-    ca.kp = cudaKernelNodeParams{};
-    ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
+    if (!to_device && d2h_ind[i]) {  // (src, dst_slot, dst_off, bytes)
+        ca.fwd_slot = fwd_dev + slot;
+        ca.ptrs[0] = &ca.src;
+        ca.ptrs[1] = &ca.fwd_slot;
+        ca.ptrs[2] = &ca.dst_off;
+        ca.ptrs[3] = &ca.bytes;
+        ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY_OUT));
+    } else {                         // (src, dst, bytes, fwd_slot, fwd_value)
+        ca.ptrs[0] = &ca.src;
+        ca.ptrs[1] = &ca.dst;
+        ca.ptrs[2] = &ca.bytes;
+        ca.ptrs[3] = &ca.fwd_slot;
+        ca.ptrs[4] = &ca.fwd_value;
+        ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
+    }
     uint32_t pieces = (ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK;
     // Reads of pinned host memory share the link with the GPU's own fetches of launch commands: eight streams that each
     // put 128 KB of reads in flight at once delay the start of every stream's next graph (measured: 15 us between graphs
@@ -424,7 +452,7 @@ int set_ctx::build_graph(int slot, int set_index) {
         if (!expr_is_zero(bd.h2d_bytes)) {
             if (h2d_sm[i]) {
                 CopyArgs ca;
-                copy_params(ca, slot, (int)i, true, ph_in, unit);
+                copy_params(ca, slot, (int)i, true, ph_in, unit, ph_out);
                 CK(cudaGraphAddKernelNode(&g.h2d_nodes[i], g.graph, nullptr, 0, &ca.kp));
             } else {
                 CK(cudaGraphAddMemcpyNode1D(&g.h2d_nodes[i], g.graph, nullptr, 0, (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, unit),
@@ -685,17 +713,17 @@ int set_ctx::bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) {
     }
     for (size_t i = 0; i < bufs.size(); ++i) {
         const set_buffer_desc& bd = bufs[i];
-        if (!expr_is_zero(bd.h2d_bytes) && (full || es.in != in)) {
+        if (!expr_is_zero(bd.h2d_bytes) && (full || es.in != in || ((int)i == fwd_buf && es.out != out))) {
             if (h2d_sm[i]) {
                 CopyArgs ca;
-                copy_params(ca, slot, (int)i, true, in, job.dims);
+                copy_params(ca, slot, (int)i, true, in, job.dims, out);
                 CK(cudaGraphExecKernelNodeSetParams(es.exec, g.h2d_nodes[i], &ca.kp));
             } else {
                 CK(cudaGraphExecMemcpyNodeSetParams1D(es.exec, g.h2d_nodes[i], (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, job.dims),
                                                       (const char*)in + eval(bd.h2d_host_off, job.dims), eval(bd.h2d_bytes, job.dims), kin));
             }
         }
-        if (!expr_is_zero(bd.d2h_bytes) && (full || es.out != out)) {
+        if (!expr_is_zero(bd.d2h_bytes) && (full || (es.out != out && !d2h_ind[i]))) {  // a forwarded destination needs no update
             if (d2h_sm[i]) {
                 CopyArgs ca;
                 copy_params(ca, slot, (int)i, false, out, job.dims);
@@ -822,7 +850,7 @@ int set_ctx::plain_job(int slot, const JobDesc& job) {
         if (!expr_is_zero(bd.h2d_bytes)) {
             if (h2d_sm[i]) {  // the same node list as the job graph, launched one by one
                 CopyArgs ca;
-                copy_params(ca, slot, (int)i, true, job.in, job.dims);
+                copy_params(ca, slot, (int)i, true, job.in, job.dims, job.out);
                 CK(cudaLaunchKernel(ca.kp.func, ca.kp.gridDim, ca.kp.blockDim, ca.ptrs, 0, st));
             } else {
                 CK(cudaMemcpyAsync((char*)sm.buf[i] + eval(bd.h2d_dev_off, job.dims), (const char*)job.in + eval(bd.h2d_host_off, job.dims),
@@ -1037,6 +1065,8 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.completion_fence < SET_FENCE_DEFAULT || cfg.completion_fence > SET_FENCE_NONE) return SET_ERR_INVALID;
     if (cfg.completion_fence == SET_FENCE_DEFAULT) cfg.completion_fence = SET_FENCE_SYSTEM;
     if (cfg.streams_per_lane < 0 || cfg.streams_per_lane > 4096) return SET_ERR_INVALID;
+    if (cfg.completion_thread < 0 || cfg.completion_thread > 2) return SET_ERR_INVALID;
+    if (cfg.completion_thread == 0) cfg.completion_thread = 1;
     // Default (measured on B200): with host I/O a job's chain is latency-bound (its copy-in waits on the link),
     // so every slot gets a CUDA stream of its own -- the paper's worker W_i = (S_i, G_i, M_i), PAPER.md:110 -- and b chains are
     // in flight instead of S (config 1 end to end 201 K -> 316 K jobs/s, config 0 227 K -> 336 K).  With device-resident I/O
@@ -1130,7 +1160,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
         c->stamp_recs.reserve(1 << 16);
     }
     if (cfg.mode == SET_MODE_SET)
-        c->sched.reset(new Scheduler(c, c->H, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us));
+        c->sched.reset(new Scheduler(c, c->H, c->b, c->q, cfg.num_dispatchers, cfg.steal_policy, cfg.spin_us, cfg.completion_thread == 1));
     *out = c;
     return SET_OK;
 }
@@ -1267,6 +1297,24 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
             c->n_sm_copies += (int)c->h2d_sm[i] + (int)c->d2h_sm[i];
         }
         for (auto& st : c->stages) c->pdl = c->pdl || (st.flags & SET_STAGE_PDL);
+        // output-address forwarding: needs an SM copy-in node to carry the address and at least one SM copy-out node to use it
+        const char* fo = getenv("SET_FORWARD_OUT");
+        if (!(fo && fo[0] == '0')) {
+            int first_in = -1;
+            bool any_out = false;
+            for (size_t i = 0; i < c->bufs.size(); ++i) {
+                if (c->h2d_sm[i] && first_in < 0) first_in = (int)i;
+                any_out = any_out || c->d2h_sm[i];
+            }
+            if (first_in >= 0 && any_out) {
+                if (cudaMalloc((void**)&c->fwd_dev, sizeof(void*) * (size_t)c->b) != cudaSuccess) {
+                    cudaGetLastError();
+                    return c->fail(SET_ERR_NOMEM, "allocation of the forwarding words failed");
+                }
+                c->fwd_buf = first_in;
+                for (size_t i = 0; i < c->bufs.size(); ++i) c->d2h_ind[i] = c->d2h_sm[i];
+            }
+        }
     }
     {
         bool in_loop = false;
@@ -1383,6 +1431,7 @@ set_status set_destroy(set_ctx* c) {
     if (c->ph_in) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_in) : cudaFreeHost(c->ph_in));
     if (c->ph_out) (c->cfg.io == SET_IO_DEVICE ? cudaFree(c->ph_out) : cudaFreeHost(c->ph_out));
     for (auto& ha : c->host_allocs) cudaFreeHost(ha.first);
+    if (c->fwd_dev) cudaFree(c->fwd_dev);
     if (c->flags_host) cudaFreeHost(c->flags_host);
     if (c->ts_host) cudaFreeHost(c->ts_host);
     for (int s = 0; s < c->H; ++s) {

@@ -188,7 +188,7 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
     SimBackend be(b, queue_capacity + 1, 2, jobs, seed, /*polled=*/(seed & 2) != 0);
     int64_t rc = 0;
     {
-        Scheduler sched(&be, num_streams, b, queue_capacity, num_dispatchers, policy, 20);
+        Scheduler sched(&be, num_streams, b, queue_capacity, num_dispatchers, policy, 20, /*poller=*/(seed >> 2) & 1);
         be.attach(&sched);
         std::atomic<int64_t> next{0};
         std::vector<std::thread> subs;

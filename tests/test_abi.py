@@ -70,7 +70,7 @@ def test_struct_sizes_match_header(libset):
     assert C.sizeof(libset.SizeExpr) == 24 and C.sizeof(libset.GridRule) == 32 and C.sizeof(libset.Tmap2D) == 40
     assert C.sizeof(libset.ArgDesc) == 8 + 24 + 8 + 40
     assert C.sizeof(libset.Stats) == 20 * 8
-    assert C.sizeof(libset.Config) == 14 * 4 + 8 + 8 + 8 + 8
+    assert C.sizeof(libset.Config) == 14 * 4 + 8 + 8 + 8 + 16
     assert C.sizeof(libset.GapStats) == 13 * 8
 
 
