@@ -19,6 +19,8 @@
  *                           or an NV_NSIGHT_INJECTION_* / NV_COMPUTE_PROFILER_* variable is set); SET_DRIVER_LOCK=0 overrides.
  *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 8: 64 KB in flight per
  *                           copy; more delays the GPU's own command fetches over the same link).
+ *   SET_FUSE_SIGNAL=0       keep the completion signal a node of its own even where the job has a single SM copy-out node that
+ *                           could carry it (for A/B measurements; read at set_register_pipeline).
  *   SET_FORWARD_OUT=0       turn output-address forwarding off (read at set_register_pipeline; for A/B measurements).  By default,
  *                           where a job graph has an SM copy-in node and SM copy-out nodes, the copy-in node carries the job's
  *                           host_out address into a per-slot device word and the copy-out nodes take their destination from
@@ -403,8 +405,10 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_COPY           15  /* (const void* src, void* dst, uint32 bytes, void** fwd_slot, void* fwd_value)  copy by the
                                     SMs; src / dst may be pinned HOST or DEVICE memory; fwd_slot != NULL: also stores
                                     fwd_value (the job's output address) into that DEVICE word                */
-#define SET_K_COPY_OUT       24  /* (const void* src, void* const* dst_slot, uint64 dst_off, uint32 bytes)  copy by the SMs
-                                    to *dst_slot + dst_off: the address the job's copy-in node forwarded       */
+#define SET_K_COPY_OUT       24  /* (const void* src, void* const* dst_slot, uint64 dst_off, uint32 bytes, uint32* flag,
+                                    uint64* stamp, uint32 fence)  copy by the SMs to *dst_slot + dst_off: the address the
+                                    job's copy-in node forwarded; flag != NULL: the block that finishes last also does what
+                                    SET_K_SIGNAL does (the job's completion signal folded into its only copy-out node)   */
 /* the two paper workloads of SURVEY.md 8(f)4 (readings S5-*, S6-*) */
 #define SET_K_SOBEL3X3_U8    17  /* (const uint8* n, uint8* e, uint32 w, uint32 h)  min(255, |gx| + |gy|), clamp-to-edge   */
 #define SET_K_MEAN3X3_U8     18  /* (const uint8* e, uint8* m, uint32 w, uint32 h)  3 x 3 sum / 9, clamp-to-edge          */

@@ -21,7 +21,8 @@ __global__ void set_k_spin(uint32_t* scratch, uint32_t ns);
 __global__ void set_k_signal(uint32_t* flag, unsigned long long* stamp, uint32_t fence);
 __global__ void set_k_stamp(unsigned long long* stamp);
 __global__ void set_k_copy(const void* src, void* dst, uint32_t bytes, void** fwd_slot, void* fwd_value);
-__global__ void set_k_copy_out(const void* src, void* const* dst_slot, unsigned long long dst_off, uint32_t bytes);
+__global__ void set_k_copy_out(const void* src, void* const* dst_slot, unsigned long long dst_off, uint32_t bytes, uint32_t* flag,
+                               unsigned long long* stamp, uint32_t fence);
 __global__ void set_k_sobel3x3_u8(const uint8_t* n, uint8_t* e, uint32_t w, uint32_t h);
 __global__ void set_k_mean3x3_u8(const uint8_t* e, uint8_t* m, uint32_t w, uint32_t h);
 __global__ void set_k_threshold_u8(const uint8_t* m, uint8_t* t, uint32_t w, uint32_t h, uint32_t thresh);

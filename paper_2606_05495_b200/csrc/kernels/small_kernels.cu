@@ -308,9 +308,31 @@ extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restr
 
 // K25: copy-out whose destination is *dst_slot + dst_off: the address the job's copy-in node left in the slot's device word.
 // Every kernel between the two is ordered behind its predecessor (plain edge or griddepcontrol.wait), so the word is visible.
+// flag != NULL: this node is also the job's completion signal (K14 folded in: one node less per job -- the GPU's front end
+// works through about three million graph nodes a second, which is what bounds the short-job configs).  Every
+// block, after its part of the copy, takes a ticket with a gpu-scope release; the block that draws the last ticket has thereby
+// acquired every other block's stores, fences them out at system scope (unless fence == 0) and stores the slot's word.
 extern "C" __global__ void __launch_bounds__(256) set_k_copy_out(const void* __restrict__ src, void* const* __restrict__ dst_slot, unsigned long long dst_off,
-                                                                 uint32_t bytes) {
+                                                                 uint32_t bytes, uint32_t* flag, unsigned long long* stamp, uint32_t fence) {
     set_pdl_sync();
     char* dst = static_cast<char*>(*reinterpret_cast<void* const volatile*>(dst_slot)) + dst_off;
     copy_bytes(src, dst, bytes);
+    if (flag) {
+        __syncthreads();  // the block's stores are ordered before thread 0's release below (cta-scope barrier, then cumulativity)
+        if (threadIdx.x == 0) {
+            uint32_t* ticket = reinterpret_cast<uint32_t*>(const_cast<void**>(dst_slot) + 1);  // the word behind the forwarded address
+            uint32_t drawn;
+            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(drawn) : "l"(ticket) : "memory");
+            if (drawn == gridDim.x - 1u) {
+                *ticket = 0u;  // for the slot's next job (ordered before its launch by the completion itself)
+                if (stamp) {
+                    unsigned long long t;
+                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+                    *reinterpret_cast<volatile unsigned long long*>(stamp) = t;
+                }
+                if (fence) asm volatile("fence.acq_rel.sys;" ::: "memory");
+                *reinterpret_cast<volatile uint32_t*>(flag) = 1u;
+            }
+        }
+    }
 }

@@ -224,7 +224,10 @@ struct set_ctx final : public Backend {
         void** fwd_slot;               // SET_K_COPY: where the copy-in node leaves the job's output address (or NULL)
         void* fwd_value;
         unsigned long long dst_off;    // SET_K_COPY_OUT: byte offset behind the forwarded address
-        void* ptrs[5];
+        uint32_t* sig_flag;            // SET_K_COPY_OUT with the completion signal folded in (else NULL)
+        unsigned long long* sig_stamp;
+        uint32_t sig_fence;
+        void* ptrs[7];
         cudaKernelNodeParams kp;
     };
     // `host` is the job's input (to_device) or output image; `fwd_out` the job's output image, forwarded by copy-in node fwd_buf
@@ -233,7 +236,8 @@ struct set_ctx final : public Backend {
     // job's first SM copy-in node fills, so a job in the steady state costs one graph-node update, not two.
     int fwd_buf = -1;                  // buffer whose H2D SM-copy node forwards; -1 = off
     bool d2h_ind[SET_MAX_BUFFERS] = {};
-    void** fwd_dev = nullptr;          // b device words
+    void** fwd_dev = nullptr;          // per slot two 8-byte device words: the forwarded address, the copy-out blocks' ticket counter
+    int fused_signal_buf = -1;         // the job's ONLY copy-out node is this buffer's SM copy and also stores the completion word
     int check_sizes(const uint32_t* dims);
     bool is_pinned(const void* p);
     void add_pinned_range(const void* p, size_t n);
@@ -323,7 +327,7 @@ void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const v
         ca.dst = (char*)slots[slot].buf[i] + eval(bd.h2d_dev_off, dims);
         ca.bytes = (uint32_t)eval(bd.h2d_bytes, dims);
         if (i == fwd_buf) {
-            ca.fwd_slot = fwd_dev + slot;
+            ca.fwd_slot = fwd_dev + 2 * (size_t)slot;
             ca.fwd_value = const_cast<void*>(fwd_out);
         }
     } else {
@@ -332,12 +336,19 @@ void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const v
         ca.bytes = (uint32_t)eval(bd.d2h_bytes, dims);
         ca.dst_off = eval(bd.d2h_host_off, dims);
     }
-    if (!to_device && d2h_ind[i]) {  // (src, dst_slot, dst_off, bytes)
-        ca.fwd_slot = fwd_dev + slot;
+    if (!to_device && d2h_ind[i]) {  // (src, dst_slot, dst_off, bytes, flag, stamp, fence)
+        ca.fwd_slot = fwd_dev + 2 * (size_t)slot;
+        const bool sig = i == fused_signal_buf;
+        ca.sig_flag = sig ? flags_dev + (size_t)slot * kFlagStride : nullptr;
+        ca.sig_stamp = sig && stamps ? ts_dev + (size_t)slot * 8 + 1 : nullptr;
+        ca.sig_fence = cfg.completion_fence == SET_FENCE_SYSTEM ? 1u : 0u;
         ca.ptrs[0] = &ca.src;
         ca.ptrs[1] = &ca.fwd_slot;
         ca.ptrs[2] = &ca.dst_off;
         ca.ptrs[3] = &ca.bytes;
+        ca.ptrs[4] = &ca.sig_flag;
+        ca.ptrs[5] = &ca.sig_stamp;
+        ca.ptrs[6] = &ca.sig_fence;
         ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY_OUT));
     } else {                         // (src, dst, bytes, fwd_slot, fwd_value)
         ca.ptrs[0] = &ca.src;
@@ -547,7 +558,10 @@ int set_ctx::build_graph(int slot, int set_index) {
             leaves.push_back(g.d2h_nodes[i]);
         }
     }
-    if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished (kernels.cu K14)
+    if (flag_poll && fused_signal_buf >= 0) {
+        // the job's only copy-out node stores the completion word itself (K25); the start stamp only has to have run before it
+        if (stamps) CK(depend(g.stamp_start_node, g.d2h_nodes[fused_signal_buf], false));
+    } else if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished (kernels.cu K14)
         std::vector<bool> leaf_is_kernel;
         for (size_t i = 0; i < bufs.size(); ++i)
             if (!expr_is_zero(bufs[i].d2h_bytes)) leaf_is_kernel.push_back(d2h_sm[i]);
@@ -1307,12 +1321,23 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
                 any_out = any_out || c->d2h_sm[i];
             }
             if (first_in >= 0 && any_out) {
-                if (cudaMalloc((void**)&c->fwd_dev, sizeof(void*) * (size_t)c->b) != cudaSuccess) {
+                if (cudaMalloc((void**)&c->fwd_dev, 2 * sizeof(void*) * (size_t)c->b) != cudaSuccess ||
+                    cudaMemset(c->fwd_dev, 0, 2 * sizeof(void*) * (size_t)c->b) != cudaSuccess) {
                     cudaGetLastError();
                     return c->fail(SET_ERR_NOMEM, "allocation of the forwarding words failed");
                 }
                 c->fwd_buf = first_in;
-                for (size_t i = 0; i < c->bufs.size(); ++i) c->d2h_ind[i] = c->d2h_sm[i];
+                int n_out = 0, only_out = -1;
+                for (size_t i = 0; i < c->bufs.size(); ++i) {
+                    c->d2h_ind[i] = c->d2h_sm[i];
+                    if (!expr_is_zero(c->bufs[i].d2h_bytes)) {
+                        n_out += 1;
+                        only_out = (int)i;
+                    }
+                }
+                // fold the completion signal into the copy-out node where the job has exactly one and the SMs do it
+                const char* fs = getenv("SET_FUSE_SIGNAL");
+                if (c->flag_poll && n_out == 1 && c->d2h_sm[only_out] && !(fs && fs[0] == '0')) c->fused_signal_buf = only_out;
             }
         }
     }

@@ -188,7 +188,9 @@ def test_every_completion_mode_delivers_every_job(libset, cb, disp):
     for config in (0, 4):
         wl = small_workload(config)
         st = check(libset, wl, list(range(wl.jobs)), callback_mode=cb, num_dispatchers=disp)
-        assert st["signal_nodes"] == (wl.jobs if cb == 3 else 0)
+        # flag-polled completion: config 4 (two copy-out nodes) keeps a signal node of its own; config 0's single SM copy-out node
+        # stores the completion word itself (SET_K_COPY_OUT), so no signal node is launched at all
+        assert st["signal_nodes"] == (wl.jobs if cb == 3 and config == 4 else 0)
         assert st["copy_nodes"] == wl.jobs * (2 if config == 0 else 1)
         assert st["max_inflight_seen"] <= wl.max_inflight
 
@@ -219,7 +221,7 @@ def test_completion_word_never_overtakes_the_output(libset):
     n = 5000 -> 20,256 bytes): a word seen early would release the slot and the check would read sentinel bytes."""
     from paper_2606_05495_b200.workloads import Workload
     st = check(libset, Workload(0, (5000,), jobs=600, num_streams=2, max_inflight=4), list(range(600)), pdl=True)
-    assert st["signal_nodes"] == 600 and st["copy_nodes"] == 1200
+    assert st["signal_nodes"] == 0 and st["copy_nodes"] == 1200       # the completion word is stored by the copy-out node itself
 
 
 def test_submit_before_register_and_double_register(libset):
@@ -950,3 +952,18 @@ def test_full_job_count_config5_and_config6(libset):
     _full_count(libset, wl, wl.jobs, 64)                         # 2,048 SSSP jobs over 64 distinct graphs
     wl = baseline_workload(6)
     _full_count(libset, wl, wl.jobs, 96)                         # 4,096 frames over 96 distinct ones
+
+
+@pytest.mark.parametrize("config", [0, 1, 5])
+@pytest.mark.parametrize("fuse,forward", [("1", "1"), ("0", "1"), ("0", "0")])
+def test_signal_fusing_and_output_forwarding_variants(libset, monkeypatch, config, fuse, forward):
+    """The three shapes of a short job's tail: completion word stored by the forwarded copy-out node (default), a signal node
+    of its own behind a forwarded copy-out node, and round 1's shape (two node updates per job, separate signal node)."""
+    from paper_2606_05495_b200.workloads import small_workload
+    monkeypatch.setenv("SET_FUSE_SIGNAL", fuse)
+    monkeypatch.setenv("SET_FORWARD_OUT", forward)
+    wl = small_workload(config)
+    n = min(wl.jobs, 64)
+    st = check(libset, wl, list(range(n)), pdl=True, debug_sentinel=0xA5A5A5A5)
+    assert st["early_completions"] == 0
+    assert st["signal_nodes"] == (0 if fuse == "1" and forward == "1" and config != 5 else n)   # config 5's copy-in is a memcpy node: nothing forwards
