@@ -209,7 +209,7 @@ MODES = {"set": 0, "plain_streams": 1, "batch_sync_graphs": 2, "single_graph": 3
 
 # graph-shape options of every arm (SET and the in-run baselines share the job graph): --sm-copy / --pdl
 OPTS = {"sm_copy_max_bytes": 0, "pdl": True, "num_dispatchers": 0, "submitters": 1, "streams_per_lane": 0, "completion_fence": 0,
-        "completion_thread": 0}
+        "completion_thread": 0, "bind_at_launch": 0}
 
 
 def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup: int, pool: int, out_ring: int,
@@ -220,7 +220,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
     o = dict(OPTS, **(opts or {}))
     ctx = setlib.Context(wl.num_streams, wl.max_inflight, mode=MODES[mode], io=setlib.IO_DEVICE if io_device else setlib.IO_HOST,
                          sm_copy_max_bytes=o["sm_copy_max_bytes"], timestamps=bool(o.get("timestamps")),
-                         streams_per_lane=o["streams_per_lane"], completion_fence=o["completion_fence"], completion_thread=o["completion_thread"],
+                         streams_per_lane=o["streams_per_lane"], completion_fence=o["completion_fence"], completion_thread=o["completion_thread"], bind_at_launch=o["bind_at_launch"],
                          **dict({"num_dispatchers": o["num_dispatchers"]}, **(ctx_kw or {})))
     try:
         ctx.register_builtin(wl.config, wl.variant, list(wl.params), pdl=o["pdl"])

@@ -17,8 +17,9 @@
  *                           executable while another launches one (profiles/r1_ncu.md).  Never set for timing.
  *                           Turned on by itself when the process runs under a CUDA injection library (CUDA_INJECTION64_PATH
  *                           or an NV_NSIGHT_INJECTION_* / NV_COMPUTE_PROFILER_* variable is set); SET_DRIVER_LOCK=0 overrides.
- *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 8: 64 KB in flight per
- *                           copy; more delays the GPU's own command fetches over the same link).
+ *   SET_COPY_MAX_BLOCKS=n   blocks of an SM copy node that READS pinned host memory (default 64 / CUDA streams, between 2 and 8:
+ *                           about 512 KB in flight over all streams saturates the link; more delays the GPU's own command
+ *                           fetches over the same link, DESIGN.md sections 5d and 11).
  *   SET_FUSE_SIGNAL=0       keep the completion signal a node of its own even where the job has a single SM copy-out node that
  *                           could carry it (for A/B measurements; read at set_register_pipeline).
  *   SET_FORWARD_OUT=0       turn output-address forwarding off (read at set_register_pipeline; for A/B measurements).  By default,
@@ -239,9 +240,12 @@ typedef struct set_config {
                                  streams in all, with SET_IO_DEVICE 1 (DESIGN.md 5b gives the measurements).  Forced to 1
                                  when the caller supplies `streams`.  The in-run baseline models use the same streams.  */
     int32_t completion_thread;/* SET_CB_FLAG_POLL: 1 = a thread of its own watches the completion words and runs Algorithm 3, the
-                                 dispatcher(s) only find and launch jobs; 2 = the dispatcher(s) poll between launches (round 1);
-                                 0 => default (1).  DESIGN.md 5d.                                                   */
-    int32_t reserved2;
+                                 dispatcher(s) only find and launch jobs; 2 = the dispatcher(s) poll between launches;
+                                 0 => default (2: measured, the extra thread buys nothing).  DESIGN.md 5d.          */
+    int32_t bind_at_launch;   /* 1 = set_submit only checks the job and queues its description; the executable is updated on the
+                                 dispatcher thread right before it is launched (the JIT update of PAPER.md:122 for every job), so
+                                 that all driver calls of a job come from one thread; 2 = set_submit updates the executable
+                                 (Algorithm 1 literally); 0 => default (2).  DESIGN.md 5d.                            */
     uint32_t debug_sentinel;  /* test hook: non-zero => at the moment a job's completion is observed (before the slot is
                                  released) the first and last 32-bit word of every D2H region of its host_out are compared
                                  with this value; a match means the completion overtook the output, counted in
@@ -456,7 +460,7 @@ int64_t set_selftest_ring(int capacity, int producers, int consumers, int64_t it
  * job completes exactly once, never more than b in flight, no slot runs two jobs at once, a stolen
  * job is bound to the thief's slot.  seed bit 0 selects SET_STEAL_RETARGET, seed bit 1 flag-polled completion
  * (the completers store the slot's word instead of calling Algorithm 3), seed bit 2 a completion thread of its own
- * (set_config.completion_thread).  Returns 0 or a negative error code. */
+ * (set_config.completion_thread), seed bit 3 bind-at-launch (set_config.bind_at_launch).  Returns 0 or a negative error code. */
 int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capacity, int num_dispatchers,
                                int submitters, int64_t jobs, uint32_t seed, uint64_t *out_steals);
 

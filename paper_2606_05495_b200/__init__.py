@@ -75,7 +75,7 @@ class Config(C.Structure):
                 ("io", C.c_int32), ("queue_capacity", C.c_int32), ("num_dispatchers", C.c_int32), ("steal_policy", C.c_int32),
                 ("callback_mode", C.c_int32), ("device", C.c_int32), ("spin_us", C.c_int32), ("sm_copy_max_bytes", C.c_int32),
                 ("timestamps", C.c_int32), ("completion_fence", C.c_int32), ("streams", C.POINTER(C.c_void_p)), ("device_arena", C.c_void_p), ("device_arena_bytes", C.c_uint64),
-                ("streams_per_lane", C.c_int32), ("completion_thread", C.c_int32), ("reserved2", C.c_int32), ("debug_sentinel", C.c_uint32)]
+                ("streams_per_lane", C.c_int32), ("completion_thread", C.c_int32), ("bind_at_launch", C.c_int32), ("debug_sentinel", C.c_uint32)]
 
 
 class Stats(C.Structure):
@@ -177,7 +177,7 @@ class Context:
                  num_dispatchers: int = 0, steal_policy: int = STEAL_SWAP, callback_mode: int = CB_DEFAULT,
                  device: int = -1, spin_us: int = 0, streams=None, device_arena: int = 0, device_arena_bytes: int = 0,
                  sm_copy_max_bytes: int = 0, timestamps: bool = False, completion_fence: int = FENCE_DEFAULT,
-                 streams_per_lane: int = 0, debug_sentinel: int = 0, completion_thread: int = 0):
+                 streams_per_lane: int = 0, debug_sentinel: int = 0, completion_thread: int = 0, bind_at_launch: int = 0):
         self._lib = load()
         self._h = C.c_void_p(None)
         cfg = Config()
@@ -188,7 +188,7 @@ class Context:
         cfg.sm_copy_max_bytes = sm_copy_max_bytes
         cfg.timestamps = 1 if timestamps else 0
         cfg.completion_fence, cfg.streams_per_lane, cfg.debug_sentinel = completion_fence, streams_per_lane, debug_sentinel
-        cfg.completion_thread = completion_thread
+        cfg.completion_thread, cfg.bind_at_launch = completion_thread, bind_at_launch
         self._streams_arr = None
         if streams is not None:
             self._streams_arr = (C.c_void_p * len(streams))(*[int(s) for s in streams])

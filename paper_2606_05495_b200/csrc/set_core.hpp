@@ -105,6 +105,9 @@ class Backend {
     // to this exec (pageable staging), so a thief must retarget this very exec instead of swapping.
     virtual int bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) = 0;
     virtual int launch(int exec, int slot, const JobDesc& job) = 0;
+    // Bind-at-launch mode only: the checks of bind() that concern the job alone (per-job sizes), made at submit time so
+    // that the caller still gets SET_ERR_SIZE synchronously.  Returns 0 or a negative set_status.
+    virtual int validate(const JobDesc&) { return 0; }
     // Called on the completing thread before the slot is released (e.g. staged D2H -> caller memory).
     virtual void finish(int exec, int slot, const JobDesc& job) = 0;
     // Called from a blocked submit/drain every kPollNs: report an asynchronous device failure (a faulting stage
@@ -174,6 +177,11 @@ class Scheduler {
     // Executables that cannot leave their slot (a job graph with a conditional loop is built per slot): a thief may only
     // use an executable of its OWN slot; if it has none free at this instant it hands the job back to the victim's queue.
     void set_slot_bound(bool v) { slot_bound_.store(v, std::memory_order_release); }
+    // Bind at launch: submit() only reserves an executable of the slot and queues the job's description; UpdateGraphParams runs
+    // on the dispatcher thread right before GraphLaunch -- the "JIT update" of PAPER.md:122 applied to every job.  All driver
+    // calls of a job then come from ONE thread: graph updates and launches go through the same driver lock, and issued from two
+    // threads they cost 0.6 + 2.3 us per job on B200, from one thread 0.3 + 1.7 us.
+    void set_bind_at_launch(bool v) { lazy_bind_.store(v, std::memory_order_release); }
 
     int slots() const { return b_; }
     int execs_per_slot() const { return epp_; }
@@ -217,7 +225,9 @@ class Scheduler {
         p.home = slot;
         p.job = job;
         bool pinned = false;
-        int rc = be_->bind(exec, slot, p.job, &pinned);  // UpdateGraphParams(J_id, i)
+        const bool lazy = lazy_bind_.load(std::memory_order_acquire);
+        int rc = lazy ? be_->validate(p.job) : be_->bind(exec, slot, p.job, &pinned);  // UpdateGraphParams(J_id, i)
+        if (lazy) p.home |= kUnboundBit;
         if (rc != 0) {
             free_execs_[slot].r.push(exec);
             space_ec_.notify_all();
@@ -289,6 +299,7 @@ class Scheduler {
 
   private:
     static constexpr int32_t kPinnedBit = 1 << 30;
+    static constexpr int32_t kUnboundBit = 1 << 29;
     static constexpr uint64_t kPollNs = 20000000ull;  // 20 ms
     template <typename T>
     struct alignas(kCacheLine) PaddedRing {
@@ -354,6 +365,7 @@ class Scheduler {
     bool launch_job(Prepared p, int w, bool stolen) {
         uint64_t t0 = now_ns();
         bool pinned = (p.home & kPinnedBit) != 0;
+        const bool unbound = (p.home & kUnboundBit) != 0;  // bind-at-launch: nothing is tied to the executable yet
         int exec = p.exec;
         int rc = 0;
         if (stolen && slot_bound_.load(std::memory_order_acquire)) {
@@ -362,7 +374,7 @@ class Scheduler {
             if (pinned || !free_execs_[w].r.try_pop(mine)) {
                 // staged data lives with the victim's executable, or every executable of w is in a submitter's hands right
                 // now: un-steal (there is room: the entry was just popped from that queue; jobs are independent, so order is free)
-                queues_[p.home & ~kPinnedBit].r.push(p);
+                queues_[p.home & ~(kPinnedBit | kUnboundBit)].r.push(p);
                 n_queued_.fetch_add(1, std::memory_order_seq_cst);
                 return false;
             }
@@ -387,6 +399,9 @@ class Scheduler {
                 // W_free's buffers and write W_free's output memory.
                 rc = be_->bind(exec, w, p.job, &dummy);
             }
+        } else if (unbound) {
+            bool dummy = false;
+            rc = be_->bind(exec, w, p.job, &dummy);  // the slot's own job: UpdateGraphParams now, on the launching thread
         }
         Running& r = running_[w];
         r.exec = exec;
@@ -505,6 +520,7 @@ class Scheduler {
     bool own_poller_ = false;
     std::atomic<bool> stop_{false};
     std::atomic<bool> slot_bound_{false};
+    std::atomic<bool> lazy_bind_{false};
     std::atomic<int> err_{0};
     CoreStats stats_;
     std::vector<std::thread> dispatchers_;

@@ -211,6 +211,7 @@ struct set_ctx final : public Backend {
     // ------------------------------------------------------------------ Backend interface
     int bind(int exec, int slot, JobDesc& job, bool* pinned_to_exec) override;
     int launch(int exec, int slot, const JobDesc& job) override;
+    int validate(const JobDesc& job) override { return check_sizes(job.dims); }
     void finish(int exec, int slot, const JobDesc& job) override;
     int poll() override;
     volatile uint32_t* done_flags() override { return flag_poll ? flags_host : nullptr; }
@@ -359,12 +360,14 @@ void set_ctx::copy_params(CopyArgs& ca, int slot, int i, bool to_device, const v
         ca.kp.func = const_cast<void*>(set_builtin_kernel(SET_K_COPY));
     }
     uint32_t pieces = (ca.bytes + SET_COPY_BYTES_PER_BLOCK - 1) / SET_COPY_BYTES_PER_BLOCK;
-    // Reads of pinned host memory share the link with the GPU's own fetches of launch commands: eight streams that each
-    // put 128 KB of reads in flight at once delay the start of every stream's next graph (measured: 15 us between graphs
-    // with 16 blocks per copy, 12 us with 4; profiles/r1_bench.md).  Eight blocks per H2D copy (64 KB in flight, the kernel
-    // strides over the rest) gave the best jobs/s; stores to host memory and HBM-to-HBM copies are not capped.
+    // Reads of pinned host memory share the link with the GPU's own fetches of launch commands: streams that each put 128 KB of
+    // reads in flight at once delay the start of every stream's next graph, and the link is saturated by about 512 KB in
+    // flight over all streams.  So a copy that reads host memory gets 64 / (CUDA streams) blocks of 8 KB, between 2 and 8 (the
+    // kernel strides over the rest).  Measured, config 1 end to end (profiles/r2_probes.md): 32 streams -- 1 / 2 / 3 / 4 / 8 / 16
+    // blocks give 367 / 380 / 373 / 353 / 325 / 303 K jobs/s (380 K is the duplex link bound); 8 streams -- 1 / 2 / 3 / 8 blocks
+    // give 163 / 194 / 203 / 219 K.  Stores to host memory and HBM-to-HBM copies are not capped.
     if (to_device && cfg.io == SET_IO_HOST) {
-        const uint32_t cap = copy_max_blocks ? copy_max_blocks : 8u;
+        const uint32_t cap = copy_max_blocks ? copy_max_blocks : (uint32_t)std::min(8, std::max(2, 64 / std::max(1, H)));
         if (pieces > cap) pieces = cap;
     }
     ca.kp.gridDim = dim3(pieces ? pieces : 1);
@@ -1080,7 +1083,12 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.completion_fence == SET_FENCE_DEFAULT) cfg.completion_fence = SET_FENCE_SYSTEM;
     if (cfg.streams_per_lane < 0 || cfg.streams_per_lane > 4096) return SET_ERR_INVALID;
     if (cfg.completion_thread < 0 || cfg.completion_thread > 2) return SET_ERR_INVALID;
-    if (cfg.completion_thread == 0) cfg.completion_thread = 1;
+    // Both defaults are round 1's arrangement: measured on B200 neither a completion thread of its own nor binding at launch moves
+    // jobs/s on configs 0 and 1 (bind falls from 0.56 to 0.27 us per job, launch rises by as much: DESIGN.md 5d), and binding at
+    // launch costs config 4 device-resident 10 % (its 3.4 us full rebinds land on the dispatcher).
+    if (cfg.completion_thread == 0) cfg.completion_thread = 2;
+    if (cfg.bind_at_launch < 0 || cfg.bind_at_launch > 2) return SET_ERR_INVALID;
+    if (cfg.bind_at_launch == 0) cfg.bind_at_launch = 2;
     // Default (measured on B200): with host I/O a job's chain is latency-bound (its copy-in waits on the link),
     // so every slot gets a CUDA stream of its own -- the paper's worker W_i = (S_i, G_i, M_i), PAPER.md:110 -- and b chains are
     // in flight instead of S (config 1 end to end 201 K -> 316 K jobs/s, config 0 227 K -> 336 K).  With device-resident I/O
@@ -1353,6 +1361,7 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     if (c->slot_graphs && c->cfg.mode == SET_MODE_PLAIN_STREAMS)
         return c->fail(SET_ERR_INVALID, "a pipeline with a loop needs a job graph: SET_MODE_PLAIN_STREAMS cannot run it");
     if (c->slot_graphs && c->sched) c->sched->set_slot_bound(true);
+    if (c->sched) c->sched->set_bind_at_launch(c->cfg.bind_at_launch == 1);
     c->nsets.resize(c->slot_graphs ? (size_t)c->b * c->epp : 1);
     if (!c->slot_graphs)
         if (int rc = c->build_graph(0, 0)) return rc;

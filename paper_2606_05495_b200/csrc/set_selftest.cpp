@@ -189,6 +189,7 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
     int64_t rc = 0;
     {
         Scheduler sched(&be, num_streams, b, queue_capacity, num_dispatchers, policy, 20, /*poller=*/(seed >> 2) & 1);
+        sched.set_bind_at_launch((seed >> 3) & 1);
         be.attach(&sched);
         std::atomic<int64_t> next{0};
         std::vector<std::thread> subs;
