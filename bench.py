@@ -747,7 +747,7 @@ def compact_line(wl, world, steps, warmup, n_jobs, ms_dev, value, ms_e2e, e2e_va
             "ms_per_step": _r(ms_dev, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype,
             "data": "synthetic",
             "config": {"workload": wl.name, "jobs_per_step_per_gpu": n_jobs, "num_streams": wl.num_streams, "max_inflight": wl.max_inflight,
-                       "streams_per_lane": detail.get("streams_per_lane"), "io": "value: HBM-resident I/O; e2e: pinned host",
+                       "streams_per_lane": detail.get("streams_per_lane"), "io": "value: HBM-resident; e2e: pinned host",
                        "l2": f"{L2_FLUSH_BYTES >> 20} MiB flush/step; {dev_arm['in_bytes'] / 1e6:.0f} MB inputs/step"},
             "clocks": clocks,
             "e2e": {"value": _r(e2e_value), "unit": "jobs/s", "h2d_bytes_per_step": int(e2e_arm["h2d_bytes"] * world),
@@ -772,7 +772,7 @@ def compact_line(wl, world, steps, warmup, n_jobs, ms_dev, value, ms_e2e, e2e_va
           # per CUDA stream: start(next job) - end(previous job); device-wide: intervals with no job in progress anywhere
           "gap_between_jobs_us": {"set": pick("set_e2e", "gap_mean_us", 2), "batch_sync": pick("batch_sync_graphs_e2e", "gap_mean_us", 2),
                                   "set_p99": pick("set_e2e", "gap_p99_us", 2), "batch_sync_p99": pick("batch_sync_graphs_e2e", "gap_p99_us", 2)},
-          "device_idle_gaps_count_meanus": {"set": [pick("set_e2e", "idle_gaps", 0), pick("set_e2e", "idle_gap_mean_us", 2)],
+          "idle_gaps_n_meanus": {"set": [pick("set_e2e", "idle_gaps", 0), pick("set_e2e", "idle_gap_mean_us", 2)],
                                             "batch_sync": [pick("batch_sync_graphs_e2e", "idle_gaps", 0), pick("batch_sync_graphs_e2e", "idle_gap_mean_us", 2)]},
           "sched_overhead_frac": {"set": pick("set_e2e", "overhead_frac", 4), "batch_sync": pick("batch_sync_graphs_e2e", "overhead_frac", 4)},
           "host_us_per_job": {"set": _r(sum(e2e_arm["host_us_per_job"][k] for k in ("submit", "launch", "callback")), 3),

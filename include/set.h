@@ -241,7 +241,8 @@ typedef struct set_config {
                                  when the caller supplies `streams`.  The in-run baseline models use the same streams.  */
     int32_t completion_thread;/* SET_CB_FLAG_POLL: 1 = a thread of its own watches the completion words and runs Algorithm 3, the
                                  dispatcher(s) only find and launch jobs; 2 = the dispatcher(s) poll between launches;
-                                 0 => default (2: measured, the extra thread buys nothing).  DESIGN.md 5d.          */
+                                 0 => default (1 from max_inflight = 16 up: +6-10 % on config 1 end to end where the host
+                                 is slow; 2 below: the hand-off costs a latency-bound config 6 %).  DESIGN.md 5d.   */
     int32_t bind_at_launch;   /* 1 = set_submit only checks the job and queues its description; the executable is updated on the
                                  dispatcher thread right before it is launched (the JIT update of PAPER.md:122 for every job), so
                                  that all driver calls of a job come from one thread; 2 = set_submit updates the executable

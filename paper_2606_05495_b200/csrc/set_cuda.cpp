@@ -1083,10 +1083,14 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     if (cfg.completion_fence == SET_FENCE_DEFAULT) cfg.completion_fence = SET_FENCE_SYSTEM;
     if (cfg.streams_per_lane < 0 || cfg.streams_per_lane > 4096) return SET_ERR_INVALID;
     if (cfg.completion_thread < 0 || cfg.completion_thread > 2) return SET_ERR_INVALID;
-    // Both defaults are round 1's arrangement: measured on B200 neither a completion thread of its own nor binding at launch moves
-    // jobs/s on configs 0 and 1 (bind falls from 0.56 to 0.27 us per job, launch rises by as much: DESIGN.md 5d), and binding at
-    // launch costs config 4 device-resident 10 % (its 3.4 us full rebinds land on the dispatcher).
-    if (cfg.completion_thread == 0) cfg.completion_thread = 2;
+    // Measured on B200: once the copy-in kernels keep the link full, config 1 end to end sits at the edge between
+    // link-bound and host-bound -- on a box whose cudaGraphLaunch takes 2.2 us instead of 1.95 us a dispatcher that also polls and
+    // completes delivers 341-355 K jobs/s, with a completion thread of its own 375-377 K (the link bound).  Binding at launch adds
+    // nothing to that (349-351 K without the thread, 376 K with it) and costs config 4 device-resident 10 % (its 3.4 us full
+    // rebinds land on the dispatcher): off by default.
+    // The hand-off from the completion thread to the dispatcher adds a fraction of a microsecond to every job's turnaround, which
+    // a latency-bound configuration feels (config 0, 8 in flight: 316 K -> 297 K jobs/s): the thread is the default from 16 slots up.
+    if (cfg.completion_thread == 0) cfg.completion_thread = cfg.max_inflight >= 16 ? 1 : 2;
     if (cfg.bind_at_launch < 0 || cfg.bind_at_launch > 2) return SET_ERR_INVALID;
     if (cfg.bind_at_launch == 0) cfg.bind_at_launch = 2;
     // Default (measured on B200): with host I/O a job's chain is latency-bound (its copy-in waits on the link),
