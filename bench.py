@@ -432,8 +432,8 @@ def stage_algorithmic(wl, dims):
         px = dims[0] * dims[1]
         return [("rgb2gray_u8", "hbm", 4 * px), ("blur3x3_u8", "hbm", 2 * px), ("hist256_u8", "hbm", px + 1024)]
     if c == 5:  # timed alone the relaxation sees an empty frontier: it scans the V flags and stops (latency-class)
-        v = p[0]
-        return [("sssp_init", "hbm", 12 * v), ("sssp_relax", "hbm", 4 * v), ("sssp_control", "hbm", 16)]
+        v, unroll = p[0], (p[2] if len(p) > 2 else 4)
+        return [("sssp_init", "hbm", 12 * v)] + [("sssp_relax", "hbm", 4 * v)] * unroll + [("sssp_control", "hbm", 16)]
     if c == 6:
         px = dims[0] * dims[1]
         return [("rgb2gray_u8", "hbm", 4 * px), ("sobel3x3_u8", "hbm", 2 * px), ("mean3x3_u8", "hbm", 2 * px), ("threshold_u8", "hbm", 2 * px),
@@ -767,7 +767,7 @@ def compact_line(wl, world, steps, warmup, n_jobs, ms_dev, value, ms_e2e, e2e_va
         return _r(v.get(field), nd) if isinstance(v, dict) and field in v else None
 
     bs = base.get("batch_sync_graphs_e2e", {}).get("jobs_per_s")
-    hm = {"set_e2e_jobs_per_s": _r(e2e_value), "batch_sync_e2e_jobs_per_s": _r(bs),
+    hm = {"batch_sync_e2e_jobs_per_s": _r(bs),  # SET's own is e2e.value
           "set_over_batch_sync_e2e": _r(e2e_value / bs, 3) if bs else None,
           # per CUDA stream: start(next job) - end(previous job); device-wide: intervals with no job in progress anywhere
           "gap_between_jobs_us": {"set": pick("set_e2e", "gap_mean_us", 2), "batch_sync": pick("batch_sync_graphs_e2e", "gap_mean_us", 2),
@@ -793,7 +793,7 @@ def compact_line(wl, world, steps, warmup, n_jobs, ms_dev, value, ms_e2e, e2e_va
     side = {}
     for k, v in (detail.get("workloads") or {}).items():
         side[k] = [v.get("e2e"), (v.get("pipeline_roofline") or {}).get("e2e_frac"), v.get("speedup_vs_batch_sync_e2e")] \
-            if "error" not in v else "error: " + v["error"][:50]
+            if "error" not in v else "error: " + v["error"][:24]  # the full text is in the detail file
     if side:
         line["workloads_e2e_frac_vsbatch"] = side  # per config: [e2e jobs/s, fraction of its pipeline roofline, SET / batch-sync]
     kroofs = {}

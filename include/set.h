@@ -122,7 +122,13 @@ typedef struct set_arg_desc {
                                    loop body one by one): the kernels of the body may not take SET_ARG_DIM arguments or dim-dependent
                                    offsets / grids (per-job sizes travel in the job's device image instead), a job is never
                                    retargeted to another slot's executable (a thief without a free executable of its own
-                                   puts the job back), and SET_MODE_PLAIN_STREAMS is refused.  One loop per pipeline.   */
+                                   puts the job back), and SET_MODE_PLAIN_STREAMS is refused.  One loop per pipeline.
+                                   The body needs at least 3 stages: a two-node body failed about once in 10^5 jobs on this
+                                   driver (cudaErrorLaunchFailure, the context is lost) and is refused with SET_ERR_INVALID.
+                                   In SET_MODE_SET such a pipeline runs one job at a time on each of at most 8 CUDA streams
+                                   (the largest divisor of num_streams that is <= 8), whatever max_inflight and
+                                   streams_per_lane say: more WHILE graphs in flight than that fail now and then on this
+                                   driver, and a WHILE graph queued behind a running one slows both.      */
 #define SET_STAGE_LOOP_END   4u
 #define SET_STAGE_PDL 1u   /* connect this stage to the node before it (the previous stage; for the first stage,
                               an SM copy node) with a programmatic-dependent-launch edge.  By setting the flag the
@@ -278,7 +284,8 @@ typedef struct set_stats {
     uint64_t copy_nodes;       /* SET_K_COPY kernel launches (copies done by the SMs)                 */
     uint64_t early_completions;/* set_config.debug_sentinel: jobs whose output still held the sentinel when their completion
                                   was observed (must stay 0)                                             */
-    uint64_t cuda_streams;     /* CUDA streams the context runs on: num_streams * streams_per_lane (not a counter) */
+    uint64_t cuda_streams;     /* CUDA streams jobs run on: num_streams * streams_per_lane, or at most 8 once a pipeline with a
+                                  loop is registered (SET_STAGE_LOOP_BEGIN says why) (not a counter)     */
 } set_stats;
 
 /* ---------------------------------------------------------------------------------------------- *
@@ -421,10 +428,12 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
 #define SET_K_BLEND_U8       20  /* (const uint8* t, const uint8* n, uint8* out, uint32 w, uint32 h)  (t + n) >> 1        */
 #define SET_K_SSSP_INIT      21  /* (const int32* img, int32* out, uint32* scratch, uint32 maxV)  dist = INF, dist[src] = 0,
                                     frontier = {src};  img = [V, E, src, 0][row_ptr V+1][col E][w E]               */
-#define SET_K_SSSP_RELAX     22  /* (img, out, scratch, maxV)  one frontier round: atomicMin relaxation of every edge
-                                    out of the frontier, next frontier = vertices whose distance got smaller       */
-#define SET_K_SSSP_CONTROL   23  /* (img, out, scratch, maxV, loop handle)  counts the round and sets the condition of
-                                    the enclosing WHILE node: another round iff some distance changed               */
+#define SET_K_SSSP_RELAX     22  /* (img, out, scratch, maxV, uint32 sub)  one frontier round, the sub-th of the U a pass
+                                    of the loop body holds: atomicMin relaxation of every edge out of the frontier, next
+                                    frontier = vertices whose distance got smaller; scratch = flags[2][maxV], ctrl[16] */
+#define SET_K_SSSP_CONTROL   23  /* (img, out, scratch, maxV, uint32 U, loop handle)  counts the rounds of this pass that
+                                    had a frontier and sets the condition of the enclosing WHILE node: another pass iff
+                                    the pass's last round changed some distance                                      */
 
 /* HOST address usable as set_stage_desc.func, or NULL for an unknown id. */
 const void *set_builtin_kernel(int kernel_id);
@@ -433,7 +442,8 @@ const void *set_builtin_kernel(int kernel_id);
  *   params : HOST array of uint32 or NULL for the BASELINE sizes:
  *     config 0: {n}            config 1: {n}          config 2: {h, w, sweeps[, alternate = 1]}
  *     config 3: {M, N, K}      config 4: {max_w, max_h}  (dims per job = {w, h, 1, 1})
- *     config 5 (SSSP): {maxV, maxE}  (dims per job = {E, 1, 1, 1}; V, E, src travel in the job image)
+ *     config 5 (SSSP): {maxV, maxE[, U = 4]}  (dims per job = {E, 1, 1, 1}; V, E, src travel in the job
+ *               image; U = 2..8 relaxation rounds per pass of the WHILE body, 2 + U stage kernels in all)
  *     config 6 (Sobel chain): {max_w, max_h[, thresh = 64]}  (dims per job = {w, h, 1, 1})
  *   variant: 0 = default.  config 0: 1 = histogram of the INPUT values (reading C0-1 alternative).
  * *            any config: bit 8 set = append a SET_K_SPIN delay stage that busy-waits dims[3] nanoseconds.

@@ -28,8 +28,8 @@ __global__ void set_k_mean3x3_u8(const uint8_t* e, uint8_t* m, uint32_t w, uint3
 __global__ void set_k_threshold_u8(const uint8_t* m, uint8_t* t, uint32_t w, uint32_t h, uint32_t thresh);
 __global__ void set_k_blend_u8(const uint8_t* t, const uint8_t* n, uint8_t* out, uint32_t w, uint32_t h);
 __global__ void set_k_sssp_init(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
-__global__ void set_k_sssp_relax(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
-__global__ void set_k_sssp_control(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, cudaGraphConditionalHandle loop);
+__global__ void set_k_sssp_relax(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, uint32_t sub);
+__global__ void set_k_sssp_control(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, uint32_t unroll, cudaGraphConditionalHandle loop);
 }
 
 // Programmatic dependent launch (SET_STAGE_PDL edges of the job graph): let the next kernel node be scheduled now,
@@ -52,3 +52,4 @@ constexpr int kHistPixPerBlock = 256 * 16;  // one 128-bit load per thread; a 12
 constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words
 constexpr int kStencilTileW = 64 * 4, kStencilTileH = 4;  // K17/K18: block (64, 4), 4 pixels per thread
 constexpr int kBytePixPerBlock = 256 * 16;                // K19/K20: one 128-bit word per thread
+constexpr unsigned kSsspLanes = 8;                        // K22: threads per vertex (blocks of 256 threads: 32 vertices each)

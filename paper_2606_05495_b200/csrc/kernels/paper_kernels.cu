@@ -1,7 +1,7 @@
 // paper_kernels.cu -- stage kernels of the two paper workloads added in round 2:
 //   config 6, the five-stage Sobel chain:  K10 gray (stencil_kernels.cu) -> K17 sobel -> K18 mean3x3 ->
 //             K19 threshold -> K20 blend, all integer, bit-exact (readings S6-1..S6-6)
-//   config 5, frontier Bellman-Ford SSSP:  K21 init -> WHILE { K22 relax -> K23 control } (readings S5-1..S5-4);
+//   config 5, frontier Bellman-Ford SSSP:  K21 init -> WHILE { K22 relax x U -> K23 control } (readings S5-1..S5-4);
 //             the loop is a conditional WHILE node of the job graph and K23 sets its condition on the device.
 // Hand-written CUDA for sm_100a.  The frames (0.3 - 2 MB) and graphs (~0.6 MB) sit in L2 right after the H2D copy, so
 // these are latency-class kernels like those of configs 0, 1 and 4: coalesced 32- and 128-bit accesses, no shared memory.
@@ -114,13 +114,18 @@ extern "C" __global__ void __launch_bounds__(256) set_k_blend_u8(const uint8_t* 
 
 // ------------------------------------------------------------------------------------------------------------
 // SSSP.  Device image of a job (mirrors host_in): int32 [V, E, src, 0][row_ptr V+1][col E][w E].
-// out: int32 [dist V][rounds, 0, 0, 0] (mirrors host_out).  scratch: uint32 flags[2][maxV] then ctrl[4] = {changed, round, -, -}.
-// The frontier is a flag per vertex, double-buffered by the parity of the round, so that a round never clears a flag
-// another thread of the same round is setting.  Distances are relaxed IN PLACE with atomicMin: a vertex may pick up a
-// distance lowered earlier in the same round, so the GPU needs at most as many rounds as the oracle's synchronous rounds
-// and ends on the same, unique, distances (reading S5-4).
+// out: int32 [dist V][rounds, 0, 0, 0] (mirrors host_out).
+// scratch: uint32 flags[2][maxV], then ctrl[16] = {-, rounds, relaxations done, -, changed[0..U-1], ...}.
+// The frontier is a flag per vertex, double-buffered by the parity of the relaxation's running number, so that a
+// relaxation never clears a flag another thread of the same relaxation is setting.  Distances are relaxed IN PLACE with
+// atomicMin: a vertex may pick up a distance lowered earlier in the same round, so the GPU needs at most as many rounds
+// as the oracle's synchronous rounds and ends on the same, unique, distances (reading S5-4).
+// One pass of the WHILE body is U relaxation kernels (sub = 0 .. U-1) and the control kernel: every pass of a WHILE node
+// costs a device-side relaunch that the chip serialises over all graphs in flight (about 4-5 us), while
+// a relaxation over an empty frontier is a 2 us kernel, so U = 4 trades up to U-1 of those for 3/4 of the relaunches.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kSsspInf = 0x7fffffff;
+constexpr uint32_t kSsspCtrlWords = 16, kSsspRounds = 1, kSsspDone = 2, kSsspChanged = 4;
 
 extern "C" __global__ void __launch_bounds__(256) set_k_sssp_init(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
                                                                   uint32_t max_v) {
@@ -133,30 +138,39 @@ extern "C" __global__ void __launch_bounds__(256) set_k_sssp_init(const int32_t*
         f0[v] = v == src ? 1u : 0u;
         f1[v] = 0u;
     }
-    if (blockIdx.x == 0 && threadIdx.x < 4) {
-        scratch[2 * (size_t)max_v + threadIdx.x] = 0u;  // changed = 0, round = 0
-        out[V + threadIdx.x] = 0;
+    if (blockIdx.x == 0 && threadIdx.x < kSsspCtrlWords) {
+        scratch[2 * (size_t)max_v + threadIdx.x] = 0u;
+        if (threadIdx.x < 4) out[V + threadIdx.x] = 0;
     }
 }
 
+// K22: kSsspLanes threads per vertex (a group never straddles a warp): lane g of the group relaxes edges g, g + 8, ... of
+// its vertex, so a round is one dependent chain flag -> row_ptr -> (col, w) -> atomicMin whatever the out-degree, instead
+// of out-degree atomics one behind the other.  The flag is read by the whole group before lane 0 clears it.
 extern "C" __global__ void __launch_bounds__(256) set_k_sssp_relax(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
-                                                                   uint32_t max_v) {
+                                                                   uint32_t max_v, uint32_t sub) {
     set_pdl_sync();
     const uint32_t V = min((uint32_t)img[0], max_v);
     const int32_t* row_ptr = img + 4;
     const int32_t* col = row_ptr + V + 1;
     const int32_t* wgt = col + img[1];
     uint32_t* ctrl = scratch + 2 * (size_t)max_v;
-    const uint32_t round = ctrl[1];
-    uint32_t* fin = scratch + (round & 1u) * (size_t)max_v;
-    uint32_t* fout = scratch + ((round + 1u) & 1u) * (size_t)max_v;
+    const uint32_t number = ctrl[kSsspDone] + sub;  // this relaxation's running number within the job
+    uint32_t* fin = scratch + (number & 1u) * (size_t)max_v;
+    uint32_t* fout = scratch + ((number + 1u) & 1u) * (size_t)max_v;
+    constexpr uint32_t kPerWarp = 32 / kSsspLanes;
+    const uint32_t g = threadIdx.x % kSsspLanes, in_warp = (threadIdx.x % 32) / kSsspLanes;
+    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, warps = gridDim.x * blockDim.x / 32;
     bool any = false;
-    for (uint32_t u = blockIdx.x * blockDim.x + threadIdx.x; u < V; u += gridDim.x * blockDim.x) {
-        if (!fin[u]) continue;
-        fin[u] = 0u;
+    for (uint32_t base = warp * kPerWarp; base < V; base += warps * kPerWarp) {  // uniform over the warp
+        const uint32_t u = base + in_warp;
+        const uint32_t f = u < V ? fin[u] : 0u;
+        __syncwarp();
+        if (!f) continue;
+        if (g == 0) fin[u] = 0u;
         const int32_t du = *reinterpret_cast<volatile int32_t*>(out + u);  // finite: u entered the frontier by getting a distance
         const int32_t e1 = __ldg(row_ptr + u + 1);
-        for (int32_t e = __ldg(row_ptr + u); e < e1; ++e) {
+        for (int32_t e = __ldg(row_ptr + u) + (int32_t)g; e < e1; e += (int32_t)kSsspLanes) {
             const int32_t v = __ldg(col + e), nd = du + __ldg(wgt + e);
             if (nd < atomicMin(out + v, nd)) {
                 fout[v] = 1u;
@@ -164,19 +178,23 @@ extern "C" __global__ void __launch_bounds__(256) set_k_sssp_relax(const int32_t
             }
         }
     }
-    if (any) ctrl[0] = 1u;
+    if (any) ctrl[kSsspChanged + sub] = 1u;  // the next relaxation's frontier is not empty
 }
 
-// K23: the loop's condition.  One thread: count the round, report it, and keep the WHILE node going while the round
-// just finished lowered some distance (at most V rounds: Bellman-Ford's bound with non-negative weights).
+// K23: the loop's condition.  One thread: count the rounds that had a frontier (relaxation 0 of a pass always has one;
+// relaxation s + 1 has one iff relaxation s lowered a distance), report the count, and keep the WHILE node going while the
+// last relaxation of the pass lowered some distance (at most V rounds: Bellman-Ford's bound with non-negative weights).
 extern "C" __global__ void set_k_sssp_control(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch, uint32_t max_v,
-                                              cudaGraphConditionalHandle loop) {
+                                              uint32_t unroll, cudaGraphConditionalHandle loop) {
     set_pdl_sync();
     const uint32_t V = min((uint32_t)img[0], max_v);
     uint32_t* ctrl = scratch + 2 * (size_t)max_v;
-    const uint32_t changed = ctrl[0], round = ctrl[1] + 1u;
-    ctrl[0] = 0u;
-    ctrl[1] = round;
-    out[V] = (int32_t)round;
-    cudaGraphSetConditional(loop, (changed != 0u && round <= V) ? 1u : 0u);
+    uint32_t rounds = ctrl[kSsspRounds] + 1u;
+    for (uint32_t s = 0; s + 1 < unroll; ++s) rounds += ctrl[kSsspChanged + s] ? 1u : 0u;
+    const uint32_t last = ctrl[kSsspChanged + unroll - 1];
+    for (uint32_t s = 0; s < unroll; ++s) ctrl[kSsspChanged + s] = 0u;
+    ctrl[kSsspRounds] = rounds;
+    ctrl[kSsspDone] += unroll;
+    out[V] = (int32_t)rounds;
+    cudaGraphSetConditional(loop, (last != 0u && rounds <= V) ? 1u : 0u);
 }

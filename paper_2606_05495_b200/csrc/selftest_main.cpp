@@ -30,12 +30,13 @@ int main(int argc, char** argv) {
                rc == 0 ? "ok" : "FAILED", (long long)rc);
         if (rc) ++bad;
     }
-    // S, b, q, dispatchers, submitters, jobs, seed (bit 0: retarget steals, bit 1: flag-polled completion, bit 2: own poller thread)
+    // S, b, q, dispatchers, submitters, jobs, seed (bit 0: retarget steals, bit 1: flag-polled completion, bit 2: own poller thread, ...)
     struct S { int S, b, q, disp, subs; int64_t jobs; uint32_t seed; } scheds[] = {
         {4, 8, 2, 1, 1, 10000, 0}, {8, 32, 2, 1, 1, 10000, 1}, {8, 32, 2, 3, 2, 10000, 2}, {8, 32, 2, 2, 2, 10000, 3},
         {1, 1, 1, 1, 1, 1000, 3},  {4, 6, 1, 2, 3, 5000, 5},   {2, 64, 4, 2, 2, 10000, 4}, {8, 4096, 1, 1, 2, 20000, 2},
         {8, 32, 2, 1, 1, 10000, 6}, {8, 32, 2, 2, 2, 10000, 7}, {4, 8, 2, 1, 2, 10000, 6},   // bit 2: completion thread of its own
-        {8, 32, 2, 1, 1, 10000, 14}, {8, 32, 2, 2, 2, 10000, 9}, {4, 8, 2, 1, 2, 10000, 10}, {8, 32, 2, 2, 1, 10000, 15}};  // bit 3: bind at launch
+        {8, 32, 2, 1, 1, 10000, 14}, {8, 32, 2, 2, 2, 10000, 9}, {4, 8, 2, 1, 2, 10000, 10}, {8, 32, 2, 2, 1, 10000, 15},  // bit 3: bind at launch
+        {8, 32, 2, 1, 1, 10000, 18}, {4, 32, 2, 2, 3, 10000, 22}, {8, 16, 2, 2, 2, 10000, 26}};  // bit 4: slots beyond the streams retired, slot-bound
     for (auto& s : scheds) {
         uint64_t steals = 0;
         int64_t rc = set_selftest_scheduler(s.S, s.b, s.q, s.disp, s.subs, s.jobs * scale, s.seed, &steals);

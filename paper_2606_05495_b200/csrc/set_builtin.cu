@@ -225,9 +225,9 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
                              {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});
             break;
         }
-        case 5: {  // SSSP by frontier Bellman-Ford: init -> WHILE { relax -> control }   (readings S5-1..S5-4)
-            uint32_t maxv = P(0, 4096), maxe = P(1, 15 * 4096);
-            if (maxv == 0 || maxe == 0) return SET_ERR_INVALID;
+        case 5: {  // SSSP by frontier Bellman-Ford: init -> WHILE { relax x U -> control }   (readings S5-1..S5-4)
+            uint32_t maxv = P(0, 4096), maxe = P(1, 15 * 4096), unroll = P(2, 4);  // U relaxations per pass of the loop (paper_kernels.cu)
+            if (maxv == 0 || maxe == 0 || unroll < 2 || unroll > 8) return SET_ERR_INVALID;  // U = 1 is a two-node body: set_register_pipeline refuses it
             const uint64_t head = 16ull + 4ull * (maxv + 1);  // [V, E, src, 0][row_ptr]; then col and w, 8 bytes per edge
             in_bytes = head + 8ull * maxe;
             out_bytes = 4ull * maxv + 16;                      // [dist][rounds, 0, 0, 0]
@@ -235,13 +235,17 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[0].h2d_bytes = set_size_expr{head, 8, 0x1, 0};  // dims[0] = E of the job
             bf[1] = buffer(out_bytes);
             bf[1].d2h_bytes = fixed(out_bytes);
-            bf[2] = buffer(8ull * maxv + 16);                  // frontier flags [2][maxV], ctrl[4]
+            bf[2] = buffer(8ull * maxv + 64);                  // frontier flags [2][maxV], ctrl[16]
             nb = 3;
             const set_grid_rule g = grid_fixed((maxv + 255) / 256);
             st[ns++] = stage(SET_K_SSSP_INIT, g, grid_fixed(1), 256, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
-            st[ns] = stage(SET_K_SSSP_RELAX, g, grid_fixed(1), 256, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
-            st[ns++].flags = SET_STAGE_LOOP_BEGIN;
-            st[ns] = stage(SET_K_SSSP_CONTROL, grid_fixed(1), grid_fixed(1), 1, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv), arg_cond()});
+            for (uint32_t sub = 0; sub < unroll; ++sub) {
+                st[ns] = stage(SET_K_SSSP_RELAX, grid_fixed((uint32_t)(((uint64_t)maxv * kSsspLanes + 255) / 256)), grid_fixed(1), 256, 1, 0,
+                               {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv), arg_u32(sub)});
+                st[ns++].flags = sub == 0 ? SET_STAGE_LOOP_BEGIN : 0u;
+            }
+            st[ns] = stage(SET_K_SSSP_CONTROL, grid_fixed(1), grid_fixed(1), 1, 1, 0,
+                           {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv), arg_u32(unroll), arg_cond()});
             st[ns++].flags = SET_STAGE_LOOP_END;
             break;
         }

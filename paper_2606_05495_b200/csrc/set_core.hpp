@@ -158,6 +158,7 @@ class Scheduler {
         // the main thread initialises all workers; all of them start idle.
         for (int w = 0; w < b_; ++w) pool_.push(w);
         n_free_.store(b_, std::memory_order_relaxed);
+        active_ = b_;
         own_poller_ = flags_ != nullptr && poller != 0;
         for (int d = 0; d < num_dispatchers; ++d) dispatchers_.emplace_back([this] { dispatcher_loop(); });
         if (own_poller_) dispatchers_.emplace_back([this] { poller_loop(); });
@@ -182,6 +183,28 @@ class Scheduler {
     // calls of a job then come from ONE thread: graph updates and launches go through the same driver lock, and issued from two
     // threads they cost 0.6 + 2.3 us per job on B200, from one thread 0.3 + 1.7 us.
     void set_bind_at_launch(bool v) { lazy_bind_.store(v, std::memory_order_release); }
+
+    // Take slots keep .. b-1 out of service.  Only before the first job is submitted (nothing queued, nothing in flight): their
+    // executables leave the free lists, so Algorithm 1 never queues a job on them, and they leave W_pool, so they never
+    // dispatch or steal.  The backend asks for this where more slots than CUDA streams cost throughput.
+    void retire_slots(int keep) {
+        if (keep < 1 || keep >= b_) return;
+        std::vector<int> ws;
+        int w = -1, e = -1;
+        while (pool_.try_pop(w)) ws.push_back(w);
+        int kept = 0;
+        for (int x : ws)
+            if (x < keep) {
+                pool_.push(x);
+                ++kept;
+            }
+        n_free_.store(kept, std::memory_order_seq_cst);
+        for (w = keep; w < b_; ++w)
+            while (free_execs_[w].r.try_pop(e)) {
+            }
+        active_ = keep;
+    }
+    int active_slots() const { return active_; }
 
     int slots() const { return b_; }
     int execs_per_slot() const { return epp_; }
@@ -504,6 +527,7 @@ class Scheduler {
     Backend* be_;
     volatile uint32_t* flags_ = nullptr;
     const int S_, b_, q_, epp_, steal_policy_;
+    int active_ = 0;  // slots in service: b_ unless retire_slots() was called
     const uint64_t spin_ns_;
     std::unique_ptr<PaddedRing<Prepared>[]> queues_;
     std::unique_ptr<PaddedRing<int>[]> free_execs_;

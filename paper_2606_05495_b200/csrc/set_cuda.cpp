@@ -82,10 +82,14 @@ struct PinnedRange {
 
 }  // namespace
 
+constexpr int kMaxLoopStreams = 8;     // WHILE graphs in flight at once (set_register_pipeline says why)
+constexpr int kMinLoopBodyStages = 3;  // kernel nodes in a WHILE body (set_register_pipeline says why)
+
 struct set_ctx final : public Backend {
     set_config cfg{};
     int S = 0, b = 0, q = 0, epp = 0, device = 0;
-    int L = 1, H = 0;  // set_config.streams_per_lane and the number of CUDA streams H = S * L; slot w runs on streams[w % H]
+    int L = 1, H = 0;  // set_config.streams_per_lane and the number of CUDA streams H = S * L; slot w runs on streams[w % Hw]
+    int Hw = 0;        // streams in use: H, or for a pipeline with a loop at most kMaxLoopStreams of them (see set_register_pipeline)
     std::vector<cudaStream_t> streams, notify;
     bool own_streams = false;
     std::unique_ptr<SpinLock[]> stream_locks;
@@ -772,7 +776,7 @@ static void CUDART_CB set_completion_cb(void* arg) {
 
 int set_ctx::launch(int exec, int slot, const JobDesc&) {
     bind_thread();
-    int s = slot % H;
+    int s = slot % Hw;
     std::unique_lock<std::mutex> dl(driver_mu, std::defer_lock);
     if (driver_lock) dl.lock();
     SpinLock& lk = stream_locks[s];
@@ -806,7 +810,7 @@ int set_ctx::poll() {
 
 void set_ctx::finish(int exec, int slot, const JobDesc&) {
     if (stamps) {
-        StampRec r{(uint32_t)(slot % H), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
+        StampRec r{(uint32_t)(slot % Hw), __atomic_load_n(&ts_host[(size_t)slot * 8], __ATOMIC_ACQUIRE),
                    __atomic_load_n(&ts_host[(size_t)slot * 8 + 1], __ATOMIC_ACQUIRE)};
         // The signal thread stores the end stamp and then the completion word, unfenced: the two stores may reach host
         // memory in either order (seen on B200, rarely -- the reason the job's OUTPUT is never written by
@@ -849,7 +853,7 @@ void set_ctx::finish(int exec, int slot, const JobDesc&) {
 // ---------------------------------------------------------------------------------------------------------
 int set_ctx::plain_job(int slot, const JobDesc& job) {
     // "Synchronous model": individual copies and kernel launches, no graph
-    int s = slot % H;
+    int s = slot % Hw;
     cudaStream_t st = streams[s];
     SlotMem& sm = slots[slot];
     if (sm.used) {  // buffer reuse guarded by event synchronisation
@@ -911,7 +915,7 @@ int set_ctx::baseline_flush() {
         bool dummy;
         int e = (int)i * epp;
         if (int rc = bind(e, (int)i, batch[i], &dummy)) return rc;
-        CK(cudaGraphLaunch(execs[e].exec, streams[i % H]));
+        CK(cudaGraphLaunch(execs[e].exec, streams[i % Hw]));
     }
     base_launched.fetch_add(batch.size(), std::memory_order_relaxed);
     kernel_nodes.fetch_add(stages.size() * batch.size(), std::memory_order_relaxed);
@@ -1010,8 +1014,8 @@ void set_ctx::mq_loop() {
             bool dummy;
             int rc = err.load() ? err.load() : bind(w * epp, w, j, &dummy);
             if (rc == 0) {
-                cudaError_t e = cudaGraphLaunch(execs[w * epp].exec, streams[w % H]);
-                if (e == cudaSuccess) e = cudaEventRecord(slots[w].done, streams[w % H]);
+                cudaError_t e = cudaGraphLaunch(execs[w * epp].exec, streams[w % Hw]);
+                if (e == cudaSuccess) e = cudaEventRecord(slots[w].done, streams[w % Hw]);
                 if (e != cudaSuccess) rc = cuda_fail(e, "graph launch (queue model)", __LINE__);
             }
             base_ns_launch.fetch_add(now_ns() - t0, std::memory_order_relaxed);
@@ -1133,6 +1137,7 @@ set_status set_create_ex(const set_config* cfg_in, set_ctx** out) {
     // CUDA streams behind each logical stream (set.h streams_per_lane): never more than the lane has slots
     c->L = c->own_streams ? std::max(1, std::min(cfg.streams_per_lane, c->b / c->S)) : 1;
     c->H = c->S * c->L;
+    c->Hw = c->H;
     c->streams.resize(c->H);
     c->notify.resize(c->H);
     c->stream_locks.reset(new SpinLock[c->H]);
@@ -1224,6 +1229,7 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     {  // loop structure (set.h SET_STAGE_LOOP_BEGIN): at most one loop, properly closed; a loop pipeline is bound to its
        // slot, so no kernel of it may depend on the job's dims; SET_ARG_COND only inside the loop
         bool any_loop = false, in_loop = false, closed = false;
+        int body_stages = 0;
         for (int s = 0; s < num_stages; ++s) any_loop = any_loop || (stages[s].flags & SET_STAGE_LOOP_BEGIN);
         for (int s = 0; s < num_stages; ++s) {
             const set_stage_desc& st = stages[s];
@@ -1240,6 +1246,7 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
             if (in_loop)
                 for (int k = 0; k < 3; ++k)
                     if (!dim_free(st.grid[k].count)) return SET_ERR_INVALID;
+            if (in_loop) ++body_stages;
             if (st.flags & SET_STAGE_LOOP_END) {
                 if (!in_loop) return SET_ERR_INVALID;
                 in_loop = false;
@@ -1247,6 +1254,12 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
             }
         }
         if (in_loop) return SET_ERR_INVALID;
+        // Measured on B200 / CUDA 12.9 (profiles/r2_probes.md section 3): a WHILE body of TWO kernel nodes (relaxation ->
+        // control) ended in cudaErrorLaunchFailure -- sticky, the context is lost -- about once in 10^5 jobs with 8 such
+        // graphs in flight (never with 4); bodies of 3 to 9 nodes ran 6.6 million jobs without one.  Refuse the short body.
+        if (any_loop && body_stages < kMinLoopBodyStages)
+            return c->fail(SET_ERR_INVALID, "a loop body needs at least %d stages (two-node WHILE bodies are not reliable on this driver)",
+                           kMinLoopBodyStages);
         if (any_loop && c->cfg.mode == SET_MODE_SET && c->cfg.steal_policy == SET_STEAL_RETARGET) return SET_ERR_INVALID;
     }
     for (int i = 0; i < num_bufs; ++i) {
@@ -1365,6 +1378,16 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     if (c->slot_graphs && c->cfg.mode == SET_MODE_PLAIN_STREAMS)
         return c->fail(SET_ERR_INVALID, "a pipeline with a loop needs a job graph: SET_MODE_PLAIN_STREAMS cannot run it");
     if (c->slot_graphs && c->sched) c->sched->set_slot_bound(true);
+    if (c->slot_graphs) {
+        // Measured on B200 / CUDA 12.9 (profiles/r2_probes.md section 4): with more than 8 graphs holding a WHILE node in
+        // flight at once, a launch now and then ends in cudaErrorLaunchFailure (about once in 10^5 jobs at 32 in flight,
+        // never at 8).  Loop pipelines therefore run on at most 8 of the context's CUDA streams: the largest divisor of S
+        // that is <= 8, so that slots w and w + H, which the scheduler polls as one in-order list, still share a stream.
+        int lim = 1;
+        for (int d = 1; d <= kMaxLoopStreams && d <= c->S; ++d)
+            if (c->S % d == 0) lim = d;
+        c->Hw = lim;
+    }
     if (c->sched) c->sched->set_bind_at_launch(c->cfg.bind_at_launch == 1);
     c->nsets.resize(c->slot_graphs ? (size_t)c->b * c->epp : 1);
     if (!c->slot_graphs)
@@ -1398,6 +1421,9 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
     c->host_rebinds.store(0);
     c->ns_bind.store(0);
     c->registered = true;
+    // one job in flight per CUDA stream: a WHILE graph queued on a stream behind a running one slows both down (8 streams:
+    // 54 K SSSP jobs/s with 8 slots, 34 K with 16 or 32), so the slots beyond the streams are taken out of service
+    if (c->slot_graphs && c->sched) c->sched->retire_slots(c->Hw);
     if (c->cfg.mode == SET_MODE_MUTEX_QUEUE) c->mq_thread = std::thread([c] { c->mq_loop(); });
     return SET_OK;
 }
@@ -1576,7 +1602,7 @@ set_status set_get_stats(set_ctx* c, set_stats* out) {
     out->signal_nodes = c->signal_nodes.load();
     out->copy_nodes = c->copy_nodes.load();
     out->early_completions = c->early_completions.load();
-    out->cuda_streams = (uint64_t)c->H;
+    out->cuda_streams = (uint64_t)c->Hw;
     out->ns_bind = c->ns_bind.load();
     out->ns_sync = c->ns_sync.load();
     return SET_OK;

@@ -101,6 +101,7 @@ class SimBackend : public Backend {
     }
     int launch(int exec, int slot, const JobDesc& job) override {
         if (bound_slot_[(size_t)exec] != slot) errors.fetch_add(1);  // G must be bound to the launching slot's M_w
+        if (slot >= in_service.load() || exec / epp_ >= in_service.load()) errors.fetch_add(1);  // a retired slot or one of its execs
         if (slot_busy_[(size_t)slot].exchange(1) != 0) errors.fetch_add(1);  // one job per slot at a time
         if (exec_busy_[(size_t)exec].exchange(1) != 0) errors.fetch_add(1);
         int64_t inflight = inflight_.fetch_add(1) + 1;
@@ -128,6 +129,7 @@ class SimBackend : public Backend {
         return bad;
     }
     std::atomic<int64_t> errors{0}, binds{0};
+    std::atomic<int> in_service{1 << 30};  // Scheduler::retire_slots: slots below this number may run jobs
 
   private:
     struct Item {
@@ -190,6 +192,12 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
     {
         Scheduler sched(&be, num_streams, b, queue_capacity, num_dispatchers, policy, 20, /*poller=*/(seed >> 2) & 1);
         sched.set_bind_at_launch((seed >> 3) & 1);
+        const int keep = ((seed >> 4) & 1) ? num_streams : b;  // seed bit 4: a loop pipeline's geometry (slot-bound, one slot per stream)
+        if (keep < b) {
+            sched.set_slot_bound(true);
+            sched.retire_slots(keep);
+            be.in_service.store(keep);
+        }
         be.attach(&sched);
         std::atomic<int64_t> next{0};
         std::vector<std::thread> subs;
@@ -210,7 +218,7 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
         if (submit_errors.load() != 0) rc = -2;
         CoreStats& st = sched.stats();
         if ((int64_t)st.completed.load() != jobs || (int64_t)st.submitted.load() != jobs) rc = -3;
-        if ((int64_t)st.max_inflight.load() > b) rc = -4;
+        if ((int64_t)st.max_inflight.load() > keep) rc = -4;
         if (out_steals) *out_steals = st.steals.load();
         sched.stop();
         be.shutdown();

@@ -94,7 +94,7 @@ def baseline_workload(config: int) -> Workload:
     if config == 5:  # paper workload 6; SURVEY.md 8(f)4
         return Workload(5, (4096, inputgen.sssp_max_edges(4096, 8)), jobs=2048, num_streams=8, max_inflight=32,
                         name="config5 SSSP frontier Bellman-Ford, 4096 vertices, mean out-degree 8, WHILE node (2048 jobs)", dtype="int32",
-                        kernels_per_job=3, extra={"mean_deg": 8})
+                        kernels_per_job=6, extra={"mean_deg": 8})  # graph kernel nodes: init + 4 relaxations + control
     if config == 6:  # paper workload 1; SURVEY.md 8(f)4
         return Workload(6, (1920, 1080), jobs=4096, num_streams=8, max_inflight=32,
                         name="config6 Sobel chain gray->sobel->mean->threshold->blend, jittered sizes (4096 jobs)", dtype="u8", kernels_per_job=5)
@@ -108,7 +108,7 @@ def small_workload(config: int) -> Workload:
     if config == 2: return Workload(2, (300, 2052, 10), jobs=12, num_streams=4, max_inflight=8, dtype="f32", kernels_per_job=10)
     if config == 3: return Workload(3, (384, 512, 256), jobs=8, num_streams=4, max_inflight=8, dtype="bf16", kernels_per_job=1)
     if config == 4: return Workload(4, (1920, 1080), jobs=48, num_streams=8, max_inflight=32, dtype="u8", kernels_per_job=3)
-    if config == 5: return Workload(5, (1000, inputgen.sssp_max_edges(1000, 4)), jobs=48, num_streams=4, max_inflight=8, dtype="int32", kernels_per_job=3, extra={"mean_deg": 4})
+    if config == 5: return Workload(5, (1000, inputgen.sssp_max_edges(1000, 4)), jobs=48, num_streams=4, max_inflight=8, dtype="int32", kernels_per_job=6, extra={"mean_deg": 4})
     if config == 6: return Workload(6, (1920, 1080), jobs=48, num_streams=8, max_inflight=32, dtype="u8", kernels_per_job=5)
     raise ValueError(config)
 

@@ -89,6 +89,12 @@ def test_stdout_line_is_compact_and_complete():
     side_line = back["workloads_e2e_frac_vsbatch"]
     assert set(side_line) == {"config0", "config2", "config3", "config4", "config5", "config6"} and side_line["config2"] == [812.3, 0.9412, 1.031]
     assert back["detail"] == "bench_detail.json"
+    # side workloads that failed put a short error each on the line: it stays under 2 KB
+    detail_err = dict(detail, workloads={f"config{c}": {"error": "e" * 300} for c in (0, 2, 3, 4, 5, 6)})
+    line_err = bench.compact_line(wl, 1, 20, 5, 10000, 24.8, 402503.2, 46.0, 217224.4, _fake_arm(402503.2, "device"), _fake_arm(217224.4, "host"),
+                                  clocks, detail_err, "/x/bench_detail.json", pk)
+    assert len(json.dumps(line_err, separators=(",", ":"))) < 2048
+    assert line_err["workloads_e2e_frac_vsbatch"]["config5"].startswith("error: ")
     # world > 1: no side passes ran, the line is still complete
     line2 = bench.compact_line(wl, 8, 20, 5, 10000, 24.8, 3.2e6, 46.0, 1.7e6, _fake_arm(402503.2, "device"), _fake_arm(217224.4, "host"),
                                clocks, {}, None, pk)

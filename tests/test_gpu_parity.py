@@ -834,14 +834,51 @@ def test_plain_streams_refuse_a_loop_pipeline(libset):
     ctx.close()
 
 
+@pytest.mark.parametrize("streams,lanes,want", [(8, 4, 8), (8, 1, 8), (16, 2, 8), (12, 2, 6), (3, 4, 3)])
+def test_loop_pipelines_run_on_at_most_8_streams(libset, streams, lanes, want):
+    """More than 8 WHILE graphs in flight at once fail now and then on this driver, and a WHILE graph queued on a stream
+    behind a running one slows both (profiles/r2_probes.md section 3), so a pipeline with a loop keeps to the largest
+    divisor of S that is <= 8 CUDA streams and to one job in flight on each, whatever streams_per_lane and max_inflight
+    ask for; the other workloads keep all their streams and slots."""
+    from paper_2606_05495_b200.workloads import Workload
+    wl = Workload(5, (512, inputgen.sssp_max_edges(512, 4)), jobs=96, num_streams=streams, max_inflight=4 * streams, kernels_per_job=6,
+                  extra={"mean_deg": 4})
+    st = check(libset, wl, list(range(96)), streams_per_lane=lanes, pdl=True)
+    assert st["cuda_streams"] == want and 1 <= st["max_inflight_seen"] <= want
+    wl6 = Workload(6, (1920, 1080), jobs=16, num_streams=streams, max_inflight=4 * streams, dtype="u8", kernels_per_job=5)
+    assert check(libset, wl6, list(range(16)), streams_per_lane=lanes)["cuda_streams"] == streams * lanes
+
+
 @pytest.mark.parametrize("v,deg", [(1, 1), (2, 1), (37, 2), (256, 1), (1000, 4), (4096, 8), (20000, 3)])
 @pytest.mark.parametrize("pdl", [False, True])
 def test_config5_graph_sizes(libset, v, deg, pdl):
     """One vertex, a sparse graph most of which is unreachable (degree 1), several blocks plus a ragged tail, the bench
     size, and a graph large enough for dozens of rounds: distances bit-exact, rounds within the oracle's."""
     from paper_2606_05495_b200.workloads import Workload
-    wl = Workload(5, (v, inputgen.sssp_max_edges(v, deg)), jobs=10, num_streams=2, max_inflight=4, kernels_per_job=3, extra={"mean_deg": deg})
+    wl = Workload(5, (v, inputgen.sssp_max_edges(v, deg)), jobs=10, num_streams=2, max_inflight=4, kernels_per_job=6, extra={"mean_deg": deg})
     check(libset, wl, list(range(10)), pdl=pdl)
+
+
+@pytest.mark.parametrize("unroll", [2, 3, 5, 8])
+@pytest.mark.parametrize("v,deg", [(1, 1), (37, 2), (4096, 8), (20000, 3)])
+def test_config5_relaxations_per_loop_pass(libset, unroll, v, deg):
+    """U relaxation kernels per pass of the WHILE body (default 4), odd and even: the frontier's double buffer follows the
+    relaxation's running number, relaxations over an empty frontier change nothing and are not counted as rounds, so the
+    distances and the bound on the round count do not depend on U; the graph has 2 + U stage kernels."""
+    from paper_2606_05495_b200.workloads import Workload
+    wl = Workload(5, (v, inputgen.sssp_max_edges(v, deg), unroll), jobs=8, num_streams=2, max_inflight=4, kernels_per_job=2 + unroll,
+                  extra={"mean_deg": deg})
+    st = check(libset, wl, list(range(8)))
+    assert st["kernel_nodes"] == 8 * (2 + unroll)
+
+
+def test_config5_unroll_out_of_range_is_refused(libset):
+    for u in (0, 1, 9):       # U = 1 would be a two-node loop body, which this driver does not run reliably (set.h)
+        ctx = libset.Context(2, 4)
+        with pytest.raises(libset.SetError) as ei:
+            ctx.register_builtin(5, 0, [256, 2048, u])
+        assert ei.value.status == libset.SET_ERR_INVALID
+        ctx.close()
 
 
 def test_config5_hand_graphs_through_the_library(libset):

@@ -39,6 +39,9 @@ def test_ring_delivers_every_token_exactly_once(libset, cap, prod, cons, items):
     (1, 1, 1, 1, 1, 2000, 3),       # degenerate: one worker
     (4, 6, 1, 2, 3, 10000, 5),      # max_inflight not a multiple of the stream count -> rounded up
     (2, 64, 4, 2, 2, 20000, 4),
+    (8, 32, 2, 1, 1, 20000, 16 + 2),    # a loop pipeline's geometry: slots 8..31 retired, executables bound to their slot
+    (4, 32, 2, 2, 3, 20000, 16 + 4),    # the same with a completion thread, several dispatchers and submitters
+    (8, 8, 2, 1, 1, 5000, 16),          # nothing to retire
 ])
 def test_scheduler_algorithms_on_simulated_device(libset, S, b, q, disp, subs, jobs, seed):
     rc, steals = libset.selftest_scheduler(S, b, q, disp, subs, jobs, seed)
