@@ -475,6 +475,34 @@ int64_t set_selftest_ring(int capacity, int producers, int consumers, int64_t it
 int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capacity, int num_dispatchers,
                                int submitters, int64_t jobs, uint32_t seed, uint64_t *out_steals);
 
+/* ---------------------------------------------------------------------------------------------- *
+ * An entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid allocation).
+ *
+ * set_sssp_noalloc: one SSSP job -- the computation of builtin config 5 ("Bellman-Ford graph traversal with
+ * frontier-based relaxation"; readings S5-1..S5-4) -- as ONE kernel launch on `stream`, without a set_ctx.
+ *   dev_image    : DEVICE, int32 [V, E, src, 0][row_ptr V+1][col E][w E], 4-byte aligned (the job image of config 5);
+ *                  read only; the caller keeps it alive and unchanged until the launch has finished on `stream`
+ *   dev_out      : DEVICE, int32 [dist V][rounds, 0, 0, 0]: written by the kernel; dist[] is the unique result
+ *                  (unreachable = 2^31 - 1), rounds counts the relaxation rounds that had a frontier
+ *   num_vertices : V of the image (the kernel reads min(image V, num_vertices) vertices); 0 = do the per-device set-up
+ *                  only and launch nothing (call this once per device before a graph capture)
+ *   stream       : a cudaStream_t passed as a plain pointer (NULL = the default stream)
+ * The kernel's scratch (frontier flags, 2 x SET_NOALLOC_MAX_VERTICES uint32 = 128 KiB) is a file-scope static __device__
+ * array: every GPU that loads the library holds it until the process exits.  The call makes no cudaMalloc, cudaFree or
+ * other allocating call; the first call on a device resolves the array's device address (cudaGetSymbolAddress).  It is
+ * asynchronous: the result is in dev_out once `stream` has reached the launch.
+ * EVERY call on a device shares the one array, and it keeps the last call's contents: the kernel writes every flag it
+ * reads before reading it, so calls one after the other -- on one stream, or ordered by events -- are independent, but
+ * two calls that OVERLAP on the GPU (different streams, no ordering) race on it and give wrong distances.
+ * Errors: SET_ERR_SIZE if num_vertices > SET_NOALLOC_MAX_VERTICES (nothing is launched), SET_ERR_INVALID (NULL
+ * pointers), SET_ERR_CUDA (no device, failed launch); the text is in set_noalloc_last_error() (per thread, valid until
+ * that thread's next call).  One block runs the job (about 100 - 200 us at V = 4096): a latency path, not a throughput one.
+ */
+#define SET_NOALLOC_MAX_VERTICES 16384
+set_status set_sssp_noalloc(const void *dev_image, void *dev_out, uint32_t num_vertices, void *stream);
+const char *set_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

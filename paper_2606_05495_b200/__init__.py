@@ -102,7 +102,7 @@ class GapStats(C.Structure):
 EXPORTS = ["set_create", "set_create_ex", "set_register_pipeline", "set_submit", "set_submit_dims", "set_submit_batch",
            "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_host_register", "set_host_unregister", "set_get_stats", "set_reset_stats", "set_get_gap_stats",
            "set_last_error", "set_get_geometry", "set_time_stage", "set_builtin_kernel", "set_builtin_pipeline",
-           "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler"]
+           "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler", "set_sssp_noalloc", "set_noalloc_last_error"]
 
 _lib = None
 
@@ -147,6 +147,9 @@ def load():
     lib.set_selftest_ring.restype = i64
     lib.set_selftest_scheduler.argtypes = [C.c_int] * 5 + [i64, C.c_uint32, C.POINTER(u64)]
     lib.set_selftest_scheduler.restype = i64
+    lib.set_sssp_noalloc.argtypes = [vp, vp, C.c_uint32, vp]
+    lib.set_noalloc_last_error.argtypes = []
+    lib.set_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
         fn = getattr(lib, name)
         if fn.restype is C.c_int and name not in ("set_selftest_find_order",):
@@ -311,6 +314,19 @@ class Context:
         out = C.c_float(0)
         self._check(self._lib.set_time_stage(self._h, stage, d, warmup, iters, C.byref(out)), "set_time_stage")
         return out.value
+
+
+NOALLOC_MAX_VERTICES = 16384  # SET_NOALLOC_MAX_VERTICES
+
+
+def sssp_noalloc(dev_image: int, dev_out: int, num_vertices: int, stream: int = 0) -> None:
+    """set_sssp_noalloc (include/set.h): one SSSP job on `stream`, scratch in the library's static device array, no
+    allocation.  dev_image / dev_out are DEVICE addresses; asynchronous.  Raises SetError (SET_ERR_SIZE beyond
+    NOALLOC_MAX_VERTICES)."""
+    lib = load()
+    rc = lib.set_sssp_noalloc(dev_image, dev_out, num_vertices, stream or None)
+    if rc != SET_OK:
+        raise SetError(rc, "set_sssp_noalloc", lib.set_noalloc_last_error().decode())
 
 
 def selftest_find_order(b: int, w: int, nonempty: int) -> int:

@@ -17,7 +17,7 @@ LIB = os.path.join(HERE, "libset.so")
 TRACE_LIB = os.path.join(HERE, "libsettrace.so")  # CUPTI gap tracer (include/set_trace.h): measurement only
 BUILD_DIR = os.path.join(HERE, "build")
 
-CUDA_SOURCES = ["kernels/small_kernels.cu", "kernels/stencil_kernels.cu", "kernels/paper_kernels.cu", "kernels/gemm_sm100.cu", "set_builtin.cu"]
+CUDA_SOURCES = ["kernels/small_kernels.cu", "kernels/stencil_kernels.cu", "kernels/paper_kernels.cu", "kernels/gemm_sm100.cu", "set_builtin.cu", "set_noalloc.cu"]
 HOST_SOURCES = ["set_cuda.cpp", "set_selftest.cpp"]
 HEADERS = ["set_core.hpp", "set_ring.hpp", "kernels/kernels.h"]
 
