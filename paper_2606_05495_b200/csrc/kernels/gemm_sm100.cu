@@ -157,33 +157,37 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 
 // GELU, erf form (reading C3-3): 0.5 z (1 + erf(z / sqrt 2)), evaluated in fp32, TWO elements per call.  The epilogue is
-// issue-bound (32,768 elements per CTA through four schedulers; the scalar version compiled to ~30 instructions per
-// element and took 6 us of the kernel's 17), so (1) erf is one branch-free expression instead of erff()'s two diverging
-// paths: erfc(|x|) = (a1 t + ... + a5 t^5) exp(-x^2), t = 1 / (1 + p |x|)  (Abramowitz & Stegun 7.1.26, |error| <= 1.5e-7
-// absolute -- more than three orders below the bf16 rounding of the output), with 1 + erf(x) = erfc(|x|) for x < 0 and
-// 2 - erfc(|x|) otherwise, which also avoids the cancellation of 1 + erf(x) on the negative side; and (2) every multiply
-// and add is a packed f32x2 instruction (sm_100 FFMA2 / FMUL2 / FADD2: two fp32 lanes per issue slot).  The 0.5 is
-// folded into the polynomial's coefficients.  Per pair: 13 packed FP, 4 MUFU, 2 LOP, 2 SEL, 1 bf16x2 convert.
+// issue- and MUFU-bound (32,768 elements per CTA through four schedulers and four 4-lane MUFU units; the scalar erff()
+// version compiled to ~30 instructions per element and took 6 us of the kernel's 17), so (1) erf is one branch-free
+// expression with ONE special-function instruction per element:
+//     erfc(|x|) = 1 / (1 + a1 |x| + ... + a6 |x|^6)^16        (Abramowitz & Stegun 7.1.28, |error| <= 3e-7 absolute;
+// the 1 / sqrt 2 of x = z / sqrt 2 is folded into the coefficients; round 2's first version used 7.1.26, which needs a
+// reciprocal AND an exponential: 2 MUFU per element, 2.1 us of MUFU time per CTA), and 0.5 z (1 + erf x) =
+// hz + |hz| (1 - erfc|x|) with hz = z / 2: for z < 0 the sum cancels to hz erfc|x| with an absolute error of an ulp of hz,
+// far below the bf16 rounding of anything that is not itself negligible (tests: <= 1 bf16 ulp where |GELU| >= 1e-3, 4e-6
+// absolute below); and (2) every multiply and add is a packed f32x2 instruction (sm_100 FFMA2 / FMUL2 / FADD2: two fp32
+// lanes per issue slot).  A power that overflows gives rcp(inf) = 0: erf = 1.  Per pair: 13 packed FP, 2 MUFU, 4 LOP.
 __device__ __forceinline__ float2 gelu_erf2(float2 z) {
-    const float2 x = __fmul2_rn(z, make_float2(0.70710678118654752440f, 0.70710678118654752440f));
-    const float2 ax = make_float2(fabsf(x.x), fabsf(x.y));
-    const float2 d = __ffma2_rn(make_float2(0.3275911f, 0.3275911f), ax, make_float2(1.0f, 1.0f));
-    float2 t;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.x) : "f"(d.x));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t.y) : "f"(d.y));
-    float2 p = __ffma2_rn(make_float2(0.5f * 1.061405429f, 0.5f * 1.061405429f), t, make_float2(0.5f * -1.453152027f, 0.5f * -1.453152027f));
-    p = __ffma2_rn(p, t, make_float2(0.5f * 1.421413741f, 0.5f * 1.421413741f));
-    p = __ffma2_rn(p, t, make_float2(0.5f * -0.284496736f, 0.5f * -0.284496736f));
-    p = __ffma2_rn(p, t, make_float2(0.5f * 0.254829592f, 0.5f * 0.254829592f));
-    // exp(-x^2) = 2^(-x^2 log2 e)
-    const float2 u = __fmul2_rn(__fmul2_rn(ax, ax), make_float2(-1.4426950408889634f, -1.4426950408889634f));
-    float2 e;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.x) : "f"(u.x));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.y) : "f"(u.y));
-    const float2 w = __fmul2_rn(__fmul2_rn(p, t), e);                          // erfc(|x|) / 2
-    const float2 c = __fadd2_rn(make_float2(1.0f, 1.0f), make_float2(-w.x, -w.y));  // 1 - erfc(|x|) / 2
-    const float2 phi = make_float2(x.x < 0.0f ? w.x : c.x, x.y < 0.0f ? w.y : c.y);  // (1 + erf(x)) / 2
-    return __fmul2_rn(z, phi);
+    constexpr float kA1 = 0.0705230784f * 0.70710678118654752440f, kA2 = 0.0422820123f * 0.5f,
+                    kA3 = 0.0092705272f * 0.35355339059327376220f, kA4 = 0.0001520143f * 0.25f,
+                    kA5 = 0.0002765672f * 0.17677669529663688110f, kA6 = 0.0000430638f * 0.125f;
+    const float2 az = make_float2(fabsf(z.x), fabsf(z.y));
+    float2 d = __ffma2_rn(make_float2(kA6, kA6), az, make_float2(kA5, kA5));
+    d = __ffma2_rn(d, az, make_float2(kA4, kA4));
+    d = __ffma2_rn(d, az, make_float2(kA3, kA3));
+    d = __ffma2_rn(d, az, make_float2(kA2, kA2));
+    d = __ffma2_rn(d, az, make_float2(kA1, kA1));
+    d = __ffma2_rn(d, az, make_float2(1.0f, 1.0f));
+    d = __fmul2_rn(d, d);
+    d = __fmul2_rn(d, d);
+    d = __fmul2_rn(d, d);
+    d = __fmul2_rn(d, d);  // (1 + ...)^16
+    float2 r;              // erfc(|x|)
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r.x) : "f"(d.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r.y) : "f"(d.y));
+    const float2 hz = __fmul2_rn(z, make_float2(0.5f, 0.5f));
+    const float2 m = __fadd2_rn(make_float2(1.0f, 1.0f), make_float2(-r.x, -r.y));  // erf(|x|)
+    return __ffma2_rn(make_float2(fabsf(hz.x), fabsf(hz.y)), m, hz);
 }
 
 }  // namespace
