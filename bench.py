@@ -280,7 +280,7 @@ def run_arm(setlib, wl, job_ids, mode: str, io_device: bool, steps: int, warmup:
                 g["overhead_frac"] = max(0.0, 1.0 - g["busy_union_us"] / (ev_ms[-1] * 1e3))
                 per_step_gaps.append(g)
                 stp = ctx.stats()
-                st_sum = stp if st_sum is None else {k: (max(st_sum[k], v) if k == "max_inflight_seen" else st_sum[k] + v) for k, v in stp.items()}
+                st_sum = stp if st_sum is None else {k: (max(st_sum[k], v) if k in ("max_inflight_seen", "cuda_streams") else st_sum[k] + v) for k, v in stp.items()}
                 ctx.reset_stats()
         st = st_sum if st_sum is not None else ctx.stats()
         gap_stats = merge_gap_stats(per_step_gaps) if per_step_gaps else None
