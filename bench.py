@@ -431,6 +431,9 @@ def stage_algorithmic(wl, dims):
     if c == 4:
         px = dims[0] * dims[1]
         return [("rgb2gray_u8", "hbm", 4 * px), ("blur3x3_u8", "hbm", 2 * px), ("hist256_u8", "hbm", px + 1024)]
+    if c == 5 and wl.variant == 1:  # one kernel runs the job: reads the image once per round at most; latency-class
+        e = p[0] * wl.extra.get("mean_deg", 8)  # image (header, row_ptr, col, w) read + distances written
+        return [("sssp_solo", "hbm", 16 + 4 * (p[0] + 1) + 8 * e + 4 * p[0] + 16)]
     if c == 5:  # timed alone the relaxation sees an empty frontier: it scans the V flags and stops (latency-class)
         v, unroll = p[0], (p[2] if len(p) > 2 else 4)
         return [("sssp_init", "hbm", 12 * v)] + [("sssp_relax", "hbm", 4 * v)] * unroll + [("sssp_control", "hbm", 16)]
@@ -973,6 +976,34 @@ def main():
                     log(f"[bench] config {c} failed: {e}")
                 _INPUTS.clear()  # the side workloads' inputs are large (config 2: 1 GB): keep only what is in use
             detail["workloads"] = others
+            # config 5, variant 1: the whole SSSP job as ONE kernel of one block instead of the WHILE-node pipeline;
+            # detail file only -- the stdout line keeps the WHILE-node pipeline, which is what SURVEY.md 8(f)4 names
+            if wl.config != 5:
+                try:
+                    import dataclasses
+                    w5 = dataclasses.replace(workload_for(5), variant=1, kernels_per_job=1)
+                    ids5 = list(range(w5.jobs))
+                    # the copy-in (16 + 4 (V + 1) + 8 E bytes, capacity 508 KB) as an SM copy: the copy engines get through about
+                    # 90 K copies of this size a second whatever the stream count; device-resident: one CUDA stream per slot
+                    vo = {"sm_copy_max_bytes": 1 << 20}
+                    v_e2e = arm(w5, ids5, "set", False, SIDE_STEPS, SIDE_WARMUP, verify=2, opts=vo)
+                    v_bat = arm(w5, ids5, "batch_sync_graphs", False, SIDE_STEPS, SIDE_WARMUP, verify=0, opts=vo)
+                    v_dev = arm(w5, ids5, "set", True, SIDE_STEPS, SIDE_WARMUP, verify=2, opts=dict(vo, streams_per_lane=4))
+                    v_ce = arm(w5, ids5, "set", False, SIDE_STEPS, SIDE_WARMUP, verify=0)
+                    bound = (others.get("config5") or {}).get("pipeline_roofline", {}).get("e2e_bound_jobs_per_s")
+                    detail["variants"] = {"config5_single_kernel": {
+                        "options": "sm_copy_max_bytes = 1 MiB (SM copy-in); device-resident arm: streams_per_lane = 4",
+                        "e2e_with_default_options_copy_engine_in": round(v_ce["jobs_per_s"], 1),
+                        "e2e": round(v_e2e["jobs_per_s"], 1), "value": round(v_dev["jobs_per_s"], 1), "batch_sync_graphs_e2e": round(v_bat["jobs_per_s"], 1),
+                        "speedup_vs_batch_sync_e2e": round(v_e2e["jobs_per_s"] / v_bat["jobs_per_s"], 3),
+                        "e2e_frac_of_link_bound": round(v_e2e["jobs_per_s"] / bound, 4) if bound else None,
+                        "mismatches": v_e2e["mismatches"] + v_dev["mismatches"],
+                        "kernels": kernel_rooflines(setlib, w5, pk, None)}}
+                    side_bad += detail["variants"]["config5_single_kernel"]["mismatches"]
+                except Exception as e:
+                    detail["variants"] = {"config5_single_kernel": {"error": str(e)[:300]}}
+                    log(f"[bench] config 5 variant 1 failed: {e}")
+                _INPUTS.clear()
         if args.sweep:
             detail["batch_sweep"] = batch_sweep(setlib, wl, ids, flush)
     detail["side_mismatches"] = side_bad

@@ -217,9 +217,10 @@ typedef struct set_config {
     int32_t callback_mode;    /* SET_CB_*                                                          */
     int32_t device;           /* CUDA device ordinal; -1 => current device                         */
     int32_t spin_us;          /* dispatcher/drain spin time before sleeping; 0 => default (50)     */
-    int32_t sm_copy_max_bytes;/* H2D/D2H copies of a fixed size up to this many bytes become kernel nodes
+    int32_t sm_copy_max_bytes;/* H2D/D2H copies of up to this many bytes become kernel nodes
                                  (SET_K_COPY: the SMs read/write pinned host memory over the link) instead of
-                                 copy-engine memcpy nodes; 0 => default (262144), -1 => never.                    */
+                                 copy-engine memcpy nodes; a copy whose size depends on the job's dims counts with the
+                                 capacity of its buffer; 0 => default (262144), -1 => never.   */
     int32_t timestamps;       /* 1: every job graph gets two extra one-thread kernel nodes that store the GPU's
                                  %globaltimer when the graph starts (a root node beside the first copy) and when it
                                  ends (the completion-signal node, or a last node of its own): the device-side gap
@@ -421,6 +422,11 @@ set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int war
                                     uint64* stamp, uint32 fence)  copy by the SMs to *dst_slot + dst_off: the address the
                                     job's copy-in node forwarded; flag != NULL: the block that finishes last also does what
                                     SET_K_SIGNAL does (the job's completion signal folded into its only copy-out node)   */
+#define SET_K_SSSP_SOLO      25  /* (img, out, scratch, maxV)  the whole SSSP job in one block of 1024 threads: K21's
+                                    initialisation, K22's relaxation round after round with a block barrier between them,
+                                    the round count; distances and frontier flags in 5 maxV bytes (flags padded to a
+                                    word) of DYNAMIC shared memory, scratch = work list uint32[maxV].  Launch with grid 1,
+                                    block 1024; maxV <= 40000.                                                          */
 /* the two paper workloads of SURVEY.md 8(f)4 (readings S5-*, S6-*) */
 #define SET_K_SOBEL3X3_U8    17  /* (const uint8* n, uint8* e, uint32 w, uint32 h)  min(255, |gx| + |gy|), clamp-to-edge   */
 #define SET_K_MEAN3X3_U8     18  /* (const uint8* e, uint8* m, uint32 w, uint32 h)  3 x 3 sum / 9, clamp-to-edge          */
@@ -446,6 +452,8 @@ const void *set_builtin_kernel(int kernel_id);
  *               image; U = 2..8 relaxation rounds per pass of the WHILE body, 2 + U stage kernels in all)
  *     config 6 (Sobel chain): {max_w, max_h[, thresh = 64]}  (dims per job = {w, h, 1, 1})
  *   variant: 0 = default.  config 0: 1 = histogram of the INPUT values (reading C0-1 alternative).
+ *            config 5: 1 = the whole job as ONE kernel of one block (SET_K_SSSP_SOLO) instead of the WHILE-node pipeline:
+ *            same buffers, same output; meant for graphs of a few thousand vertices.
  * *            any config: bit 8 set = append a SET_K_SPIN delay stage that busy-waits dims[3] nanoseconds.
  *   stages/bufs : HOST arrays with room for SET_MAX_STAGES / SET_MAX_BUFFERS entries.
  *   host_in_bytes/host_out_bytes : HOST, may be NULL; maximum byte size of a job's host images.
@@ -488,16 +496,16 @@ int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capa
  *   num_vertices : V of the image (the kernel reads min(image V, num_vertices) vertices); 0 = do the per-device set-up
  *                  only and launch nothing (call this once per device before a graph capture)
  *   stream       : a cudaStream_t passed as a plain pointer (NULL = the default stream)
- * The kernel's scratch (frontier flags, 2 x SET_NOALLOC_MAX_VERTICES uint32 = 128 KiB) is a file-scope static __device__
- * array: every GPU that loads the library holds it until the process exits.  The call makes no cudaMalloc, cudaFree or
+ * The kernel's scratch (its work list of frontier vertices, SET_NOALLOC_MAX_VERTICES uint32 = 64 KiB) is a file-scope static
+ * __device__ array: every GPU that loads the library holds it until the process exits.  The call makes no cudaMalloc, cudaFree or
  * other allocating call; the first call on a device resolves the array's device address (cudaGetSymbolAddress).  It is
  * asynchronous: the result is in dev_out once `stream` has reached the launch.
- * EVERY call on a device shares the one array, and it keeps the last call's contents: the kernel writes every flag it
+ * EVERY call on a device shares the one array, and it keeps the last call's contents: the kernel writes every entry it
  * reads before reading it, so calls one after the other -- on one stream, or ordered by events -- are independent, but
  * two calls that OVERLAP on the GPU (different streams, no ordering) race on it and give wrong distances.
  * Errors: SET_ERR_SIZE if num_vertices > SET_NOALLOC_MAX_VERTICES (nothing is launched), SET_ERR_INVALID (NULL
  * pointers), SET_ERR_CUDA (no device, failed launch); the text is in set_noalloc_last_error() (per thread, valid until
- * that thread's next call).  One block runs the job (about 100 - 200 us at V = 4096): a latency path, not a throughput one.
+ * that thread's next call).  One block runs the job: a latency path, not a throughput one.
  */
 #define SET_NOALLOC_MAX_VERTICES 16384
 set_status set_sssp_noalloc(const void *dev_image, void *dev_out, uint32_t num_vertices, void *stream);

@@ -247,7 +247,7 @@ set_k_gemm_bias_gelu_bf16(const __grid_constant__ CUtensorMap tmA, const __grid_
     // Programmatic dependent launch (set.h SET_STAGE_PDL): the prologue above (tensor-map prefetch, barrier init) and the
     // TMEM allocation below may overlap the node before this one; nothing may read A, B or bias, or write C, before that
     // node's writes are visible.  Both instructions do nothing over an ordinary edge.
-    set_pdl_sync();
+    set_pdl_sync(bias);
     // The producer warp goes straight to its first loads; the TMEM allocation (0.2 - 0.4 us) runs beside their latency.
     uint32_t tmem_base = 0;
     if (warp != 0) {

@@ -29,6 +29,7 @@ __global__ void set_k_threshold_u8(const uint8_t* m, uint8_t* t, uint32_t w, uin
 __global__ void set_k_blend_u8(const uint8_t* t, const uint8_t* n, uint8_t* out, uint32_t w, uint32_t h);
 __global__ void set_k_sssp_init(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
 __global__ void set_k_sssp_relax(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, uint32_t sub);
+__global__ void set_k_sssp_solo(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v);
 __global__ void set_k_sssp_control(const int32_t* img, int32_t* out, uint32_t* scratch, uint32_t max_v, uint32_t unroll, cudaGraphConditionalHandle loop);
 }
 
@@ -36,9 +37,20 @@ __global__ void set_k_sssp_control(const int32_t* img, int32_t* out, uint32_t* s
 // then wait until every kernel this one depends on has finished and its writes are visible.  Both instructions do
 // nothing in a kernel that was launched over an ordinary edge, so every built-in kernel starts with this.
 #ifdef __CUDACC__
-__device__ __forceinline__ void set_pdl_sync() {
+// The pointers a kernel READS what earlier nodes wrote through are passed in and come back "laundered" through an empty asm
+// placed after the wait.  Without that the compiler may issue a load through a `const T* __restrict__` parameter BEFORE the
+// wait: it treats such loads as invariant (ld.global.nc), and invariant loads are not held back by a "memory" clobber.
+// Seen in SASS: K21's load of V sat in front of ACQBULK and read what the slot's previous job had left (round 2).
+template <typename T>  // T: a pointer type, __restrict__ and all
+__device__ __forceinline__ void set_pdl_launder(T& p) {
+    static_assert(sizeof(T) == 8, "pointers only");
+    asm volatile("" : "+l"(p));
+}
+template <typename... P>
+__device__ __forceinline__ void set_pdl_sync(P&... inputs) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    (set_pdl_launder(inputs), ...);
 }
 #endif
 
@@ -52,4 +64,7 @@ constexpr int kHistPixPerBlock = 256 * 16;  // one 128-bit load per thread; a 12
 constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words
 constexpr int kStencilTileW = 64 * 4, kStencilTileH = 4;  // K17/K18: block (64, 4), 4 pixels per thread
 constexpr int kBytePixPerBlock = 256 * 16;                // K19/K20: one 128-bit word per thread
+constexpr int kSsspSoloThreads = 1024;                    // K25: one block runs the job
+constexpr unsigned kSsspSoloMaxV = 40000;                 // K25: 5 bytes of shared memory per vertex (200 KB of the SM's 227)
+extern "C" uint32_t set_sssp_solo_smem_bytes(uint32_t max_v);
 constexpr unsigned kSsspLanes = 8;                        // K22: threads per vertex (blocks of 256 threads: 32 vertices each)

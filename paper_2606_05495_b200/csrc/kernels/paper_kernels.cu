@@ -2,7 +2,8 @@
 //   config 6, the five-stage Sobel chain:  K10 gray (stencil_kernels.cu) -> K17 sobel -> K18 mean3x3 ->
 //             K19 threshold -> K20 blend, all integer, bit-exact (readings S6-1..S6-6)
 //   config 5, frontier Bellman-Ford SSSP:  K21 init -> WHILE { K22 relax x U -> K23 control } (readings S5-1..S5-4);
-//             the loop is a conditional WHILE node of the job graph and K23 sets its condition on the device.
+//             the loop is a conditional WHILE node of the job graph and K23 sets its condition on the device;
+//             variant 1: K25, the whole job in one kernel of one block.
 // Hand-written CUDA for sm_100a.  The frames (0.3 - 2 MB) and graphs (~0.6 MB) sit in L2 right after the H2D copy, so
 // these are latency-class kernels like those of configs 0, 1 and 4: coalesced 32- and 128-bit accesses, no shared memory.
 #include "kernels.h"
@@ -56,7 +57,7 @@ __device__ __forceinline__ void stencil3x3_u8(const uint8_t* __restrict__ in, ui
 
 // K17: e = min(255, |gx| + |gy|), gx = [-1 0 1; -2 0 2; -1 0 1] * n, gy = its transpose (reading S6-2).
 extern "C" __global__ void __launch_bounds__(256) set_k_sobel3x3_u8(const uint8_t* __restrict__ n, uint8_t* __restrict__ e, uint32_t w, uint32_t h) {
-    set_pdl_sync();
+    set_pdl_sync(n);
     stencil3x3_u8(n, e, w, h, [](int a, int b, int c, int d, int, int f, int g, int hh, int i) -> uint32_t {
         const int gx = (c - a) + 2 * (f - d) + (i - g);
         const int gy = (g - a) + 2 * (hh - b) + (i - c);
@@ -67,7 +68,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_sobel3x3_u8(const uint8_
 
 // K18: m = (sum of the 3 x 3 neighbourhood) / 9, integer division (reading S6-3).
 extern "C" __global__ void __launch_bounds__(256) set_k_mean3x3_u8(const uint8_t* __restrict__ e, uint8_t* __restrict__ m, uint32_t w, uint32_t h) {
-    set_pdl_sync();
+    set_pdl_sync(e);
     stencil3x3_u8(e, m, w, h, [](int a, int b, int c, int d, int ee, int f, int g, int hh, int i) -> uint32_t {
         return (uint32_t)(a + b + c + d + ee + f + g + hh + i) / 9u;
     });
@@ -76,7 +77,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_mean3x3_u8(const uint8_t
 // K19: t = m >= thresh ? 255 : 0 (reading S6-4).  16 pixels per thread: one 128-bit load, one 128-bit store.
 extern "C" __global__ void __launch_bounds__(256) set_k_threshold_u8(const uint8_t* __restrict__ m, uint8_t* __restrict__ t, uint32_t w, uint32_t h,
                                                                       uint32_t thresh) {
-    set_pdl_sync();
+    set_pdl_sync(m);
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     const uint32_t th4 = thresh * 0x01010101u;
@@ -96,7 +97,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_threshold_u8(const uint8
 // K20: out = (128 t + 128 n) >> 8 = (t + n) >> 1 per byte (reading S6-5): the halving add without rounding.
 extern "C" __global__ void __launch_bounds__(256) set_k_blend_u8(const uint8_t* __restrict__ t, const uint8_t* __restrict__ n, uint8_t* __restrict__ out,
                                                                   uint32_t w, uint32_t h) {
-    set_pdl_sync();
+    set_pdl_sync(t, n);
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     if (p0 + 15 < npix && ((reinterpret_cast<uintptr_t>(t) | reinterpret_cast<uintptr_t>(n) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0) {
@@ -129,7 +130,7 @@ constexpr uint32_t kSsspCtrlWords = 16, kSsspRounds = 1, kSsspDone = 2, kSsspCha
 
 extern "C" __global__ void __launch_bounds__(256) set_k_sssp_init(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
                                                                   uint32_t max_v) {
-    set_pdl_sync();
+    set_pdl_sync(img);
     const uint32_t V = min((uint32_t)img[0], max_v), src = (uint32_t)img[2];
     uint32_t* f0 = scratch;
     uint32_t* f1 = scratch + max_v;
@@ -149,7 +150,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_sssp_init(const int32_t*
 // of out-degree atomics one behind the other.  The flag is read by the whole group before lane 0 clears it.
 extern "C" __global__ void __launch_bounds__(256) set_k_sssp_relax(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch,
                                                                    uint32_t max_v, uint32_t sub) {
-    set_pdl_sync();
+    set_pdl_sync(img);
     const uint32_t V = min((uint32_t)img[0], max_v);
     const int32_t* row_ptr = img + 4;
     const int32_t* col = row_ptr + V + 1;
@@ -186,7 +187,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_sssp_relax(const int32_t
 // last relaxation of the pass lowered some distance (at most V rounds: Bellman-Ford's bound with non-negative weights).
 extern "C" __global__ void set_k_sssp_control(const int32_t* __restrict__ img, int32_t* __restrict__ out, uint32_t* __restrict__ scratch, uint32_t max_v,
                                               uint32_t unroll, cudaGraphConditionalHandle loop) {
-    set_pdl_sync();
+    set_pdl_sync(img);
     const uint32_t V = min((uint32_t)img[0], max_v);
     uint32_t* ctrl = scratch + 2 * (size_t)max_v;
     uint32_t rounds = ctrl[kSsspRounds] + 1u;
@@ -197,4 +198,77 @@ extern "C" __global__ void set_k_sssp_control(const int32_t* __restrict__ img, i
     ctrl[kSsspDone] += unroll;
     out[V] = (int32_t)rounds;
     cudaGraphSetConditional(loop, (last != 0u && rounds <= V) ? 1u : 0u);
+}
+
+// K25: the whole SSSP job in ONE kernel of ONE block (config 5 variant 1, and set_sssp_noalloc): initialisation, every
+// round, the round count -- with __syncthreads() between rounds instead of a pass of a WHILE node (a device-side relaunch
+// of 4 - 5 us that the chip serialises over all graphs in flight).  Same image, same out, same result as
+// K21-K23.  The distances and the frontier flags live in SHARED memory for the whole job (one SM's atomic and scattered
+// store traffic to L2 bounded the first version: 150 us per job at V = 4096 with everything in global memory); global
+// memory sees the read-only graph, the work list and, at the end, one coalesced store of the distances.
+// A round is two phases of the block:
+//   A  every thread looks at the frontier flags of its own vertices (one 32-bit load = 4 byte flags), clears them and
+//      appends the flagged vertices to the work list (position from a shared-memory counter);
+//   B  groups of kSsspLanes threads take the list's vertices and relax their out-edges in place with atomicMin (K22's
+//      relaxation), flagging every vertex whose distance got smaller for the next round.
+// Phases never overlap, so ONE flag array is enough, and only frontier vertices cost a dependent chain of loads.
+// Dynamic shared memory: set_sssp_solo_smem_bytes(max_v) = int32 dist[max_v] + byte flags[max_v]; scratch (global): the
+// work list, uint32[max_v].  Everything the job reads from either it writes first: an earlier job's leftovers never matter.
+// A block is the limit of this variant (max_v <= kSsspSoloMaxV so that the distances fit one SM's shared memory; a round
+// of a full frontier is V / 128 steps of the block): it is meant for graphs of a few thousand vertices -- the paper's
+// "many small jobs" -- and the WHILE-node pipeline stays the general one.
+extern "C" uint32_t set_sssp_solo_smem_bytes(uint32_t max_v) { return 4u * max_v + ((max_v + 3u) & ~3u); }
+
+extern "C" __global__ void __launch_bounds__(kSsspSoloThreads) set_k_sssp_solo(const int32_t* __restrict__ img, int32_t* __restrict__ out,
+                                                                               uint32_t* __restrict__ scratch, uint32_t max_v) {
+    set_pdl_sync(img);
+    extern __shared__ __align__(16) uint8_t solo_smem[];
+    __shared__ uint32_t s_n[2];  // length of the work list, by the parity of the round
+    int32_t* dist = reinterpret_cast<int32_t*>(solo_smem);
+    uint32_t* flag_words = reinterpret_cast<uint32_t*>(solo_smem + 4u * (size_t)max_v);
+    uint8_t* flags = reinterpret_cast<uint8_t*>(flag_words);
+    uint32_t* list = scratch;
+    const uint32_t V = min((uint32_t)img[0], max_v), src = (uint32_t)img[2];
+    const int32_t* row_ptr = img + 4;
+    const int32_t* col = row_ptr + V + 1;
+    const int32_t* wgt = col + img[1];
+    const uint32_t words = (V + 3u) / 4u;
+    for (uint32_t v = threadIdx.x; v < V; v += kSsspSoloThreads) dist[v] = v == src ? 0 : kSsspInf;
+    for (uint32_t w = threadIdx.x; w < words; w += kSsspSoloThreads) flag_words[w] = (src < V && src / 4u == w) ? 1u << (8u * (src % 4u)) : 0u;
+    if (threadIdx.x < 2) s_n[threadIdx.x] = 0u;
+    const uint32_t g = threadIdx.x % kSsspLanes, group = threadIdx.x / kSsspLanes;
+    constexpr uint32_t kGroups = kSsspSoloThreads / kSsspLanes;
+    uint32_t rounds = 0;
+    for (;;) {
+        __syncthreads();  // the flags and distances of the previous round (or the initialisation) are visible to the block
+        uint32_t* n_now = &s_n[rounds & 1u];
+        for (uint32_t w = threadIdx.x; w < words; w += kSsspSoloThreads) {  // phase A
+            const uint32_t f = flag_words[w];
+            if (f == 0u) continue;
+            flag_words[w] = 0u;
+            const uint32_t cnt = (f & 1u) + ((f >> 8) & 1u) + ((f >> 16) & 1u) + ((f >> 24) & 1u);
+            uint32_t pos = atomicAdd(n_now, cnt);
+#pragma unroll
+            for (uint32_t b = 0; b < 4; ++b)
+                if ((f >> (8u * b)) & 1u) list[pos++] = 4u * w + b;
+        }
+        __syncthreads();
+        const uint32_t n = *n_now;
+        if (n == 0u) break;                          // the frontier is empty: done
+        rounds += 1u;                                // a round that had a frontier
+        if (threadIdx.x == 0) s_n[rounds & 1u] = 0u;  // the next round's counter: last read before the barrier above
+        for (uint32_t i = group; i < n; i += kGroups) {  // phase B
+            const uint32_t u = list[i];
+            const int32_t du = *reinterpret_cast<volatile int32_t*>(dist + u);  // finite: u entered the frontier by getting a distance
+            const int32_t e1 = __ldg(row_ptr + u + 1);
+            for (int32_t e = __ldg(row_ptr + u) + (int32_t)g; e < e1; e += (int32_t)kSsspLanes) {
+                const int32_t v = __ldg(col + e), nd = du + __ldg(wgt + e);
+                if (nd < atomicMin(dist + v, nd)) flags[v] = 1u;
+            }
+        }
+        if (rounds > V) break;  // at most V rounds: Bellman-Ford's bound with non-negative weights (uniform over the block)
+    }
+    __syncthreads();
+    for (uint32_t v = threadIdx.x; v < V; v += kSsspSoloThreads) out[v] = dist[v];
+    if (threadIdx.x < 4) out[V + threadIdx.x] = threadIdx.x == 0 ? (int32_t)rounds : 0;
 }

@@ -32,7 +32,7 @@ __device__ __forceinline__ bool aligned16(const void* a, const void* b = nullptr
 // thread totals -> 32 warp totals scanned by warp 0 in shared memory -> carry from the previous chunk.
 extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t* __restrict__ in, int32_t* __restrict__ out,
                                                                   uint32_t n) {
-    set_pdl_sync();
+    set_pdl_sync(in);
     __shared__ int warp_tot[32];
     __shared__ int chunk_tot;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -83,7 +83,7 @@ extern "C" __global__ void __launch_bounds__(1024) set_k_scan_i32(const int32_t*
 // summed, one bin per thread.
 extern "C" __global__ void __launch_bounds__(256) set_k_hist_mod64(const int32_t* __restrict__ in, uint32_t* __restrict__ hist,
                                                                    uint32_t n) {
-    set_pdl_sync();
+    set_pdl_sync(in);
     __shared__ uint32_t h[8][64 + 1];
     const int tid = threadIdx.x, wid = tid >> 5;
     const uint32_t n4 = n / 4;
@@ -124,7 +124,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_hist_mod64(const int32_t
 // K3..K6: one fp32 operation per element per kernel (reading C1-5: the chain stays unfused).  256 threads x 4
 // elements per block; __fmul_rn/__fadd_rn are never contracted into an FMA (reading C1-1).
 extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* __restrict__ x, float* __restrict__ y, uint32_t n) {
-    set_pdl_sync();
+    set_pdl_sync(x);
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(x, y)) {
         float4 v = *reinterpret_cast<const float4*>(x + i);
@@ -139,7 +139,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_affine_f32(const float* 
 }
 
 extern "C" __global__ void __launch_bounds__(256) set_k_add_bias_f32(float* __restrict__ y, const float* __restrict__ bias, uint32_t n) {
-    set_pdl_sync();
+    set_pdl_sync(bias);
     uint32_t i = 4u * (blockIdx.x * 256u + threadIdx.x);
     if (i + 3 < n && aligned16(y, bias)) {
         float4 v = *reinterpret_cast<float4*>(y + i);
@@ -190,7 +190,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_square_f32(float* __rest
 // the 1e-6 tolerance of the double-accumulated oracle; measured ~1e-8).
 extern "C" __global__ void __launch_bounds__(1024) set_k_block_sum_f32(const float* __restrict__ y, float* __restrict__ out,
                                                                        uint32_t n) {
-    set_pdl_sync();
+    set_pdl_sync(y);
     __shared__ float wsum[32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     float acc = 0.0f;
@@ -297,16 +297,16 @@ __device__ __forceinline__ void copy_bytes(const void* __restrict__ src, void* _
 }  // namespace
 
 // fwd_slot != NULL: the copy-in node also carries the job's OUTPUT address into the slot's device word, from which the
-// copy-out node (K25) takes its destination -- so that a job costs ONE graph-node update instead of two (the update and the
+// copy-out node (K24) takes its destination -- so that a job costs ONE graph-node update instead of two (the update and the
 // launch go through the same driver lock, about 0.5 us per node: DESIGN.md 5d).
 extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restrict__ src, void* __restrict__ dst, uint32_t bytes, void** fwd_slot,
                                                              void* fwd_value) {
-    set_pdl_sync();
+    set_pdl_sync(src);
     if (fwd_slot && blockIdx.x == 0 && threadIdx.x == 0) *fwd_slot = fwd_value;
     copy_bytes(src, dst, bytes);
 }
 
-// K25: copy-out whose destination is *dst_slot + dst_off: the address the job's copy-in node left in the slot's device word.
+// K24: copy-out whose destination is *dst_slot + dst_off: the address the job's copy-in node left in the slot's device word.
 // Every kernel between the two is ordered behind its predecessor (plain edge or griddepcontrol.wait), so the word is visible.
 // flag != NULL: this node is also the job's completion signal (K14 folded in: one node less per job -- the GPU's front end
 // works through about three million graph nodes a second, which is what bounds the short-job configs).  Every
@@ -314,7 +314,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_copy(const void* __restr
 // acquired every other block's stores, fences them out at system scope (unless fence == 0) and stores the slot's word.
 extern "C" __global__ void __launch_bounds__(256) set_k_copy_out(const void* __restrict__ src, void* const* __restrict__ dst_slot, unsigned long long dst_off,
                                                                  uint32_t bytes, uint32_t* flag, unsigned long long* stamp, uint32_t fence) {
-    set_pdl_sync();
+    set_pdl_sync(src, dst_slot);
     char* dst = static_cast<char*>(*reinterpret_cast<void* const volatile*>(dst_slot)) + dst_off;
     copy_bytes(src, dst, bytes);
     if (flag) {

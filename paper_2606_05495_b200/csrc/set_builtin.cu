@@ -109,6 +109,7 @@ extern "C" const void* set_builtin_kernel(int id) {
         case SET_K_SSSP_INIT: return (const void*)set_k_sssp_init;
         case SET_K_SSSP_RELAX: return (const void*)set_k_sssp_relax;
         case SET_K_SSSP_CONTROL: return (const void*)set_k_sssp_control;
+        case SET_K_SSSP_SOLO: return (const void*)set_k_sssp_solo;
         default: return nullptr;
     }
 }
@@ -237,6 +238,12 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[1].d2h_bytes = fixed(out_bytes);
             bf[2] = buffer(8ull * maxv + 64);                  // frontier flags [2][maxV], ctrl[16]
             nb = 3;
+            if (variant == 1) {  // the whole job in one kernel of one block: no WHILE node (K25)
+                if (maxv > kSsspSoloMaxV) return SET_ERR_INVALID;  // the distances must fit one SM's shared memory
+                st[ns++] = stage(SET_K_SSSP_SOLO, grid_fixed(1), grid_fixed(1), kSsspSoloThreads, 1, set_sssp_solo_smem_bytes(maxv),
+                                 {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
+                break;
+            }
             const set_grid_rule g = grid_fixed((maxv + 255) / 256);
             st[ns++] = stage(SET_K_SSSP_INIT, g, grid_fixed(1), 256, 1, 0, {arg_buf(0), arg_buf(1), arg_buf(2), arg_u32(maxv)});
             for (uint32_t sub = 0; sub < unroll; ++sub) {

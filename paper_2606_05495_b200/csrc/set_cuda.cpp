@@ -566,7 +566,7 @@ int set_ctx::build_graph(int slot, int set_index) {
         }
     }
     if (flag_poll && fused_signal_buf >= 0) {
-        // the job's only copy-out node stores the completion word itself (K25); the start stamp only has to have run before it
+        // the job's only copy-out node stores the completion word itself (K24); the start stamp only has to have run before it
         if (stamps) CK(depend(g.stamp_start_node, g.d2h_nodes[fused_signal_buf], false));
     } else if (flag_poll) {  // completion signal: runs after every D2H copy of the job has finished (kernels.cu K14)
         std::vector<bool> leaf_is_kernel;
@@ -1323,14 +1323,18 @@ set_status set_register_pipeline(set_ctx* c, const set_stage_desc* stages, int n
             return c->fail(SET_ERR_NOMEM, "pinned placeholder allocation failed");
         }
     }
-    // ---- which copies become SET_K_COPY kernel nodes: fixed size (the grid never changes), at most sm_copy_max_bytes
+    // ---- which copies become SET_K_COPY kernel nodes: at most sm_copy_max_bytes; a size that depends on the job's dims counts
+    // with its buffer's capacity (the node's byte count and grid are part of the per-job update either way)
     {
         // default 256 KiB: below that a copy-engine node costs more in engine hand-off than the copy itself, across the
         // host link and (SET_IO_DEVICE) inside HBM alike (profiles/r1_bench.md, graph_variants)
         int64_t lim = c->cfg.sm_copy_max_bytes != 0 ? c->cfg.sm_copy_max_bytes : 262144;
         for (size_t i = 0; i < c->bufs.size(); ++i) {
             const set_buffer_desc& bd = c->bufs[i];
-            auto small = [&](const set_size_expr& e) { return e.per_unit == 0 && e.fixed > 0 && (int64_t)e.fixed <= lim; };
+            auto small = [&](const set_size_expr& e) {
+                if (expr_is_zero(e)) return false;
+                return (int64_t)(e.per_unit == 0 ? e.fixed : bd.bytes) <= lim;
+            };
             c->h2d_sm[i] = small(bd.h2d_bytes);
             c->d2h_sm[i] = small(bd.d2h_bytes);
             c->n_sm_copies += (int)c->h2d_sm[i] + (int)c->d2h_sm[i];

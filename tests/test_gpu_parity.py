@@ -872,6 +872,43 @@ def test_config5_relaxations_per_loop_pass(libset, unroll, v, deg):
     assert st["kernel_nodes"] == 8 * (2 + unroll)
 
 
+@pytest.mark.parametrize("v,deg", [(1, 1), (2, 1), (37, 2), (256, 1), (1000, 4), (4096, 8), (20000, 3)])
+@pytest.mark.parametrize("pdl", [False, True])
+def test_config5_single_kernel_variant(libset, v, deg, pdl):
+    """Variant 1 of config 5: the whole job in ONE kernel of one block (SET_K_SSSP_SOLO), no WHILE node.  Same images, same
+    outputs, same rule: distances bit for bit, rounds within the oracle's; more jobs than slots, so every slot's scratch is
+    reused by a job with another graph."""
+    from paper_2606_05495_b200.workloads import Workload
+    wl = Workload(5, (v, inputgen.sssp_max_edges(v, deg)), variant=1, jobs=24, num_streams=4, max_inflight=8, kernels_per_job=1,
+                  extra={"mean_deg": deg})
+    st = check(libset, wl, list(range(24)), pdl=pdl)
+    assert st["kernel_nodes"] == 24 and st["cuda_streams"] >= 4       # an ordinary pipeline: no loop, all streams in use
+
+
+def test_config5_single_kernel_variant_at_the_bench_size_in_every_model(libset):
+    from paper_2606_05495_b200.workloads import baseline_workload
+    import dataclasses
+    wl = dataclasses.replace(baseline_workload(5), variant=1, kernels_per_job=1, jobs=256)
+    for mode in (0, 1, 2, 3, 4):
+        check(libset, wl, list(range(256 if mode == 0 else 40)), mode=mode)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_copies_of_a_job_dependent_size_as_sm_copies(libset, variant):
+    """Config 5's copy-in is 16 + 4 (V + 1) + 8 E bytes, E per job: with sm_copy_max_bytes above the buffer's capacity it is an
+    SM copy node whose byte count and grid are updated per job (two SM copies per job then: in and out); the default limit
+    keeps the copy engine for it at the bench size.  Jobs of different E alternate on every slot."""
+    from paper_2606_05495_b200.workloads import Workload
+    v, deg = 4096, 8
+    wl = Workload(5, (v, inputgen.sssp_max_edges(v, deg)), variant=variant, jobs=40, num_streams=4, max_inflight=8,
+                  kernels_per_job=1 if variant else 6, extra={"mean_deg": deg})
+    assert len({wl.dims(j)[0] for j in range(40)}) > 30                       # the sizes really differ
+    st = check(libset, wl, list(range(40)), sm_copy_max_bytes=1 << 20)
+    assert st["copy_nodes"] == 2 * 40
+    st = check(libset, wl, list(range(8)))
+    assert st["copy_nodes"] == 8                                              # default: copy-out only
+
+
 def test_config5_unroll_out_of_range_is_refused(libset):
     for u in (0, 1, 9):       # U = 1 would be a two-node loop body, which this driver does not run reliably (set.h)
         ctx = libset.Context(2, 4)
@@ -1003,4 +1040,5 @@ def test_signal_fusing_and_output_forwarding_variants(libset, monkeypatch, confi
     n = min(wl.jobs, 64)
     st = check(libset, wl, list(range(n)), pdl=True, debug_sentinel=0xA5A5A5A5)
     assert st["early_completions"] == 0
-    assert st["signal_nodes"] == (0 if fuse == "1" and forward == "1" and config != 5 else n)   # config 5's copy-in is a memcpy node: nothing forwards
+    # config 5's copy-in has a job-dependent size: it is an SM copy too while its buffer's capacity is within sm_copy_max_bytes
+    assert st["signal_nodes"] == (0 if fuse == "1" and forward == "1" else n)
