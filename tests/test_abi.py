@@ -112,3 +112,38 @@ def test_product_does_not_import_oracle():
             assert "paper_2606_05495_b200" not in src.replace("imports nothing from\npaper_2606_05495_b200", "") or f in ("__init__.py", "oracle.h")
             assert not re.search(r"^\s*(import|from)\s+paper_2606_05495_b200", src, flags=re.M), f
             assert "set.h" not in src and "libset" not in src, f
+
+
+def test_no_global_memory_access_is_scheduled_before_griddepcontrol_wait(libset):
+    """Every built-in kernel starts with griddepcontrol.launch_dependents / .wait (kernels.h set_pdl_sync) so that it may sit
+    behind a programmatic edge.  The compiler once moved an invariant load (`const T* __restrict__` parameter, ld.global.nc)
+    in front of the wait -- a stale read of the slot's previous job -- so the SASS of every kernel is scanned:
+    no global load, store, atomic or TMA load may precede ACQBULK (the wait)."""
+    import shutil
+    import subprocess
+    from paper_2606_05495_b200 import build as b
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    objs = [os.path.join(b.BUILD_DIR, f) for f in sorted(os.listdir(b.BUILD_DIR)) if f.startswith("kernels_") and f.endswith(".o")]
+    assert len(objs) >= 4
+    seen, bad = set(), []
+    mem = re.compile(r"\b(LDG|LD\.E|STG|ST\.E|ATOMG?|RED|UTMALDG|UTMASTG)\b")
+    for o in objs:
+        sass = subprocess.run([cuobjdump, "-sass", o], capture_output=True, text=True, check=True).stdout
+        fn, waited = None, False
+        for ln in sass.splitlines():
+            m = re.search(r"Function : (\S+)", ln)
+            if m:
+                fn, waited = m.group(1), False
+                continue
+            if fn is None or not re.search(r"/\*[0-9a-f]{4,}\*/", ln):
+                continue
+            if "ACQBULK" in ln:
+                waited = True
+                seen.add(fn)
+            elif not waited and mem.search(ln):
+                bad.append((fn, ln.strip()[:90]))
+    assert not bad, bad[:5]
+    kernels = {n for n in seen if n.startswith("set_k_")}
+    assert len(kernels) >= 25, sorted(kernels)          # every set_k_* kernel has the wait
