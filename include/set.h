@@ -57,6 +57,7 @@ typedef int32_t set_status;
 #define SET_ERR_NOMEM    (-3) /* host or device allocation failed                                  */
 #define SET_ERR_STATE    (-4) /* call out of order (submit before register, register twice, ...)   */
 #define SET_ERR_SIZE     (-5) /* a per-job size computed from dims exceeds a registered buffer     */
+#define SET_ERR_BUSY     (-6) /* set_try_submit_dims: no executable is free right now (not an error state)   */
 
 #define SET_MAX_STAGES  16
 #define SET_MAX_BUFFERS  8
@@ -329,6 +330,10 @@ set_status set_register_pipeline(set_ctx *ctx, const set_stage_desc *stages, int
 set_status set_submit(set_ctx *ctx, uint64_t job_id, const void *host_in, void *host_out);
 set_status set_submit_dims(set_ctx *ctx, uint64_t job_id, const void *host_in, void *host_out,
                            const uint32_t dims[SET_MAX_DIMS]);
+/* set_submit_dims that never blocks: SET_ERR_BUSY if no executable is free right now (nothing was queued, the context is
+ * unchanged and stays usable); SET_MODE_SET only (SET_ERR_STATE otherwise).  The building block of set_multi_submit_dims. */
+set_status set_try_submit_dims(set_ctx *ctx, uint64_t job_id, const void *host_in, void *host_out,
+                               const uint32_t dims[SET_MAX_DIMS]);
 /* n submissions in one call (same semantics as n calls in order).  host_ins/host_outs: HOST arrays of
  * n pointers; dims: HOST array[n][4] or NULL; job_ids: HOST array[n] or NULL (then first_id + i). */
 set_status set_submit_batch(set_ctx *ctx, int64_t n, uint64_t first_id, const uint64_t *job_ids,
@@ -482,6 +487,36 @@ int64_t set_selftest_ring(int capacity, int producers, int consumers, int64_t it
  * (set_config.completion_thread), seed bit 3 bind-at-launch (set_config.bind_at_launch).  Returns 0 or a negative error code. */
 int64_t set_selftest_scheduler(int num_streams, int max_inflight, int queue_capacity, int num_dispatchers,
                                int submitters, int64_t jobs, uint32_t seed, uint64_t *out_steals);
+
+/* ---------------------------------------------------------------------------------------------- *
+ * Several scheduler instances behind one submit call ("one scheduler instance per GPU (own streams, slots,
+ * execs); job_id mod n_gpu as home, host-side stealing across instances"; PAPER.md:122 for the retarget-to-thief idea).
+ * No collective, no device-to-device traffic: jobs are independent and live in host memory; an instance is a whole set_ctx
+ * on the device it was given, and two instances may share a device.  Host buffers must be reachable from every device
+ * (set_host_alloc memory is: it is allocated portable).  Unmeasured on more than one GPU.
+ *
+ * set_multi_create      : cfg as for set_create_ex (cfg->device is ignored), devices: HOST array[num_instances] of CUDA
+ *                         ordinals, 1 <= num_instances <= 64.  SET_MODE_SET only.  *out is NULL on failure.
+ * set_multi_register_pipeline : the same pipeline on every instance (arguments as set_register_pipeline).
+ * set_multi_submit_dims : home = job_id mod num_instances.  If the home instance has no free executable at this instant
+ *                         the job goes to the first other instance (home + 1, home + 2, ... cyclically) that has one -- the
+ *                         idle instance steals at the host, before anything was bound -- and if none has, the call blocks
+ *                         on the home instance (back-pressure).  Thread-safe like set_submit.  dims may be NULL.
+ * set_multi_drain       : set_drain of every instance; returns the first failing status.
+ * set_multi_instance    : the i-th set_ctx (for set_host_alloc, set_get_stats, set_last_error), NULL if out of range.
+ * set_multi_stolen      : jobs that ran on an instance other than their home since creation.
+ * set_multi_destroy     : drains and destroys every instance.
+ */
+typedef struct set_multi set_multi;
+set_status set_multi_create(const set_config *cfg, int num_instances, const int *devices, set_multi **out);
+set_status set_multi_register_pipeline(set_multi *m, const set_stage_desc *stages, int num_stages,
+                                       const set_buffer_desc *bufs, int num_bufs);
+set_status set_multi_submit_dims(set_multi *m, uint64_t job_id, const void *host_in, void *host_out,
+                                 const uint32_t dims[SET_MAX_DIMS]);
+set_status set_multi_drain(set_multi *m);
+set_ctx *set_multi_instance(set_multi *m, int i);
+uint64_t set_multi_stolen(set_multi *m);
+set_status set_multi_destroy(set_multi *m);
 
 /* ---------------------------------------------------------------------------------------------- *
  * An entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight

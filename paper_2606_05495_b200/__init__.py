@@ -18,7 +18,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libset.so")
 
-SET_OK, SET_ERR_INVALID, SET_ERR_CUDA, SET_ERR_NOMEM, SET_ERR_STATE, SET_ERR_SIZE = 0, -1, -2, -3, -4, -5
+SET_OK, SET_ERR_INVALID, SET_ERR_CUDA, SET_ERR_NOMEM, SET_ERR_STATE, SET_ERR_SIZE, SET_ERR_BUSY = 0, -1, -2, -3, -4, -5, -6
 SET_MAX_STAGES, SET_MAX_BUFFERS, SET_MAX_ARGS, SET_MAX_DIMS = 16, 8, 12, 4
 MODE_SET, MODE_PLAIN_STREAMS, MODE_BATCH_SYNC, MODE_SINGLE_GRAPH, MODE_MUTEX_QUEUE = 0, 1, 2, 3, 4
 IO_HOST, IO_DEVICE = 0, 1
@@ -33,7 +33,7 @@ BUF_ZERO = 1
 VARIANT_SPIN = 0x100
 
 _STATUS_NAMES = {0: "SET_OK", -1: "SET_ERR_INVALID", -2: "SET_ERR_CUDA", -3: "SET_ERR_NOMEM", -4: "SET_ERR_STATE",
-                 -5: "SET_ERR_SIZE"}
+                 -5: "SET_ERR_SIZE", -6: "SET_ERR_BUSY"}
 
 
 class SetError(RuntimeError):
@@ -102,7 +102,9 @@ class GapStats(C.Structure):
 EXPORTS = ["set_create", "set_create_ex", "set_register_pipeline", "set_submit", "set_submit_dims", "set_submit_batch",
            "set_drain", "set_destroy", "set_host_alloc", "set_host_free", "set_host_register", "set_host_unregister", "set_get_stats", "set_reset_stats", "set_get_gap_stats",
            "set_last_error", "set_get_geometry", "set_time_stage", "set_builtin_kernel", "set_builtin_pipeline",
-           "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler", "set_sssp_noalloc", "set_noalloc_last_error"]
+           "set_selftest_find_order", "set_selftest_ring", "set_selftest_scheduler", "set_sssp_noalloc", "set_noalloc_last_error",
+           "set_try_submit_dims", "set_multi_create", "set_multi_register_pipeline", "set_multi_submit_dims", "set_multi_drain",
+           "set_multi_instance", "set_multi_stolen", "set_multi_destroy"]
 
 _lib = None
 
@@ -147,6 +149,16 @@ def load():
     lib.set_selftest_ring.restype = i64
     lib.set_selftest_scheduler.argtypes = [C.c_int] * 5 + [i64, C.c_uint32, C.POINTER(u64)]
     lib.set_selftest_scheduler.restype = i64
+    lib.set_try_submit_dims.argtypes = [vp, u64, vp, vp, C.POINTER(C.c_uint32)]
+    lib.set_multi_create.argtypes = [C.POINTER(Config), C.c_int, C.POINTER(C.c_int), C.POINTER(vp)]
+    lib.set_multi_register_pipeline.argtypes = [vp, C.POINTER(StageDesc), C.c_int, C.POINTER(BufferDesc), C.c_int]
+    lib.set_multi_submit_dims.argtypes = [vp, u64, vp, vp, C.POINTER(C.c_uint32)]
+    lib.set_multi_drain.argtypes = [vp]
+    lib.set_multi_instance.argtypes = [vp, C.c_int]
+    lib.set_multi_instance.restype = vp
+    lib.set_multi_stolen.argtypes = [vp]
+    lib.set_multi_stolen.restype = u64
+    lib.set_multi_destroy.argtypes = [vp]
     lib.set_sssp_noalloc.argtypes = [vp, vp, C.c_uint32, vp]
     lib.set_noalloc_last_error.argtypes = []
     lib.set_noalloc_last_error.restype = C.c_char_p
@@ -314,6 +326,76 @@ class Context:
         out = C.c_float(0)
         self._check(self._lib.set_time_stage(self._h, stage, d, warmup, iters, C.byref(out)), "set_time_stage")
         return out.value
+
+
+class MultiContext:
+    """set_multi (include/set.h): one scheduler instance per entry of `devices` behind one submit call; a job's home is
+    job_id mod n, an instance with room takes a job whose home is full.  Argument marshalling only."""
+
+    def __init__(self, devices, num_streams: int, max_inflight: int, queue_capacity: int = 0, sm_copy_max_bytes: int = 0,
+                 streams_per_lane: int = 0, completion_thread: int = 0):
+        self._lib = load()
+        self._h = C.c_void_p(None)
+        cfg = Config()
+        cfg.struct_bytes = C.sizeof(Config)
+        cfg.num_streams, cfg.max_inflight, cfg.mode, cfg.io = num_streams, max_inflight, MODE_SET, IO_HOST
+        cfg.queue_capacity, cfg.sm_copy_max_bytes, cfg.streams_per_lane, cfg.completion_thread = queue_capacity, sm_copy_max_bytes, streams_per_lane, completion_thread
+        self.n = len(devices)
+        dev = (C.c_int * self.n)(*[int(d) for d in devices])
+        rc = self._lib.set_multi_create(C.byref(cfg), self.n, dev, C.byref(self._h))
+        if rc != SET_OK:
+            raise SetError(rc, "set_multi_create")
+
+    def _check(self, rc: int, what: str):
+        if rc != SET_OK:
+            detail = " | ".join(filter(None, ((self._lib.set_last_error(self.instance(i)) or b"").decode() for i in range(self.n))))
+            raise SetError(rc, what, detail)
+
+    def instance(self, i: int) -> int:
+        return self._lib.set_multi_instance(self._h, i)
+
+    def register_builtin(self, config: int, variant: int = 0, params=None, pdl: bool = False):
+        st, ns, bf, nb, hin, hout = builtin_pipeline(config, variant, params)
+        if pdl:
+            for i in range(ns):
+                st[i].flags |= STAGE_PDL
+        self._check(self._lib.set_multi_register_pipeline(self._h, st, ns, bf, nb), "set_multi_register_pipeline")
+        return hin, hout
+
+    def submit(self, job_id: int, host_in: int, host_out: int, dims=None):
+        d = None if dims is None else (C.c_uint32 * 4)(*(list(dims) + [1] * (4 - len(dims))))
+        self._check(self._lib.set_multi_submit_dims(self._h, job_id, host_in, host_out, d), "set_multi_submit_dims")
+
+    def drain(self):
+        self._check(self._lib.set_multi_drain(self._h), "set_multi_drain")
+
+    def stolen(self) -> int:
+        return int(self._lib.set_multi_stolen(self._h))
+
+    def stats(self, i: int) -> dict:
+        s = Stats()
+        self._check(self._lib.set_get_stats(self.instance(i), C.byref(s)), "set_get_stats")
+        return s.as_dict()
+
+    def host_alloc(self, nbytes: int) -> int:
+        p = self._lib.set_host_alloc(self.instance(0), nbytes)
+        if not p:
+            raise SetError(SET_ERR_NOMEM, f"set_host_alloc({nbytes})")
+        return p
+
+    def host_free(self, p: int):
+        self._lib.set_host_free(self.instance(0), p)
+
+    def close(self):
+        if self._h:
+            self._lib.set_multi_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
 
 
 NOALLOC_MAX_VERTICES = 16384  # SET_NOALLOC_MAX_VERTICES

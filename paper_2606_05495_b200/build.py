@@ -18,7 +18,7 @@ TRACE_LIB = os.path.join(HERE, "libsettrace.so")  # CUPTI gap tracer (include/se
 BUILD_DIR = os.path.join(HERE, "build")
 
 CUDA_SOURCES = ["kernels/small_kernels.cu", "kernels/stencil_kernels.cu", "kernels/paper_kernels.cu", "kernels/gemm_sm100.cu", "set_builtin.cu", "set_noalloc.cu"]
-HOST_SOURCES = ["set_cuda.cpp", "set_selftest.cpp"]
+HOST_SOURCES = ["set_cuda.cpp", "set_selftest.cpp", "set_multi.cpp"]
 HEADERS = ["set_core.hpp", "set_ring.hpp", "kernels/kernels.h"]
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

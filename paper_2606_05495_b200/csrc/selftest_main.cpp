@@ -36,7 +36,8 @@ int main(int argc, char** argv) {
         {1, 1, 1, 1, 1, 1000, 3},  {4, 6, 1, 2, 3, 5000, 5},   {2, 64, 4, 2, 2, 10000, 4}, {8, 4096, 1, 1, 2, 20000, 2},
         {8, 32, 2, 1, 1, 10000, 6}, {8, 32, 2, 2, 2, 10000, 7}, {4, 8, 2, 1, 2, 10000, 6},   // bit 2: completion thread of its own
         {8, 32, 2, 1, 1, 10000, 14}, {8, 32, 2, 2, 2, 10000, 9}, {4, 8, 2, 1, 2, 10000, 10}, {8, 32, 2, 2, 1, 10000, 15},  // bit 3: bind at launch
-        {8, 32, 2, 1, 1, 10000, 18}, {4, 32, 2, 2, 3, 10000, 22}, {8, 16, 2, 2, 2, 10000, 26}};  // bit 4: slots beyond the streams retired, slot-bound
+        {8, 32, 2, 1, 1, 10000, 18}, {4, 32, 2, 2, 3, 10000, 22}, {8, 16, 2, 2, 2, 10000, 26},  // bit 4: slots beyond the streams retired, slot-bound
+        {2, 4, 1, 1, 3, 10000, 32}, {8, 32, 2, 2, 2, 10000, 38}};  // bit 5: non-blocking submits that are retried
     for (auto& s : scheds) {
         uint64_t steals = 0;
         int64_t rc = set_selftest_scheduler(s.S, s.b, s.q, s.disp, s.subs, s.jobs * scale, s.seed, &steals);

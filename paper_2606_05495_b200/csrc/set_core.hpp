@@ -221,7 +221,8 @@ class Scheduler {
     // The paper's submitter claims job indices from a shared array with compare_exchange(c_next, id, id+1);
     // here the caller hands the job over, so the claim degenerates to a fetch_add that yields the ticket used
     // to pick the first queue to look at ("monitors all queues for available slots").
-    int submit(JobDesc job) {
+    static constexpr int kWouldBlock = -6;  // SET_ERR_BUSY: a non-blocking submit found no free executable
+    int submit(JobDesc job, bool blocking = true) {
         uint64_t t0 = now_ns();
         if (int e = error()) return e;
         uint64_t ticket = c_next_.fetch_add(1, std::memory_order_relaxed);
@@ -239,6 +240,7 @@ class Scheduler {
             }
             if (slot >= 0) break;
             if (int e = error()) return e;
+            if (!blocking) return kWouldBlock;  // nothing was taken, nothing to undo (the ticket only picks where the scan starts)
             stats_.submit_stalls.fetch_add(1, std::memory_order_relaxed);
             if (space_ec_.wait(seen, spin_ns_, kPollNs))
                 if (int e = be_->poll()) set_error(e);

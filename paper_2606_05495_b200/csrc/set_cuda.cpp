@@ -1453,6 +1453,19 @@ set_status set_submit(set_ctx* c, uint64_t job_id, const void* host_in, void* ho
     return set_submit_dims(c, job_id, host_in, host_out, nullptr);
 }
 
+set_status set_try_submit_dims(set_ctx* c, uint64_t job_id, const void* host_in, void* host_out, const uint32_t dims[SET_MAX_DIMS]) {
+    if (!c || !host_in || !host_out) return SET_ERR_INVALID;
+    if (int e = c->err.load()) return e;
+    if (!c->registered) return SET_ERR_STATE;
+    if (c->cfg.mode != SET_MODE_SET) return SET_ERR_STATE;  // the baseline models have no queue to find full
+    JobDesc j;
+    j.id = job_id;
+    j.in = host_in;
+    j.out = host_out;
+    if (dims) memcpy(j.dims, dims, sizeof(j.dims));
+    return c->sched->submit(j, /*blocking=*/false);
+}
+
 set_status set_submit_batch(set_ctx* c, int64_t n, uint64_t first_id, const uint64_t* job_ids, const void* const* host_ins,
                             void* const* host_outs, const uint32_t* dims) {
     if (!c || n < 0 || (n > 0 && (!host_ins || !host_outs))) return SET_ERR_INVALID;

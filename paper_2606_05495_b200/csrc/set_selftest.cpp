@@ -201,7 +201,7 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
         be.attach(&sched);
         std::atomic<int64_t> next{0};
         std::vector<std::thread> subs;
-        std::atomic<int64_t> submit_errors{0};
+        std::atomic<int64_t> submit_errors{0}, would_block{0};
         for (int s = 0; s < submitters; ++s)
             subs.emplace_back([&] {
                 for (;;) {
@@ -209,7 +209,16 @@ extern "C" int64_t set_selftest_scheduler(int num_streams, int max_inflight, int
                     if (j >= jobs) break;
                     JobDesc d;
                     d.id = (uint64_t)j;
-                    if (sched.submit(d) != 0) submit_errors.fetch_add(1);
+                    if ((seed >> 5) & 1) {  // seed bit 5: non-blocking submits, retried while every executable is taken (set_try_submit_dims)
+                        int rc;
+                        while ((rc = sched.submit(d, /*blocking=*/false)) == Scheduler::kWouldBlock) {
+                            would_block.fetch_add(1);
+                            std::this_thread::yield();
+                        }
+                        if (rc != 0) submit_errors.fetch_add(1);
+                    } else if (sched.submit(d) != 0) {
+                        submit_errors.fetch_add(1);
+                    }
                 }
             });
         for (auto& t : subs) t.join();

@@ -84,6 +84,12 @@ def test_invalid_arguments_are_rejected_without_a_device(libset):
     assert lib.set_drain(None) == libset.SET_ERR_INVALID
     assert lib.set_destroy(None) == libset.SET_OK
     assert lib.set_last_error(None) == b""
+    assert lib.set_try_submit_dims(None, 0, None, None, None) == libset.SET_ERR_INVALID
+    m = C.c_void_p(None)
+    assert lib.set_multi_create(None, 2, None, C.byref(m)) == libset.SET_ERR_INVALID and not m
+    assert lib.set_multi_submit_dims(None, 0, None, None, None) == libset.SET_ERR_INVALID
+    assert lib.set_multi_drain(None) == libset.SET_ERR_INVALID
+    assert lib.set_multi_destroy(None) == libset.SET_OK and lib.set_multi_stolen(None) == 0 and not lib.set_multi_instance(None, 0)
 
 
 def test_no_cpu_fallback_without_gpu(libset):

@@ -812,6 +812,86 @@ def test_maximum_depth_4096_in_flight(libset):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
+# one scheduler instance per GPU behind one submit call, host-side stealing across instances.  One GPU here:
+# both instances sit on device 0 (set.h allows it), which exercises everything but the second device.
+# ---------------------------------------------------------------------------------------------------------------------
+def _multi_run(libset, m, wl, job_ids):
+    from paper_2606_05495_b200.workloads import PinnedArena
+    ins = [wl.make_input(j) for j in job_ids]
+    arena = PinnedArena(m, sum(x.nbytes + 512 for x in ins) + len(ins) * (wl.out_bytes() + 512) + 4096)
+    bufs = []
+    for x in ins:
+        a_in, v_in = arena.take(x.nbytes)
+        v_in[:] = x
+        a_out, v_out = arena.take(wl.out_bytes())
+        v_out[:] = SENTINEL
+        bufs.append((a_in, a_out, v_out))
+    for k, j in enumerate(job_ids):
+        m.submit(j, bufs[k][0], bufs[k][1])
+    m.drain()
+    for k in range(len(job_ids)):
+        compare(wl, np.array(bufs[k][2], copy=True), oracle_out(wl, ins[k], (1, 1, 1, 1)))
+    bufs = None
+    arena.free()
+
+
+@pytest.mark.parametrize("config", [0, 1])
+def test_multi_instance_front_end_routes_jobs_to_their_home(libset, config):
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(config)
+    n = 300
+    with libset.MultiContext([0, 0, 0], 2, 8) as m:
+        m.register_builtin(config, 0, list(wl.params), pdl=True)
+        _multi_run(libset, m, wl, list(range(n)))
+        done = [m.stats(i)["completed"] for i in range(3)]
+        assert sum(done) == n and m.stolen() <= n
+        # a job runs at home unless home was full at that instant: whatever was not stolen ran at job_id mod 3
+        assert all(abs(d - n // 3) <= m.stolen() for d in done), (done, m.stolen())
+
+
+def test_multi_instance_front_end_steals_when_home_is_full(libset):
+    """Every job id is even, so instance 0 is everybody's home; with one slot and two executables it is full most of the time
+    and instance 1 takes what it cannot: every output is still F(in) of its own job, and instance 1 ran exactly the stolen jobs."""
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(1)
+    n = 400
+    with libset.MultiContext([0, 0], 1, 1, queue_capacity=1) as m:
+        m.register_builtin(1, 0, list(wl.params))
+        _multi_run(libset, m, wl, [2 * k for k in range(n)])
+        s0, s1 = m.stats(0), m.stats(1)
+        assert s0["completed"] + s1["completed"] == n
+        assert m.stolen() == s1["completed"] and m.stolen() > 0
+        assert s0["max_inflight_seen"] <= 1 and s1["max_inflight_seen"] <= 1
+
+
+def test_try_submit_reports_busy_and_leaves_the_context_usable(libset):
+    import ctypes as C
+    from paper_2606_05495_b200.workloads import PinnedArena, small_workload
+    wl = small_workload(1)
+    lib = libset.load()
+    with libset.Context(1, 1, queue_capacity=1) as ctx:
+        ctx.register_builtin(1, 0, list(wl.params))
+        x = wl.make_input(0)
+        arena = PinnedArena(ctx, x.nbytes + 64 * 512 + 4096)
+        a_in, v_in = arena.take(x.nbytes)
+        v_in[:] = x
+        outs = [arena.take(4) for _ in range(64)]
+        codes = [lib.set_try_submit_dims(ctx._h, k, a_in, outs[k][0], None) for k in range(64)]
+        ctx.drain()
+        assert set(codes) <= {libset.SET_OK, libset.SET_ERR_BUSY} and codes[0] == libset.SET_OK
+        assert codes.count(libset.SET_ERR_BUSY) > 0                       # two executables, 64 submissions in a few microseconds
+        assert ctx.stats()["completed"] == codes.count(libset.SET_OK)
+        want = oracle_out(wl, x, (1, 1, 1, 1))
+        for k, c in enumerate(codes):
+            if c == libset.SET_OK:
+                compare(wl, np.array(outs[k][1], copy=True), want)
+        ctx.submit(99, a_in, outs[0][0])                                  # still usable
+        ctx.drain()
+        v_in = outs = None
+        arena.free()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
 # the two paper workloads of SURVEY.md 8(f)4: SSSP with a conditional WHILE node (config 5), Sobel chain (config 6)
 # ---------------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("config", [5, 6])

@@ -42,6 +42,8 @@ def test_ring_delivers_every_token_exactly_once(libset, cap, prod, cons, items):
     (8, 32, 2, 1, 1, 20000, 16 + 2),    # a loop pipeline's geometry: slots 8..31 retired, executables bound to their slot
     (4, 32, 2, 2, 3, 20000, 16 + 4),    # the same with a completion thread, several dispatchers and submitters
     (8, 8, 2, 1, 1, 5000, 16),          # nothing to retire
+    (2, 4, 1, 1, 3, 20000, 32),         # non-blocking submits (set_try_submit_dims) retried by three submitters against 4 slots
+    (8, 32, 2, 2, 2, 20000, 32 + 4 + 2),
 ])
 def test_scheduler_algorithms_on_simulated_device(libset, S, b, q, disp, subs, jobs, seed):
     rc, steals = libset.selftest_scheduler(S, b, q, disp, subs, jobs, seed)
