@@ -62,7 +62,6 @@ constexpr int kGrayPixPerBlock = 256 * 16;
 constexpr int kBlurTileW = 512, kBlurTileH = 16;  // 32 lanes x 16 pixels, 4 warps x 4 rows (a 1280 x 720 frame: 135 blocks)
 constexpr int kHistPixPerBlock = 256 * 16;  // one 128-bit load per thread; a 1280 x 720 frame: 225 blocks
 constexpr int kCopyBytesPerBlock = 256 * 16 * 2;  // set_k_copy: 256 threads x two 128-bit words
-constexpr int kStencilTileW = 64 * 4, kStencilTileH = 4;  // K17/K18: block (64, 4), 4 pixels per thread
 constexpr int kBytePixPerBlock = 256 * 16;                // K19/K20: one 128-bit word per thread
 constexpr int kSsspSoloThreads = 1024;                    // K25: one block runs the job
 constexpr unsigned kSsspSoloMaxV = 40000;                 // K25: 5 bytes of shared memory per vertex (200 KB of the SM's 227)

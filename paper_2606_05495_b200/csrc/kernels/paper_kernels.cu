@@ -5,73 +5,188 @@
 //             the loop is a conditional WHILE node of the job graph and K23 sets its condition on the device;
 //             variant 1: K25, the whole job in one kernel of one block.
 // Hand-written CUDA for sm_100a.  The frames (0.3 - 2 MB) and graphs (~0.6 MB) sit in L2 right after the H2D copy, so
-// these are latency-class kernels like those of configs 0, 1 and 4: coalesced 32- and 128-bit accesses, no shared memory.
+// these are latency-class kernels like those of configs 0, 1 and 4: coalesced 128-bit accesses; only K25 uses shared memory.
 #include "kernels.h"
 
 namespace {
 
-// ---- 3 x 3 neighbourhoods on a byte image, clamp-to-edge: a thread produces 4 horizontally adjacent pixels --------------
-// rows[r][c]: row y-1+r, column x0-1+c, c = 0..5.  Fast path (w % 4 == 0, so every row starts 4-byte aligned and x0 is a
-// multiple of 4): one 32-bit load for the four centre pixels plus one byte on either side.
-__device__ __forceinline__ void load_row6(const uint8_t* __restrict__ row, uint32_t x0, uint32_t w, bool fast, int (&p)[6]) {
-    if (fast) {
-        const uint32_t v = __ldg(reinterpret_cast<const uint32_t*>(row + x0));
-        p[1] = v & 0xff;
-        p[2] = (v >> 8) & 0xff;
-        p[3] = (v >> 16) & 0xff;
-        p[4] = v >> 24;
-        p[0] = x0 ? __ldg(row + x0 - 1) : p[1];
-        p[5] = x0 + 4 < w ? __ldg(row + x0 + 4) : p[4];
-    } else {
+// ---- 3 x 3 neighbourhoods on a byte image, clamp-to-edge, in K11's arrangement (stencil_kernels.cu) ---------------------
+// blockDim = (32, 4), tile = 512 pixels x 16 rows: a lane owns 16 pixels (one 128-bit word) of 4 consecutive rows.  The six
+// input rows of a lane (4 + the row above and below) are loaded before the first add; horizontal neighbours come from the
+// adjacent lanes by shuffle.  Per row, sums are kept as two 16-bit halves per register (the even pixels b0, b2 and the odd
+// pixels b1, b3 of each 32-bit word): every partial sum below fits 16 bits, so packed adds never carry between the halves.
+struct Packed16 {
+    uint32_t ev[4], od[4];
+};
+// left / right neighbours of the even and of the odd pixels of word k, as packed halves
+__device__ __forceinline__ void neighbours(const uint32_t (&x)[4], int k, uint32_t lb, uint32_t rb, uint32_t& ev, uint32_t& od, uint32_t& le,
+                                           uint32_t& re, uint32_t& lo, uint32_t& ro) {
+    ev = x[k] & 0x00ff00ffu;          // (b0, b2)
+    od = (x[k] >> 8) & 0x00ff00ffu;   // (b1, b3)
+    const uint32_t prev_b3 = k == 0 ? lb : x[k - 1] >> 24;
+    const uint32_t next_b0 = k == 3 ? rb : x[k + 1] & 0xffu;
+    le = (od << 16) | prev_b3;        // left of (b0, b2) = (b-1, b1)
+    re = od;                          // right of (b0, b2) = (b1, b3)
+    lo = ev;                          // left of (b1, b3) = (b0, b2)
+    ro = (ev >> 16) | (next_b0 << 16);  // right of (b1, b3) = (b2, b4)
+}
+// per row: horizontal [1 c 1] sums (c = 1: <= 765, c = 2: <= 1020) and biased horizontal differences right - left + 255 (0 .. 510)
+template <uint32_t kCentre>
+__device__ __forceinline__ Packed16 hsum16(const uint4& wd, uint32_t lb, uint32_t rb) {
+    const uint32_t x[4] = {wd.x, wd.y, wd.z, wd.w};
+    Packed16 r;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) {
-            int x = (int)x0 - 1 + c;
-            x = x < 0 ? 0 : (x >= (int)w ? (int)w - 1 : x);
-            p[c] = __ldg(row + x);
-        }
+    for (int k = 0; k < 4; ++k) {
+        uint32_t ev, od, le, re, lo, ro;
+        neighbours(x, k, lb, rb, ev, od, le, re, lo, ro);
+        r.ev[k] = le + kCentre * ev + re;
+        r.od[k] = lo + kCentre * od + ro;
+    }
+    return r;
+}
+__device__ __forceinline__ Packed16 hdiff16(const uint4& wd, uint32_t lb, uint32_t rb) {
+    const uint32_t x[4] = {wd.x, wd.y, wd.z, wd.w};
+    Packed16 r;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        uint32_t ev, od, le, re, lo, ro;
+        neighbours(x, k, lb, rb, ev, od, le, re, lo, ro);
+        r.ev[k] = (re + 0x00ff00ffu) - le;  // each half: 255 - left >= 0, so no borrow crosses into the other half
+        r.od[k] = (ro + 0x00ff00ffu) - lo;
+    }
+    return r;
+}
+// The lane's 16 pixels of rows r0 - 1 .. r0 + 4 (clamped) and the pixel on either side of them (clamped at the image's edge).
+struct Lane16 {
+    uint4 wd[6];
+    uint32_t lb[6], rb[6];
+};
+__device__ __forceinline__ void load_lane16(const uint8_t* __restrict__ in, uint32_t w, uint32_t h, uint32_t r0, uint32_t x16, bool active, Lane16& L) {
+    const uint32_t lane = threadIdx.x;
+    uint32_t le[6], re[6];  // edge pixels fetched from memory by the warp's first / last lane
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const uint32_t rr = min(max((int)r0 - 1 + k, 0), (int)h - 1);
+        const uint8_t* row = in + (size_t)rr * w;
+        L.wd[k] = active ? __ldg(reinterpret_cast<const uint4*>(row + x16)) : make_uint4(0, 0, 0, 0);
+        le[k] = (active && lane == 0 && x16 > 0) ? __ldg(row + x16 - 1) : 0u;
+        re[k] = (active && lane == 31 && x16 + 16 < w) ? __ldg(row + x16 + 16) : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        uint32_t lb = __shfl_up_sync(0xffffffffu, L.wd[k].w >> 24, 1);
+        uint32_t rb = __shfl_down_sync(0xffffffffu, L.wd[k].x & 0xffu, 1);
+        if (lane == 0) lb = x16 > 0 ? le[k] : (L.wd[k].x & 0xffu);  // clamp at the left edge
+        if (x16 + 16 >= w) rb = L.wd[k].w >> 24;                    // clamp at the right edge
+        else if (lane == 31) rb = re[k];
+        L.lb[k] = lb;
+        L.rb[k] = rb;
     }
 }
-
+// ragged width (rows are not 16-byte aligned): the thread's 16 x 4 pixels one by one, nine clamped taps each
 template <typename F>
-__device__ __forceinline__ void stencil3x3_u8(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, uint32_t w, uint32_t h, F f) {
-    const uint32_t x0 = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
-    const uint32_t y = blockIdx.y * blockDim.y + threadIdx.y;
-    if (x0 >= w || y >= h) return;
-    const bool fast = (w & 3u) == 0 && (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (reinterpret_cast<uintptr_t>(out) & 3u) == 0;
-    const uint32_t yu = y ? y - 1 : 0, yd = y + 1 < h ? y + 1 : h - 1;
-    int r[3][6];
-    load_row6(in + (size_t)yu * w, x0, w, fast, r[0]);
-    load_row6(in + (size_t)y * w, x0, w, fast, r[1]);
-    load_row6(in + (size_t)yd * w, x0, w, fast, r[2]);
-    uint32_t o[4];
+__device__ __forceinline__ void stencil_ragged(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, uint32_t w, uint32_t h, uint32_t r0, F f) {
+    const uint32_t x0 = (blockIdx.x * 32u + threadIdx.x) * 16u;
+    for (uint32_t r = r0; r < min(r0 + 4u, h); ++r)
+        for (uint32_t x = x0; x < min(x0 + 16u, w); ++x) {
+            int t[9];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) o[k] = f(r[0][k], r[0][k + 1], r[0][k + 2], r[1][k], r[1][k + 1], r[1][k + 2], r[2][k], r[2][k + 1], r[2][k + 2]);
-    if (fast) {
-        *reinterpret_cast<uint32_t*>(out + (size_t)y * w + x0) = o[0] | (o[1] << 8) | (o[2] << 16) | (o[3] << 24);
-    } else {
-        for (uint32_t k = 0; k < 4 && x0 + k < w; ++k) out[(size_t)y * w + x0 + k] = (uint8_t)o[k];
-    }
+            for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+                for (int dx = -1; dx <= 1; ++dx) {
+                    const int yy = min(max((int)r + dy, 0), (int)h - 1), xx = min(max((int)x + dx, 0), (int)w - 1);
+                    t[(dy + 1) * 3 + dx + 1] = in[(size_t)yy * w + xx];
+                }
+            out[(size_t)r * w + x] = (uint8_t)f(t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8]);
+        }
 }
+__device__ __forceinline__ uint32_t interleave(uint32_t ev, uint32_t od) { return (ev & 0x00ff00ffu) | ((od & 0x00ff00ffu) << 8); }
 
 }  // namespace
 
 // K17: e = min(255, |gx| + |gy|), gx = [-1 0 1; -2 0 2; -1 0 1] * n, gy = its transpose (reading S6-2).
-extern "C" __global__ void __launch_bounds__(256) set_k_sobel3x3_u8(const uint8_t* __restrict__ n, uint8_t* __restrict__ e, uint32_t w, uint32_t h) {
+// gx = vertical [1 2 1] of the rows' horizontal differences (right - left), gy = the bottom row's horizontal [1 2 1] sum
+// minus the top row's.  Both are carried with a bias of 1020 so that the packed halves stay non-negative (0 .. 2040).
+extern "C" __global__ void __launch_bounds__(128) set_k_sobel3x3_u8(const uint8_t* __restrict__ n, uint8_t* __restrict__ e, uint32_t w, uint32_t h) {
     set_pdl_sync(n);
-    stencil3x3_u8(n, e, w, h, [](int a, int b, int c, int d, int, int f, int g, int hh, int i) -> uint32_t {
-        const int gx = (c - a) + 2 * (f - d) + (i - g);
-        const int gy = (g - a) + 2 * (hh - b) + (i - c);
-        const int m = abs(gx) + abs(gy);
-        return (uint32_t)(m > 255 ? 255 : m);
-    });
+    const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
+    if ((w & 15u) != 0) {
+        stencil_ragged(n, e, w, h, r0, [](int a, int b, int c, int d, int, int f, int g, int hh, int i) -> uint32_t {
+            const int gx = (c - a) + 2 * (f - d) + (i - g);
+            const int gy = (g - a) + 2 * (hh - b) + (i - c);
+            const int m = abs(gx) + abs(gy);
+            return (uint32_t)(m > 255 ? 255 : m);
+        });
+        return;
+    }
+    const uint32_t x16 = (blockIdx.x * 32u + threadIdx.x) * 16u;
+    const bool active = x16 < w;
+    if (r0 >= h) return;  // warp-uniform
+    Lane16 L;
+    load_lane16(n, w, h, r0, x16, active, L);
+    Packed16 hd[6], hs[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        hd[k] = hdiff16(L.wd[k], L.lb[k], L.rb[k]);
+        hs[k] = hsum16<2>(L.wd[k], L.lb[k], L.rb[k]);
+    }
+    if (!active) return;
+    constexpr uint32_t kBias = 0x03fc03fcu;  // 1020 in both halves
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (r0 + k >= h) break;
+        uint32_t o[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t m[2];
+#pragma unroll
+            for (int par = 0; par < 2; ++par) {  // even pixels, odd pixels
+                const uint32_t* d0 = par ? hd[k].od : hd[k].ev;
+                const uint32_t* d1 = par ? hd[k + 1].od : hd[k + 1].ev;
+                const uint32_t* d2 = par ? hd[k + 2].od : hd[k + 2].ev;
+                const uint32_t* s0 = par ? hs[k].od : hs[k].ev;
+                const uint32_t* s2 = par ? hs[k + 2].od : hs[k + 2].ev;
+                const uint32_t gxb = d0[q] + 2u * d1[q] + d2[q];   // gx + 1020 per half
+                const uint32_t gyb = s2[q] + (kBias - s0[q]);      // gy + 1020 per half (s0 <= 1020: no borrow)
+                const uint32_t ax = __vabsdiffu2(gxb, kBias), ay = __vabsdiffu2(gyb, kBias);
+                m[par] = __vminu2(ax + ay, 0x00ff00ffu);           // |gx| + |gy| <= 2040: no carry between the halves
+            }
+            o[q] = interleave(m[0], m[1]);
+        }
+        *reinterpret_cast<uint4*>(e + (size_t)(r0 + k) * w + x16) = make_uint4(o[0], o[1], o[2], o[3]);
+    }
 }
 
-// K18: m = (sum of the 3 x 3 neighbourhood) / 9, integer division (reading S6-3).
-extern "C" __global__ void __launch_bounds__(256) set_k_mean3x3_u8(const uint8_t* __restrict__ e, uint8_t* __restrict__ m, uint32_t w, uint32_t h) {
+// K18: m = (sum of the 3 x 3 neighbourhood) / 9, integer division (reading S6-3).  Sum <= 2295; floor(v / 9) =
+// (v * 7282) >> 16 for every v in that range (checked exhaustively in tests/test_host_logic.py).
+extern "C" __global__ void __launch_bounds__(128) set_k_mean3x3_u8(const uint8_t* __restrict__ e, uint8_t* __restrict__ m, uint32_t w, uint32_t h) {
     set_pdl_sync(e);
-    stencil3x3_u8(e, m, w, h, [](int a, int b, int c, int d, int ee, int f, int g, int hh, int i) -> uint32_t {
-        return (uint32_t)(a + b + c + d + ee + f + g + hh + i) / 9u;
-    });
+    const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
+    if ((w & 15u) != 0) {
+        stencil_ragged(e, m, w, h, r0, [](int a, int b, int c, int d, int ee, int f, int g, int hh, int i) -> uint32_t {
+            return (uint32_t)(a + b + c + d + ee + f + g + hh + i) / 9u;
+        });
+        return;
+    }
+    const uint32_t x16 = (blockIdx.x * 32u + threadIdx.x) * 16u;
+    const bool active = x16 < w;
+    if (r0 >= h) return;  // warp-uniform
+    Lane16 L;
+    load_lane16(e, w, h, r0, x16, active, L);
+    Packed16 hs[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) hs[k] = hsum16<1>(L.wd[k], L.lb[k], L.rb[k]);
+    if (!active) return;
+    auto div9 = [](uint32_t v) { return (((v & 0xffffu) * 7282u) >> 16) | ((((v >> 16) * 7282u) >> 16) << 16); };
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (r0 + k >= h) break;
+        uint32_t o[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            o[q] = interleave(div9(hs[k].ev[q] + hs[k + 1].ev[q] + hs[k + 2].ev[q]), div9(hs[k].od[q] + hs[k + 1].od[q] + hs[k + 2].od[q]));
+        *reinterpret_cast<uint4*>(m + (size_t)(r0 + k) * w + x16) = make_uint4(o[0], o[1], o[2], o[3]);
+    }
 }
 
 // K19: t = m >= thresh ? 255 : 0 (reading S6-4).  16 pixels per thread: one 128-bit load, one 128-bit store.

@@ -270,12 +270,12 @@ extern "C" set_status set_builtin_pipeline(int config, int variant, const uint32
             bf[3] = buffer(maxpix);  // pong; the blended output ends here
             bf[3].d2h_bytes = scaled(1, WH);
             nb = 4;
-            const set_grid_rule gx = grid_div(scaled(1, 0x1), kStencilTileW), gy = grid_div(scaled(1, 0x2), kStencilTileH);
+            const set_grid_rule gx = grid_div(scaled(1, 0x1), kBlurTileW), gy = grid_div(scaled(1, 0x2), kBlurTileH);  // K11's tile
             const set_grid_rule gp = grid_div(scaled(1, WH), kBytePixPerBlock);
             st[ns++] = stage(SET_K_RGB2GRAY_U8, grid_div(scaled(1, WH), kGrayPixPerBlock), grid_fixed(1), 256, 1, 0,
                              {arg_buf(0), arg_buf(1), arg_dim(0), arg_dim(1)});
-            st[ns++] = stage(SET_K_SOBEL3X3_U8, gx, gy, 64, 4, 0, {arg_buf(1), arg_buf(2), arg_dim(0), arg_dim(1)});
-            st[ns++] = stage(SET_K_MEAN3X3_U8, gx, gy, 64, 4, 0, {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});
+            st[ns++] = stage(SET_K_SOBEL3X3_U8, gx, gy, 32, 4, 0, {arg_buf(1), arg_buf(2), arg_dim(0), arg_dim(1)});
+            st[ns++] = stage(SET_K_MEAN3X3_U8, gx, gy, 32, 4, 0, {arg_buf(2), arg_buf(3), arg_dim(0), arg_dim(1)});
             st[ns++] = stage(SET_K_THRESHOLD_U8, gp, grid_fixed(1), 256, 1, 0, {arg_buf(3), arg_buf(2), arg_dim(0), arg_dim(1), arg_u32(thresh)});
             st[ns++] = stage(SET_K_BLEND_U8, gp, grid_fixed(1), 256, 1, 0, {arg_buf(2), arg_buf(1), arg_buf(3), arg_dim(0), arg_dim(1)});
             break;

@@ -1064,13 +1064,14 @@ def test_config6_ragged_frames(libset, size):
     check(libset, wl, list(range(3)))
 
 
+@pytest.mark.parametrize("size", [(328, 77), (336, 77), (1040, 19), (512, 16)])
 @pytest.mark.parametrize("upto", [2, 3, 4])
-def test_config6_stage_by_stage(libset, upto):
+def test_config6_stage_by_stage(libset, upto, size):
     """The Sobel chain truncated after the edge (2), mean (3) and threshold (4) stages, with that stage's buffer copied
     back: every intermediate image bit for bit against the oracle's stage functions."""
     import oracle
     from paper_2606_05495_b200.workloads import PinnedArena
-    w, h = 328, 77
+    w, h = size    # a ragged width (per-pixel path); multiples of 16: part of a 512-pixel tile, two tiles and a bit, exactly one tile
     st, ns, bf, nb, _, _ = libset.builtin_pipeline(6, 0, [w, h])
     assert ns == 5 and nb == 4
     src_buf = {2: 2, 3: 3, 4: 2}[upto]                         # sobel -> buffer 2, mean -> 3, threshold -> 2

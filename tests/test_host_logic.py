@@ -69,3 +69,8 @@ def test_scheduler_core_is_clean_under_thread_sanitizer():
                        env=dict(os.environ, TSAN_OPTIONS="halt_on_error=0 exitcode=66"))
     assert "SELFTEST OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
     assert r.returncode == 0 and "WARNING: ThreadSanitizer" not in r.stderr, r.stderr[-3000:]
+
+
+def test_divide_by_nine_multiplier_is_exact_on_the_mean_filters_range():
+    """K18 (set_k_mean3x3_u8) divides the 3 x 3 sum (at most 9 * 255) by 9 as (v * 7282) >> 16 in each 16-bit half."""
+    assert all((v * 7282) >> 16 == v // 9 for v in range(9 * 255 + 1))
