@@ -393,7 +393,9 @@ set_status set_get_geometry(set_ctx *ctx, int *out_slots, int *out_streams, int 
 
 /* Time stage `stage` alone on slot 0's buffers and stream: a graph holding a chain of `iters` launches of the
  * stage's kernel (no host launch cost between them), run once or more for warm-up (`warmup` > 0) and then once
- * bracketed by CUDA events on that stream; dims as in set_submit_dims (NULL => all 1).
+ * bracketed by CUDA events on that stream; dims as in set_submit_dims (NULL => all 1).  The launches are chained by
+ * plain edges, or by programmatic edges if the stage was registered with SET_STAGE_PDL (what the kernel costs behind
+ * another kernel of such a job graph: the next launch is already resident while this one drains).
  * out_avg_us: HOST, average microseconds per launch.  Requires a drained context. */
 set_status set_time_stage(set_ctx *ctx, int stage, const uint32_t *dims, int warmup, int iters,
                           float *out_avg_us);

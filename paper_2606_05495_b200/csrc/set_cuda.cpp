@@ -1750,7 +1750,18 @@ set_status set_time_stage(set_ctx* c, int stage, const uint32_t* dims, int warmu
         kp.sharedMemBytes = sd.smem_bytes;
         kp.kernelParams = ap.ptrs;
         cudaGraphNode_t node;
-        er = cudaGraphAddKernelNode(&node, g, prev ? &prev : nullptr, prev ? 1 : 0, &kp);
+        if (prev && (sd.flags & SET_STAGE_PDL)) {
+            // the stage was registered with a programmatic edge in front of it: chain it the same way, so that the figure is
+            // what the kernel costs behind another kernel of a job graph (the next launch is resident while this one drains)
+            er = cudaGraphAddKernelNode(&node, g, nullptr, 0, &kp);
+            cudaGraphEdgeData ed{};
+            ed.from_port = cudaGraphKernelNodePortProgrammatic;
+            ed.to_port = 0;
+            ed.type = cudaGraphDependencyTypeProgrammatic;
+            if (er == cudaSuccess) er = cudaGraphAddDependencies_v2(g, &prev, &node, &ed, 1);
+        } else {
+            er = cudaGraphAddKernelNode(&node, g, prev ? &prev : nullptr, prev ? 1 : 0, &kp);
+        }
         prev = node;
     }
     if (er == cudaSuccess) er = cudaGraphInstantiate(&ge, g, 0);

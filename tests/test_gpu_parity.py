@@ -811,6 +811,19 @@ def test_maximum_depth_4096_in_flight(libset):
         ctx.close()
 
 
+def test_time_stage_chains_by_plain_or_programmatic_edges(libset):
+    """set_time_stage (bench.py's kernel rooflines): a chain of launches by plain edges, or by programmatic edges when the
+    stage carries SET_STAGE_PDL; both run, give a sane time, leave the context usable and its results right."""
+    from paper_2606_05495_b200.workloads import small_workload
+    wl = small_workload(1)
+    for pdl in (False, True):
+        with libset.Context(2, 4) as ctx:
+            ctx.register_builtin(1, 0, list(wl.params), pdl=pdl)
+            ts = [ctx.time_stage(k, None, warmup=2, iters=20) for k in range(ctx.num_stages)]
+            assert all(0.2 < t < 100.0 for t in ts), ts
+        check(libset, wl, list(range(8)), pdl=pdl)
+
+
 # ---------------------------------------------------------------------------------------------------------------------
 # SURVEY.md 8(e): one scheduler instance per GPU behind one submit call, host-side stealing across instances.  One GPU here:
 # both instances sit on device 0 (set.h allows it), which exercises everything but the second device.
