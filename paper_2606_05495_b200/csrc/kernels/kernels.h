@@ -52,6 +52,15 @@ __device__ __forceinline__ void set_pdl_sync(P&... inputs) {
     asm volatile("griddepcontrol.wait;" ::: "memory");
     (set_pdl_launder(inputs), ...);
 }
+// The same without the early trigger, for kernels whose grid covers a frame (K10-K12, K17-K20): with launch_dependents at the
+// top, the NEXT kernel's blocks become resident at once and sit on SM slots and registers, spinning in their wait, while
+// blocks of THIS kernel have yet to start -- config 6 device-resident ran at 119 K jobs/s with the trigger and 145 K without
+// (profiles/r2_probes.md section 8).  Without a trigger the dependent launches when this grid completes, as over a plain edge.
+template <typename... P>
+__device__ __forceinline__ void set_pdl_wait(P&... inputs) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    (set_pdl_launder(inputs), ...);
+}
 #endif
 
 // Tile shapes the host-side grid rules in set_builtin.cu must agree with.

@@ -108,7 +108,7 @@ __device__ __forceinline__ uint32_t interleave(uint32_t ev, uint32_t od) { retur
 // gx = vertical [1 2 1] of the rows' horizontal differences (right - left), gy = the bottom row's horizontal [1 2 1] sum
 // minus the top row's.  Both are carried with a bias of 1020 so that the packed halves stay non-negative (0 .. 2040).
 extern "C" __global__ void __launch_bounds__(128) set_k_sobel3x3_u8(const uint8_t* __restrict__ n, uint8_t* __restrict__ e, uint32_t w, uint32_t h) {
-    set_pdl_sync(n);
+    set_pdl_wait(n);
     const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
     if ((w & 15u) != 0) {
         stencil_ragged(n, e, w, h, r0, [](int a, int b, int c, int d, int, int f, int g, int hh, int i) -> uint32_t {
@@ -160,7 +160,7 @@ extern "C" __global__ void __launch_bounds__(128) set_k_sobel3x3_u8(const uint8_
 // K18: m = (sum of the 3 x 3 neighbourhood) / 9, integer division (reading S6-3).  Sum <= 2295; floor(v / 9) =
 // (v * 7282) >> 16 for every v in that range (checked exhaustively in tests/test_host_logic.py).
 extern "C" __global__ void __launch_bounds__(128) set_k_mean3x3_u8(const uint8_t* __restrict__ e, uint8_t* __restrict__ m, uint32_t w, uint32_t h) {
-    set_pdl_sync(e);
+    set_pdl_wait(e);
     const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
     if ((w & 15u) != 0) {
         stencil_ragged(e, m, w, h, r0, [](int a, int b, int c, int d, int ee, int f, int g, int hh, int i) -> uint32_t {
@@ -192,7 +192,7 @@ extern "C" __global__ void __launch_bounds__(128) set_k_mean3x3_u8(const uint8_t
 // K19: t = m >= thresh ? 255 : 0 (reading S6-4).  16 pixels per thread: one 128-bit load, one 128-bit store.
 extern "C" __global__ void __launch_bounds__(256) set_k_threshold_u8(const uint8_t* __restrict__ m, uint8_t* __restrict__ t, uint32_t w, uint32_t h,
                                                                       uint32_t thresh) {
-    set_pdl_sync(m);
+    set_pdl_wait(m);
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     const uint32_t th4 = thresh * 0x01010101u;
@@ -212,7 +212,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_threshold_u8(const uint8
 // K20: out = (128 t + 128 n) >> 8 = (t + n) >> 1 per byte (reading S6-5): the halving add without rounding.
 extern "C" __global__ void __launch_bounds__(256) set_k_blend_u8(const uint8_t* __restrict__ t, const uint8_t* __restrict__ n, uint8_t* __restrict__ out,
                                                                   uint32_t w, uint32_t h) {
-    set_pdl_sync(t, n);
+    set_pdl_wait(t, n);
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     if (p0 + 15 < npix && ((reinterpret_cast<uintptr_t>(t) | reinterpret_cast<uintptr_t>(n) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0) {

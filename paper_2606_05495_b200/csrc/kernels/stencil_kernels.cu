@@ -95,7 +95,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_jacobi5_f32(const float*
 // ------------------------------------------------------------------------------------------------------------
 extern "C" __global__ void __launch_bounds__(256) set_k_rgb2gray_u8(const uint8_t* __restrict__ rgb, uint8_t* __restrict__ gray,
                                                                     uint32_t w, uint32_t h) {
-    set_pdl_sync(rgb);
+    set_pdl_wait(rgb);
     const uint32_t npix = w * h;
     const uint32_t p0 = (blockIdx.x * 256u + threadIdx.x) * 16u;
     if (p0 + 15 < npix) {
@@ -152,7 +152,7 @@ __device__ __forceinline__ HRow hsum16(const uint4& wd, uint32_t lb, uint32_t rb
 
 extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t* __restrict__ g, uint8_t* __restrict__ out, uint32_t w,
                                                                    uint32_t h) {
-    set_pdl_sync(g);
+    set_pdl_wait(g);
     const uint32_t r0 = blockIdx.y * kBlurTileH + threadIdx.y * 4u;
     if ((w & 15u) == 0) {
         const uint32_t lane = threadIdx.x;
@@ -217,7 +217,7 @@ extern "C" __global__ void __launch_bounds__(256) set_k_blur3x3_u8(const uint8_t
 // ------------------------------------------------------------------------------------------------------------
 extern "C" __global__ void __launch_bounds__(256) set_k_hist256_u8(const uint8_t* __restrict__ p, uint32_t* __restrict__ hist,
                                                                    uint32_t w, uint32_t h) {
-    set_pdl_sync(p);
+    set_pdl_wait(p);
     static_assert(kHistPixPerBlock == 256 * 16, "one 128-bit load per thread");
     const uint32_t n = w * h;
     __shared__ uint32_t sh[8][256];
