@@ -135,7 +135,10 @@ typedef struct set_arg_desc {
                               an SM copy node) with a programmatic-dependent-launch edge.  By setting the flag the
                               caller asserts that the kernel executes griddepcontrol.wait before it reads or writes
                               job data; every built-in kernel does (the tcgen05 GEMM after its barrier / TMEM set-up,
-                              before its first TMA load).  Ignored where the predecessor is a copy-engine node.  */
+                              before its first TMA load).  A kernel that also executes griddepcontrol.launch_dependents
+                              early lets the NEXT node's blocks become resident while it still runs: the built-in kernels
+                              with a handful of blocks do, those whose grid covers a frame do not (their dependents
+                              would only sit on SM resources).  Ignored where the predecessor is a copy-engine node.  */
 
 /* One stage = one kernel node of the job graph ("nodes are initialized with the target
  * function, input arguments, grid and block dimensions").  Stages run in list order. */
